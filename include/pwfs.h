@@ -1,0 +1,152 @@
+/*
+ * pwfs.h -- C ABI of libpwfs.so: the modulated pyramid wavefront-sensor forward
+ * model on one NVIDIA B200 (sm_100a), hand-written CUDA, no cuFFT.
+ *
+ * What the library computes (one "frame" per input phase screen):
+ *   for each of K points on the modulation circle build the pupil phasor
+ *   A exp(i(phi + tilt_k)), zero-pad it into an M x M grid, 2-D DFT to the focal
+ *   plane, multiply by the four-face pyramid phase mask, inverse 2-D DFT back
+ *   to the pupil plane, accumulate |E|^2 over k; rebin the four pupil images to
+ *   n_sub x n_sub subaperture pixels each (one 2n_sub x 2n_sub detector frame)
+ *   and reduce them to normalised x/y slopes over the valid subapertures.
+ *
+ * Where this is defined.  The paper names the object and its wiring only:
+ * "apply a transformation from focal plane to pupil plane emulating an optical
+ * pyramid" (sec. 2); parameters pup_diam / pup_dist / mod_amp /
+ * output_resolution / wavelengthInNm (Table 1);
+ * pyr.in_ef -> pyr.out_i -> ccd.in_i, ccd.out_pixels ->
+ * sc.in_pixels -> sc.out_slopes; GPU-resident data passed
+ * by opaque handle (sec. 6); "Pyramid ... propagation (from
+ * wavefront to detector plane)" is one of the GPU-accelerated routines
+ * (PAPER.md:L342).  The arithmetic is BASELINE.json `north_star`, written out
+ * as steps O0..O9 in SURVEY.md section 8(c) and restated with every reading of
+ * a silent point in DESIGN.md.
+ *
+ * Conventions
+ *   - 2-D arrays are row-major [y][x] (x fast).  Phase is in radians at the
+ *     sensing wavelength.  1 lambda/D of tilt = 2 pi across the N pupil pixels.
+ *   - Every function returns PWFS_OK (0) or a negative pwfs_status; nothing
+ *     throws or aborts across this boundary and there is no global mutable state.
+ *   - A handle owns its device tables and scratch memory.  The caller owns
+ *     pupil_amp (host memory, copied by pwfs_create) and the phase / frames /
+ *     slopes buffers.  A handle is not thread-safe; distinct handles are.
+ *   - Non-finite phase values propagate to the outputs (no checking on the hot
+ *     path).
+ */
+#ifndef PWFS_H
+#define PWFS_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pwfs pwfs_t; /* opaque */
+
+typedef enum {
+    PWFS_OK = 0,
+    PWFS_EINVAL = -1,       /* bad parameter, NULL pointer, geometry that leaves the grid, n_valid == 0 */
+    PWFS_ENOMEM = -2,       /* host or device allocation failed */
+    PWFS_ECUDA = -3,        /* a CUDA runtime call failed (see pwfs_last_cuda_error) */
+    PWFS_EUNSUPPORTED = -4  /* valid request this build has no kernel for (e.g. M/32 not instantiated) */
+} pwfs_status;
+
+/* Parameters of one sensor (names follow PAPER.md Table 1 where
+ * the paper has one: n_subap = pup_diam, mod_radius = mod_amp). */
+typedef struct {
+    int32_t n_pupil;        /* N >= 2 : pupil sampling, D spans exactly N px                  */
+    int32_t m_grid;         /* M : FFT grid.  Even, M >= 2N, M = 32*R with R in the built set
+                               (pwfs_supported_grid); R is 2/3/5-smooth, R <= 32              */
+    const float *pupil_amp; /* HOST ptr, N*N floats row-major [y][x]; amplitude A >= 0; copied */
+    int32_t mask_shift_px;  /* s : pupil-image offset in px (mask phase 2 pi s (|u~|+|v~|)/M).
+                               <= 0 selects the default M/4 (needs M % 4 == 0).
+                               Needs N <= 2 s and s <= M/2 - N/2 (windows disjoint, in grid)  */
+    float mod_radius;       /* r >= 0 in lambda/D                                             */
+    int32_t mod_points;     /* K >= 1 points equally spaced on the circle (K=1, r=0: none)    */
+    float mod_angle0;       /* theta_0 [rad] of point 0, counter-clockwise from +x            */
+    int32_t n_subap;        /* n_sub in [1, N]: subapertures across one pupil image;
+                               binning b = N / n_sub need not be an integer (area weights)    */
+    float illum_thresh;     /* valid iff illumination >= thresh * full subaperture; <= 0 -> 0.5 */
+    int32_t slope_norm;     /* 0: divide by the mean valid-subaperture flux (default);
+                               1: divide by the subaperture's own flux                        */
+    int32_t device;         /* CUDA device ordinal                                            */
+} pwfs_params;
+
+/* Build a sensor: validates p, computes all tables on the host in double
+ * precision (tilt tables, mask, twiddles, rebin weights, valid mask), uploads
+ * them.  Scratch memory is allocated lazily by the first pwfs_run and reused.
+ * On failure *out is set to NULL.  Defined by: north_star "pwfs_create(pupil,
+ * M, mask params, mod radius, K, binning)". */
+int pwfs_create(const pwfs_params *p, pwfs_t **out);
+
+/* Detector size (2*n_sub) and number of valid subapertures.  Either pointer
+ * may be NULL. */
+int pwfs_info(const pwfs_t *h, int32_t *det_size, int32_t *n_valid);
+
+/* Copy the n_sub*n_sub valid-subaperture mask (row-major [j][i], 1 = valid,
+ * same mask for all four pupil images) to HOST memory. */
+int pwfs_valid_mask(const pwfs_t *h, uint8_t *host_mask);
+
+/* The hot path.  d_phase: DEVICE float [B][N][N] (radians).  d_frames: DEVICE
+ * float [B][2n_sub][2n_sub], frame[qy*n_sub + j][qx*n_sub + i] = area-weighted
+ * SUM of I = mean_k |E_k|^2 over subaperture (j,i) of the pupil image at
+ * (M/2 + (2qx-1)s, M/2 + (2qy-1)s).  d_slopes: DEVICE float [B][2*n_valid] =
+ * [Sx(valid subaps, row-major) ..., Sy(...)], Sx = ((a+c)-(b+d))/norm,
+ * Sy = ((a+b)-(c+d))/norm with a,b,c,d the tiles (qx,qy) = (0,0),(1,0),(0,1),
+ * (1,1); may be NULL.  cuda_stream: a cudaStream_t (NULL = default stream).
+ * Asynchronous: work is enqueued on the stream and the call returns; buffers
+ * must stay alive until the stream reaches that point.  B = 0 is a no-op.
+ * Does not allocate once scratch has been sized for a batch this large.
+ * Defined by: north_star "pwfs_run(phase batch -> frames, slopes)". */
+int pwfs_run(pwfs_t *h, const float *d_phase, int32_t B, float *d_frames, float *d_slopes,
+             void *cuda_stream);
+
+/* Same computation with HOST buffers (h_slopes may be NULL): copies the phase
+ * batch host->device, runs, copies frames and slopes device->host on an
+ * internal stream and returns after they have arrived (synchronous).  Pinned
+ * host memory makes the copies asynchronous to the kernels of the previous
+ * chunk; pageable memory works but is slower. */
+int pwfs_run_host(pwfs_t *h, const float *h_phase, int32_t B, float *h_frames, float *h_slopes);
+
+/* Release everything the handle owns.  NULL-safe. */
+void pwfs_destroy(pwfs_t *h);
+
+/* Static description of a status code. */
+const char *pwfs_strerror(int code);
+
+/* cudaError_t (as int) of the last failing CUDA call on this handle, 0 if none. */
+int pwfs_last_cuda_error(const pwfs_t *h);
+
+/* 1 if this build has kernels for an M-point grid, else 0. */
+int pwfs_supported_grid(int32_t m_grid);
+
+/* Scheduling knobs (0 keeps the built-in heuristic): frames processed per
+ * kernel chunk, and the number of ways the K modulation points are split
+ * across warps in the column pass.  Results do not depend on them beyond FP32
+ * summation order. */
+int pwfs_set_schedule(pwfs_t *h, int32_t frames_per_chunk, int32_t k_split);
+
+/* Instrumentation.  Kernel classes: 0 = row pass (phasor + x-convolution),
+ * 1 = column pass (y-convolution + |E|^2 accumulation + y-rebin),
+ * 2 = x-rebin, 3 = slopes.  pwfs_set_timing(h, 1) makes pwfs_run bracket every
+ * kernel with CUDA events on the caller's stream; pwfs_get_timing then
+ * synchronises those events and returns, for everything run since timing was
+ * enabled (or last read), the summed device time per class in milliseconds and
+ * the launch count per class.  launches[] is counted even when timing is off. */
+#define PWFS_NUM_KERNEL_CLASSES 4
+int pwfs_set_timing(pwfs_t *h, int32_t enable);
+int pwfs_get_timing(pwfs_t *h, float ms[PWFS_NUM_KERNEL_CLASSES],
+                    int64_t launches[PWFS_NUM_KERNEL_CLASSES]);
+
+/* Internal geometry, for reports: n_cols = pupil-plane columns actually
+ * computed (<= 2N), k_unique = distinct x-tilts among the K modulation points
+ * (the row pass is shared between points with equal x-tilt), frames_per_chunk
+ * and k_split as they would be used for a batch of B frames. */
+int pwfs_geometry(const pwfs_t *h, int32_t B, int32_t *n_cols, int32_t *k_unique,
+                  int32_t *frames_per_chunk, int32_t *k_split);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PWFS_H */

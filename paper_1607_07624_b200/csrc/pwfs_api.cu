@@ -1,0 +1,555 @@
+// pwfs_api.cu -- C ABI of libpwfs.so (include/pwfs.h): parameter validation,
+// host-side table construction (double precision), scratch management, kernel
+// dispatch and instrumentation.  No torch types, no cuFFT, no CPU fallback: every
+// step of the path runs in the kernels of pwfs_kernels.cuh.
+#include "../../include/pwfs.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "pwfs_kernels.cuh"
+
+using namespace pwk;
+
+namespace {
+
+constexpr double kTwoPi = 6.283185307179586476925286766559;
+
+// ---- per-grid kernel configurations (R1 = M/32, NB, warps/CTA row pass, column pass)
+using Cfg4 = PassCfg<4, 8, 4, 4>;     // M = 128
+using Cfg8 = PassCfg<8, 4, 4, 4>;     // M = 256
+using Cfg10 = PassCfg<10, 3, 16, 4>;  // M = 320
+using Cfg15 = PassCfg<15, 2, 8, 4>;   // M = 480
+using Cfg16 = PassCfg<16, 2, 8, 4>;   // M = 512
+using Cfg20 = PassCfg<20, 1, 16, 4>;  // M = 640
+using Cfg25 = PassCfg<25, 1, 16, 4>;  // M = 800
+using Cfg32 = PassCfg<32, 1, 16, 4>;  // M = 1024
+
+struct Launcher {
+    int R1, NB, WPB_X, WPB_Y, RPC;
+    size_t smem_x, smem_y;
+    const void *xfn, *yfn;
+    void (*launch_x)(dim3, cudaStream_t, const DevTables &, const float *, float2 *);
+    void (*launch_y)(dim3, cudaStream_t, const DevTables &, const float2 *, float *, int);
+};
+
+template <class C>
+void launch_x_t(dim3 grid, cudaStream_t st, const DevTables &t, const float *phase, float2 *T) {
+    xpass_kernel<C><<<grid, 32 * C::WPB_X, C::smem_x, st>>>(t, phase, T);
+}
+template <class C>
+void launch_y_t(dim3 grid, cudaStream_t st, const DevTables &t, const float2 *T, float *colbin, int ksplit) {
+    ypass_kernel<C><<<grid, 32 * C::WPB_Y, C::smem_y, st>>>(t, T, colbin, ksplit);
+}
+template <class C>
+Launcher make_launcher() {
+    Launcher l;
+    l.R1 = C::R1; l.NB = C::NB; l.WPB_X = C::WPB_X; l.WPB_Y = C::WPB_Y; l.RPC = C::RPC;
+    l.smem_x = C::smem_x; l.smem_y = C::smem_y;
+    l.xfn = (const void *)xpass_kernel<C>;
+    l.yfn = (const void *)ypass_kernel<C>;
+    l.launch_x = launch_x_t<C>;
+    l.launch_y = launch_y_t<C>;
+    return l;
+}
+
+bool find_launcher(int M, Launcher *out) {
+    if (M % 32) return false;
+    switch (M / 32) {
+        case 4: *out = make_launcher<Cfg4>(); return true;
+        case 8: *out = make_launcher<Cfg8>(); return true;
+        case 10: *out = make_launcher<Cfg10>(); return true;
+        case 15: *out = make_launcher<Cfg15>(); return true;
+        case 16: *out = make_launcher<Cfg16>(); return true;
+        case 20: *out = make_launcher<Cfg20>(); return true;
+        case 25: *out = make_launcher<Cfg25>(); return true;
+        case 32: *out = make_launcher<Cfg32>(); return true;
+        default: return false;
+    }
+}
+
+struct TimedSpan { cudaEvent_t a, b; int cls; };
+
+}  // namespace
+
+struct pwfs {
+    pwfs_params prm;
+    int device = 0;
+    int s = 0;
+    Launcher L{};
+    DevTables tab{};
+    std::vector<void *> dev_allocs;          // table memory
+    std::vector<uint8_t> valid;              // host copy of the valid mask
+    // scratch
+    float2 *T = nullptr; size_t T_elems = 0;
+    float *colbin = nullptr; size_t colbin_elems = 0;
+    // host-buffer path
+    cudaStream_t hstream = nullptr;
+    float *d_phase = nullptr, *d_frames = nullptr, *d_slopes = nullptr;
+    size_t d_cap_frames = 0;
+    // schedule
+    int user_fpc = 0, user_ksplit = 0;
+    int num_sms = 148;
+    size_t scratch_budget = (size_t)4 << 30;
+    // instrumentation
+    int timing = 0;
+    std::vector<TimedSpan> spans;
+    std::vector<cudaEvent_t> event_pool;
+    float ms_acc[PWFS_NUM_KERNEL_CLASSES] = {0, 0, 0, 0};
+    int64_t launches[PWFS_NUM_KERNEL_CLASSES] = {0, 0, 0, 0};
+    int last_cuda = 0;
+};
+
+namespace {
+
+#define PWFS_CUDA(h, call)                                         \
+    do {                                                           \
+        cudaError_t e__ = (call);                                  \
+        if (e__ != cudaSuccess) { (h)->last_cuda = (int)e__; return PWFS_ECUDA; } \
+    } while (0)
+
+template <typename T>
+int upload(pwfs *h, const std::vector<T> &v, const T **dst) {
+    void *d = nullptr;
+    size_t bytes = std::max<size_t>(v.size(), 1) * sizeof(T);
+    cudaError_t e = cudaMalloc(&d, bytes);
+    if (e != cudaSuccess) { h->last_cuda = (int)e; return e == cudaErrorMemoryAllocation ? PWFS_ENOMEM : PWFS_ECUDA; }
+    h->dev_allocs.push_back(d);
+    if (!v.empty()) {
+        e = cudaMemcpy(d, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) { h->last_cuda = (int)e; return PWFS_ECUDA; }
+    }
+    *dst = (const T *)d;
+    return PWFS_OK;
+}
+
+// Area-overlap rebin tables for one axis (O7): detector bin jj = q*n_sub + i takes
+// source px p in [floor(i N / n_sub), ceil((i+1) N / n_sub)) of window q with weight
+// |[p,p+1) n [i b,(i+1) b)| = integer / n_sub; `start` is the grid coordinate of the
+// first source px in the corner-placed frame used by the kernels.
+void build_rebin(int N, int M, int s, int n_sub, std::vector<int> &start, std::vector<int> &cnt,
+                 std::vector<float> &w, int &cmax, double yscale) {
+    const int D = 2 * n_sub;
+    std::vector<std::vector<double>> ws(D);
+    start.assign(D, 0); cnt.assign(D, 0); cmax = 0;
+    for (int jj = 0; jj < D; ++jj) {
+        const int q = jj / n_sub, i = jj % n_sub;
+        const long long lo_bin = (long long)i * N, hi_bin = (long long)(i + 1) * N;
+        const int p0 = (int)(lo_bin / n_sub);
+        const int p1 = (int)((hi_bin + n_sub - 1) / n_sub);     // exclusive
+        const int g = q == 0 ? (M - s) % M : s % M;              // window origin, corner-placed grid
+        start[jj] = (g + p0) % M;
+        for (int p = p0; p < p1; ++p) {
+            const long long lo = std::max<long long>((long long)p * n_sub, lo_bin);
+            const long long hi = std::min<long long>((long long)(p + 1) * n_sub, hi_bin);
+            ws[jj].push_back((double)(hi - lo) / (double)n_sub * yscale);
+        }
+        cnt[jj] = (int)ws[jj].size();
+        cmax = std::max(cmax, cnt[jj]);
+    }
+    w.assign((size_t)D * cmax, 0.f);
+    for (int jj = 0; jj < D; ++jj)
+        for (int c = 0; c < cnt[jj]; ++c) w[(size_t)jj * cmax + c] = (float)ws[jj][c];
+}
+
+// Valid-subaperture mask (O8): illumination = area-weighted sum of A^2, valid iff
+// >= thresh * b^2 * max A^2.  Integer-scaled weights (x n_sub per axis) make every
+// term an integer for binary A, so ties at exactly 50 % are decided exactly.
+int build_valid(int N, int n_sub, const float *A, double thresh, std::vector<uint8_t> &valid,
+                std::vector<int> &vidx) {
+    double amax2 = 0.0;
+    for (size_t t = 0; t < (size_t)N * N; ++t) amax2 = std::max(amax2, (double)A[t] * (double)A[t]);
+    valid.assign((size_t)n_sub * n_sub, 0);
+    vidx.clear();
+    if (!(amax2 > 0.0)) return 0;
+    auto overlap = [&](int i, int p) -> long long {
+        long long lo = std::max<long long>((long long)p * n_sub, (long long)i * N);
+        long long hi = std::min<long long>((long long)(p + 1) * n_sub, (long long)(i + 1) * N);
+        return hi > lo ? hi - lo : 0;
+    };
+    const double full = (double)N * (double)N * amax2;
+    for (int j = 0; j < n_sub; ++j) {
+        const int py0 = (int)(((long long)j * N) / n_sub), py1 = (int)((((long long)j + 1) * N + n_sub - 1) / n_sub);
+        for (int i = 0; i < n_sub; ++i) {
+            const int px0 = (int)(((long long)i * N) / n_sub), px1 = (int)((((long long)i + 1) * N + n_sub - 1) / n_sub);
+            double ill = 0.0;
+            for (int py = py0; py < py1; ++py)
+                for (int px = px0; px < px1; ++px) {
+                    const double a = (double)A[(size_t)py * N + px];
+                    ill += (double)(overlap(j, py) * overlap(i, px)) * a * a;
+                }
+            if (ill >= thresh * full) {
+                valid[(size_t)j * n_sub + i] = 1;
+                vidx.push_back(j * n_sub + i);
+            }
+        }
+    }
+    return (int)vidx.size();
+}
+
+int build_tables(pwfs *h) {
+    const pwfs_params &p = h->prm;
+    const int N = p.n_pupil, M = p.m_grid, K = p.mod_points, n_sub = p.n_subap, s = h->s;
+    const int R1 = h->L.R1;
+    DevTables &t = h->tab;
+    t.N = N; t.M = M; t.NP = (N + 15) / 16 * 16; t.K = K;
+    t.D = 2 * n_sub; t.n_sub = n_sub; t.slope_norm = p.slope_norm;
+
+    // O0: modulation points; distinct x-tilts (the row pass depends on k only through dx_k)
+    std::vector<double> dx(K), dy(K), ux;
+    std::vector<int> jx(K);
+    for (int k = 0; k < K; ++k) {
+        const double th = (double)p.mod_angle0 + kTwoPi * (double)k / (double)K;
+        dx[k] = (double)p.mod_radius * std::cos(th);
+        dy[k] = (double)p.mod_radius * std::sin(th);
+        int found = -1;
+        for (size_t u = 0; u < ux.size(); ++u)
+            if (std::fabs(ux[u] - dx[k]) <= 1e-9 * std::max(1.0, (double)p.mod_radius)) { found = (int)u; break; }
+        if (found < 0) { found = (int)ux.size(); ux.push_back(dx[k]); }
+        jx[k] = found;
+    }
+    t.KX = (int)ux.size();
+    const double c = 0.5 * (double)(N - 1);
+    std::vector<float> txt((size_t)t.KX * N);
+    for (int j = 0; j < t.KX; ++j)
+        for (int x = 0; x < N; ++x) {
+            double turns = ux[j] * ((double)x - c) / (double)N;       // O1, x part, in turns
+            turns -= std::nearbyint(turns);
+            txt[(size_t)j * N + x] = (float)turns;
+        }
+    std::vector<float2> tyt((size_t)K * N);
+    for (int k = 0; k < K; ++k)
+        for (int y = 0; y < N; ++y) {
+            double turns = dy[k] * ((double)y - c) / (double)N;       // O1, y part
+            turns -= std::nearbyint(turns);
+            tyt[(size_t)k * N + y] = make_float2((float)std::cos(kTwoPi * turns), (float)std::sin(kTwoPi * turns));
+        }
+    // twiddles between the two register stages, and the 1-D mask a(u)/M (O4; 1/M = O5's scale per axis)
+    std::vector<float2> tw((size_t)R1 * 32), am((size_t)R1 * 32);
+    for (int k1 = 0; k1 < R1; ++k1)
+        for (int n2 = 0; n2 < 32; ++n2) {
+            const double ang = -kTwoPi * (double)((k1 * n2) % M) / (double)M;
+            tw[(size_t)k1 * 32 + n2] = make_float2((float)std::cos(ang), (float)std::sin(ang));
+            const int u = k1 + R1 * n2;                               // n2 plays k2 here
+            const int us = u < M / 2 ? u : u - M;
+            const long long num = ((long long)s * std::abs(us)) % M;
+            const double am_ang = kTwoPi * (double)num / (double)M;
+            am[(size_t)k1 * 32 + n2] = make_float2((float)(std::cos(am_ang) / M), (float)(std::sin(am_ang) / M));
+        }
+    // columns of the pupil plane that fall inside a window (corner-placed grid: origins M-s and s)
+    std::vector<int> xc_of_x(M, -1), colx;
+    for (int q = 0; q < 2; ++q) {
+        const int g = q == 0 ? (M - s) % M : s % M;
+        for (int pp = 0; pp < N; ++pp) xc_of_x[(g + pp) % M] = 0;
+    }
+    for (int x = 0; x < M; ++x)
+        if (xc_of_x[x] == 0) { xc_of_x[x] = (int)colx.size(); colx.push_back(x); }
+    t.ncols = (int)colx.size();
+    // rebin tables (same for both axes; the y copy carries no extra scale)
+    std::vector<int> rb_start, rb_cnt;
+    std::vector<float> rb_w;
+    build_rebin(N, M, s, n_sub, rb_start, rb_cnt, rb_w, t.cmax, 1.0);
+    // valid mask
+    std::vector<int> vidx;
+    const double thr = p.illum_thresh > 0.f ? (double)p.illum_thresh : 0.5;
+    t.n_valid = build_valid(N, n_sub, p.pupil_amp, thr, h->valid, vidx);
+    if (t.n_valid == 0) return PWFS_EINVAL;
+
+    std::vector<float> amp(p.pupil_amp, p.pupil_amp + (size_t)N * N);
+    int rc;
+    if ((rc = upload(h, amp, &t.amp))) return rc;
+    if ((rc = upload(h, txt, &t.txt))) return rc;
+    if ((rc = upload(h, tyt, &t.tyt))) return rc;
+    if ((rc = upload(h, jx, &t.jx))) return rc;
+    if ((rc = upload(h, tw, &t.tw))) return rc;
+    if ((rc = upload(h, am, &t.am))) return rc;
+    if ((rc = upload(h, colx, &t.colx))) return rc;
+    if ((rc = upload(h, xc_of_x, &t.xc_of_x))) return rc;
+    if ((rc = upload(h, rb_start, &t.rb_start))) return rc;
+    if ((rc = upload(h, rb_cnt, &t.rb_cnt))) return rc;
+    if ((rc = upload(h, rb_w, &t.rb_w))) return rc;
+    if ((rc = upload(h, vidx, &t.vidx))) return rc;
+    return PWFS_OK;
+}
+
+// frames per chunk and k-split for a batch of B frames
+void schedule(const pwfs *h, int B, int *fpc, int *ksplit) {
+    const DevTables &t = h->tab;
+    const size_t T_frame = (size_t)t.KX * t.ncols * t.NP * sizeof(float2);
+    const int col_warps = (t.ncols + h->L.NB - 1) / h->L.NB;           // column-pass warps per frame
+    const int slots = h->num_sms * 12;                                  // resident warps we aim to fill
+    int F = h->user_fpc > 0 ? h->user_fpc : (8 * slots + col_warps - 1) / col_warps;
+    const size_t maxF = std::max<size_t>(1, h->scratch_budget / std::max<size_t>(T_frame, 1));
+    F = (int)std::min<size_t>((size_t)F, maxF);
+    F = std::max(1, std::min(F, std::max(B, 1)));
+    int ks = h->user_ksplit > 0 ? h->user_ksplit : 1;
+    if (h->user_ksplit <= 0) {
+        // too few warps for the machine: split the modulation loop, keeping >= 4 points per warp
+        while ((long long)F * col_warps * ks < 2LL * slots && t.K / (ks * 2) >= 4) ks *= 2;
+    }
+    ks = std::max(1, std::min(ks, t.K));
+    *fpc = F; *ksplit = ks;
+}
+
+int ensure_scratch(pwfs *h, int F, int ksplit) {
+    const DevTables &t = h->tab;
+    const size_t needT = (size_t)F * t.KX * t.ncols * t.NP;
+    const size_t needC = (size_t)F * ksplit * t.ncols * t.D;
+    if (needT > h->T_elems) {
+        if (h->T) cudaFree(h->T);
+        h->T = nullptr; h->T_elems = 0;
+        cudaError_t e = cudaMalloc((void **)&h->T, needT * sizeof(float2));
+        if (e != cudaSuccess) { h->last_cuda = (int)e; return e == cudaErrorMemoryAllocation ? PWFS_ENOMEM : PWFS_ECUDA; }
+        h->T_elems = needT;
+    }
+    if (needC > h->colbin_elems) {
+        if (h->colbin) cudaFree(h->colbin);
+        h->colbin = nullptr; h->colbin_elems = 0;
+        cudaError_t e = cudaMalloc((void **)&h->colbin, needC * sizeof(float));
+        if (e != cudaSuccess) { h->last_cuda = (int)e; return e == cudaErrorMemoryAllocation ? PWFS_ENOMEM : PWFS_ECUDA; }
+        h->colbin_elems = needC;
+    }
+    return PWFS_OK;
+}
+
+struct SpanGuard {
+    pwfs *h; cudaStream_t st; int cls; cudaEvent_t a = nullptr, b = nullptr;
+    SpanGuard(pwfs *h_, cudaStream_t st_, int cls_) : h(h_), st(st_), cls(cls_) {
+        h->launches[cls]++;
+        if (!h->timing) return;
+        auto get = [&]() {
+            cudaEvent_t e = nullptr;
+            if (!h->event_pool.empty()) { e = h->event_pool.back(); h->event_pool.pop_back(); }
+            else cudaEventCreate(&e);
+            return e;
+        };
+        a = get(); b = get();
+        cudaEventRecord(a, st);
+    }
+    ~SpanGuard() {
+        if (!a) return;
+        cudaEventRecord(b, st);
+        h->spans.push_back({a, b, cls});
+    }
+};
+
+}  // namespace
+
+extern "C" {
+
+const char *pwfs_strerror(int code) {
+    switch (code) {
+        case PWFS_OK: return "ok";
+        case PWFS_EINVAL: return "invalid argument";
+        case PWFS_ENOMEM: return "out of memory";
+        case PWFS_ECUDA: return "CUDA runtime error";
+        case PWFS_EUNSUPPORTED: return "grid size not supported by this build";
+        default: return "unknown pwfs status";
+    }
+}
+
+int pwfs_supported_grid(int32_t m_grid) {
+    Launcher l;
+    return find_launcher(m_grid, &l) ? 1 : 0;
+}
+
+int pwfs_create(const pwfs_params *p, pwfs_t **out) {
+    if (out) *out = nullptr;
+    if (!p || !out || !p->pupil_amp) return PWFS_EINVAL;
+    const int N = p->n_pupil, M = p->m_grid;
+    if (N < 2 || M < 2 * N || (M & 1)) return PWFS_EINVAL;
+    if (p->mod_points < 1 || !(p->mod_radius >= 0.f) || !std::isfinite(p->mod_radius) || !std::isfinite(p->mod_angle0))
+        return PWFS_EINVAL;
+    if (p->n_subap < 1 || p->n_subap > N) return PWFS_EINVAL;
+    if (p->slope_norm != 0 && p->slope_norm != 1) return PWFS_EINVAL;
+    if (p->illum_thresh > 1.f || !std::isfinite(p->illum_thresh)) return PWFS_EINVAL;
+    int s = p->mask_shift_px;
+    if (s <= 0) { if (M % 4) return PWFS_EINVAL; s = M / 4; }
+    if (2 * s < N || s > M / 2 - N / 2) return PWFS_EINVAL;
+    for (size_t i = 0; i < (size_t)N * N; ++i)
+        if (!(p->pupil_amp[i] >= 0.f) || !std::isfinite(p->pupil_amp[i])) return PWFS_EINVAL;
+    Launcher L;
+    if (!find_launcher(M, &L)) return PWFS_EUNSUPPORTED;
+
+    pwfs *h = new (std::nothrow) pwfs();
+    if (!h) return PWFS_ENOMEM;
+    h->prm = *p; h->s = s; h->L = L; h->device = p->device;
+    int rc = PWFS_OK;
+    cudaError_t e = cudaSetDevice(p->device);
+    if (e != cudaSuccess) { h->last_cuda = (int)e; rc = PWFS_ECUDA; }
+    if (!rc) {
+        cudaDeviceProp prop;
+        e = cudaGetDeviceProperties(&prop, p->device);
+        if (e != cudaSuccess) { h->last_cuda = (int)e; rc = PWFS_ECUDA; }
+        else {
+            h->num_sms = prop.multiProcessorCount;
+            if (prop.major < 10) rc = PWFS_EUNSUPPORTED;   // built for sm_100a only
+        }
+    }
+    if (!rc) {
+        e = cudaFuncSetAttribute(L.xfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem_x);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(L.yfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem_y);
+        if (e != cudaSuccess) { h->last_cuda = (int)e; rc = PWFS_ECUDA; }
+    }
+    if (!rc) {
+        const char *env = std::getenv("PWFS_SCRATCH_MB");
+        if (env && std::atol(env) > 0) h->scratch_budget = (size_t)std::atol(env) << 20;
+        rc = build_tables(h);
+    }
+    h->prm.pupil_amp = nullptr;   // the caller keeps ownership; we hold a device copy only
+    if (rc) { pwfs_destroy(h); return rc; }
+    *out = h;
+    return PWFS_OK;
+}
+
+void pwfs_destroy(pwfs_t *h) {
+    if (!h) return;
+    cudaSetDevice(h->device);
+    for (void *d : h->dev_allocs) cudaFree(d);
+    if (h->T) cudaFree(h->T);
+    if (h->colbin) cudaFree(h->colbin);
+    if (h->d_phase) cudaFree(h->d_phase);
+    if (h->d_frames) cudaFree(h->d_frames);
+    if (h->d_slopes) cudaFree(h->d_slopes);
+    if (h->hstream) cudaStreamDestroy(h->hstream);
+    for (auto &sp : h->spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
+    for (auto ev : h->event_pool) cudaEventDestroy(ev);
+    delete h;
+}
+
+int pwfs_info(const pwfs_t *h, int32_t *det_size, int32_t *n_valid) {
+    if (!h) return PWFS_EINVAL;
+    if (det_size) *det_size = h->tab.D;
+    if (n_valid) *n_valid = h->tab.n_valid;
+    return PWFS_OK;
+}
+
+int pwfs_valid_mask(const pwfs_t *h, uint8_t *host_mask) {
+    if (!h || !host_mask) return PWFS_EINVAL;
+    std::memcpy(host_mask, h->valid.data(), h->valid.size());
+    return PWFS_OK;
+}
+
+int pwfs_last_cuda_error(const pwfs_t *h) { return h ? h->last_cuda : 0; }
+
+int pwfs_set_schedule(pwfs_t *h, int32_t frames_per_chunk, int32_t k_split) {
+    if (!h || frames_per_chunk < 0 || k_split < 0 || k_split > h->tab.K) return PWFS_EINVAL;
+    h->user_fpc = frames_per_chunk;
+    h->user_ksplit = k_split;
+    return PWFS_OK;
+}
+
+int pwfs_geometry(const pwfs_t *h, int32_t B, int32_t *n_cols, int32_t *k_unique, int32_t *frames_per_chunk,
+                  int32_t *k_split) {
+    if (!h) return PWFS_EINVAL;
+    int F, ks;
+    schedule(h, B, &F, &ks);
+    if (n_cols) *n_cols = h->tab.ncols;
+    if (k_unique) *k_unique = h->tab.KX;
+    if (frames_per_chunk) *frames_per_chunk = F;
+    if (k_split) *k_split = ks;
+    return PWFS_OK;
+}
+
+int pwfs_set_timing(pwfs_t *h, int32_t enable) {
+    if (!h) return PWFS_EINVAL;
+    h->timing = enable ? 1 : 0;
+    return PWFS_OK;
+}
+
+int pwfs_get_timing(pwfs_t *h, float ms[PWFS_NUM_KERNEL_CLASSES], int64_t launches[PWFS_NUM_KERNEL_CLASSES]) {
+    if (!h) return PWFS_EINVAL;
+    for (auto &sp : h->spans) {
+        PWFS_CUDA(h, cudaEventSynchronize(sp.b));
+        float m = 0.f;
+        PWFS_CUDA(h, cudaEventElapsedTime(&m, sp.a, sp.b));
+        h->ms_acc[sp.cls] += m;
+        h->event_pool.push_back(sp.a);
+        h->event_pool.push_back(sp.b);
+    }
+    h->spans.clear();
+    for (int i = 0; i < PWFS_NUM_KERNEL_CLASSES; ++i) {
+        if (ms) ms[i] = h->ms_acc[i];
+        if (launches) launches[i] = h->launches[i];
+        h->ms_acc[i] = 0.f;
+        h->launches[i] = 0;
+    }
+    return PWFS_OK;
+}
+
+int pwfs_run(pwfs_t *h, const float *d_phase, int32_t B, float *d_frames, float *d_slopes, void *cuda_stream) {
+    if (!h || B < 0) return PWFS_EINVAL;
+    if (B == 0) return PWFS_OK;
+    if (!d_phase || !d_frames) return PWFS_EINVAL;
+    PWFS_CUDA(h, cudaSetDevice(h->device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const DevTables &t = h->tab;
+    int F, ks;
+    schedule(h, B, &F, &ks);
+    int rc = ensure_scratch(h, F, ks);
+    if (rc) return rc;
+    const Launcher &L = h->L;
+    const size_t NN = (size_t)t.N * t.N, DD = (size_t)t.D * t.D;
+    for (int f0 = 0; f0 < B; f0 += F) {
+        const int Fc = std::min(F, B - f0);
+        {   // K1: phasor + x-convolution (a1, a3, a4, a5 along x)
+            SpanGuard g(h, st, 0);
+            L.launch_x(dim3((t.N + L.RPC - 1) / L.RPC, t.KX, Fc), st, t, d_phase + (size_t)f0 * NN, h->T);
+        }
+        {   // K2: y-convolution + |E|^2 over k + y-rebin (a3, a4, a5 along y, a6, a7)
+            SpanGuard g(h, st, 1);
+            const int per_cta = L.NB * L.WPB_Y;
+            L.launch_y(dim3((t.ncols + per_cta - 1) / per_cta, ks, Fc), st, t, h->T, h->colbin, ks);
+        }
+        {   // K3a: x-rebin (a7)
+            SpanGuard g(h, st, 2);
+            const int threads = std::min(256, (t.D + 31) / 32 * 32);
+            xrebin_kernel<<<dim3(t.D, Fc), threads, 0, st>>>(t, h->colbin, d_frames + (size_t)f0 * DD, ks,
+                                                             1.0f / (float)t.K);
+        }
+        if (d_slopes) {   // K3b: slopes (a8)
+            SpanGuard g(h, st, 3);
+            slopes_kernel<<<Fc, 256, 0, st>>>(t, d_frames + (size_t)f0 * DD, d_slopes + (size_t)f0 * 2 * t.n_valid);
+        }
+        PWFS_CUDA(h, cudaGetLastError());
+    }
+    return PWFS_OK;
+}
+
+int pwfs_run_host(pwfs_t *h, const float *h_phase, int32_t B, float *h_frames, float *h_slopes) {
+    if (!h || B < 0) return PWFS_EINVAL;
+    if (B == 0) return PWFS_OK;
+    if (!h_phase || !h_frames) return PWFS_EINVAL;
+    PWFS_CUDA(h, cudaSetDevice(h->device));
+    const DevTables &t = h->tab;
+    const size_t NN = (size_t)t.N * t.N, DD = (size_t)t.D * t.D, SS = (size_t)2 * t.n_valid;
+    if (!h->hstream) PWFS_CUDA(h, cudaStreamCreateWithFlags(&h->hstream, cudaStreamNonBlocking));
+    if ((size_t)B > h->d_cap_frames) {
+        if (h->d_phase) cudaFree(h->d_phase);
+        if (h->d_frames) cudaFree(h->d_frames);
+        if (h->d_slopes) cudaFree(h->d_slopes);
+        h->d_phase = h->d_frames = h->d_slopes = nullptr; h->d_cap_frames = 0;
+        cudaError_t e = cudaMalloc((void **)&h->d_phase, (size_t)B * NN * sizeof(float));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_frames, (size_t)B * DD * sizeof(float));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_slopes, (size_t)B * SS * sizeof(float));
+        if (e != cudaSuccess) { h->last_cuda = (int)e; return e == cudaErrorMemoryAllocation ? PWFS_ENOMEM : PWFS_ECUDA; }
+        h->d_cap_frames = (size_t)B;
+    }
+    PWFS_CUDA(h, cudaMemcpyAsync(h->d_phase, h_phase, (size_t)B * NN * sizeof(float), cudaMemcpyHostToDevice, h->hstream));
+    int rc = pwfs_run(h, h->d_phase, B, h->d_frames, h_slopes ? h->d_slopes : nullptr, h->hstream);
+    if (rc) return rc;
+    PWFS_CUDA(h, cudaMemcpyAsync(h_frames, h->d_frames, (size_t)B * DD * sizeof(float), cudaMemcpyDeviceToHost, h->hstream));
+    if (h_slopes)
+        PWFS_CUDA(h, cudaMemcpyAsync(h_slopes, h->d_slopes, (size_t)B * SS * sizeof(float), cudaMemcpyDeviceToHost, h->hstream));
+    PWFS_CUDA(h, cudaStreamSynchronize(h->hstream));
+    return PWFS_OK;
+}
+
+}  // extern "C"

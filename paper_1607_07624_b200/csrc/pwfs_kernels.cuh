@@ -1,0 +1,328 @@
+// pwfs_kernels.cuh -- the sm_100a kernels of the pyramid-WFS hot path.
+//
+// Structure.  The 2-D operator IDFT2 . mask . DFT2 with the
+// separable pyramid mask m(u,v) = a(u) a(v) factors into two 1-D circular
+// convolutions, E = Cy (P Cx^T), C = IDFT diag(a) DFT.  So instead of four 1-D
+// passes with three round trips there are two fused passes with one:
+//
+//   xpass (K1): for every pupil ROW y (N of them, not M) and every distinct
+//               x-tilt j: phasor A exp(i(phi + tilt_x)) -> length-M DFT over x
+//               -> * a(u) -> inverse DFT -> keep only the window columns ->
+//               T[f][j][xc][y]  (transposed so the column pass reads coalesced).
+//   ypass (K2): one warp per needed COLUMN xc, looping over its modulation
+//               points k: load T[.., xc, :] * tilt_y,k(y) -> DFT over y -> * a(v)
+//               -> inverse DFT -> |E|^2 accumulated in registers over k ->
+//               area-weighted rebin along y -> colbin[f][ks][xc][jy].
+//   xrebin (K3a), slopes (K3b): finish the detector frame and the slopes.
+//
+// A length-M transform, M = 32*R1, is done by ONE WARP in two register stages
+// with one shared-memory exchange: lane n2 does a DFT of size R1 over
+// x[32 n1 + n2] (coalesced loads), the warp exchanges through padded shared
+// memory, lane k1 does a DFT of size 32 over n2.  The inverse runs the same
+// graph backwards, so forward+mask+inverse needs two exchanges and no
+// bit-reversal, and results come back in natural order in the lane that loaded
+// them.  To keep all 32 lanes busy in the size-32 stage when R1 < 32 a warp
+// works on NB transforms at once (NB*R1 ~ 32).
+#pragma once
+#include "pwfs_dft.cuh"
+
+namespace pwk {
+
+constexpr float kInv2PiHi = 0.15915493667125702f;   // fl32(1/(2 pi))
+constexpr float kInv2PiLo = 6.4206382e-09f;          // 1/(2 pi) - kInv2PiHi
+constexpr int kPitch = 33;  // float2 row pitch of the exchange buffer: conflict-free LDS.64/STS.64
+
+template <int R1_, int NB_, int WPB_X_, int WPB_Y_>
+struct PassCfg {
+    static constexpr int R1 = R1_;           // M / 32
+    static constexpr int NB = NB_;           // transforms a warp works on at once
+    static constexpr int M = 32 * R1_;
+    static constexpr int ITEMS = NB_ * R1_;  // size-32 DFTs per warp batch
+    static constexpr int ROUNDS = (ITEMS + 31) / 32;
+    static constexpr int WARP_BUF = ITEMS * kPitch + 1;   // float2 per warp (+1: staggers warps across banks)
+    static constexpr int TAB = R1_ * kPitch;              // float2 per table (twiddle, mask)
+    static constexpr int WPB_X = WPB_X_;     // warps per CTA, row pass
+    static constexpr int WPB_Y = WPB_Y_;     // warps per CTA, column pass
+    static constexpr int RPC = NB_ * WPB_X_; // rows per CTA, row pass
+    static constexpr size_t smem_x = (size_t)(WPB_X_ * WARP_BUF + 2 * TAB) * sizeof(float2);
+    static constexpr size_t smem_y = (size_t)(WPB_Y_ * WARP_BUF + 2 * TAB) * sizeof(float2);
+};
+
+// Device-side view of a sensor's tables (all pointers are device memory).
+struct DevTables {
+    int N, M, NP;             // pupil px, grid, padded y-pitch of T
+    int K, KX;                // modulation points, distinct x-tilts
+    int ncols;                // pupil-plane columns computed
+    int D, n_sub, cmax;       // detector size 2 n_sub, rebin support
+    int n_valid, slope_norm;
+    const float *amp;         // [N][N]
+    const float *txt;         // [KX][N]  x-tilt in turns, reduced to [-0.5, 0.5)
+    const float2 *tyt;        // [K][N]   exp(i tilt_y,k(y))
+    const int *jx;            // [K]      x-tilt index of modulation point k
+    const float2 *tw;         // [R1][32] exp(-2 pi i k1 n2 / M)
+    const float2 *am;         // [R1][32] a(k1 + R1 k2) / M
+    const int *colx;          // [ncols]  grid x of compact column xc
+    const int *xc_of_x;       // [M]      compact column of grid x (or -1)
+    const int *rb_start;      // [D]      first source px (grid coordinate) of detector bin
+    const int *rb_cnt;        // [D]
+    const float *rb_w;        // [D][cmax] area weights
+    const int *vidx;          // [n_valid] j*n_sub + i of valid subapertures, row-major
+};
+
+__device__ __forceinline__ void load_tables(float2 *s_tw, float2 *s_am, const DevTables &t, int R1) {
+    for (int i = threadIdx.x; i < R1 * 32; i += blockDim.x) {
+        int k1 = i >> 5, n2 = i & 31;
+        s_tw[k1 * kPitch + n2] = t.tw[i];
+        s_am[k1 * kPitch + n2] = t.am[i];
+    }
+}
+
+// Size-32 stage for the warp's current batch: for every (transform b, k1):
+// twiddle, DFT over n2, mask, inverse DFT, conjugate twiddle; in place in `buf`.
+template <class C>
+__device__ __forceinline__ void stage32(float2 *buf, const float2 *s_tw, const float2 *s_am, int lane) {
+#pragma unroll
+    for (int rd = 0; rd < C::ROUNDS; ++rd) {
+        int w = rd * 32 + lane;
+        if (w < C::ITEMS) {
+            int k1 = w % C::R1;
+            float2 *row = buf + w * kPitch;
+            const float2 *twr = s_tw + k1 * kPitch;
+            const float2 *amr = s_am + k1 * kPitch;
+            float2 u[32];
+#pragma unroll
+            for (int n2 = 0; n2 < 32; ++n2) u[n2] = cmul(row[n2], twr[n2]);
+            Dft<32, -1>::run(u);
+#pragma unroll
+            for (int k2 = 0; k2 < 32; ++k2) u[k2] = cmul(u[k2], amr[k2]);
+            Dft<32, +1>::run(u);
+#pragma unroll
+            for (int n2 = 0; n2 < 32; ++n2) row[n2] = cmulc(u[n2], twr[n2]);
+        }
+    }
+}
+
+// ------------------------------------------------------------------ K1 ------
+// grid (ceil(N/RPC), KX, F); block 32*WPB_X.  Warp wl of the CTA owns rows
+// y0 + wl*NB + b, b < NB.
+template <class C>
+__global__ void __launch_bounds__(32 * C::WPB_X)
+xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ T) {
+    extern __shared__ float2 smem[];
+    float2 *s_tw = smem;
+    float2 *s_am = smem + C::TAB;
+    float2 *s_buf = smem + 2 * C::TAB;
+    const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
+    const int N = t.N;
+    const int j = blockIdx.y, f = blockIdx.z;
+    const int y0 = blockIdx.x * C::RPC;
+    float2 *buf = s_buf + wl * C::WARP_BUF;
+
+    load_tables(s_tw, s_am, t, C::R1);
+
+    const float *ph_f = phase + (size_t)f * N * N;
+    const float *txt = t.txt + (size_t)j * N;
+    // step A: phasor, DFT of size R1 over n1 (x = 32 n1 + lane)
+#pragma unroll
+    for (int b = 0; b < C::NB; ++b) {
+        const int y = y0 + wl * C::NB + b;
+        float2 v[C::R1];
+#pragma unroll
+        for (int n1 = 0; n1 < C::R1; ++n1) {
+            const int x = 32 * n1 + lane;
+            float2 p = make_float2(0.f, 0.f);
+            if (y < N && x < N) {
+                const float a = __ldg(t.amp + (size_t)y * N + x);
+                const float ph = __ldg(ph_f + (size_t)y * N + x);
+                // phase in turns, reduced: ph/(2 pi) with a two-term constant
+                // 1/(2 pi) = kInv2PiHi + kInv2PiLo (float pair); q is exact, the FMAs keep the product's low bits
+                const float q = rintf(ph * kInv2PiHi);
+                float tr = fmaf(ph, kInv2PiHi, -q);
+                tr = fmaf(ph, kInv2PiLo, tr);
+                tr += __ldg(txt + x);
+                tr -= rintf(tr);
+                float sn, cs;
+                __sincosf(tr * 6.283185307179586f, &sn, &cs);
+                p = make_float2(a * cs, a * sn);
+            }
+            v[n1] = p;
+        }
+        Dft<C::R1, -1>::run(v);
+#pragma unroll
+        for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitch + lane] = v[k1];
+    }
+    __syncthreads();   // tables loaded + this warp's stores visible
+    stage32<C>(buf, s_tw, s_am, lane);
+    __syncwarp();
+    // step A': inverse DFT of size R1 over k1 -> x = 32 n1 + lane; stage for the transposed store
+#pragma unroll
+    for (int b = 0; b < C::NB; ++b) {
+        float2 v[C::R1];
+#pragma unroll
+        for (int k1 = 0; k1 < C::R1; ++k1) v[k1] = buf[(b * C::R1 + k1) * kPitch + lane];
+        Dft<C::R1, +1>::run(v);
+#pragma unroll
+        for (int n1 = 0; n1 < C::R1; ++n1) buf[(b * C::R1 + n1) * kPitch + lane] = v[n1];
+    }
+    __syncthreads();
+    // transposed write-out: T[f][j][xc][y], RPC consecutive y per column
+    float2 *Tj = T + ((size_t)f * t.KX + j) * (size_t)t.ncols * t.NP;
+    const int total = C::RPC * t.ncols;
+    for (int idx = threadIdx.x; idx < total; idx += 32 * C::WPB_X) {
+        const int r = idx % C::RPC, xc = idx / C::RPC;
+        const int y = y0 + r;
+        if (y < N) {
+            const int x = __ldg(t.colx + xc);
+            const int w2 = r / C::NB, b = r % C::NB;
+            Tj[(size_t)xc * t.NP + y] = s_buf[w2 * C::WARP_BUF + (b * C::R1 + (x >> 5)) * kPitch + (x & 31)];
+        }
+    }
+}
+
+// ------------------------------------------------------------------ K2 ------
+// grid (ceil(ncols / (NB*WPB_Y)), ksplit, F); block 32*WPB_Y.  Warps are
+// independent: warp -> NB adjacent columns, loops over its share of k.
+template <class C>
+__global__ void __launch_bounds__(32 * C::WPB_Y)
+ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colbin, int ksplit) {
+    extern __shared__ float2 smem[];
+    float2 *s_tw = smem;
+    float2 *s_am = smem + C::TAB;
+    float2 *s_buf = smem + 2 * C::TAB;
+    const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
+    const int N = t.N;
+    const int ks = blockIdx.y, f = blockIdx.z;
+    const int xc0 = (blockIdx.x * C::WPB_Y + wl) * C::NB;
+    float2 *buf = s_buf + wl * C::WARP_BUF;
+
+    load_tables(s_tw, s_am, t, C::R1);
+    __syncthreads();
+    if (xc0 >= t.ncols) return;
+
+    float acc[C::NB][C::R1];
+#pragma unroll
+    for (int b = 0; b < C::NB; ++b)
+#pragma unroll
+        for (int n1 = 0; n1 < C::R1; ++n1) acc[b][n1] = 0.f;
+
+    const int k_lo = (int)(((long long)ks * t.K) / ksplit), k_hi = (int)(((long long)(ks + 1) * t.K) / ksplit);
+    for (int k = k_lo; k < k_hi; ++k) {
+        const int j = __ldg(t.jx + k);
+        const float2 *Tj = T + ((size_t)f * t.KX + j) * (size_t)t.ncols * t.NP;
+        const float2 *ty = t.tyt + (size_t)k * N;
+#pragma unroll
+        for (int b = 0; b < C::NB; ++b) {
+            const int xc = xc0 + b;
+            float2 v[C::R1];
+#pragma unroll
+            for (int n1 = 0; n1 < C::R1; ++n1) {
+                const int y = 32 * n1 + lane;
+                float2 p = make_float2(0.f, 0.f);
+                if (y < N && xc < t.ncols) p = cmul(__ldg(Tj + (size_t)xc * t.NP + y), __ldg(ty + y));
+                v[n1] = p;
+            }
+            Dft<C::R1, -1>::run(v);
+#pragma unroll
+            for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitch + lane] = v[k1];
+        }
+        __syncwarp();
+        stage32<C>(buf, s_tw, s_am, lane);
+        __syncwarp();
+#pragma unroll
+        for (int b = 0; b < C::NB; ++b) {
+            float2 v[C::R1];
+#pragma unroll
+            for (int k1 = 0; k1 < C::R1; ++k1) v[k1] = buf[(b * C::R1 + k1) * kPitch + lane];
+            Dft<C::R1, +1>::run(v);
+#pragma unroll
+            for (int n1 = 0; n1 < C::R1; ++n1) acc[b][n1] = fmaf(v[n1].x, v[n1].x, fmaf(v[n1].y, v[n1].y, acc[b][n1]));
+        }
+        // next iteration's step-A stores touch only this lane's column, which only this lane read
+    }
+    // y-rebin: column of summed intensity -> 2 n_sub detector rows
+    float *colI = reinterpret_cast<float *>(buf);          // NB*M floats <= buffer
+    __syncwarp();
+#pragma unroll
+    for (int b = 0; b < C::NB; ++b)
+#pragma unroll
+        for (int n1 = 0; n1 < C::R1; ++n1) colI[b * C::M + 32 * n1 + lane] = acc[b][n1];
+    __syncwarp();
+    const int D = t.D, cmax = t.cmax;
+    for (int b = 0; b < C::NB; ++b) {
+        const int xc = xc0 + b;
+        if (xc >= t.ncols) break;
+        float *out = colbin + (((size_t)f * ksplit + ks) * t.ncols + xc) * D;
+        for (int jj = lane; jj < D; jj += 32) {
+            int y = __ldg(t.rb_start + jj);
+            const int cnt = __ldg(t.rb_cnt + jj);
+            const float *w = t.rb_w + (size_t)jj * cmax;
+            float s = 0.f;
+            for (int c = 0; c < cnt; ++c) {
+                s = fmaf(__ldg(w + c), colI[b * C::M + y], s);
+                if (++y == C::M) y = 0;
+            }
+            out[jj] = s;
+        }
+    }
+}
+
+// ------------------------------------------------------------------ K3a -----
+// frame[f][jy][jx] = (1/K) sum_ks sum_c wx[jx][c] colbin[f][ks][xc(jx,c)][jy]
+// grid (D (jx), F); block covers jy.
+__global__ void xrebin_kernel(DevTables t, const float *__restrict__ colbin, float *__restrict__ frames,
+                              int ksplit, float scale) {
+    const int jx = blockIdx.x, f = blockIdx.y;
+    const int D = t.D;
+    int x = __ldg(t.rb_start + jx);
+    const int cnt = __ldg(t.rb_cnt + jx);
+    const float *w = t.rb_w + (size_t)jx * t.cmax;
+    for (int jy = threadIdx.x; jy < D; jy += blockDim.x) {
+        float s = 0.f;
+        int xx = x;
+        for (int c = 0; c < cnt; ++c) {
+            const int xc = __ldg(t.xc_of_x + xx);
+            const float wc = __ldg(w + c);
+            for (int ks = 0; ks < ksplit; ++ks)
+                s = fmaf(wc, __ldg(colbin + (((size_t)f * ksplit + ks) * t.ncols + xc) * D + jy), s);
+            if (++xx == t.M) xx = 0;
+        }
+        frames[((size_t)f * D + jy) * D + jx] = s * scale;
+    }
+}
+
+// ------------------------------------------------------------------ K3b -----
+// One CTA per frame: nbar = mean over valid subaps of a+b+c+d, then slopes.
+__global__ void slopes_kernel(DevTables t, const float *__restrict__ frames, float *__restrict__ slopes) {
+    __shared__ float red[32];
+    __shared__ float s_nbar;
+    const int f = blockIdx.x, D = t.D, ns = t.n_sub, nv = t.n_valid;
+    const float *fr = frames + (size_t)f * D * D;
+    float part = 0.f;
+    for (int i = threadIdx.x; i < nv; i += blockDim.x) {
+        const int id = __ldg(t.vidx + i), jj = id / ns, ii = id % ns;
+        part += (fr[jj * D + ii] + fr[jj * D + ns + ii]) + (fr[(ns + jj) * D + ii] + fr[(ns + jj) * D + ns + ii]);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = part;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        float v = (threadIdx.x < (blockDim.x >> 5)) ? red[threadIdx.x] : 0.f;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (threadIdx.x == 0) s_nbar = v / (float)nv;
+    }
+    __syncthreads();
+    const float nbar = s_nbar;
+    float *out = slopes + (size_t)f * 2 * nv;
+    for (int i = threadIdx.x; i < nv; i += blockDim.x) {
+        const int id = __ldg(t.vidx + i), jj = id / ns, ii = id % ns;
+        const float a = fr[jj * D + ii], b = fr[jj * D + ns + ii];
+        const float c = fr[(ns + jj) * D + ii], d = fr[(ns + jj) * D + ns + ii];
+        const float den = t.slope_norm == 1 ? ((a + b) + (c + d)) : nbar;
+        out[i] = ((a + c) - (b + d)) / den;
+        out[nv + i] = ((a + b) - (c + d)) / den;
+    }
+}
+
+}  // namespace pwk

@@ -1,0 +1,229 @@
+"""Thin Python binding of libpwfs.so (include/pwfs.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI; PyTorch is
+used for device memory and streams.  There is no CPU fallback: if the library
+has not been built (python -m paper_1607_07624_b200.build) or no CUDA device is
+present, construction raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpwfs.so")
+
+PWFS_OK, PWFS_EINVAL, PWFS_ENOMEM, PWFS_ECUDA, PWFS_EUNSUPPORTED = 0, -1, -2, -3, -4
+NUM_KERNEL_CLASSES = 4
+KERNEL_CLASSES = ("xpass", "ypass", "xrebin", "slopes")
+
+EXPORTS = ("pwfs_create", "pwfs_info", "pwfs_valid_mask", "pwfs_run", "pwfs_run_host",
+           "pwfs_destroy", "pwfs_strerror", "pwfs_last_cuda_error", "pwfs_supported_grid",
+           "pwfs_set_schedule", "pwfs_set_timing", "pwfs_get_timing", "pwfs_geometry")
+
+
+class pwfs_params(C.Structure):
+    _fields_ = [("n_pupil", C.c_int32), ("m_grid", C.c_int32), ("pupil_amp", C.POINTER(C.c_float)),
+                ("mask_shift_px", C.c_int32), ("mod_radius", C.c_float), ("mod_points", C.c_int32),
+                ("mod_angle0", C.c_float), ("n_subap", C.c_int32), ("illum_thresh", C.c_float),
+                ("slope_norm", C.c_int32), ("device", C.c_int32)]
+
+
+class PwfsError(RuntimeError):
+    def __init__(self, code: int, what: str, detail: str = ""):
+        self.code = code
+        super().__init__(f"{what}: {detail or code}")
+
+
+_lib = None
+
+
+def load_library() -> C.CDLL:
+    """dlopen libpwfs.so and declare every prototype of include/pwfs.h."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise FileNotFoundError(
+            f"{LIB_PATH} is missing: build it with `python -m paper_1607_07624_b200.build` "
+            "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    vp, i32 = C.c_void_p, C.c_int32
+    lib.pwfs_create.argtypes = [C.POINTER(pwfs_params), C.POINTER(vp)]
+    lib.pwfs_create.restype = C.c_int
+    lib.pwfs_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i32)]
+    lib.pwfs_info.restype = C.c_int
+    lib.pwfs_valid_mask.argtypes = [vp, vp]
+    lib.pwfs_valid_mask.restype = C.c_int
+    lib.pwfs_run.argtypes = [vp, vp, i32, vp, vp, vp]
+    lib.pwfs_run.restype = C.c_int
+    lib.pwfs_run_host.argtypes = [vp, vp, i32, vp, vp]
+    lib.pwfs_run_host.restype = C.c_int
+    lib.pwfs_destroy.argtypes = [vp]
+    lib.pwfs_destroy.restype = None
+    lib.pwfs_strerror.argtypes = [C.c_int]
+    lib.pwfs_strerror.restype = C.c_char_p
+    lib.pwfs_last_cuda_error.argtypes = [vp]
+    lib.pwfs_last_cuda_error.restype = C.c_int
+    lib.pwfs_supported_grid.argtypes = [i32]
+    lib.pwfs_supported_grid.restype = C.c_int
+    lib.pwfs_set_schedule.argtypes = [vp, i32, i32]
+    lib.pwfs_set_schedule.restype = C.c_int
+    lib.pwfs_set_timing.argtypes = [vp, i32]
+    lib.pwfs_set_timing.restype = C.c_int
+    lib.pwfs_get_timing.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_int64)]
+    lib.pwfs_get_timing.restype = C.c_int
+    lib.pwfs_geometry.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.POINTER(i32)]
+    lib.pwfs_geometry.restype = C.c_int
+    _lib = lib
+    return lib
+
+
+def strerror(code: int) -> str:
+    return load_library().pwfs_strerror(code).decode()
+
+
+def supported_grid(m_grid: int) -> bool:
+    return bool(load_library().pwfs_supported_grid(m_grid))
+
+
+class PWFS:
+    """One pyramid sensor on one GPU: pwfs_create / pwfs_run / pwfs_destroy."""
+
+    def __init__(self, pupil_amp: np.ndarray, m_grid: int, mod_radius: float, mod_points: int,
+                 n_subap: int, mask_shift_px: int = 0, mod_angle0: float = 0.0,
+                 illum_thresh: float = 0.5, slope_norm: int = 0, device: int = 0):
+        self._h = None
+        self._lib = load_library()
+        amp = np.ascontiguousarray(pupil_amp, dtype=np.float32)
+        if amp.ndim != 2 or amp.shape[0] != amp.shape[1]:
+            raise ValueError("pupil_amp must be a square 2-D array")
+        prm = pwfs_params(amp.shape[0], m_grid, amp.ctypes.data_as(C.POINTER(C.c_float)),
+                          mask_shift_px, mod_radius, mod_points, mod_angle0, n_subap, illum_thresh,
+                          slope_norm, device)
+        h = C.c_void_p()
+        rc = self._lib.pwfs_create(C.byref(prm), C.byref(h))
+        if rc != PWFS_OK:
+            raise PwfsError(rc, "pwfs_create", strerror(rc))
+        self._h = h
+        self.device = device
+        self.n_pupil = amp.shape[0]
+        self.m_grid = m_grid
+        self.mod_points = mod_points
+        det, nv = C.c_int32(), C.c_int32()
+        self._check(self._lib.pwfs_info(self._h, C.byref(det), C.byref(nv)), "pwfs_info")
+        self.det_size, self.n_valid = det.value, nv.value
+
+    # -- plumbing ---------------------------------------------------------
+    def _check(self, rc: int, what: str):
+        if rc != PWFS_OK:
+            detail = strerror(rc)
+            if rc == PWFS_ECUDA and self._h:
+                detail += f" (cudaError {self._lib.pwfs_last_cuda_error(self._h)})"
+            raise PwfsError(rc, what, detail)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.pwfs_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    # -- queries ----------------------------------------------------------
+    def valid_mask(self) -> np.ndarray:
+        ns = self.det_size // 2
+        out = np.empty((ns, ns), dtype=np.uint8)
+        self._check(self._lib.pwfs_valid_mask(self._h, out.ctypes.data_as(C.c_void_p)), "pwfs_valid_mask")
+        return out
+
+    def geometry(self, batch: int) -> dict:
+        a, b, c, d = C.c_int32(), C.c_int32(), C.c_int32(), C.c_int32()
+        self._check(self._lib.pwfs_geometry(self._h, batch, C.byref(a), C.byref(b), C.byref(c), C.byref(d)),
+                    "pwfs_geometry")
+        return dict(n_cols=a.value, k_unique=b.value, frames_per_chunk=c.value, k_split=d.value)
+
+    def set_schedule(self, frames_per_chunk: int = 0, k_split: int = 0):
+        self._check(self._lib.pwfs_set_schedule(self._h, frames_per_chunk, k_split), "pwfs_set_schedule")
+
+    def set_timing(self, enable: bool):
+        self._check(self._lib.pwfs_set_timing(self._h, int(enable)), "pwfs_set_timing")
+
+    def get_timing(self) -> Tuple[dict, dict]:
+        ms = (C.c_float * NUM_KERNEL_CLASSES)()
+        n = (C.c_int64 * NUM_KERNEL_CLASSES)()
+        self._check(self._lib.pwfs_get_timing(self._h, ms, n), "pwfs_get_timing")
+        return ({k: float(ms[i]) for i, k in enumerate(KERNEL_CLASSES)},
+                {k: int(n[i]) for i, k in enumerate(KERNEL_CLASSES)})
+
+    # -- the hot path -----------------------------------------------------
+    def run(self, phase, frames=None, slopes=None, want_slopes: bool = True, stream=None):
+        """phase: CUDA float32 tensor [B,N,N] (or [N,N]).  Returns (frames, slopes)
+        CUDA tensors [B,2n_sub,2n_sub], [B,2 n_valid]; asynchronous on `stream`
+        (default: torch's current stream)."""
+        import torch
+        if not (isinstance(phase, torch.Tensor) and phase.is_cuda and phase.dtype == torch.float32):
+            raise TypeError("phase must be a CUDA float32 tensor")
+        if phase.device.index != self.device:
+            raise ValueError("phase lives on another device than the sensor")
+        if phase.dim() == 2:
+            phase = phase.unsqueeze(0)
+        phase = phase.contiguous()
+        B, N = phase.shape[0], self.n_pupil
+        if tuple(phase.shape[1:]) != (N, N):
+            raise ValueError(f"phase must be [B,{N},{N}]")
+        D = self.det_size
+        if frames is None:
+            frames = torch.empty((B, D, D), dtype=torch.float32, device=phase.device)
+        if slopes is None and want_slopes:
+            slopes = torch.empty((B, 2 * self.n_valid), dtype=torch.float32, device=phase.device)
+        st = stream if stream is not None else torch.cuda.current_stream(phase.device)
+        rc = self._lib.pwfs_run(self._h, C.c_void_p(phase.data_ptr()), B, C.c_void_p(frames.data_ptr()),
+                                C.c_void_p(slopes.data_ptr()) if slopes is not None else None,
+                                C.c_void_p(st.cuda_stream))
+        self._check(rc, "pwfs_run")
+        return frames, slopes
+
+    def run_host(self, phase, frames=None, slopes=None, want_slopes: bool = True):
+        """Same with HOST buffers (numpy arrays or CPU torch tensors, float32,
+        ideally pinned): host->device, run, device->host inside the call."""
+        def ptr_shape(a):
+            if isinstance(a, np.ndarray):
+                assert a.dtype == np.float32 and a.flags.c_contiguous
+                return a.ctypes.data, a.shape
+            assert a.dtype.is_floating_point and a.element_size() == 4 and a.is_contiguous() and not a.is_cuda
+            return a.data_ptr(), tuple(a.shape)
+        p, shp = ptr_shape(phase)
+        B = 1 if len(shp) == 2 else shp[0]
+        D = self.det_size
+        if frames is None:
+            frames = np.empty((B, D, D), dtype=np.float32)
+        if slopes is None and want_slopes:
+            slopes = np.empty((B, 2 * self.n_valid), dtype=np.float32)
+        fp, _ = ptr_shape(frames)
+        sp = ptr_shape(slopes)[0] if slopes is not None else None
+        rc = self._lib.pwfs_run_host(self._h, C.c_void_p(p), B, C.c_void_p(fp),
+                                     C.c_void_p(sp) if sp is not None else None)
+        self._check(rc, "pwfs_run_host")
+        return frames, slopes
+
+
+def from_config(cfg, device: int = 0, **overrides) -> PWFS:
+    """Build the sensor of a workloads.WfsConfig."""
+    from . import workloads
+    kw = dict(pupil_amp=workloads.make_pupil(cfg), m_grid=cfg.m_grid, mod_radius=cfg.mod_radius,
+              mod_points=cfg.mod_points, n_subap=cfg.n_subap, device=device)
+    kw.update(overrides)
+    return PWFS(**kw)

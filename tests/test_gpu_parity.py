@@ -1,0 +1,212 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the
+same seeded float32 inputs, element by element.
+
+Bar (BASELINE.json north_star, reading A14): per frame
+    max |dI| / max I <= 1e-4   on the detector frame,
+    |d slope|        <= 1e-4   per element (absolute),
+valid masks bit-exact.  Small cases run every frame through the oracle; at the
+five full BASELINE.json sizes a sample of frames is compared (the oracle needs
+seconds per frame there) in the launch configuration bench.py times.
+"""
+import numpy as np
+import pytest
+
+from paper_1607_07624_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL_FRAME = 1e-4
+TOL_SLOPE = 1e-4
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch
+
+
+def _compare(frames_gpu, slopes_gpu, frames_ref, slopes_ref):
+    frames_gpu = np.asarray(frames_gpu, dtype=np.float64)
+    slopes_gpu = np.asarray(slopes_gpu, dtype=np.float64)
+    assert frames_gpu.shape == frames_ref.shape and slopes_gpu.shape == slopes_ref.shape
+    assert np.isfinite(frames_gpu).all() and np.isfinite(slopes_gpu).all()
+    worst_f = worst_s = 0.0
+    for b in range(frames_ref.shape[0]):
+        ef = np.abs(frames_gpu[b] - frames_ref[b]).max() / frames_ref[b].max()
+        es = np.abs(slopes_gpu[b] - slopes_ref[b]).max()
+        worst_f, worst_s = max(worst_f, ef), max(worst_s, es)
+    assert worst_f <= TOL_FRAME, f"frame error {worst_f:.3e} > {TOL_FRAME}"
+    assert worst_s <= TOL_SLOPE, f"slope error {worst_s:.3e} > {TOL_SLOPE}"
+    return worst_f, worst_s
+
+
+def _run_both(torch, A, M, r, K, ns, phase, **kw):
+    from oracle import pwfs_oracle as orc
+    from paper_1607_07624_b200.pwfs import PWFS
+    sensor = PWFS(A, M, r, K, ns, **kw)
+    try:
+        v_ref, nv_ref = orc.valid_mask(A, ns, kw.get("illum_thresh", 0.5))
+        assert sensor.n_valid == nv_ref
+        assert np.array_equal(sensor.valid_mask(), v_ref)              # bit-exact mask
+        fr, sl = sensor.run(torch.from_numpy(phase).cuda())
+        torch.cuda.synchronize()
+        fr_ref, sl_ref = orc.pwfs_run(A, M, r, K, ns, phase, s=kw.get("mask_shift_px", 0),
+                                      theta0=kw.get("mod_angle0", 0.0),
+                                      thresh=kw.get("illum_thresh", 0.5),
+                                      norm_mode=kw.get("slope_norm", 0))
+        return _compare(fr.cpu().numpy(), sl.cpu().numpy(), fr_ref, sl_ref)
+    finally:
+        sensor.close()
+
+
+# ------------------------------------------------------------------ configs --
+def test_cfg1_every_frame(torch_cuda):
+    cfg = wl.CONFIGS["cfg1_tiny"]
+    A = wl.make_pupil(cfg)
+    phase = wl.phase_batch(cfg)                                         # all 10 steps
+    _run_both(torch_cuda, A, cfg.m_grid, cfg.mod_radius, cfg.mod_points, cfg.n_subap, phase)
+
+
+@pytest.mark.parametrize("name,frames", [("cfg2_flao", 6), ("cfg3_npot", 3), ("cfg4_elt", 2), ("cfg5_multi", 12)])
+def test_full_size_configs_sampled_frames(torch_cuda, name, frames):
+    """Full BASELINE.json sizes.  The GPU runs a batch large enough to use the
+    same chunked launch configuration as bench.py; the oracle checks the first
+    `frames` of them (cfg5: one step = all 12 sensor instances)."""
+    from oracle import pwfs_oracle as orc
+    from paper_1607_07624_b200.pwfs import from_config
+    torch = torch_cuda
+    cfg = wl.CONFIGS[name]
+    A = wl.make_pupil(cfg)
+    steps = max(1, frames // cfg.instances)
+    phase = wl.phase_batch(cfg, steps=steps)[:frames]
+    reps = 24 if name != "cfg4_elt" else 20
+    big = np.concatenate([phase] * (reps // frames + 1))[:max(reps, frames)]
+    sensor = from_config(cfg)
+    try:
+        fr, sl = sensor.run(torch.from_numpy(big).cuda())
+        torch.cuda.synchronize()
+        fr, sl = fr.cpu().numpy(), sl.cpu().numpy()
+        fr_ref, sl_ref = orc.pwfs_run(A, cfg.m_grid, cfg.mod_radius, cfg.mod_points, cfg.n_subap, phase)
+        _compare(fr[:frames], sl[:frames], fr_ref, sl_ref)
+        # the batch repeats the sample: every repeat must reproduce it bit for bit
+        for i in range(frames, big.shape[0]):
+            assert np.array_equal(fr[i], fr[i % frames]) and np.array_equal(sl[i], sl[i % frames])
+    finally:
+        sensor.close()
+
+
+# -------------------------------------------------------------- edge cases ---
+@pytest.mark.parametrize("N,M,ns,K,r", [
+    (64, 128, 16, 12, 3.0),      # cfg1 geometry
+    (60, 128, 23, 5, 1.5),       # non-integer binning, K % 4 != 0, margins (M > 2N)
+    (50, 128, 7, 1, 0.0),        # unmodulated, ragged N (not a multiple of 16 or 32)
+    (128, 256, 32, 8, 2.0),      # M = 256
+    (250, 512, 50, 6, 2.5),      # M = 512, ragged N
+    (300, 640, 30, 4, 1.0),      # M = 640
+    (37, 320, 37, 3, 0.7),       # tiny pupil in a large grid, b = 1
+])
+def test_geometries(torch_cuda, N, M, ns, K, r):
+    rng = np.random.default_rng(N * 7 + M)
+    c = (np.arange(N) - (N - 1) / 2.0)
+    X, Y = np.meshgrid(c, c)
+    A = (np.hypot(X, Y) <= N / 2.0).astype(np.float32)
+    phase = (rng.standard_normal((3, N, N)) * 3.0).astype(np.float32)
+    phase[1] = wl.tilt_phase(N, 0.3, -0.2)
+    _run_both(torch_cuda, A, M, r, K, ns, phase)
+
+
+def test_options_shift_angle_threshold_norm(torch_cuda):
+    N, M, ns = 48, 128, 12
+    rng = np.random.default_rng(5)
+    A = (rng.random((N, N)) > 0.15).astype(np.float32) * (0.5 + rng.random((N, N))).astype(np.float32)
+    phase = (rng.standard_normal((2, N, N)) * 2.0).astype(np.float32)
+    _run_both(torch_cuda, A, M, 2.0, 7, ns, phase, mask_shift_px=30, mod_angle0=0.4,
+              illum_thresh=0.3, slope_norm=1)
+    _run_both(torch_cuda, A, M, 2.0, 7, ns, phase, mask_shift_px=24, mod_angle0=-1.1)
+
+
+def test_large_phase_values_are_range_reduced(torch_cuda):
+    cfg = wl.CONFIGS["cfg1_tiny"]
+    A = wl.make_pupil(cfg)
+    phase = wl.phase_batch(cfg, steps=2) * 8.0                          # ~ +-500 rad
+    assert np.abs(phase).max() > 200
+    _run_both(torch_cuda, A, cfg.m_grid, cfg.mod_radius, cfg.mod_points, cfg.n_subap,
+              phase.astype(np.float32))
+
+
+def test_empty_batch_and_single_frame(torch_cuda):
+    from paper_1607_07624_b200.pwfs import from_config
+    torch = torch_cuda
+    cfg = wl.CONFIGS["cfg1_tiny"]
+    sensor = from_config(cfg)
+    try:
+        fr, sl = sensor.run(torch.empty((0, cfg.n_pupil, cfg.n_pupil), dtype=torch.float32, device="cuda"))
+        assert fr.shape == (0, cfg.det_size, cfg.det_size) and sl.shape == (0, 2 * sensor.n_valid)
+        ph = torch.from_numpy(wl.phase_batch(cfg, steps=1)[0]).cuda()   # [N,N]
+        fr1, sl1 = sensor.run(ph)
+        assert fr1.shape == (1, cfg.det_size, cfg.det_size)
+        fr2, _ = sensor.run(ph, want_slopes=False)
+        assert torch.equal(fr1, fr2)
+    finally:
+        sensor.close()
+
+
+def test_schedule_knobs_do_not_change_results(torch_cuda):
+    from paper_1607_07624_b200.pwfs import from_config
+    torch = torch_cuda
+    cfg = wl.CONFIGS["cfg1_tiny"]
+    phase = torch.from_numpy(wl.phase_batch(cfg, steps=7)).cuda()
+    sensor = from_config(cfg)
+    try:
+        base_f, base_s = sensor.run(phase)
+        for fpc, ks in [(1, 1), (3, 2), (7, 4), (2, 12)]:
+            sensor.set_schedule(fpc, ks)
+            f, s = sensor.run(phase)
+            assert (f - base_f).abs().max() <= 2e-6 * base_f.abs().max()
+            assert (s - base_s).abs().max() <= 1e-5
+    finally:
+        sensor.close()
+
+
+def test_host_buffer_entry_point_matches_device_entry_point(torch_cuda):
+    from paper_1607_07624_b200.pwfs import from_config
+    torch = torch_cuda
+    cfg = wl.CONFIGS["cfg1_tiny"]
+    phase = wl.phase_batch(cfg, steps=4)
+    sensor = from_config(cfg)
+    try:
+        fd, sd = sensor.run(torch.from_numpy(phase).cuda())
+        pinned = torch.from_numpy(phase).pin_memory()
+        fh = torch.empty((4, cfg.det_size, cfg.det_size), dtype=torch.float32).pin_memory()
+        sh = torch.empty((4, 2 * sensor.n_valid), dtype=torch.float32).pin_memory()
+        sensor.run_host(pinned, fh, sh)
+        assert torch.equal(fd.cpu(), fh) and torch.equal(sd.cpu(), sh)
+        fn, sn = sensor.run_host(phase)                                # pageable numpy
+        assert np.array_equal(fn, fh.numpy()) and np.array_equal(sn, sh.numpy())
+    finally:
+        sensor.close()
+
+
+def test_bad_parameters_are_rejected(torch_cuda):
+    from paper_1607_07624_b200.pwfs import PWFS, PwfsError, PWFS_EINVAL, PWFS_EUNSUPPORTED
+    A = np.ones((32, 32), np.float32)
+    for kw, code in [
+        (dict(m_grid=96), PWFS_EUNSUPPORTED),          # 96/32 = 3 not built
+        (dict(m_grid=60), PWFS_EINVAL),                # M < 2N
+        (dict(mod_points=0), PWFS_EINVAL),
+        (dict(mod_radius=-1.0), PWFS_EINVAL),
+        (dict(n_subap=0), PWFS_EINVAL),
+        (dict(n_subap=33), PWFS_EINVAL),
+        (dict(mask_shift_px=10), PWFS_EINVAL),         # 2 s < N : windows overlap
+        (dict(mask_shift_px=60), PWFS_EINVAL),         # window leaves the grid
+        (dict(slope_norm=2), PWFS_EINVAL),
+    ]:
+        args = dict(pupil_amp=A, m_grid=128, mod_radius=1.0, mod_points=4, n_subap=8)
+        args.update(kw)
+        with pytest.raises(PwfsError) as ei:
+            PWFS(**args)
+        assert ei.value.code == code, kw
+    with pytest.raises(PwfsError):                      # no light: n_valid == 0
+        PWFS(np.zeros((32, 32), np.float32), 128, 1.0, 4, 8)
