@@ -1,0 +1,292 @@
+#!/usr/bin/env python
+"""bench.py -- pyramid-WFS frames/s and fraction of roofline on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--config cfg4_elt] [--no-cpu-baseline]
+
+One "step" = one pass of the whole hot path (phasor+tilt -> pad -> FFT2 -> mask
+-> IFFT2 -> sum_k |E|^2 -> rebin -> slopes) over the full batch of the named
+config (cfg4_elt: 100 frames x 48 modulation points), through the C ABI.
+Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for every field.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import statistics
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1607_07624_b200 import workloads as wl  # noqa: E402
+
+METRIC = "pyramid_wfs_frames_per_s"
+UNIT = "frames/s"
+# FP32 "alu" roofline: 148 SMs x 128 FP32 lanes x 2 flop/FMA x 1.965 GHz
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+L2_FLUSH_BYTES = 256 << 20
+
+
+def nominal_flops_per_modpoint(M: int) -> float:
+    """2 transforms x 5 M^2 log2(M^2) per modulation point."""
+    return 2.0 * 5.0 * M * M * math.log2(M * M)
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons during the timed region (NVML)."""
+
+    def __init__(self, index: int):
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _loop(self):
+        nv = self.nv
+        names = {}
+        for nm in dir(nv):
+            if nm.startswith("nvmlClocksThrottleReason") and isinstance(getattr(nv, nm), int):
+                names[getattr(nv, nm)] = nm.replace("nvmlClocksThrottleReason", "")
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, nm in names.items():
+                    if bit and (mask & bit) == bit and nm not in ("None", "All"):
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            self._stop.wait(0.05)
+
+    def start(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._loop, daemon=True)
+            self._thr.start()
+
+    def stop(self) -> dict:
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+        norm = {"GpuIdle": "gpu_idle", "ApplicationsClocksSetting": "applications_clocks_setting",
+                "SwPowerCap": "sw_power_cap", "HwSlowdown": "hw_slowdown", "SyncBoost": "sync_boost",
+                "SwThermalSlowdown": "sw_thermal_slowdown", "HwThermalSlowdown": "hw_thermal_slowdown",
+                "HwPowerBrakeSlowdown": "hw_power_brake_slowdown", "DisplayClockSetting": "display_clock_setting"}
+        return {"sm_mhz": statistics.median(self.samples) if self.samples else None,
+                "sm_max_mhz": self.max_mhz, "samples": len(self.samples),
+                "reasons": sorted(norm.get(r, r) for r in self.reasons if r != "GpuIdle")}
+
+
+def time_oracle(cfg, frames: int):
+    """The oracle as it stands on the host cores: seconds for `frames` frames."""
+    from oracle import pwfs_oracle as orc
+    A = wl.make_pupil(cfg)
+    steps = max(1, math.ceil(frames / cfg.instances))
+    phase = wl.phase_batch(cfg, steps=steps)[:frames]
+    orc.valid_mask(A, cfg.n_subap)                       # library load / build outside the clock
+    t0 = time.perf_counter()
+    orc.pwfs_run(A, cfg.m_grid, cfg.mod_radius, cfg.mod_points, cfg.n_subap, phase)
+    return time.perf_counter() - t0, orc.num_threads()
+
+
+def oracle_sample_frames(cfg) -> int:
+    """Frames the oracle gets through in roughly 10-30 s on ~8 cores."""
+    cost = cfg.mod_points * 2 * cfg.m_grid ** 2 * math.log2(cfg.m_grid)      # ~ relative cost/frame
+    ref = 48 * 2 * 1024 ** 2 * 10                                            # cfg4: ~3.5 s/frame on 8 cores
+    return max(1, min(cfg.batch, int(round(4 * ref / cost))))
+
+
+def run_reference(args, cfg):
+    """--impl reference: the CPU oracle (this tier's reference arm), rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    frames = 1 if cfg.m_grid >= 800 else oracle_sample_frames(cfg)
+    for _ in range(args.warmup):
+        time_oracle(cfg, 1)
+    tot, cores = 0.0, 0
+    for _ in range(args.steps):
+        dt, cores = time_oracle(cfg, frames)
+        tot += dt
+    value = frames * args.steps / tot
+    sample = f"{frames} frame(s) of {cfg.name} per step, all {cfg.mod_points} modulation points"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": cfg.name, "frames_per_step": frames},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, cfg):
+    import torch
+    import torch.distributed as dist
+    from paper_1607_07624_b200.pwfs import from_config
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+
+    # weak scaling: every rank runs the full batch of the config on its own seeded slice of time
+    steps_cfg = cfg.steps
+    phase_np = wl.phase_batch(cfg, steps=steps_cfg, first_step=rank * steps_cfg)
+    B = phase_np.shape[0]
+    sensor = from_config(cfg, device=local)
+    geo = sensor.geometry(B)
+    phase = torch.from_numpy(phase_np).to(dev)
+    D, nv = sensor.det_size, sensor.n_valid
+    frames = torch.empty((B, D, D), dtype=torch.float32, device=dev)
+    slopes = torch.empty((B, 2 * nv), dtype=torch.float32, device=dev)
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream(dev)
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize(dev)
+
+    def max_over_ranks(x: float) -> float:
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    # ---- device-resident timing (value) -------------------------------------
+    for _ in range(args.warmup):
+        sensor.run(phase, frames, slopes)
+    barrier()
+    sensor.get_timing()                                  # reset counters
+    sensor.set_timing(True)
+    sampler = ClockSampler(local)
+    ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    sampler.start()
+    barrier()
+    for i in range(args.steps):
+        flush.zero_()                                    # evict L2 between timed steps (not timed)
+        ev0[i].record(stream)
+        sensor.run(phase, frames, slopes)
+        ev1[i].record(stream)
+    barrier()
+    clocks = sampler.stop()
+    ms_total = sum(a.elapsed_time(b) for a, b in zip(ev0, ev1))
+    kernel_ms, launches = sensor.get_timing()
+    sensor.set_timing(False)
+    ms_total = max_over_ranks(ms_total)
+    ms_per_step = ms_total / args.steps
+    value = world * B * args.steps / (ms_total * 1e-3)
+
+    # ---- end to end through the host-buffer entry point (e2e) ----------------
+    h_phase = torch.from_numpy(phase_np).pin_memory()
+    h_frames = torch.empty((B, D, D), dtype=torch.float32).pin_memory()
+    h_slopes = torch.empty((B, 2 * nv), dtype=torch.float32).pin_memory()
+    for _ in range(max(1, args.warmup // 2)):
+        sensor.run_host(h_phase, h_frames, h_slopes)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        sensor.run_host(h_phase, h_frames, h_slopes)     # synchronous: returns when results are on the host
+    barrier()
+    e2e_s = max_over_ranks(time.perf_counter() - t0)
+    e2e_value = world * B * args.steps / e2e_s
+    same = bool(np.array_equal(h_frames.numpy(), frames.cpu().numpy()))
+
+    if rank == 0:
+        M, K = cfg.m_grid, cfg.mod_points
+        # dominant kernel = column pass; its share of the nominal work is the y-direction
+        # transforms, i.e. half of 2 x 5 M^2 log2(M^2) per modulation point
+        dom = max(kernel_ms, key=kernel_ms.get)
+        n_launch = max(1, launches[dom])
+        units_per_launch = B * K * args.steps / n_launch                 # modulation points per launch
+        share = {"xpass": 0.5, "ypass": 0.5}.get(dom, 0.0)
+        flops_per_launch = share * nominal_flops_per_modpoint(M) * units_per_launch
+        avg_launch_s = kernel_ms[dom] * 1e-3 / n_launch
+        achieved = flops_per_launch / avg_launch_s / 1e12 if avg_launch_s > 0 else 0.0
+        path_tflops = nominal_flops_per_modpoint(M) * B * K / (ms_per_step * 1e-3) / 1e12
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tpath):
+            with open(tpath) as fh:
+                traffic = json.load(fh).get(cfg.name, {}).get(dom)
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": cfg.name, "n_pupil": cfg.n_pupil, "m_grid": M, "mod_points": K,
+                       "mod_radius": cfg.mod_radius, "n_subap": cfg.n_subap, "frames_per_step": B,
+                       "frames_per_chunk": geo["frames_per_chunk"], "k_split": geo["k_split"],
+                       "k_unique_xtilts": geo["k_unique"], "columns_computed": geo["n_cols"],
+                       "l2": f"flushed between timed steps ({L2_FLUSH_BYTES >> 20} MiB memset, untimed)",
+                       "parallelism": f"frames sharded over {world} GPU(s), no collective"},
+            "modpoint_ffts_per_s": value * K,
+            "transforms_2d_per_s": 2 * value * K,
+            "roofline": {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": FP32_PEAK_TFLOPS,
+                         "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS, "traffic": traffic,
+                         "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (guide unit counts/clocks)",
+                         "launch_ms": avg_launch_s * 1e3, "launches": n_launch,
+                         "nominal_flops_per_launch": flops_per_launch,
+                         "path_achieved": path_tflops, "path_frac": path_tflops / FP32_PEAK_TFLOPS,
+                         "kernel_ms_per_step": {k: v / args.steps for k, v in kernel_ms.items()}},
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h_phase.numel() * 4),
+                    "d2h_bytes_per_step": int(h_frames.numel() * 4 + h_slopes.numel() * 4),
+                    "matches_device_path": same},
+            "gpu_launches": int(sum(launches.values())),
+            "clocks": clocks,
+        }
+        if not args.no_cpu_baseline:
+            nfr = oracle_sample_frames(cfg)
+            dt, cores = time_oracle(cfg, nfr)
+            line["cpu_baseline"] = {"value": nfr / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                    "sample": f"{nfr} frame(s) of {cfg.name}, all {K} modulation points, {dt:.1f} s"}
+        print(json.dumps(line), flush=True)
+    sensor.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--config", default="cfg4_elt", choices=wl.CONFIG_ORDER)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.steps < 1 or args.warmup < 0:
+        raise SystemExit("bench.py: need --steps >= 1 and --warmup >= 0")
+    cfg = wl.CONFIGS[args.config]
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_ours(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

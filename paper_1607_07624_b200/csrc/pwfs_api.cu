@@ -30,7 +30,13 @@ using Cfg15 = PassCfg<15, 2, 8, 4>;   // M = 480
 using Cfg16 = PassCfg<16, 2, 8, 4>;   // M = 512
 using Cfg20 = PassCfg<20, 1, 16, 4>;  // M = 640
 using Cfg25 = PassCfg<25, 1, 16, 4>;  // M = 800
-using Cfg32 = PassCfg<32, 1, 16, 4>;  // M = 1024
+#ifndef PWFS_C32_WX
+#define PWFS_C32_WX 8
+#define PWFS_C32_WY 4
+#define PWFS_C32_MX 2
+#define PWFS_C32_MY 2
+#endif
+using Cfg32 = PassCfg<32, 1, PWFS_C32_WX, PWFS_C32_WY, PWFS_C32_MX, PWFS_C32_MY>;  // M = 1024
 
 struct Launcher {
     int R1, NB, WPB_X, WPB_Y, RPC;
@@ -63,14 +69,30 @@ Launcher make_launcher() {
 bool find_launcher(int M, Launcher *out) {
     if (M % 32) return false;
     switch (M / 32) {
+#if !defined(PWFS_ONLY_R1) || PWFS_ONLY_R1 == 4
         case 4: *out = make_launcher<Cfg4>(); return true;
+#endif
+#if !defined(PWFS_ONLY_R1) || PWFS_ONLY_R1 == 8
         case 8: *out = make_launcher<Cfg8>(); return true;
+#endif
+#if !defined(PWFS_ONLY_R1) || PWFS_ONLY_R1 == 10
         case 10: *out = make_launcher<Cfg10>(); return true;
+#endif
+#if !defined(PWFS_ONLY_R1) || PWFS_ONLY_R1 == 15
         case 15: *out = make_launcher<Cfg15>(); return true;
+#endif
+#if !defined(PWFS_ONLY_R1) || PWFS_ONLY_R1 == 16
         case 16: *out = make_launcher<Cfg16>(); return true;
+#endif
+#if !defined(PWFS_ONLY_R1) || PWFS_ONLY_R1 == 20
         case 20: *out = make_launcher<Cfg20>(); return true;
+#endif
+#if !defined(PWFS_ONLY_R1) || PWFS_ONLY_R1 == 25
         case 25: *out = make_launcher<Cfg25>(); return true;
+#endif
+#if !defined(PWFS_ONLY_R1) || PWFS_ONLY_R1 == 32
         case 32: *out = make_launcher<Cfg32>(); return true;
+#endif
         default: return false;
     }
 }
@@ -199,7 +221,7 @@ int build_tables(pwfs *h) {
     const int N = p.n_pupil, M = p.m_grid, K = p.mod_points, n_sub = p.n_subap, s = h->s;
     const int R1 = h->L.R1;
     DevTables &t = h->tab;
-    t.N = N; t.M = M; t.NP = (N + 15) / 16 * 16; t.K = K;
+    t.N = N; t.M = M; t.NP = (N + 31) / 32 * 32; t.K = K;
     t.D = 2 * n_sub; t.n_sub = n_sub; t.slope_norm = p.slope_norm;
 
     // O0: modulation points; distinct x-tilts (the row pass depends on k only through dx_k)
@@ -224,12 +246,12 @@ int build_tables(pwfs *h) {
             turns -= std::nearbyint(turns);
             txt[(size_t)j * N + x] = (float)turns;
         }
-    std::vector<float2> tyt((size_t)K * N);
+    std::vector<float2> tyt((size_t)K * t.NP, make_float2(0.f, 0.f));   // zero in the padding y >= N
     for (int k = 0; k < K; ++k)
         for (int y = 0; y < N; ++y) {
             double turns = dy[k] * ((double)y - c) / (double)N;       // O1, y part
             turns -= std::nearbyint(turns);
-            tyt[(size_t)k * N + y] = make_float2((float)std::cos(kTwoPi * turns), (float)std::sin(kTwoPi * turns));
+            tyt[(size_t)k * t.NP + y] = make_float2((float)std::cos(kTwoPi * turns), (float)std::sin(kTwoPi * turns));
         }
     // twiddles between the two register stages, and the 1-D mask a(u)/M (O4; 1/M = O5's scale per axis)
     std::vector<float2> tw((size_t)R1 * 32), am((size_t)R1 * 32);
@@ -501,7 +523,7 @@ int pwfs_run(pwfs_t *h, const float *d_phase, int32_t B, float *d_frames, float 
         const int Fc = std::min(F, B - f0);
         {   // K1: phasor + x-convolution (a1, a3, a4, a5 along x)
             SpanGuard g(h, st, 0);
-            L.launch_x(dim3((t.N + L.RPC - 1) / L.RPC, t.KX, Fc), st, t, d_phase + (size_t)f0 * NN, h->T);
+            L.launch_x(dim3((t.NP + L.RPC - 1) / L.RPC, t.KX, Fc), st, t, d_phase + (size_t)f0 * NN, h->T);
         }
         {   // K2: y-convolution + |E|^2 over k + y-rebin (a3, a4, a5 along y, a6, a7)
             SpanGuard g(h, st, 1);

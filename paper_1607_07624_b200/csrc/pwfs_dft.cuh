@@ -1,12 +1,21 @@
-// pwfs_dft.cuh -- small complex-FP32 DFTs held entirely in registers.
+// pwfs_dft.cuh -- small complex-FP32 DFTs held entirely in registers, written
+// with Blackwell's packed FP32x2 instructions (FADD2 / FMUL2 / FFMA2).
 //
 // Dft<N, DIR>::run(x) replaces x[0..N) (natural order) by its unnormalised DFT
 // X[k] = sum_n x[n] exp(DIR 2 pi i n k / N), DIR = -1 forward / +1 inverse, for
-// any 2/3/5-smooth N.  Everything is resolved at compile time: the recursion
-// (decimation in time, radix 4 where possible, else 2, 3, 5), every array index
-// and every twiddle factor, so after inlining the arrays live in registers and
-// twiddles are FMA immediates.  Trivial twiddles (1, -1, +-i, (+-1+-i)/sqrt2)
-// cost no multiply.  These are the butterflies of steps a3/a5.
+// any 2/3/5-smooth N.  DftP<N, DIR, NZ> is the same transform when x[NZ..N) is
+// known to be zero at compile time (zero-padded input: those butterflies and
+// twiddles are never emitted, and x[NZ..N) is never read).
+//
+// Everything is resolved at compile time: the recursion (decimation in time,
+// radix 4 where possible, else 2, 3, 5), every array index and every twiddle, so
+// after inlining the arrays live in registers and twiddles are immediates.
+//
+// A complex number is a float2 = one 64-bit register pair, so on sm_100a
+//   complex add / sub / add of +-i*b          = 1 FADD2 (operand swap/negate modifiers)
+//   complex * compile-time or run-time twiddle = 1 FMUL2 + 1 FFMA2
+// i.e. half the issue slots of scalar code for the same FP32 pipe time.  These
+// are the butterflies of steps a3/a5.
 #pragma once
 #include <cuda_runtime.h>
 #include <utility>
@@ -20,7 +29,7 @@ __device__ __forceinline__ void sfor_impl(F &&f, std::integer_sequence<int, Is..
 }
 template <int N, typename F>
 __device__ __forceinline__ void sfor(F &&f) {
-    sfor_impl(f, std::make_integer_sequence<int, N>{});
+    if constexpr (N > 0) sfor_impl(f, std::make_integer_sequence<int, N>{});
 }
 
 // ------------------------------------------------- compile-time cos / sin ---
@@ -55,22 +64,36 @@ __host__ __device__ constexpr cs cossin2pi(long long num, long long den) {
         default: return {s, -c};
     }
 }
+__host__ __device__ constexpr int cdiv(int a, int b) { return (a + b - 1) / b; }
+__host__ __device__ constexpr int imin(int a, int b) { return a < b ? a : b; }
+__host__ __device__ constexpr int imax(int a, int b) { return a > b ? a : b; }
 }  // namespace ct
 
 // ----------------------------------------------------- complex primitives ---
-__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
-__device__ __forceinline__ float2 cmul(float2 a, float2 w) {
-    return make_float2(fmaf(-a.y, w.y, a.x * w.x), fmaf(a.y, w.x, a.x * w.y));
-}
-__device__ __forceinline__ float2 cmulc(float2 a, float2 w) {  // a * conj(w)
-    return make_float2(fmaf(a.y, w.y, a.x * w.x), fmaf(a.y, w.x, -a.x * w.y));
-}
-// multiply by DIR*i
+__device__ __forceinline__ float2 bc(float v) { return make_float2(v, v); }
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
+// a + DIR*i*b  and  a - DIR*i*b   (one FADD2 each: swapped halves, one negated)
 template <int DIR>
-__device__ __forceinline__ float2 mul_i(float2 a) {
-    if constexpr (DIR > 0) return make_float2(-a.y, a.x);
-    else return make_float2(a.y, -a.x);
+__device__ __forceinline__ float2 cadd_i(float2 a, float2 b) {
+    if constexpr (DIR > 0) return __fadd2_rn(a, make_float2(-b.y, b.x));
+    else return __fadd2_rn(a, make_float2(b.y, -b.x));
+}
+template <int DIR>
+__device__ __forceinline__ float2 csub_i(float2 a, float2 b) { return cadd_i<-DIR>(a, b); }
+// a * w, run-time w:  t = a.y*(w.y, w.x);  r = a.x*w + (-t.x, t.y)      (FMUL2 + FFMA2)
+__device__ __forceinline__ float2 cmul(float2 a, float2 w) {
+    const float2 t = __fmul2_rn(bc(a.y), make_float2(w.y, w.x));
+    return __ffma2_rn(bc(a.x), w, make_float2(-t.x, t.y));
+}
+// a * conj(w) = w.x*a + w.y*(a.y, -a.x):  t = w.y*(a.y, a.x);  r = w.x*a + (t.x, -t.y)
+__device__ __forceinline__ float2 cmulc(float2 a, float2 w) {
+    const float2 t = __fmul2_rn(bc(w.y), make_float2(a.y, a.x));
+    return __ffma2_rn(bc(w.x), a, make_float2(t.x, -t.y));
+}
+// a * (c + i s) with compile-time c, s:  c*a + s*(-a.y, a.x)             (FMUL2 + FFMA2, immediates)
+__device__ __forceinline__ float2 cmul_const(float2 a, float c, float s) {
+    return __ffma2_rn(bc(c), a, __fmul2_rn(bc(s), make_float2(-a.y, a.x)));
 }
 
 // a * exp(DIR 2 pi i NUM/DEN) with the constant folded at compile time.
@@ -88,111 +111,159 @@ __device__ __forceinline__ float2 mul_w(float2 a) {
         return make_float2(-a.y, a.x);
     } else if constexpr (4 * num == 3 * DEN) {        // -i
         return make_float2(a.y, -a.x);
-    } else if constexpr ((8 * num) % DEN == 0) {      // (+-1 +- i)/sqrt2
+    } else if constexpr ((8 * num) % DEN == 0) {      // (+-1 +- i)/sqrt2: one FADD2 + one FMUL2
         constexpr float h = 0.70710678118654752440f;
-        if constexpr (c > 0 && s > 0) return make_float2((a.x - a.y) * h, (a.x + a.y) * h);
-        else if constexpr (c < 0 && s > 0) return make_float2((-a.x - a.y) * h, (a.x - a.y) * h);
-        else if constexpr (c < 0 && s < 0) return make_float2((a.y - a.x) * h, (-a.x - a.y) * h);
-        else return make_float2((a.x + a.y) * h, (a.y - a.x) * h);
+        // (1+i)a = a + i a ; (-1+i)a = -(a - i a) ; (-1-i)a = -(a + i a) ; (1-i)a = a - i a
+        if constexpr (c > 0 && s > 0) return __fmul2_rn(__fadd2_rn(a, make_float2(-a.y, a.x)), bc(h));
+        else if constexpr (c < 0 && s > 0) return __fmul2_rn(__fadd2_rn(a, make_float2(a.y, -a.x)), bc(-h));
+        else if constexpr (c < 0 && s < 0) return __fmul2_rn(__fadd2_rn(a, make_float2(-a.y, a.x)), bc(-h));
+        else return __fmul2_rn(__fadd2_rn(a, make_float2(a.y, -a.x)), bc(h));
     } else {
-        return make_float2(fmaf(-s, a.y, c * a.x), fmaf(s, a.x, c * a.y));
+        return cmul_const(a, c, s);
     }
 }
 
-// ------------------------------------------------------------- butterflies --
-template <int N, int DIR>
-struct Dft;
+// ------------------------------------------------- prime-size butterflies ---
+// Bfly<P, DIR, PZ>: DFT of size P whose inputs x[PZ..P) are zero (never read).
+template <int P, int DIR, int PZ>
+struct Bfly;
 
-template <int DIR>
-struct Dft<1, DIR> {
-    __device__ __forceinline__ static void run(float2 (&)[1]) {}
-};
-
-template <int DIR>
-struct Dft<2, DIR> {
+template <int DIR, int PZ>
+struct Bfly<2, DIR, PZ> {
     __device__ __forceinline__ static void run(float2 (&x)[2]) {
-        float2 a = x[0], b = x[1];
-        x[0] = cadd(a, b);
-        x[1] = csub(a, b);
+        if constexpr (PZ >= 2) {
+            const float2 a = x[0], b = x[1];
+            x[0] = cadd(a, b);
+            x[1] = csub(a, b);
+        } else {
+            x[1] = x[0];
+        }
     }
 };
 
-template <int DIR>
-struct Dft<3, DIR> {
+template <int DIR, int PZ>
+struct Bfly<3, DIR, PZ> {
     __device__ __forceinline__ static void run(float2 (&x)[3]) {
         constexpr float s60 = 0.86602540378443864676f * (float)DIR;
-        float2 a = x[0], b = x[1], c = x[2];
-        float2 t = cadd(b, c), u = csub(b, c);
-        x[0] = cadd(a, t);
-        float2 m = make_float2(fmaf(-0.5f, t.x, a.x), fmaf(-0.5f, t.y, a.y));
-        // X1 = m + i*DIR*s*u,  X2 = m - i*DIR*s*u
-        x[1] = make_float2(fmaf(-s60, u.y, m.x), fmaf(s60, u.x, m.y));
-        x[2] = make_float2(fmaf(s60, u.y, m.x), fmaf(-s60, u.x, m.y));
+        if constexpr (PZ == 1) {
+            x[1] = x[0]; x[2] = x[0];
+        } else {
+            const float2 a = x[0], b = x[1];
+            float2 t = b, u = b;
+            if constexpr (PZ >= 3) { t = cadd(b, x[2]); u = csub(b, x[2]); }
+            x[0] = cadd(a, t);
+            const float2 m = __ffma2_rn(bc(-0.5f), t, a);
+            const float2 iu = make_float2(-u.y, u.x);
+            x[1] = __ffma2_rn(bc(s60), iu, m);      // m + i DIR s u
+            x[2] = __ffma2_rn(bc(-s60), iu, m);     // m - i DIR s u
+        }
     }
 };
 
-template <int DIR>
-struct Dft<4, DIR> {
+template <int DIR, int PZ>
+struct Bfly<4, DIR, PZ> {
     __device__ __forceinline__ static void run(float2 (&x)[4]) {
-        float2 t0 = cadd(x[0], x[2]), t1 = csub(x[0], x[2]);
-        float2 t2 = cadd(x[1], x[3]), t3 = mul_i<DIR>(csub(x[1], x[3]));
-        x[0] = cadd(t0, t2);
-        x[1] = cadd(t1, t3);
-        x[2] = csub(t0, t2);
-        x[3] = csub(t1, t3);
+        if constexpr (PZ == 1) {
+            x[1] = x[0]; x[2] = x[0]; x[3] = x[0];
+        } else if constexpr (PZ == 2) {             // X_j = a + w^j b, w = DIR i
+            const float2 a = x[0], b = x[1];
+            x[0] = cadd(a, b);
+            x[1] = cadd_i<DIR>(a, b);
+            x[2] = csub(a, b);
+            x[3] = csub_i<DIR>(a, b);
+        } else {
+            const float2 t0 = cadd(x[0], x[2]), t1 = csub(x[0], x[2]);
+            float2 t2 = x[1], t3 = x[1];
+            if constexpr (PZ >= 4) { t2 = cadd(x[1], x[3]); t3 = csub(x[1], x[3]); }
+            x[0] = cadd(t0, t2);
+            x[1] = cadd_i<DIR>(t1, t3);
+            x[2] = csub(t0, t2);
+            x[3] = csub_i<DIR>(t1, t3);
+        }
     }
 };
 
-template <int DIR>
-struct Dft<5, DIR> {
+template <int DIR, int PZ>
+struct Bfly<5, DIR, PZ> {
     __device__ __forceinline__ static void run(float2 (&x)[5]) {
         constexpr float c1 = 0.30901699437494742410f;    // cos 72
         constexpr float c2 = -0.80901699437494742410f;   // cos 144
         constexpr float s1 = 0.95105651629515357212f * (float)DIR;   // sin 72
         constexpr float s2 = 0.58778525229247312917f * (float)DIR;   // sin 144
-        float2 a = x[0];
-        float2 t1 = cadd(x[1], x[4]), t2 = cadd(x[2], x[3]);
-        float2 t3 = csub(x[1], x[4]), t4 = csub(x[2], x[3]);
-        x[0] = cadd(a, cadd(t1, t2));
-        float2 m1 = make_float2(fmaf(c2, t2.x, fmaf(c1, t1.x, a.x)), fmaf(c2, t2.y, fmaf(c1, t1.y, a.y)));
-        float2 m2 = make_float2(fmaf(c1, t2.x, fmaf(c2, t1.x, a.x)), fmaf(c1, t2.y, fmaf(c2, t1.y, a.y)));
-        float2 n1 = make_float2(fmaf(s2, t4.x, s1 * t3.x), fmaf(s2, t4.y, s1 * t3.y));
-        float2 n2 = make_float2(fmaf(-s1, t4.x, s2 * t3.x), fmaf(-s1, t4.y, s2 * t3.y));
-        // X1 = m1 + i n1, X4 = m1 - i n1, X2 = m2 + i n2, X3 = m2 - i n2  (DIR folded in s1, s2)
-        x[1] = make_float2(m1.x - n1.y, m1.y + n1.x);
-        x[4] = make_float2(m1.x + n1.y, m1.y - n1.x);
-        x[2] = make_float2(m2.x - n2.y, m2.y + n2.x);
-        x[3] = make_float2(m2.x + n2.y, m2.y - n2.x);
+        if constexpr (PZ == 1) {
+            x[1] = x[0]; x[2] = x[0]; x[3] = x[0]; x[4] = x[0];
+        } else {
+            const float2 a = x[0];
+            float2 t1 = x[1], t3 = x[1];
+            if constexpr (PZ >= 5) { t1 = cadd(x[1], x[4]); t3 = csub(x[1], x[4]); }
+            float2 m1 = __ffma2_rn(bc(c1), t1, a), m2 = __ffma2_rn(bc(c2), t1, a);
+            float2 n1 = __fmul2_rn(bc(s1), t3), n2 = __fmul2_rn(bc(s2), t3);
+            float2 x0 = cadd(a, t1);
+            if constexpr (PZ >= 3) {
+                float2 t2 = x[2], t4 = x[2];
+                if constexpr (PZ >= 4) { t2 = cadd(x[2], x[3]); t4 = csub(x[2], x[3]); }
+                x0 = cadd(x0, t2);
+                m1 = __ffma2_rn(bc(c2), t2, m1);
+                m2 = __ffma2_rn(bc(c1), t2, m2);
+                n1 = __ffma2_rn(bc(s2), t4, n1);
+                n2 = __ffma2_rn(bc(-s1), t4, n2);
+            }
+            // X1 = m1 + i n1, X4 = m1 - i n1, X2 = m2 + i n2, X3 = m2 - i n2  (DIR folded in s1, s2)
+            x[0] = x0;
+            x[1] = cadd_i<1>(m1, n1);
+            x[4] = csub_i<1>(m1, n1);
+            x[2] = cadd_i<1>(m2, n2);
+            x[3] = csub_i<1>(m2, n2);
+        }
     }
 };
 
-// Composite N = P*Q, decimation in time:
+// ------------------------------------------------------ composite lengths ---
+// N = P*Q, decimation in time:
 //   Y_p = DFT_Q( x[P q' + p] ),  X[q + Q j] = sum_p W_P^{p j} ( W_N^{p q} Y_p[q] ).
-template <int N, int DIR>
-struct Dft {
+// With x[NZ..N) = 0 sub-sequence p has ceil((NZ-p)/P) leading non-zeros and only
+// the first min(P, NZ) sub-sequences are non-zero at all.
+template <int N, int DIR, int NZ>
+struct DftP {
+    static_assert(NZ >= 1 && NZ <= N, "DftP: 1 <= NZ <= N");
     static constexpr int P = (N % 4 == 0) ? 4 : (N % 2 == 0) ? 2 : (N % 3 == 0) ? 3 : 5;
     static constexpr int Q = N / P;
-    static_assert(N % P == 0 && Q >= 1, "Dft: length must be 2/3/5-smooth");
+    static_assert(N == 1 || N % P == 0, "DftP: length must be 2/3/5-smooth");
+    static constexpr int PZ = ct::imin(P, NZ);
+
     __device__ __forceinline__ static void run(float2 (&x)[N]) {
-        float2 y[P][Q];
-        sfor<P>([&](auto pc) {
-            constexpr int p = decltype(pc)::value;
-            float2 sub[Q];
-            sfor<Q>([&](auto qc) { constexpr int q = decltype(qc)::value; sub[q] = x[P * q + p]; });
-            Dft<Q, DIR>::run(sub);
-            sfor<Q>([&](auto qc) { constexpr int q = decltype(qc)::value; y[p][q] = sub[q]; });
-        });
-        sfor<Q>([&](auto qc) {
-            constexpr int q = decltype(qc)::value;
-            float2 t[P];
-            sfor<P>([&](auto pc) {
+        if constexpr (N == 1) {
+        } else if constexpr (NZ == 1) {              // DFT of a delta at 0 is constant
+            sfor<N - 1>([&](auto ic) { x[decltype(ic)::value + 1] = x[0]; });
+        } else if constexpr (Q == 1) {
+            Bfly<P, DIR, PZ>::run(x);
+        } else {
+            float2 y[P][Q];
+            sfor<PZ>([&](auto pc) {
                 constexpr int p = decltype(pc)::value;
-                t[p] = mul_w<p * q, N, DIR>(y[p][q]);
+                constexpr int NZp = ct::cdiv(NZ - p, P);
+                float2 sub[Q];
+                sfor<NZp>([&](auto qc) { constexpr int q = decltype(qc)::value; sub[q] = x[P * q + p]; });
+                DftP<Q, DIR, NZp>::run(sub);
+                sfor<Q>([&](auto qc) { constexpr int q = decltype(qc)::value; y[p][q] = sub[q]; });
             });
-            Dft<P, DIR>::run(t);
-            sfor<P>([&](auto jc) { constexpr int j = decltype(jc)::value; x[q + Q * j] = t[j]; });
-        });
+            sfor<Q>([&](auto qc) {
+                constexpr int q = decltype(qc)::value;
+                float2 t[P];
+                sfor<PZ>([&](auto pc) {
+                    constexpr int p = decltype(pc)::value;
+                    t[p] = mul_w<p * q, N, DIR>(y[p][q]);
+                });
+                Bfly<P, DIR, PZ>::run(t);
+                sfor<P>([&](auto jc) { constexpr int j = decltype(jc)::value; x[q + Q * j] = t[j]; });
+            });
+        }
     }
+};
+
+template <int N, int DIR>
+struct Dft {
+    __device__ __forceinline__ static void run(float2 (&x)[N]) { DftP<N, DIR, N>::run(x); }
 };
 
 }  // namespace pwk

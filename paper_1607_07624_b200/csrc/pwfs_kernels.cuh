@@ -32,17 +32,20 @@ constexpr float kInv2PiHi = 0.15915493667125702f;   // fl32(1/(2 pi))
 constexpr float kInv2PiLo = 6.4206382e-09f;          // 1/(2 pi) - kInv2PiHi
 constexpr int kPitch = 33;  // float2 row pitch of the exchange buffer: conflict-free LDS.64/STS.64
 
-template <int R1_, int NB_, int WPB_X_, int WPB_Y_>
+template <int R1_, int NB_, int WPB_X_, int WPB_Y_, int MINB_X_ = 1, int MINB_Y_ = 1>
 struct PassCfg {
     static constexpr int R1 = R1_;           // M / 32
     static constexpr int NB = NB_;           // transforms a warp works on at once
     static constexpr int M = 32 * R1_;
+    static constexpr int NZ = (R1_ + 1) / 2; // M >= 2N  =>  at most ceil(R1/2) non-zero inputs per lane
     static constexpr int ITEMS = NB_ * R1_;  // size-32 DFTs per warp batch
     static constexpr int ROUNDS = (ITEMS + 31) / 32;
     static constexpr int WARP_BUF = ITEMS * kPitch + 1;   // float2 per warp (+1: staggers warps across banks)
     static constexpr int TAB = R1_ * kPitch;              // float2 per table (twiddle, mask)
     static constexpr int WPB_X = WPB_X_;     // warps per CTA, row pass
     static constexpr int WPB_Y = WPB_Y_;     // warps per CTA, column pass
+    static constexpr int MINB_X = MINB_X_;   // CTAs per SM the register allocation must allow
+    static constexpr int MINB_Y = MINB_Y_;
     static constexpr int RPC = NB_ * WPB_X_; // rows per CTA, row pass
     static constexpr size_t smem_x = (size_t)(WPB_X_ * WARP_BUF + 2 * TAB) * sizeof(float2);
     static constexpr size_t smem_y = (size_t)(WPB_Y_ * WARP_BUF + 2 * TAB) * sizeof(float2);
@@ -50,14 +53,14 @@ struct PassCfg {
 
 // Device-side view of a sensor's tables (all pointers are device memory).
 struct DevTables {
-    int N, M, NP;             // pupil px, grid, padded y-pitch of T
+    int N, M, NP;             // pupil px, grid, y-pitch of T and tyt (N rounded up to 32; padding is zero)
     int K, KX;                // modulation points, distinct x-tilts
     int ncols;                // pupil-plane columns computed
     int D, n_sub, cmax;       // detector size 2 n_sub, rebin support
     int n_valid, slope_norm;
     const float *amp;         // [N][N]
     const float *txt;         // [KX][N]  x-tilt in turns, reduced to [-0.5, 0.5)
-    const float2 *tyt;        // [K][N]   exp(i tilt_y,k(y))
+    const float2 *tyt;        // [K][NP]  exp(i tilt_y,k(y)), zero for y >= N
     const int *jx;            // [K]      x-tilt index of modulation point k
     const float2 *tw;         // [R1][32] exp(-2 pi i k1 n2 / M)
     const float2 *am;         // [R1][32] a(k1 + R1 k2) / M
@@ -103,10 +106,10 @@ __device__ __forceinline__ void stage32(float2 *buf, const float2 *s_tw, const f
 }
 
 // ------------------------------------------------------------------ K1 ------
-// grid (ceil(N/RPC), KX, F); block 32*WPB_X.  Warp wl of the CTA owns rows
-// y0 + wl*NB + b, b < NB.
+// grid (ceil(NP/RPC), KX, F); block 32*WPB_X.  Warp wl of the CTA owns rows
+// y0 + wl*NB + b, b < NB.  Rows N <= y < NP carry a zero phasor and come out zero.
 template <class C>
-__global__ void __launch_bounds__(32 * C::WPB_X)
+__global__ void __launch_bounds__(32 * C::WPB_X, C::MINB_X)
 xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ T) {
     extern __shared__ float2 smem[];
     float2 *s_tw = smem;
@@ -120,34 +123,36 @@ xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ 
 
     load_tables(s_tw, s_am, t, C::R1);
 
-    const float *ph_f = phase + (size_t)f * N * N;
-    const float *txt = t.txt + (size_t)j * N;
-    // step A: phasor, DFT of size R1 over n1 (x = 32 n1 + lane)
+    const float *txt = t.txt + (size_t)j * N + lane;
+    // step A: phasor, zero-padded DFT of size R1 over n1 (x = 32 n1 + lane)
 #pragma unroll
     for (int b = 0; b < C::NB; ++b) {
         const int y = y0 + wl * C::NB + b;
+        const float *ph_row = phase + ((size_t)f * N + y) * N + lane;
+        const float *a_row = t.amp + (size_t)y * N + lane;
+        float ph[C::NZ], am[C::NZ], tx[C::NZ];
+#pragma unroll
+        for (int n1 = 0; n1 < C::NZ; ++n1) {
+            const bool ok = (y < N) && (32 * n1 + lane < N);
+            ph[n1] = ok ? __ldg(ph_row + 32 * n1) : 0.f;
+            am[n1] = ok ? __ldg(a_row + 32 * n1) : 0.f;
+            tx[n1] = ok ? __ldg(txt + 32 * n1) : 0.f;
+        }
         float2 v[C::R1];
 #pragma unroll
-        for (int n1 = 0; n1 < C::R1; ++n1) {
-            const int x = 32 * n1 + lane;
-            float2 p = make_float2(0.f, 0.f);
-            if (y < N && x < N) {
-                const float a = __ldg(t.amp + (size_t)y * N + x);
-                const float ph = __ldg(ph_f + (size_t)y * N + x);
-                // phase in turns, reduced: ph/(2 pi) with a two-term constant
-                // 1/(2 pi) = kInv2PiHi + kInv2PiLo (float pair); q is exact, the FMAs keep the product's low bits
-                const float q = rintf(ph * kInv2PiHi);
-                float tr = fmaf(ph, kInv2PiHi, -q);
-                tr = fmaf(ph, kInv2PiLo, tr);
-                tr += __ldg(txt + x);
-                tr -= rintf(tr);
-                float sn, cs;
-                __sincosf(tr * 6.283185307179586f, &sn, &cs);
-                p = make_float2(a * cs, a * sn);
-            }
-            v[n1] = p;
+        for (int n1 = 0; n1 < C::NZ; ++n1) {
+            // phase in turns: ph/(2 pi) with 1/(2 pi) = kInv2PiHi + kInv2PiLo; q is an exact integer and
+            // the FMAs keep the low bits of the product, so the reduction costs no accuracy at |ph| ~ 100 rad
+            const float q = rintf(ph[n1] * kInv2PiHi);
+            float tr = fmaf(ph[n1], kInv2PiHi, -q);
+            tr = fmaf(ph[n1], kInv2PiLo, tr);
+            tr += tx[n1];
+            tr -= rintf(tr);
+            float sn, cs;
+            __sincosf(tr * 6.283185307179586f, &sn, &cs);
+            v[n1] = make_float2(am[n1] * cs, am[n1] * sn);
         }
-        Dft<C::R1, -1>::run(v);
+        DftP<C::R1, -1, C::NZ>::run(v);
 #pragma unroll
         for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitch + lane] = v[k1];
     }
@@ -171,7 +176,7 @@ xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ 
     for (int idx = threadIdx.x; idx < total; idx += 32 * C::WPB_X) {
         const int r = idx % C::RPC, xc = idx / C::RPC;
         const int y = y0 + r;
-        if (y < N) {
+        if (y < t.NP) {
             const int x = __ldg(t.colx + xc);
             const int w2 = r / C::NB, b = r % C::NB;
             Tj[(size_t)xc * t.NP + y] = s_buf[w2 * C::WARP_BUF + (b * C::R1 + (x >> 5)) * kPitch + (x & 31)];
@@ -181,16 +186,18 @@ xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ 
 
 // ------------------------------------------------------------------ K2 ------
 // grid (ceil(ncols / (NB*WPB_Y)), ksplit, F); block 32*WPB_Y.  Warps are
-// independent: warp -> NB adjacent columns, loops over its share of k.
+// independent: warp -> NB adjacent columns, loops over its share of k.  The
+// inputs of modulation point k+1 are fetched into registers while point k is
+// being transformed (T streams from HBM/L2 once; nothing else leaves the SM).
 template <class C>
-__global__ void __launch_bounds__(32 * C::WPB_Y)
+__global__ void __launch_bounds__(32 * C::WPB_Y, C::MINB_Y)
 ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colbin, int ksplit) {
     extern __shared__ float2 smem[];
     float2 *s_tw = smem;
     float2 *s_am = smem + C::TAB;
     float2 *s_buf = smem + 2 * C::TAB;
     const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
-    const int N = t.N;
+    const int NP = t.NP;
     const int ks = blockIdx.y, f = blockIdx.z;
     const int xc0 = (blockIdx.x * C::WPB_Y + wl) * C::NB;
     float2 *buf = s_buf + wl * C::WARP_BUF;
@@ -206,22 +213,32 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
         for (int n1 = 0; n1 < C::R1; ++n1) acc[b][n1] = 0.f;
 
     const int k_lo = (int)(((long long)ks * t.K) / ksplit), k_hi = (int)(((long long)(ks + 1) * t.K) / ksplit);
+    const size_t frame_stride = (size_t)t.ncols * NP;
+    const float2 *Tf = T + (size_t)f * t.KX * frame_stride + (size_t)xc0 * NP + lane;
+
+    float2 pre[C::NB][C::NZ];
+    auto fetch = [&](int k) {
+        const float2 *src = Tf + (size_t)__ldg(t.jx + k) * frame_stride;
+#pragma unroll
+        for (int b = 0; b < C::NB; ++b)
+#pragma unroll
+            for (int n1 = 0; n1 < C::NZ; ++n1)
+                pre[b][n1] = (32 * n1 < NP && xc0 + b < t.ncols) ? __ldg(src + (size_t)b * NP + 32 * n1)
+                                                                 : make_float2(0.f, 0.f);
+    };
+    if (k_lo < k_hi) fetch(k_lo);
     for (int k = k_lo; k < k_hi; ++k) {
-        const int j = __ldg(t.jx + k);
-        const float2 *Tj = T + ((size_t)f * t.KX + j) * (size_t)t.ncols * t.NP;
-        const float2 *ty = t.tyt + (size_t)k * N;
+        const float2 *ty = t.tyt + (size_t)k * NP + lane;
+        float2 tyv[C::NZ];
+#pragma unroll
+        for (int n1 = 0; n1 < C::NZ; ++n1) tyv[n1] = (32 * n1 < NP) ? __ldg(ty + 32 * n1) : make_float2(0.f, 0.f);
 #pragma unroll
         for (int b = 0; b < C::NB; ++b) {
-            const int xc = xc0 + b;
             float2 v[C::R1];
 #pragma unroll
-            for (int n1 = 0; n1 < C::R1; ++n1) {
-                const int y = 32 * n1 + lane;
-                float2 p = make_float2(0.f, 0.f);
-                if (y < N && xc < t.ncols) p = cmul(__ldg(Tj + (size_t)xc * t.NP + y), __ldg(ty + y));
-                v[n1] = p;
-            }
-            Dft<C::R1, -1>::run(v);
+            for (int n1 = 0; n1 < C::NZ; ++n1) v[n1] = cmul(pre[b][n1], tyv[n1]);
+            if (b == C::NB - 1 && k + 1 < k_hi) fetch(k + 1);
+            DftP<C::R1, -1, C::NZ>::run(v);
 #pragma unroll
             for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitch + lane] = v[k1];
         }

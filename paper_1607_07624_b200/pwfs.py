@@ -14,7 +14,7 @@ from typing import Optional, Tuple
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libpwfs.so")
+LIB_PATH = os.environ.get("PWFS_LIB_PATH") or os.path.join(_HERE, "libpwfs.so")
 
 PWFS_OK, PWFS_EINVAL, PWFS_ENOMEM, PWFS_ECUDA, PWFS_EUNSUPPORTED = 0, -1, -2, -3, -4
 NUM_KERNEL_CLASSES = 4
