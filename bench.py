@@ -137,6 +137,7 @@ def run_reference(args, cfg):
 def run_ours(args, cfg):
     import torch
     import torch.distributed as dist
+    from paper_1607_07624_b200 import sharding
     from paper_1607_07624_b200.pwfs import from_config
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -170,11 +171,7 @@ def run_ours(args, cfg):
             torch.cuda.synchronize(dev)
 
     def max_over_ranks(x: float) -> float:
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return sharding.max_over_ranks(x, dev)
 
     # ---- device-resident timing (value) -------------------------------------
     for _ in range(args.warmup):

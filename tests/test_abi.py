@@ -1,0 +1,95 @@
+"""The C-ABI library loads here (no GPU) and exports every symbol include/pwfs.h
+declares; entry points that need no device behave as documented and the ones
+that do fail loudly instead of falling back to a CPU path."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_1607_07624_b200 import build, pwfs
+    build.build()                                   # nvcc cross-compiles without a GPU
+    return pwfs.load_library()
+
+
+def _declared_functions():
+    src = open(os.path.join(ROOT, "include", "pwfs.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(pwfs_[a-z_]+)\s*\(", src)))
+
+
+def test_header_symbols_are_exported(lib):
+    from paper_1607_07624_b200 import pwfs
+    names = _declared_functions()
+    assert len(names) >= 13 and "pwfs_create" in names and "pwfs_run" in names and "pwfs_destroy" in names
+    for n in names:
+        assert hasattr(lib, n), f"libpwfs.so does not export {n}"
+    assert sorted(pwfs.EXPORTS) == names             # the binding covers the whole header
+
+
+def test_params_struct_layout_matches_header():
+    from paper_1607_07624_b200.pwfs import pwfs_params
+    fields = [f[0] for f in pwfs_params._fields_]
+    src = open(os.path.join(ROOT, "include", "pwfs.h")).read()
+    body = src[src.index("typedef struct {"):src.index("} pwfs_params;")]
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    declared = re.findall(r"\b(?:int32_t|float|const float \*)\s*(\w+);", body)
+    assert declared == fields
+    assert C.sizeof(pwfs_params) == 48
+
+
+def test_strerror_and_supported_grid(lib):
+    from paper_1607_07624_b200 import pwfs
+    assert pwfs.strerror(0) == "ok"
+    assert "invalid" in pwfs.strerror(pwfs.PWFS_EINVAL)
+    assert "memory" in pwfs.strerror(pwfs.PWFS_ENOMEM)
+    assert "CUDA" in pwfs.strerror(pwfs.PWFS_ECUDA)
+    assert "unknown" in pwfs.strerror(-99)
+    for m in (128, 256, 320, 480, 512, 640, 800, 1024):
+        assert pwfs.supported_grid(m)
+    for m in (0, 96, 100, 2048, 1000):
+        assert not pwfs.supported_grid(m)
+
+
+def test_null_and_invalid_arguments_do_not_crash(lib):
+    from paper_1607_07624_b200 import pwfs
+    h = C.c_void_p()
+    assert lib.pwfs_create(None, C.byref(h)) == pwfs.PWFS_EINVAL
+    amp = np.ones((8, 8), np.float32)
+    prm = pwfs.pwfs_params(8, 10, amp.ctypes.data_as(C.POINTER(C.c_float)), 0, 1.0, 4, 0.0, 2, 0.5, 0, 0)
+    assert lib.pwfs_create(C.byref(prm), C.byref(h)) == pwfs.PWFS_EINVAL      # M < 2N
+    assert h.value is None
+    prm.m_grid = 96
+    assert lib.pwfs_create(C.byref(prm), C.byref(h)) == pwfs.PWFS_EUNSUPPORTED
+    lib.pwfs_destroy(None)                                                      # NULL-safe
+    assert lib.pwfs_info(None, None, None) == pwfs.PWFS_EINVAL
+    assert lib.pwfs_run(None, None, 1, None, None, None) == pwfs.PWFS_EINVAL
+    assert lib.pwfs_last_cuda_error(None) == 0
+
+
+def test_no_cpu_fallback_without_a_device(lib):
+    """Without a CUDA device construction must raise (PWFS_ECUDA), never compute."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    from paper_1607_07624_b200.pwfs import PWFS, PwfsError, PWFS_ECUDA
+    with pytest.raises(PwfsError) as ei:
+        PWFS(np.ones((32, 32), np.float32), 128, 1.0, 4, 8)
+    assert ei.value.code == PWFS_ECUDA
+
+
+def test_product_path_does_not_touch_the_oracle():
+    pkg = os.path.join(ROOT, "paper_1607_07624_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for fn in files:
+            if fn.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, fn)).read()
+                assert "pwfs_oracle" not in txt and "from oracle" not in txt and "import oracle" not in txt, fn
+    otxt = open(os.path.join(ROOT, "oracle", "pwfs_oracle.py")).read() + open(os.path.join(ROOT, "oracle", "pwfs_oracle.c")).read()
+    assert "import paper_1607_07624_b200" not in otxt and "from paper_1607_07624_b200" not in otxt and "libpwfs.so" not in otxt
