@@ -225,11 +225,15 @@ def run_ours(args, cfg):
         avg_launch_s = kernel_ms[dom] * 1e-3 / n_launch
         achieved = flops_per_launch / avg_launch_s / 1e12 if avg_launch_s > 0 else 0.0
         path_tflops = nominal_flops_per_modpoint(M) * B * K / (ms_per_step * 1e-3) / 1e12
-        traffic = None
-        tpath = os.path.join(ROOT, "profiles", "traffic.json")
+        traffic = None                                                   # dram bytes per launch, from the committed ncu capture
+        tpath = os.path.join(ROOT, "profiles", "traffic.csv")
         if os.path.exists(tpath):
+            import csv
             with open(tpath) as fh:
-                traffic = json.load(fh).get(cfg.name, {}).get(dom)
+                for row in csv.DictReader(fh):
+                    if row["config"] == cfg.name and row["kernel"] == dom:
+                        per_frame = float(row["dram_bytes_per_launch"]) / float(row["frames_per_launch"])
+                        traffic = per_frame * B * args.steps / n_launch
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
