@@ -46,52 +46,55 @@ struct Launcher {
     void (*launch_y)(dim3, cudaStream_t, const DevTables &, const float2 *, float *, int);
 };
 
-template <class C>
+template <class C, bool QM>
 void launch_x_t(dim3 grid, cudaStream_t st, const DevTables &t, const float *phase, float2 *T) {
-    xpass_kernel<C><<<grid, 32 * C::WPB_X, C::smem_x, st>>>(t, phase, T);
+    xpass_kernel<C, QM><<<grid, 32 * C::WPB_X, C::smem_x, st>>>(t, phase, T);
 }
-template <class C>
+template <class C, bool QM>
 void launch_y_t(dim3 grid, cudaStream_t st, const DevTables &t, const float2 *T, float *colbin, int ksplit) {
-    ypass_kernel<C><<<grid, 32 * C::WPB_Y, C::smem_y, st>>>(t, T, colbin, ksplit);
+    ypass_kernel<C, QM><<<grid, 32 * C::WPB_Y, C::smem_y, st>>>(t, T, colbin, ksplit);
 }
-template <class C>
-Launcher make_launcher() {
+template <class C, bool QM>
+Launcher make_launcher_q() {
     Launcher l;
     l.R1 = C::R1; l.NB = C::NB; l.WPB_X = C::WPB_X; l.WPB_Y = C::WPB_Y; l.RPC = C::RPC;
     l.smem_x = C::smem_x; l.smem_y = C::smem_y;
-    l.xfn = (const void *)xpass_kernel<C>;
-    l.yfn = (const void *)ypass_kernel<C>;
-    l.launch_x = launch_x_t<C>;
-    l.launch_y = launch_y_t<C>;
+    l.xfn = (const void *)xpass_kernel<C, QM>;
+    l.yfn = (const void *)ypass_kernel<C, QM>;
+    l.launch_x = launch_x_t<C, QM>;
+    l.launch_y = launch_y_t<C, QM>;
     return l;
 }
+// quarter = the mask shift is exactly M/4: kernels with the table-free power-of-i mask
+template <class C>
+Launcher make_launcher(bool quarter) { return quarter ? make_launcher_q<C, true>() : make_launcher_q<C, false>(); }
 
-bool find_launcher(int M, Launcher *out) {
+bool find_launcher(int M, bool quarter, Launcher *out) {
     if (M % 32) return false;
     switch (M / 32) {
 #if !defined(PWFS_ONLY_R1) || PWFS_ONLY_R1 == 4
-        case 4: *out = make_launcher<Cfg4>(); return true;
+        case 4: *out = make_launcher<Cfg4>(quarter); return true;
 #endif
 #if !defined(PWFS_ONLY_R1) || PWFS_ONLY_R1 == 8
-        case 8: *out = make_launcher<Cfg8>(); return true;
+        case 8: *out = make_launcher<Cfg8>(quarter); return true;
 #endif
 #if !defined(PWFS_ONLY_R1) || PWFS_ONLY_R1 == 10
-        case 10: *out = make_launcher<Cfg10>(); return true;
+        case 10: *out = make_launcher<Cfg10>(quarter); return true;
 #endif
 #if !defined(PWFS_ONLY_R1) || PWFS_ONLY_R1 == 15
-        case 15: *out = make_launcher<Cfg15>(); return true;
+        case 15: *out = make_launcher<Cfg15>(quarter); return true;
 #endif
 #if !defined(PWFS_ONLY_R1) || PWFS_ONLY_R1 == 16
-        case 16: *out = make_launcher<Cfg16>(); return true;
+        case 16: *out = make_launcher<Cfg16>(quarter); return true;
 #endif
 #if !defined(PWFS_ONLY_R1) || PWFS_ONLY_R1 == 20
-        case 20: *out = make_launcher<Cfg20>(); return true;
+        case 20: *out = make_launcher<Cfg20>(quarter); return true;
 #endif
 #if !defined(PWFS_ONLY_R1) || PWFS_ONLY_R1 == 25
-        case 25: *out = make_launcher<Cfg25>(); return true;
+        case 25: *out = make_launcher<Cfg25>(quarter); return true;
 #endif
 #if !defined(PWFS_ONLY_R1) || PWFS_ONLY_R1 == 32
-        case 32: *out = make_launcher<Cfg32>(); return true;
+        case 32: *out = make_launcher<Cfg32>(quarter); return true;
 #endif
         default: return false;
     }
@@ -105,6 +108,7 @@ struct pwfs {
     pwfs_params prm;
     int device = 0;
     int s = 0;
+    bool quarter = false;                    // s == M/4: table-free mask kernels
     Launcher L{};
     DevTables tab{};
     std::vector<void *> dev_allocs;          // table memory
@@ -263,7 +267,7 @@ int build_tables(pwfs *h) {
             const int us = u < M / 2 ? u : u - M;
             const long long num = ((long long)s * std::abs(us)) % M;
             const double am_ang = kTwoPi * (double)num / (double)M;
-            am[(size_t)k1 * 32 + n2] = make_float2((float)(std::cos(am_ang) / M), (float)(std::sin(am_ang) / M));
+            am[(size_t)k1 * 32 + n2] = make_float2((float)(std::cos(am_ang) / M), (float)(std::sin(am_ang) / M));   // table path only (s != M/4)
         }
     // columns of the pupil plane that fall inside a window (corner-placed grid: origins M-s and s)
     std::vector<int> xc_of_x(M, -1), colx;
@@ -379,7 +383,7 @@ const char *pwfs_strerror(int code) {
 
 int pwfs_supported_grid(int32_t m_grid) {
     Launcher l;
-    return find_launcher(m_grid, &l) ? 1 : 0;
+    return find_launcher(m_grid, false, &l) ? 1 : 0;
 }
 
 int pwfs_create(const pwfs_params *p, pwfs_t **out) {
@@ -398,11 +402,11 @@ int pwfs_create(const pwfs_params *p, pwfs_t **out) {
     for (size_t i = 0; i < (size_t)N * N; ++i)
         if (!(p->pupil_amp[i] >= 0.f) || !std::isfinite(p->pupil_amp[i])) return PWFS_EINVAL;
     Launcher L;
-    if (!find_launcher(M, &L)) return PWFS_EUNSUPPORTED;
+    if (!find_launcher(M, 4 * s == M, &L)) return PWFS_EUNSUPPORTED;
 
     pwfs *h = new (std::nothrow) pwfs();
     if (!h) return PWFS_ENOMEM;
-    h->prm = *p; h->s = s; h->L = L; h->device = p->device;
+    h->prm = *p; h->s = s; h->quarter = (4 * s == M); h->L = L; h->device = p->device;
     int rc = PWFS_OK;
     cudaError_t e = cudaSetDevice(p->device);
     if (e != cudaSuccess) { h->last_cuda = (int)e; rc = PWFS_ECUDA; }
@@ -533,8 +537,10 @@ int pwfs_run(pwfs_t *h, const float *d_phase, int32_t B, float *d_frames, float 
         {   // K3a: x-rebin (a7)
             SpanGuard g(h, st, 2);
             const int threads = std::min(256, (t.D + 31) / 32 * 32);
+            // 1/K of O6; the quarter-mask kernels leave O5's 1/M per axis (1/M^4 on |E|^2) to this scale
+            const double m4 = h->quarter ? std::pow((double)t.M, 4.0) : 1.0;
             xrebin_kernel<<<dim3(t.D, Fc), threads, 0, st>>>(t, h->colbin, d_frames + (size_t)f0 * DD, ks,
-                                                             1.0f / (float)t.K);
+                                                             (float)(1.0 / ((double)t.K * m4)));
         }
         if (d_slopes) {   // K3b: slopes (a8)
             SpanGuard g(h, st, 3);

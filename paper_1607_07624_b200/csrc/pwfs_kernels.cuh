@@ -72,17 +72,47 @@ struct DevTables {
     const int *vidx;          // [n_valid] j*n_sub + i of valid subapertures, row-major
 };
 
+template <bool QM>
 __device__ __forceinline__ void load_tables(float2 *s_tw, float2 *s_am, const DevTables &t, int R1) {
     for (int i = threadIdx.x; i < R1 * 32; i += blockDim.x) {
         int k1 = i >> 5, n2 = i & 31;
         s_tw[k1 * kPitch + n2] = t.tw[i];
-        s_am[k1 * kPitch + n2] = t.am[i];
+        if constexpr (!QM) s_am[k1 * kPitch + n2] = t.am[i];
     }
+}
+
+// Inverse DFT-32 whose inputs x[16..32) carry a run-time sign sg = +-1 (both halves of sg2):
+// X = IDFT32(x[0..16), sg * x[16..32)).  Split 32 = 16 x 2: the size-2 butterflies on the pairs
+// (x[p], x[p+16]) absorb the sign as FFMA2s in place of FADD2s, so it costs nothing.
+__device__ __forceinline__ void idft32_signed_upper(float2 (&x)[32], float2 sg2) {
+    float2 e[16], o[16];
+    const float2 nsg2 = make_float2(-sg2.x, -sg2.y);
+    sfor<16>([&](auto pc) {
+        constexpr int p = decltype(pc)::value;
+        e[p] = __ffma2_rn(x[p + 16], sg2, x[p]);
+        o[p] = mul_w<p, 32, +1>(__ffma2_rn(x[p + 16], nsg2, x[p]));
+    });
+    Dft<16, +1>::run(e);
+    Dft<16, +1>::run(o);
+    sfor<16>([&](auto jc) {
+        constexpr int j = decltype(jc)::value;
+        x[2 * j] = e[j];
+        x[2 * j + 1] = o[j];
+    });
 }
 
 // Size-32 stage for the warp's current batch: for every (transform b, k1):
 // twiddle, DFT over n2, mask, inverse DFT, conjugate twiddle; in place in `buf`.
-template <class C>
+//
+// QM = true is the default mask s = M/4 (M % 4 == 0), whose 1-D factor is a power of i:
+// a(u) = i^|u~|, i.e. i^u for u < M/2 and i^-u above.  With u = k1 + R1 k2 (k2 >= 16 <=> u >= M/2)
+//   a(u) = i^k1 * i^(R1 k2)              k2 < 16
+//        = i^k1 * (-1)^k1 * i^(-R1 k2)   k2 >= 16
+// i^(+-R1 k2) is a compile-time swap/negate (operand modifiers, no instruction), (-1)^k1 is a
+// per-lane sign absorbed by idft32_signed_upper, and i^k1 is applied where k1 is a compile-time
+// register index (step A' of the callers, apply_ipow_k1).  The mask and its table cost nothing;
+// the 1/M per axis moves into the final frame scale.
+template <class C, bool QM>
 __device__ __forceinline__ void stage32(float2 *buf, const float2 *s_tw, const float2 *s_am, int lane) {
 #pragma unroll
     for (int rd = 0; rd < C::ROUNDS; ++rd) {
@@ -91,24 +121,45 @@ __device__ __forceinline__ void stage32(float2 *buf, const float2 *s_tw, const f
             int k1 = w % C::R1;
             float2 *row = buf + w * kPitch;
             const float2 *twr = s_tw + k1 * kPitch;
-            const float2 *amr = s_am + k1 * kPitch;
             float2 u[32];
 #pragma unroll
             for (int n2 = 0; n2 < 32; ++n2) u[n2] = cmul(row[n2], twr[n2]);
             Dft<32, -1>::run(u);
+            if constexpr (QM) {
+                sfor<32>([&](auto kc) {
+                    constexpr int k2 = decltype(kc)::value;
+                    constexpr int e = k2 < 16 ? (C::R1 * k2) % 4 : (4 - (C::R1 * k2) % 4) % 4;
+                    u[k2] = mul_w<e, 4, +1>(u[k2]);
+                });
+                const float sg = (k1 & 1) ? -1.f : 1.f;
+                idft32_signed_upper(u, make_float2(sg, sg));
+            } else {
+                const float2 *amr = s_am + k1 * kPitch;
 #pragma unroll
-            for (int k2 = 0; k2 < 32; ++k2) u[k2] = cmul(u[k2], amr[k2]);
-            Dft<32, +1>::run(u);
+                for (int k2 = 0; k2 < 32; ++k2) u[k2] = cmul(u[k2], amr[k2]);
+                Dft<32, +1>::run(u);
+            }
 #pragma unroll
             for (int n2 = 0; n2 < 32; ++n2) row[n2] = cmulc(u[n2], twr[n2]);
         }
     }
 }
 
+// i^k1 of the quarter mask, applied to the register that holds index k1 (free: operand modifiers).
+template <int R1, bool QM>
+__device__ __forceinline__ void apply_ipow_k1(float2 (&v)[R1]) {
+    if constexpr (QM) {
+        sfor<R1>([&](auto kc) {
+            constexpr int k1 = decltype(kc)::value;
+            v[k1] = mul_w<k1 % 4, 4, +1>(v[k1]);
+        });
+    }
+}
+
 // ------------------------------------------------------------------ K1 ------
 // grid (ceil(NP/RPC), KX, F); block 32*WPB_X.  Warp wl of the CTA owns rows
 // y0 + wl*NB + b, b < NB.  Rows N <= y < NP carry a zero phasor and come out zero.
-template <class C>
+template <class C, bool QM>
 __global__ void __launch_bounds__(32 * C::WPB_X, C::MINB_X)
 xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ T) {
     extern __shared__ float2 smem[];
@@ -121,7 +172,7 @@ xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ 
     const int y0 = blockIdx.x * C::RPC;
     float2 *buf = s_buf + wl * C::WARP_BUF;
 
-    load_tables(s_tw, s_am, t, C::R1);
+    load_tables<QM>(s_tw, s_am, t, C::R1);
 
     const float *txt = t.txt + (size_t)j * N + lane;
     // step A: phasor, zero-padded DFT of size R1 over n1 (x = 32 n1 + lane)
@@ -157,7 +208,7 @@ xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ 
         for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitch + lane] = v[k1];
     }
     __syncthreads();   // tables loaded + this warp's stores visible
-    stage32<C>(buf, s_tw, s_am, lane);
+    stage32<C, QM>(buf, s_tw, s_am, lane);
     __syncwarp();
     // step A': inverse DFT of size R1 over k1 -> x = 32 n1 + lane; stage for the transposed store
 #pragma unroll
@@ -165,6 +216,7 @@ xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ 
         float2 v[C::R1];
 #pragma unroll
         for (int k1 = 0; k1 < C::R1; ++k1) v[k1] = buf[(b * C::R1 + k1) * kPitch + lane];
+        apply_ipow_k1<C::R1, QM>(v);
         Dft<C::R1, +1>::run(v);
 #pragma unroll
         for (int n1 = 0; n1 < C::R1; ++n1) buf[(b * C::R1 + n1) * kPitch + lane] = v[n1];
@@ -189,7 +241,7 @@ xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ 
 // independent: warp -> NB adjacent columns, loops over its share of k.  The
 // inputs of modulation point k+1 are fetched into registers while point k is
 // being transformed (T streams from HBM/L2 once; nothing else leaves the SM).
-template <class C>
+template <class C, bool QM>
 __global__ void __launch_bounds__(32 * C::WPB_Y, C::MINB_Y)
 ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colbin, int ksplit) {
     extern __shared__ float2 smem[];
@@ -202,7 +254,7 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
     const int xc0 = (blockIdx.x * C::WPB_Y + wl) * C::NB;
     float2 *buf = s_buf + wl * C::WARP_BUF;
 
-    load_tables(s_tw, s_am, t, C::R1);
+    load_tables<QM>(s_tw, s_am, t, C::R1);
     __syncthreads();
     if (xc0 >= t.ncols) return;
 
@@ -243,13 +295,14 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
             for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitch + lane] = v[k1];
         }
         __syncwarp();
-        stage32<C>(buf, s_tw, s_am, lane);
+        stage32<C, QM>(buf, s_tw, s_am, lane);
         __syncwarp();
 #pragma unroll
         for (int b = 0; b < C::NB; ++b) {
             float2 v[C::R1];
 #pragma unroll
             for (int k1 = 0; k1 < C::R1; ++k1) v[k1] = buf[(b * C::R1 + k1) * kPitch + lane];
+            apply_ipow_k1<C::R1, QM>(v);
             Dft<C::R1, +1>::run(v);
 #pragma unroll
             for (int n1 = 0; n1 < C::R1; ++n1) acc[b][n1] = fmaf(v[n1].x, v[n1].x, fmaf(v[n1].y, v[n1].y, acc[b][n1]));
