@@ -123,18 +123,74 @@ __device__ __forceinline__ float2 mul_w(float2 a) {
     }
 }
 
+// ------------------------------------------ twiddles in "1 + i tau" form -----
+// A twiddle multiply followed by the butterfly's add/sub costs FMUL2 + FFMA2 + FADD2.
+// Writing w = sigma * i^rot * (1 + i tau), |tau| <= 1 (rot = nearest quadrant, sigma = cos,
+// tau = tan of the remainder), the product splits into
+//     u = y + i tau y          one FFMA2 (none for tau = 0, one FADD2 for tau = +-1),
+//     i^rot                    operand swap/negate modifiers, no instruction,
+//     sigma                    a real scale that the NEXT add absorbs: a + sigma*u is one FFMA2
+// (Linzer-Feig style scaling).  So a non-trivial twiddle costs one packed instruction
+// instead of two; the butterflies below take the pending scales of their inputs as a
+// compile-time set S (S::s(p) = scale of input p, S::s(0) = 1).
+namespace ct {
+struct lf { double sigma; int rot; double tau; };
+__host__ __device__ constexpr lf lf_of(long long num, long long den) {
+    num = pmod(num, den);
+    long long q = (8 * num + den) / (2 * den);
+    double r = (double)(4 * num - q * den) / (double)(4 * den);
+    double a = 2.0 * kPi * r;
+    bool exact = (4 * num == q * den);
+    double c = exact ? 1.0 : cos_poly(a);
+    double s = exact ? 0.0 : sin_poly(a);
+    return {c, (int)(q & 3), s / c};
+}
+}  // namespace ct
+
+struct OneS { __host__ __device__ static constexpr float s(int) { return 1.f; } };
+// scales of the inputs t[p] = W_N^{DIR p q} y[p] of combine step q
+template <int N, int Q_, int DIR>
+struct TwS {
+    __host__ __device__ static constexpr float s(int p) { return (float)ct::lf_of((long long)DIR * p * Q_, N).sigma; }
+};
+
+template <int E>
+__device__ __forceinline__ float2 rot_i(float2 a) {      // a * i^E
+    if constexpr ((E & 3) == 0) return a;
+    else if constexpr ((E & 3) == 1) return make_float2(-a.y, a.x);
+    else if constexpr ((E & 3) == 2) return make_float2(-a.x, -a.y);
+    else return make_float2(a.y, -a.x);
+}
+// i^rot (y + i tau y) for w = exp(DIR 2 pi i NUM/DEN); the factor sigma stays pending
+template <int NUM, int DEN, int DIR>
+__device__ __forceinline__ float2 lf_pre(float2 y) {
+    constexpr ct::lf w = ct::lf_of((long long)DIR * NUM, DEN);
+    constexpr float tau = (float)w.tau;
+    float2 u;
+    if constexpr (tau == 0.f) u = y;
+    else if constexpr (tau == 1.f) u = __fadd2_rn(y, make_float2(-y.y, y.x));
+    else if constexpr (tau == -1.f) u = __fadd2_rn(y, make_float2(y.y, -y.x));
+    else u = __ffma2_rn(bc(tau), make_float2(-y.y, y.x), y);
+    return rot_i<w.rot>(u);
+}
+// a + c*b, compile-time real c
+#define PWK_AXPY(c, b, a) (((c) == 1.f) ? __fadd2_rn((a), (b)) : ((c) == -1.f) ? __fadd2_rn((a), make_float2(-(b).x, -(b).y)) : __ffma2_rn(bc(c), (b), (a)))
+
 // ------------------------------------------------- prime-size butterflies ---
-// Bfly<P, DIR, PZ>: DFT of size P whose inputs x[PZ..P) are zero (never read).
+// Bfly<P, DIR, PZ>::run<S>: DFT of size P of the inputs S::s(p) * x[p]; x[PZ..P) are zero
+// (never read).
 template <int P, int DIR, int PZ>
 struct Bfly;
 
 template <int DIR, int PZ>
 struct Bfly<2, DIR, PZ> {
+    template <class S = OneS>
     __device__ __forceinline__ static void run(float2 (&x)[2]) {
+        constexpr float s1 = S::s(1);
         if constexpr (PZ >= 2) {
             const float2 a = x[0], b = x[1];
-            x[0] = cadd(a, b);
-            x[1] = csub(a, b);
+            x[0] = PWK_AXPY(s1, b, a);
+            x[1] = PWK_AXPY(-s1, b, a);
         } else {
             x[1] = x[0];
         }
@@ -143,70 +199,95 @@ struct Bfly<2, DIR, PZ> {
 
 template <int DIR, int PZ>
 struct Bfly<3, DIR, PZ> {
+    template <class S = OneS>
     __device__ __forceinline__ static void run(float2 (&x)[3]) {
         constexpr float s60 = 0.86602540378443864676f * (float)DIR;
+        constexpr float s1 = S::s(1);
         if constexpr (PZ == 1) {
             x[1] = x[0]; x[2] = x[0];
         } else {
-            const float2 a = x[0], b = x[1];
-            float2 t = b, u = b;
-            if constexpr (PZ >= 3) { t = cadd(b, x[2]); u = csub(b, x[2]); }
-            x[0] = cadd(a, t);
-            const float2 m = __ffma2_rn(bc(-0.5f), t, a);
+            const float2 a = x[0];
+            float2 t = x[1], u = x[1];                 // true values carry s1
+            if constexpr (PZ >= 3) {
+                constexpr float r = S::s(2) / s1;
+                t = PWK_AXPY(r, x[2], x[1]);
+                u = PWK_AXPY(-r, x[2], x[1]);
+            }
+            x[0] = PWK_AXPY(s1, t, a);
+            const float2 m = __ffma2_rn(bc(-0.5f * s1), t, a);
             const float2 iu = make_float2(-u.y, u.x);
-            x[1] = __ffma2_rn(bc(s60), iu, m);      // m + i DIR s u
-            x[2] = __ffma2_rn(bc(-s60), iu, m);     // m - i DIR s u
+            x[1] = __ffma2_rn(bc(s60 * s1), iu, m);      // m + i DIR s u
+            x[2] = __ffma2_rn(bc(-s60 * s1), iu, m);     // m - i DIR s u
         }
     }
 };
 
 template <int DIR, int PZ>
 struct Bfly<4, DIR, PZ> {
+    template <class S = OneS>
     __device__ __forceinline__ static void run(float2 (&x)[4]) {
+        constexpr float s1 = S::s(1);
         if constexpr (PZ == 1) {
             x[1] = x[0]; x[2] = x[0]; x[3] = x[0];
-        } else if constexpr (PZ == 2) {             // X_j = a + w^j b, w = DIR i
-            const float2 a = x[0], b = x[1];
-            x[0] = cadd(a, b);
-            x[1] = cadd_i<DIR>(a, b);
-            x[2] = csub(a, b);
-            x[3] = csub_i<DIR>(a, b);
+        } else if constexpr (PZ == 2) {             // X_j = a + w^j s1 b, w = DIR i
+            const float2 a = x[0], b = x[1], ib = rot_i<DIR>(x[1]);
+            x[0] = PWK_AXPY(s1, b, a);
+            x[1] = PWK_AXPY(s1, ib, a);
+            x[2] = PWK_AXPY(-s1, b, a);
+            x[3] = PWK_AXPY(-s1, ib, a);
         } else {
-            const float2 t0 = cadd(x[0], x[2]), t1 = csub(x[0], x[2]);
-            float2 t2 = x[1], t3 = x[1];
-            if constexpr (PZ >= 4) { t2 = cadd(x[1], x[3]); t3 = csub(x[1], x[3]); }
-            x[0] = cadd(t0, t2);
-            x[1] = cadd_i<DIR>(t1, t3);
-            x[2] = csub(t0, t2);
-            x[3] = csub_i<DIR>(t1, t3);
+            constexpr float s2 = S::s(2);
+            const float2 t0 = PWK_AXPY(s2, x[2], x[0]), t1 = PWK_AXPY(-s2, x[2], x[0]);
+            float2 t2 = x[1], t3 = x[1];                // true values carry s1
+            if constexpr (PZ >= 4) {
+                constexpr float r = S::s(3) / s1;
+                t2 = PWK_AXPY(r, x[3], x[1]);
+                t3 = PWK_AXPY(-r, x[3], x[1]);
+            }
+            const float2 it3 = rot_i<DIR>(t3);
+            x[0] = PWK_AXPY(s1, t2, t0);
+            x[1] = PWK_AXPY(s1, it3, t1);
+            x[2] = PWK_AXPY(-s1, t2, t0);
+            x[3] = PWK_AXPY(-s1, it3, t1);
         }
     }
 };
 
 template <int DIR, int PZ>
 struct Bfly<5, DIR, PZ> {
+    template <class S = OneS>
     __device__ __forceinline__ static void run(float2 (&x)[5]) {
         constexpr float c1 = 0.30901699437494742410f;    // cos 72
         constexpr float c2 = -0.80901699437494742410f;   // cos 144
         constexpr float s1 = 0.95105651629515357212f * (float)DIR;   // sin 72
         constexpr float s2 = 0.58778525229247312917f * (float)DIR;   // sin 144
+        constexpr float g1 = S::s(1);                    // pending scale of x[1] (and of t1, t3)
         if constexpr (PZ == 1) {
             x[1] = x[0]; x[2] = x[0]; x[3] = x[0]; x[4] = x[0];
         } else {
             const float2 a = x[0];
             float2 t1 = x[1], t3 = x[1];
-            if constexpr (PZ >= 5) { t1 = cadd(x[1], x[4]); t3 = csub(x[1], x[4]); }
-            float2 m1 = __ffma2_rn(bc(c1), t1, a), m2 = __ffma2_rn(bc(c2), t1, a);
-            float2 n1 = __fmul2_rn(bc(s1), t3), n2 = __fmul2_rn(bc(s2), t3);
-            float2 x0 = cadd(a, t1);
+            if constexpr (PZ >= 5) {
+                constexpr float r = S::s(4) / g1;
+                t1 = PWK_AXPY(r, x[4], x[1]);
+                t3 = PWK_AXPY(-r, x[4], x[1]);
+            }
+            float2 m1 = __ffma2_rn(bc(c1 * g1), t1, a), m2 = __ffma2_rn(bc(c2 * g1), t1, a);
+            float2 n1 = __fmul2_rn(bc(s1 * g1), t3), n2 = __fmul2_rn(bc(s2 * g1), t3);
+            float2 x0 = PWK_AXPY(g1, t1, a);
             if constexpr (PZ >= 3) {
+                constexpr float g2 = S::s(2);            // pending scale of x[2] (and of t2, t4)
                 float2 t2 = x[2], t4 = x[2];
-                if constexpr (PZ >= 4) { t2 = cadd(x[2], x[3]); t4 = csub(x[2], x[3]); }
-                x0 = cadd(x0, t2);
-                m1 = __ffma2_rn(bc(c2), t2, m1);
-                m2 = __ffma2_rn(bc(c1), t2, m2);
-                n1 = __ffma2_rn(bc(s2), t4, n1);
-                n2 = __ffma2_rn(bc(-s1), t4, n2);
+                if constexpr (PZ >= 4) {
+                    constexpr float r = S::s(3) / g2;
+                    t2 = PWK_AXPY(r, x[3], x[2]);
+                    t4 = PWK_AXPY(-r, x[3], x[2]);
+                }
+                x0 = PWK_AXPY(g2, t2, x0);
+                m1 = __ffma2_rn(bc(c2 * g2), t2, m1);
+                m2 = __ffma2_rn(bc(c1 * g2), t2, m2);
+                n1 = __ffma2_rn(bc(s2 * g2), t4, n1);
+                n2 = __ffma2_rn(bc(-s1 * g2), t4, n2);
             }
             // X1 = m1 + i n1, X4 = m1 - i n1, X2 = m2 + i n2, X3 = m2 - i n2  (DIR folded in s1, s2)
             x[0] = x0;
@@ -236,7 +317,7 @@ struct DftP {
         } else if constexpr (NZ == 1) {              // DFT of a delta at 0 is constant
             sfor<N - 1>([&](auto ic) { x[decltype(ic)::value + 1] = x[0]; });
         } else if constexpr (Q == 1) {
-            Bfly<P, DIR, PZ>::run(x);
+            Bfly<P, DIR, PZ>::template run<OneS>(x);
         } else {
             float2 y[P][Q];
             sfor<PZ>([&](auto pc) {
@@ -252,9 +333,9 @@ struct DftP {
                 float2 t[P];
                 sfor<PZ>([&](auto pc) {
                     constexpr int p = decltype(pc)::value;
-                    t[p] = mul_w<p * q, N, DIR>(y[p][q]);
+                    t[p] = lf_pre<p * q, N, DIR>(y[p][q]);
                 });
-                Bfly<P, DIR, PZ>::run(t);
+                Bfly<P, DIR, PZ>::template run<TwS<N, q, DIR>>(t);
                 sfor<P>([&](auto jc) { constexpr int j = decltype(jc)::value; x[q + Q * j] = t[j]; });
             });
         }
