@@ -42,13 +42,13 @@ struct Launcher {
     int R1, NB, WPB_X, WPB_Y, RPC;
     size_t smem_x, smem_y;
     const void *xfn, *yfn;
-    void (*launch_x)(dim3, cudaStream_t, const DevTables &, const float *, float2 *);
+    void (*launch_x)(dim3, cudaStream_t, const DevTables &, const float *, float2 *, int);
     void (*launch_y)(dim3, cudaStream_t, const DevTables &, const float2 *, float *, int);
 };
 
 template <class C, bool QM>
-void launch_x_t(dim3 grid, cudaStream_t st, const DevTables &t, const float *phase, float2 *T) {
-    xpass_kernel<C, QM><<<grid, 32 * C::WPB_X, C::smem_x, st>>>(t, phase, T);
+void launch_x_t(dim3 grid, cudaStream_t st, const DevTables &t, const float *phase, float2 *T, int jsplit) {
+    xpass_kernel<C, QM><<<grid, 32 * C::WPB_X, QM ? C::smem_x_q : C::smem_x_t, st>>>(t, phase, T, jsplit);
 }
 template <class C, bool QM>
 void launch_y_t(dim3 grid, cudaStream_t st, const DevTables &t, const float2 *T, float *colbin, int ksplit) {
@@ -58,7 +58,7 @@ template <class C, bool QM>
 Launcher make_launcher_q() {
     Launcher l;
     l.R1 = C::R1; l.NB = C::NB; l.WPB_X = C::WPB_X; l.WPB_Y = C::WPB_Y; l.RPC = C::RPC;
-    l.smem_x = C::smem_x; l.smem_y = C::smem_y;
+    l.smem_x = QM ? C::smem_x_q : C::smem_x_t; l.smem_y = C::smem_y;
     l.xfn = (const void *)xpass_kernel<C, QM>;
     l.yfn = (const void *)ypass_kernel<C, QM>;
     l.launch_x = launch_x_t<C, QM>;
@@ -243,12 +243,13 @@ int build_tables(pwfs *h) {
     }
     t.KX = (int)ux.size();
     const double c = 0.5 * (double)(N - 1);
-    std::vector<float> txt((size_t)t.KX * N);
+    t.NXP = 32 * ((R1 + 1) / 2);                                      // >= N because M >= 2N
+    std::vector<float2> txc((size_t)t.KX * t.NXP, make_float2(0.f, 0.f));   // zero in the padding x >= N
     for (int j = 0; j < t.KX; ++j)
         for (int x = 0; x < N; ++x) {
-            double turns = ux[j] * ((double)x - c) / (double)N;       // O1, x part, in turns
+            double turns = ux[j] * ((double)x - c) / (double)N;       // O1, x part
             turns -= std::nearbyint(turns);
-            txt[(size_t)j * N + x] = (float)turns;
+            txc[(size_t)j * t.NXP + x] = make_float2((float)std::cos(kTwoPi * turns), (float)std::sin(kTwoPi * turns));
         }
     std::vector<float2> tyt((size_t)K * t.NP, make_float2(0.f, 0.f));   // zero in the padding y >= N
     for (int k = 0; k < K; ++k)
@@ -291,7 +292,7 @@ int build_tables(pwfs *h) {
     std::vector<float> amp(p.pupil_amp, p.pupil_amp + (size_t)N * N);
     int rc;
     if ((rc = upload(h, amp, &t.amp))) return rc;
-    if ((rc = upload(h, txt, &t.txt))) return rc;
+    if ((rc = upload(h, txc, &t.txc))) return rc;
     if ((rc = upload(h, tyt, &t.tyt))) return rc;
     if ((rc = upload(h, jx, &t.jx))) return rc;
     if ((rc = upload(h, tw, &t.tw))) return rc;
@@ -308,7 +309,7 @@ int build_tables(pwfs *h) {
 // frames per chunk and k-split for a batch of B frames
 void schedule(const pwfs *h, int B, int *fpc, int *ksplit) {
     const DevTables &t = h->tab;
-    const size_t T_frame = (size_t)t.KX * t.ncols * t.NP * sizeof(float2);
+    const size_t T_frame = (size_t)t.KX * t.M * t.NP * sizeof(float2);   // T[f][j][x][y], x over the whole grid
     const int col_warps = (t.ncols + h->L.NB - 1) / h->L.NB;           // column-pass warps per frame
     const int slots = h->num_sms * 12;                                  // resident warps we aim to fill
     int F = h->user_fpc > 0 ? h->user_fpc : (8 * slots + col_warps - 1) / col_warps;
@@ -326,7 +327,7 @@ void schedule(const pwfs *h, int B, int *fpc, int *ksplit) {
 
 int ensure_scratch(pwfs *h, int F, int ksplit) {
     const DevTables &t = h->tab;
-    const size_t needT = (size_t)F * t.KX * t.ncols * t.NP;
+    const size_t needT = (size_t)F * t.KX * t.M * t.NP;
     const size_t needC = (size_t)F * ksplit * t.ncols * t.D;
     if (needT > h->T_elems) {
         if (h->T) cudaFree(h->T);
@@ -527,7 +528,12 @@ int pwfs_run(pwfs_t *h, const float *d_phase, int32_t B, float *d_frames, float 
         const int Fc = std::min(F, B - f0);
         {   // K1: phasor + x-convolution (a1, a3, a4, a5 along x)
             SpanGuard g(h, st, 0);
-            L.launch_x(dim3((t.NP + L.RPC - 1) / L.RPC, t.KX, Fc), st, t, d_phase + (size_t)f0 * NN, h->T);
+            // split the x-tilt loop only as far as needed to fill the machine (>= 8 waves of 2 CTAs/SM),
+            // keeping >= 3 tilts per CTA so the one-off phasor stays amortised
+            const int row_ctas = (t.NP + L.RPC - 1) / L.RPC;
+            int jsplit = 1;
+            while ((long long)row_ctas * Fc * jsplit < 16LL * h->num_sms && t.KX / (jsplit + 1) >= 3) ++jsplit;
+            L.launch_x(dim3(row_ctas, jsplit, Fc), st, t, d_phase + (size_t)f0 * NN, h->T, jsplit);
         }
         {   // K2: y-convolution + |E|^2 over k + y-rebin (a3, a4, a5 along y, a6, a7)
             SpanGuard g(h, st, 1);

@@ -31,6 +31,7 @@ namespace pwk {
 constexpr float kInv2PiHi = 0.15915493667125702f;   // fl32(1/(2 pi))
 constexpr float kInv2PiLo = 6.4206382e-09f;          // 1/(2 pi) - kInv2PiHi
 constexpr int kPitch = 33;  // float2 row pitch of the exchange buffer: conflict-free LDS.64/STS.64
+constexpr int kTB = 8;      // the row pass writes T[f][j][x][y] in runs of kTB consecutive y (64 bytes) per column
 
 template <int R1_, int NB_, int WPB_X_, int WPB_Y_, int MINB_X_ = 1, int MINB_Y_ = 1>
 struct PassCfg {
@@ -40,26 +41,32 @@ struct PassCfg {
     static constexpr int NZ = (R1_ + 1) / 2; // M >= 2N  =>  at most ceil(R1/2) non-zero inputs per lane
     static constexpr int ITEMS = NB_ * R1_;  // size-32 DFTs per warp batch
     static constexpr int ROUNDS = (ITEMS + 31) / 32;
-    static constexpr int WARP_BUF = ITEMS * kPitch + 1;   // float2 per warp (+1: staggers warps across banks)
+    // float2 per warp.  The row pass's write-out reads TB rows (= TB/NB warps' buffers) x a few adjacent
+    // columns per instruction: a warp stride of 2 (mod 16) 64-bit banks keeps those reads conflict-free.
+    static constexpr int WARP_BUF = (ITEMS * kPitch + 15) / 16 * 16 + 2;
     static constexpr int TAB = R1_ * kPitch;              // float2 per table (twiddle, mask)
     static constexpr int WPB_X = WPB_X_;     // warps per CTA, row pass
     static constexpr int WPB_Y = WPB_Y_;     // warps per CTA, column pass
     static constexpr int MINB_X = MINB_X_;   // CTAs per SM the register allocation must allow
     static constexpr int MINB_Y = MINB_Y_;
     static constexpr int RPC = NB_ * WPB_X_; // rows per CTA, row pass
-    static constexpr size_t smem_x = (size_t)(WPB_X_ * WARP_BUF + 2 * TAB) * sizeof(float2);
+    static_assert(RPC % kTB == 0, "row pass: rows per CTA must be whole y-blocks of T");
+    // row pass: tables (no mask table for the quarter mask) + exchange buffers + base phasor [RPC][NZ][32]
+    static constexpr size_t smem_x_q = (size_t)(WPB_X_ * WARP_BUF + 1 * TAB + RPC * NZ * 32) * sizeof(float2);
+    static constexpr size_t smem_x_t = (size_t)(WPB_X_ * WARP_BUF + 2 * TAB + RPC * NZ * 32) * sizeof(float2);
     static constexpr size_t smem_y = (size_t)(WPB_Y_ * WARP_BUF + 2 * TAB) * sizeof(float2);
 };
 
 // Device-side view of a sensor's tables (all pointers are device memory).
 struct DevTables {
-    int N, M, NP;             // pupil px, grid, y-pitch of T and tyt (N rounded up to 32; padding is zero)
+    int N, M, NP;             // pupil px, grid, y-extent of T and tyt (N rounded up to 32; padding is zero)
+    int NXP;                  // x-pitch of txc (32 * ceil(R1/2) >= N; padding is zero)
     int K, KX;                // modulation points, distinct x-tilts
     int ncols;                // pupil-plane columns computed
     int D, n_sub, cmax;       // detector size 2 n_sub, rebin support
     int n_valid, slope_norm;
     const float *amp;         // [N][N]
-    const float *txt;         // [KX][N]  x-tilt in turns, reduced to [-0.5, 0.5)
+    const float2 *txc;        // [KX][NXP] exp(i tilt_x,j(x)), zero for x >= N
     const float2 *tyt;        // [K][NP]  exp(i tilt_y,k(y)), zero for y >= N
     const int *jx;            // [K]      x-tilt index of modulation point k
     const float2 *tw;         // [R1][32] exp(-2 pi i k1 n2 / M)
@@ -157,39 +164,48 @@ __device__ __forceinline__ void apply_ipow_k1(float2 (&v)[R1]) {
 }
 
 // ------------------------------------------------------------------ K1 ------
-// grid (ceil(NP/RPC), KX, F); block 32*WPB_X.  Warp wl of the CTA owns rows
-// y0 + wl*NB + b, b < NB.  Rows N <= y < NP carry a zero phasor and come out zero.
+// grid (ceil(NP/RPC), jsplit, F); block 32*WPB_X.  Warp wl of the CTA owns rows
+// y0 + wl*NB + b, b < NB, of frame f and loops over its share of the distinct x-tilts j.
+//
+// The base phasor A exp(i phi) is computed ONCE (one range-reduced MUFU sincos per pupil
+// pixel per CTA) and parked in shared memory; per x-tilt it is multiplied by the table
+// exp(i tilt_x,j(x)) -- the tilt is separable, so this is the whole k-dependence of the
+// row pass.  Rows N <= y < NP carry a zero phasor and come out zero.
+//
+// The last register stage is done "transposed": thread (r, n2) takes row r of the CTA
+// (another warp's exchange buffer) and column residue n2, so that adjacent lanes hold
+// adjacent rows y of the same column x = 32 n1 + n2 and the results go straight from
+// registers to T[f][j][x][y] as runs of >= 64 bytes -- no staging pass for the transposition.
 template <class C, bool QM>
 __global__ void __launch_bounds__(32 * C::WPB_X, C::MINB_X)
-xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ T) {
+xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ T, int jsplit) {
     extern __shared__ float2 smem[];
     float2 *s_tw = smem;
-    float2 *s_am = smem + C::TAB;
-    float2 *s_buf = smem + 2 * C::TAB;
+    float2 *s_am = smem + C::TAB;                              // unused (zero-sized) when QM
+    float2 *s_buf = smem + (QM ? 1 : 2) * C::TAB;
+    float2 *s_p = s_buf + C::WPB_X * C::WARP_BUF;              // [RPC][NZ][32] base phasor
     const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
     const int N = t.N;
-    const int j = blockIdx.y, f = blockIdx.z;
+    const int js = blockIdx.y, f = blockIdx.z;
     const int y0 = blockIdx.x * C::RPC;
     float2 *buf = s_buf + wl * C::WARP_BUF;
+    float2 *pw = s_p + (size_t)wl * C::NB * C::NZ * 32 + lane;
 
     load_tables<QM>(s_tw, s_am, t, C::R1);
 
-    const float *txt = t.txt + (size_t)j * N + lane;
-    // step A: phasor, zero-padded DFT of size R1 over n1 (x = 32 n1 + lane)
+    // a1: base phasor of this warp's rows, x = 32 n1 + lane
 #pragma unroll
     for (int b = 0; b < C::NB; ++b) {
         const int y = y0 + wl * C::NB + b;
         const float *ph_row = phase + ((size_t)f * N + y) * N + lane;
         const float *a_row = t.amp + (size_t)y * N + lane;
-        float ph[C::NZ], am[C::NZ], tx[C::NZ];
+        float ph[C::NZ], am[C::NZ];
 #pragma unroll
         for (int n1 = 0; n1 < C::NZ; ++n1) {
             const bool ok = (y < N) && (32 * n1 + lane < N);
             ph[n1] = ok ? __ldg(ph_row + 32 * n1) : 0.f;
             am[n1] = ok ? __ldg(a_row + 32 * n1) : 0.f;
-            tx[n1] = ok ? __ldg(txt + 32 * n1) : 0.f;
         }
-        float2 v[C::R1];
 #pragma unroll
         for (int n1 = 0; n1 < C::NZ; ++n1) {
             // phase in turns: ph/(2 pi) with 1/(2 pi) = kInv2PiHi + kInv2PiLo; q is an exact integer and
@@ -197,42 +213,73 @@ xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ 
             const float q = rintf(ph[n1] * kInv2PiHi);
             float tr = fmaf(ph[n1], kInv2PiHi, -q);
             tr = fmaf(ph[n1], kInv2PiLo, tr);
-            tr += tx[n1];
-            tr -= rintf(tr);
             float sn, cs;
             __sincosf(tr * 6.283185307179586f, &sn, &cs);
-            v[n1] = make_float2(am[n1] * cs, am[n1] * sn);
+            pw[(b * C::NZ + n1) * 32] = make_float2(am[n1] * cs, am[n1] * sn);
         }
-        DftP<C::R1, -1, C::NZ>::run(v);
-#pragma unroll
-        for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitch + lane] = v[k1];
     }
-    __syncthreads();   // tables loaded + this warp's stores visible
-    stage32<C, QM>(buf, s_tw, s_am, lane);
-    __syncwarp();
-    // step A': inverse DFT of size R1 over k1 -> x = 32 n1 + lane; stage for the transposed store
+
+    // transposed last stage: this thread's items (r, n2), it < NB, and which of their outputs
+    // x = 32 n1 + n2 lie inside a pupil-image window (bit n1 of wmask[it])
+    int item_src[C::NB];          // exchange-buffer offset of (row r, k1 = 0, n2)
+    int item_dst[C::NB];          // T offset of (x = n2, y = y0 + r) within the (f, j) slab
+    unsigned wmask[C::NB];
 #pragma unroll
-    for (int b = 0; b < C::NB; ++b) {
-        float2 v[C::R1];
-#pragma unroll
-        for (int k1 = 0; k1 < C::R1; ++k1) v[k1] = buf[(b * C::R1 + k1) * kPitch + lane];
-        apply_ipow_k1<C::R1, QM>(v);
-        Dft<C::R1, +1>::run(v);
-#pragma unroll
-        for (int n1 = 0; n1 < C::R1; ++n1) buf[(b * C::R1 + n1) * kPitch + lane] = v[n1];
+    for (int it = 0; it < C::NB; ++it) {
+        const int i = threadIdx.x + it * 32 * C::WPB_X;
+        const int r = i % C::RPC, n2 = i / C::RPC;
+        item_src[it] = (r / C::NB) * C::WARP_BUF + (r % C::NB) * C::R1 * kPitch + n2;
+        item_dst[it] = n2 * t.NP + y0 + r;
+        unsigned m = 0;
+        if (y0 + r < t.NP)
+            for (int n1 = 0; n1 < C::R1; ++n1) m |= (__ldg(t.xc_of_x + 32 * n1 + n2) >= 0 ? 1u : 0u) << n1;
+        wmask[it] = m;
     }
-    __syncthreads();
-    // transposed write-out: T[f][j][xc][y], RPC consecutive y per column
-    float2 *Tj = T + ((size_t)f * t.KX + j) * (size_t)t.ncols * t.NP;
-    const int total = C::RPC * t.ncols;
-    for (int idx = threadIdx.x; idx < total; idx += 32 * C::WPB_X) {
-        const int r = idx % C::RPC, xc = idx / C::RPC;
-        const int y = y0 + r;
-        if (y < t.NP) {
-            const int x = __ldg(t.colx + xc);
-            const int w2 = r / C::NB, b = r % C::NB;
-            Tj[(size_t)xc * t.NP + y] = s_buf[w2 * C::WARP_BUF + (b * C::R1 + (x >> 5)) * kPitch + (x & 31)];
+
+    const int j_lo = (int)(((long long)js * t.KX) / jsplit), j_hi = (int)(((long long)(js + 1) * t.KX) / jsplit);
+    const size_t slab = (size_t)t.M * t.NP;
+    const int n1_stride = 32 * t.NP;
+    __syncthreads();   // tables loaded (s_p is private to the warp that wrote it)
+    for (int j = j_lo; j < j_hi; ++j) {
+        // step A: x-tilt, zero-padded DFT of size R1 over n1
+        float2 tx[C::NZ];
+        {
+            const float2 *txj = t.txc + (size_t)j * t.NXP + lane;
+#pragma unroll
+            for (int n1 = 0; n1 < C::NZ; ++n1) tx[n1] = __ldg(txj + 32 * n1);
         }
+#pragma unroll
+        for (int b = 0; b < C::NB; ++b) {
+            float2 v[C::R1];
+#pragma unroll
+            for (int n1 = 0; n1 < C::NZ; ++n1) v[n1] = cmul(pw[(b * C::NZ + n1) * 32], tx[n1]);
+            DftP<C::R1, -1, C::NZ>::run(v);
+#pragma unroll
+            for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitch + lane] = v[k1];
+        }
+        __syncwarp();
+        stage32<C, QM>(buf, s_tw, s_am, lane);
+        // pull the next tilt's table row (NXP float2 = NZ * 2 cache lines) into L1 while the last stage runs
+        if (j + 1 < j_hi && threadIdx.x < 2 * C::NZ)
+            asm volatile("prefetch.global.L1 [%0];" ::"l"(t.txc + (size_t)(j + 1) * t.NXP + 16 * threadIdx.x));
+        __syncthreads();
+        // step A'': inverse DFT of size R1 over k1 for item (r, n2) -> T[f][j][32 n1 + n2][y0 + r]
+        float2 *Tj = T + ((size_t)f * t.KX + j) * slab;
+#pragma unroll
+        for (int it = 0; it < C::NB; ++it) {
+            float2 v[C::R1];
+            const float2 *src = s_buf + item_src[it];
+#pragma unroll
+            for (int k1 = 0; k1 < C::R1; ++k1) v[k1] = src[k1 * kPitch];
+            apply_ipow_k1<C::R1, QM>(v);
+            Dft<C::R1, +1>::run(v);
+            float2 *dst = Tj + item_dst[it];
+            const unsigned m = wmask[it];
+#pragma unroll
+            for (int n1 = 0; n1 < C::R1; ++n1)
+                if ((m >> n1) & 1u) dst[n1 * n1_stride] = v[n1];
+        }
+        __syncthreads();   // the next x-tilt overwrites the buffers
     }
 }
 
@@ -265,8 +312,12 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
         for (int n1 = 0; n1 < C::R1; ++n1) acc[b][n1] = 0.f;
 
     const int k_lo = (int)(((long long)ks * t.K) / ksplit), k_hi = (int)(((long long)(ks + 1) * t.K) / ksplit);
-    const size_t frame_stride = (size_t)t.ncols * NP;
-    const float2 *Tf = T + (size_t)f * t.KX * frame_stride + (size_t)xc0 * NP + lane;
+    // T[f][j][x][y]: grid column x of compact column xc from the colx table (windows may leave gaps)
+    const size_t frame_stride = (size_t)t.M * NP;
+    const float2 *Tf = T + (size_t)f * t.KX * frame_stride + lane;
+    int colofs[C::NB];
+#pragma unroll
+    for (int b = 0; b < C::NB; ++b) colofs[b] = (xc0 + b < t.ncols) ? __ldg(t.colx + xc0 + b) * NP : 0;
 
     float2 pre[C::NB][C::NZ];
     auto fetch = [&](int k) {
@@ -275,7 +326,7 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
         for (int b = 0; b < C::NB; ++b)
 #pragma unroll
             for (int n1 = 0; n1 < C::NZ; ++n1)
-                pre[b][n1] = (32 * n1 < NP && xc0 + b < t.ncols) ? __ldg(src + (size_t)b * NP + 32 * n1)
+                pre[b][n1] = (32 * n1 < NP && xc0 + b < t.ncols) ? __ldg(src + colofs[b] + 32 * n1)
                                                                  : make_float2(0.f, 0.f);
     };
     if (k_lo < k_hi) fetch(k_lo);
