@@ -25,11 +25,11 @@ constexpr double kTwoPi = 6.283185307179586476925286766559;
 // ---- per-grid kernel configurations (R1 = M/32, NB, warps/CTA row pass, column pass)
 using Cfg4 = PassCfg<4, 8, 4, 4>;     // M = 128
 using Cfg8 = PassCfg<8, 4, 4, 4>;     // M = 256
-using Cfg10 = PassCfg<10, 3, 16, 4>;  // M = 320
-using Cfg15 = PassCfg<15, 2, 8, 4>;   // M = 480
-using Cfg16 = PassCfg<16, 2, 8, 4>;   // M = 512
-using Cfg20 = PassCfg<20, 1, 16, 4>;  // M = 640
-using Cfg25 = PassCfg<25, 1, 16, 4>;  // M = 800
+using Cfg10 = PassCfg<10, 3, 8, 4, 2, 1>;  // M = 320
+using Cfg15 = PassCfg<15, 2, 8, 4, 2, 1>;   // M = 480
+using Cfg16 = PassCfg<16, 2, 8, 4, 2, 1>;   // M = 512
+using Cfg20 = PassCfg<20, 1, 8, 4, 2, 1>;  // M = 640
+using Cfg25 = PassCfg<25, 1, 8, 4, 2, 1>;  // M = 800
 #ifndef PWFS_C32_WX
 #define PWFS_C32_WX 8
 #define PWFS_C32_WY 4
