@@ -198,6 +198,35 @@ def run_ours(args, cfg):
     ms_per_step = ms_total / args.steps
     value = world * B * args.steps / (ms_total * 1e-3)
 
+    # ---- closed-loop latency: one frame per call (B = 1), eager and replayed from a CUDA graph
+    latency = None
+    if rank == 0:
+        ph1 = phase[:1].contiguous()
+        fr1 = torch.empty((1, D, D), dtype=torch.float32, device=dev)
+        sl1 = torch.empty((1, 2 * nv), dtype=torch.float32, device=dev)
+        reps = 100
+
+        def timed(fn):
+            for _ in range(5):
+                fn()
+            torch.cuda.synchronize(dev)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            for _ in range(reps):
+                fn()
+            b.record(stream)
+            torch.cuda.synchronize(dev)
+            return a.elapsed_time(b) / reps
+
+        eager_ms = timed(lambda: sensor.run(ph1, fr1, sl1))
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):                    # pwfs_run only enqueues kernels: capturable as is
+            sensor.run(ph1, fr1, sl1)
+        graph_ms = timed(graph.replay)
+        latency = {"frames_per_call": 1, "eager_ms": eager_ms, "cuda_graph_ms": graph_ms, "calls": reps,
+                   "note": "back-to-back calls on one stream, device time per call (CUDA events)"}
+        del graph
+
     # ---- end to end through the host-buffer entry point (e2e) ----------------
     h_phase = torch.from_numpy(phase_np).pin_memory()
     h_frames = torch.empty((B, D, D), dtype=torch.float32).pin_memory()
@@ -257,6 +286,7 @@ def run_ours(args, cfg):
                     "d2h_bytes_per_step": int(h_frames.numel() * 4 + h_slopes.numel() * 4),
                     "matches_device_path": same},
             "gpu_launches": int(sum(launches.values())),
+            "latency_b1": latency,
             "clocks": clocks,
         }
         if not args.no_cpu_baseline:

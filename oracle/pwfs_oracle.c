@@ -300,6 +300,61 @@ int orc_intensity(int N, int M, const float *A, const float *phi, int K, double 
     return err;
 }
 
+/* ---------------------------------------- f3: tilt list and field stop ---- */
+
+/* Focal-plane field stop (Table 1
+ * `pyramid`: "Requested field-of-view [arcsec]", key lost in extraction).
+ * Reading F3a: the stop is the SQUARE |u~| <= h and |v~| <= h in
+ * focal-plane bins (signed frequencies as in O4), transmission 1 inside and 0
+ * outside, multiplied into the pyramid mask:  m[v][u] <- m[v][u] * stop.
+ * h < 0 means "no stop" (mask untouched). */
+void orc_field_stop(int M, double h, zc *m) {
+    if (h < 0.0) return;
+    for (int v = 0; v < M; ++v) {
+        int vs = (v < M / 2) ? v : v - M;
+        for (int u = 0; u < M; ++u) {
+            int us = (u < M / 2) ? u : u - M;
+            if ((double)abs(us) > h || (double)abs(vs) > h) m[(size_t)v * M + u] = 0.0;
+        }
+    }
+}
+
+/* O6 generalised to an arbitrary list of tilts with weights (SURVEY.md 8(f)
+ * row f3: "replace the K-point circle by an arbitrary list (dx,dy,w) -- covers
+ * extended/resolved sources"; "resolved sources", L77):
+ *   I = sum_k w_k |E_k|^2 / sum_k w_k,   E_k from O1..O5 with tilt (dx_k, dy_k).
+ * Reading F3b: weights are non-negative and normalised by their sum, so the
+ * uniform circle list reproduces O6 exactly.  Sequential over k (no threads:
+ * this entry is for small pins and parity samples). */
+int orc_intensity_list(int N, int M, const float *A, const float *phi, int n_pts,
+                       const double *dx, const double *dy, const double *w, const zc *mask,
+                       double *Iout, int use_naive) {
+    if (n_pts < 1 || N < 1 || M < N) return ORC_EINVAL;
+    size_t MM = (size_t)M * M;
+    double wsum = 0.0;
+    for (int k = 0; k < n_pts; ++k) {
+        if (!(w[k] >= 0.0)) return ORC_EINVAL;
+        wsum += w[k];
+    }
+    if (!(wsum > 0.0)) return ORC_EINVAL;
+    zc *E = (zc *)malloc(sizeof(zc) * MM);
+    if (!E) return ORC_ENOMEM;
+    for (size_t i = 0; i < MM; ++i) Iout[i] = 0.0;
+    int rc = ORC_OK;
+    for (int k = 0; k < n_pts && !rc; ++k) {
+        rc = orc_field(N, M, A, phi, dx[k], dy[k], mask, E, NULL, use_naive);
+        if (!rc)
+            for (size_t i = 0; i < MM; ++i) {
+                double re = creal(E[i]), im = cimag(E[i]);
+                Iout[i] += w[k] * (re * re + im * im);
+            }
+    }
+    if (!rc)
+        for (size_t i = 0; i < MM; ++i) Iout[i] /= wsum;
+    free(E);
+    return rc;
+}
+
 /* ------------------------------------------- O7..O9: detector, slopes ---- */
 
 /* O7 weights: W[i][p] = | [p, p+1) intersect [i b, (i+1) b) |, b = N/n_sub,
@@ -449,6 +504,40 @@ int orc_pwfs_run(int N, int M, const float *A, int s, double r, int K, double th
     if (!rc) orc_pyramid_mask(M, (double)s, mask);                  /* O4 */
     for (int bb = 0; bb < B && !rc; ++bb) {
         rc = orc_intensity(N, M, A, phase + (size_t)bb * N * N, K, r, theta0, mask, Ifull, 0);
+        if (!rc) rc = orc_frame(N, M, s, n_sub, Ifull, frames + (size_t)bb * D * D);   /* O7 */
+        if (!rc && slopes) {
+            int n2 = orc_slopes(n_sub, frames + (size_t)bb * D * D, valid, norm_mode,
+                                slopes + (size_t)bb * 2 * nv);      /* O9 */
+            if (n2 != nv) rc = ORC_EINVAL;
+        }
+    }
+    free(valid); free(mask); free(Ifull);
+    return rc ? rc : nv;
+}
+
+/* Whole path with the f3 generalisations: tilt list (dx,dy,w) in lambda/D in
+ * place of the circle and an optional square field stop of half-width
+ * stop_h focal-plane bins (< 0: none).  Otherwise identical to orc_pwfs_run. */
+int orc_pwfs_run_list(int N, int M, const float *A, int s, int n_pts, const double *dx,
+                      const double *dy, const double *w, double stop_h, int n_sub, double thresh,
+                      int norm_mode, int B, const float *phase, double *frames, double *slopes) {
+    if (N < 2 || M < 2 * N || (M & 1) || n_pts < 1 || B < 0) return ORC_EINVAL;
+    if (s <= 0) { if (M % 4) return ORC_EINVAL; s = M / 4; }
+    if (2 * s < N || s > M / 2 - N / 2) return ORC_EINVAL;
+    size_t MM = (size_t)M * M;
+    int D = 2 * n_sub;
+    unsigned char *valid = (unsigned char *)malloc((size_t)n_sub * n_sub);
+    zc *mask = (zc *)malloc(sizeof(zc) * MM);
+    double *Ifull = (double *)malloc(sizeof(double) * MM);
+    if (!valid || !mask || !Ifull) { free(valid); free(mask); free(Ifull); return ORC_ENOMEM; }
+    int nv = orc_valid_mask(N, n_sub, A, thresh, valid);            /* O8 */
+    int rc = (nv > 0) ? ORC_OK : ORC_EINVAL;
+    if (!rc) {
+        orc_pyramid_mask(M, (double)s, mask);                       /* O4 */
+        orc_field_stop(M, stop_h, mask);                            /* f3 */
+    }
+    for (int bb = 0; bb < B && !rc; ++bb) {
+        rc = orc_intensity_list(N, M, A, phase + (size_t)bb * N * N, n_pts, dx, dy, w, mask, Ifull, 0);
         if (!rc) rc = orc_frame(N, M, s, n_sub, Ifull, frames + (size_t)bb * D * D);   /* O7 */
         if (!rc && slopes) {
             int n2 = orc_slopes(n_sub, frames + (size_t)bb * D * D, valid, norm_mode,

@@ -73,6 +73,12 @@ def _load():
         lib.orc_slopes.restype = i
         lib.orc_pwfs_run.argtypes = [i, i, p, i, d, i, d, i, d, i, i, p, p, p]
         lib.orc_pwfs_run.restype = i
+        lib.orc_field_stop.argtypes = [i, d, p]
+        lib.orc_field_stop.restype = None
+        lib.orc_intensity_list.argtypes = [i, i, p, p, i, p, p, p, p, p, i]
+        lib.orc_intensity_list.restype = i
+        lib.orc_pwfs_run_list.argtypes = [i, i, p, i, i, p, p, p, d, i, d, i, i, p, p, p]
+        lib.orc_pwfs_run_list.restype = i
         _lib = lib
     return _lib
 
@@ -220,4 +226,47 @@ def pwfs_run(A, M, r, K, n_sub, phase, s=0, theta0=0.0, thresh=0.5, norm_mode=0)
                               float(thresh), norm_mode, B, _ptr(phase), _ptr(frames), _ptr(slp))
     _check(rc, "pwfs_run")
     assert rc == nv
+    return frames, slp
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def field_stop(mask, h):
+    """mask * (square stop |u~|,|v~| <= h bins); h < 0: unchanged."""
+    m = _c128(mask).copy()
+    _load().orc_field_stop(m.shape[0], float(h), _ptr(m))
+    return m
+
+
+def intensity_list(A, phi, M, dx, dy, w, mask=None, s=None, naive=False):
+    """Full-resolution I = sum_k w_k |E_k|^2 / sum_k w_k for a list of tilts."""
+    A, phi = _f32(A), _f32(phi)
+    dx, dy, w = _f64(dx), _f64(dy), _f64(w)
+    N = A.shape[0]
+    if mask is None:
+        mask = pyramid_mask(M, M // 4 if s is None else s)
+    mask = _c128(mask)
+    out = np.empty((M, M), dtype=np.float64)
+    _check(_load().orc_intensity_list(N, M, _ptr(A), _ptr(phi), dx.size, _ptr(dx), _ptr(dy), _ptr(w),
+                                      _ptr(mask), _ptr(out), int(naive)), "intensity_list")
+    return out
+
+
+def pwfs_run_list(A, M, dx, dy, w, n_sub, phase, s=0, stop_h=-1.0, thresh=0.5, norm_mode=0):
+    """Whole path with a weighted tilt list and an optional square field stop."""
+    A, phase = _f32(A), _f32(phase)
+    dx, dy, w = _f64(dx), _f64(dy), _f64(w)
+    N = A.shape[0]
+    if phase.ndim == 2:
+        phase = phase[None]
+    B = phase.shape[0]
+    _, nv = valid_mask(A, n_sub, thresh)
+    frames = np.empty((B, 2 * n_sub, 2 * n_sub), dtype=np.float64)
+    slp = np.empty((B, 2 * nv), dtype=np.float64)
+    rc = _load().orc_pwfs_run_list(N, M, _ptr(A), int(s), dx.size, _ptr(dx), _ptr(dy), _ptr(w),
+                                   float(stop_h), n_sub, float(thresh), norm_mode, B, _ptr(phase),
+                                   _ptr(frames), _ptr(slp))
+    _check(rc, "pwfs_run_list")
     return frames, slp
