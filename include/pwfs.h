@@ -80,6 +80,33 @@ typedef struct {
  * M, mask params, mod radius, K, binning)". */
 int pwfs_create(const pwfs_params *p, pwfs_t **out);
 
+/* Extensions of the sensor model, all optional.
+ *   Tilt list: n_tilts > 0 replaces the modulation circle (mod_radius, mod_points,
+ *   mod_angle0 are then ignored) by the points (tilt_x[k], tilt_y[k]) in lambda/D
+ *   with non-negative weights tilt_w[k] (NULL = uniform; only ratios matter):
+ *       I = sum_k w_k |E_k|^2 / sum_k w_k.
+ *   This is how an extended / resolved reference source, or any non-circular
+ *   modulation, is given ("resolved sources", L77 "Extended (non
+ *   point-like) reference source studies").  The uniform circle list reproduces
+ *   pwfs_create exactly.  The row pass is shared between points of equal tilt_x.
+ *   Field stop: field_stop_px >= 0 multiplies the pyramid mask by the SQUARE stop
+ *   |u~| <= h and |v~| <= h (h = field_stop_px in focal-plane bins, signed
+ *   frequencies u~ in [-M/2, M/2); 1 lambda/D = M/N bins): the focal-plane
+ *   field of view (Table 1 `pyramid`, "Requested
+ *   field-of-view [arcsec]").  < 0, or >= M/2, means no stop.  A square stop keeps
+ *   the mask separable; a stop selects the table-mask kernels.
+ * All pointers are HOST memory, copied by the call. */
+typedef struct {
+    int32_t n_tilts;
+    const float *tilt_x;
+    const float *tilt_y;
+    const float *tilt_w;
+    float field_stop_px;
+} pwfs_ext;
+
+/* pwfs_create with the extensions above; x == NULL is pwfs_create. */
+int pwfs_create_ex(const pwfs_params *p, const pwfs_ext *x, pwfs_t **out);
+
 /* Detector size (2*n_sub) and number of valid subapertures.  Either pointer
  * may be NULL. */
 int pwfs_info(const pwfs_t *h, int32_t *det_size, int32_t *n_valid);

@@ -108,7 +108,9 @@ struct pwfs {
     pwfs_params prm;
     int device = 0;
     int s = 0;
-    bool quarter = false;                    // s == M/4: table-free mask kernels
+    bool quarter = false;                    // s == M/4 and no field stop: table-free mask kernels
+    std::vector<double> list_dx, list_dy, list_w;   // f3: weighted tilt list (empty: the circle of prm)
+    double stop_h = -1.0;                    // f3: square field stop half-width [focal bins], < 0 none
     Launcher L{};
     DevTables tab{};
     std::vector<void *> dev_allocs;          // table memory
@@ -222,22 +224,35 @@ int build_valid(int N, int n_sub, const float *A, double thresh, std::vector<uin
 
 int build_tables(pwfs *h) {
     const pwfs_params &p = h->prm;
-    const int N = p.n_pupil, M = p.m_grid, K = p.mod_points, n_sub = p.n_subap, s = h->s;
+    const bool listed = !h->list_dx.empty();
+    const int N = p.n_pupil, M = p.m_grid, K = listed ? (int)h->list_dx.size() : p.mod_points, n_sub = p.n_subap, s = h->s;
     const int R1 = h->L.R1;
     DevTables &t = h->tab;
     t.N = N; t.M = M; t.NP = (N + 31) / 32 * 32; t.K = K;
     t.D = 2 * n_sub; t.n_sub = n_sub; t.slope_norm = p.slope_norm;
 
     // O0: modulation points; distinct x-tilts (the row pass depends on k only through dx_k)
-    std::vector<double> dx(K), dy(K), ux;
+    // f3: an explicit list (dx, dy, w) replaces the circle; I = sum_k w_k |E_k|^2 / sum_k w_k.  The weight
+    // rides on the y-tilt phasor as sqrt(w_k K / sum w), so the kernels and their 1/K scale are unchanged.
+    std::vector<double> dx(K), dy(K), ux, amp_k(K, 1.0);
     std::vector<int> jx(K);
+    double wsum = 0.0, tmax = (double)p.mod_radius;
+    if (listed) {
+        for (int k = 0; k < K; ++k) { wsum += h->list_w[k]; tmax = std::max(tmax, std::fabs(h->list_dx[k])); }
+        for (int k = 0; k < K; ++k) amp_k[k] = std::sqrt(h->list_w[k] * (double)K / wsum);
+    }
     for (int k = 0; k < K; ++k) {
-        const double th = (double)p.mod_angle0 + kTwoPi * (double)k / (double)K;
-        dx[k] = (double)p.mod_radius * std::cos(th);
-        dy[k] = (double)p.mod_radius * std::sin(th);
+        if (listed) {
+            dx[k] = h->list_dx[k];
+            dy[k] = h->list_dy[k];
+        } else {
+            const double th = (double)p.mod_angle0 + kTwoPi * (double)k / (double)K;
+            dx[k] = (double)p.mod_radius * std::cos(th);
+            dy[k] = (double)p.mod_radius * std::sin(th);
+        }
         int found = -1;
         for (size_t u = 0; u < ux.size(); ++u)
-            if (std::fabs(ux[u] - dx[k]) <= 1e-9 * std::max(1.0, (double)p.mod_radius)) { found = (int)u; break; }
+            if (std::fabs(ux[u] - dx[k]) <= 1e-9 * std::max(1.0, tmax)) { found = (int)u; break; }
         if (found < 0) { found = (int)ux.size(); ux.push_back(dx[k]); }
         jx[k] = found;
     }
@@ -256,7 +271,8 @@ int build_tables(pwfs *h) {
         for (int y = 0; y < N; ++y) {
             double turns = dy[k] * ((double)y - c) / (double)N;       // O1, y part
             turns -= std::nearbyint(turns);
-            tyt[(size_t)k * t.NP + y] = make_float2((float)std::cos(kTwoPi * turns), (float)std::sin(kTwoPi * turns));
+            tyt[(size_t)k * t.NP + y] = make_float2((float)(amp_k[k] * std::cos(kTwoPi * turns)),
+                                                    (float)(amp_k[k] * std::sin(kTwoPi * turns)));
         }
     // twiddles between the two register stages, and the 1-D mask a(u)/M (O4; 1/M = O5's scale per axis)
     std::vector<float2> tw((size_t)R1 * 32), am((size_t)R1 * 32);
@@ -268,7 +284,9 @@ int build_tables(pwfs *h) {
             const int us = u < M / 2 ? u : u - M;
             const long long num = ((long long)s * std::abs(us)) % M;
             const double am_ang = kTwoPi * (double)num / (double)M;
-            am[(size_t)k1 * 32 + n2] = make_float2((float)(std::cos(am_ang) / M), (float)(std::sin(am_ang) / M));   // table path only (s != M/4)
+            // table path only (s != M/4 or a field stop): f3's square stop |u~| <= h is separable too
+            const double pass = (h->stop_h >= 0.0 && (double)std::abs(us) > h->stop_h) ? 0.0 : 1.0;
+            am[(size_t)k1 * 32 + n2] = make_float2((float)(pass * std::cos(am_ang) / M), (float)(pass * std::sin(am_ang) / M));
         }
     // columns of the pupil plane that fall inside a window (corner-placed grid: origins M-s and s)
     std::vector<int> xc_of_x(M, -1), colx;
@@ -387,13 +405,29 @@ int pwfs_supported_grid(int32_t m_grid) {
     return find_launcher(m_grid, false, &l) ? 1 : 0;
 }
 
-int pwfs_create(const pwfs_params *p, pwfs_t **out) {
+int pwfs_create(const pwfs_params *p, pwfs_t **out) { return pwfs_create_ex(p, nullptr, out); }
+
+int pwfs_create_ex(const pwfs_params *p, const pwfs_ext *x, pwfs_t **out) {
     if (out) *out = nullptr;
     if (!p || !out || !p->pupil_amp) return PWFS_EINVAL;
     const int N = p->n_pupil, M = p->m_grid;
     if (N < 2 || M < 2 * N || (M & 1)) return PWFS_EINVAL;
-    if (p->mod_points < 1 || !(p->mod_radius >= 0.f) || !std::isfinite(p->mod_radius) || !std::isfinite(p->mod_angle0))
+    const bool listed = x && x->n_tilts > 0;
+    if (x && x->n_tilts < 0) return PWFS_EINVAL;
+    if (listed) {
+        if (!x->tilt_x || !x->tilt_y) return PWFS_EINVAL;
+        double wsum = 0.0;
+        for (int k = 0; k < x->n_tilts; ++k) {
+            if (!std::isfinite(x->tilt_x[k]) || !std::isfinite(x->tilt_y[k])) return PWFS_EINVAL;
+            const float w = x->tilt_w ? x->tilt_w[k] : 1.f;
+            if (!(w >= 0.f) || !std::isfinite(w)) return PWFS_EINVAL;
+            wsum += (double)w;
+        }
+        if (!(wsum > 0.0)) return PWFS_EINVAL;
+    } else if (p->mod_points < 1 || !(p->mod_radius >= 0.f) || !std::isfinite(p->mod_radius) || !std::isfinite(p->mod_angle0))
         return PWFS_EINVAL;
+    if (x && std::isnan(x->field_stop_px)) return PWFS_EINVAL;
+    const double stop_h = (x && x->field_stop_px >= 0.f && (double)x->field_stop_px < 0.5 * M) ? (double)x->field_stop_px : -1.0;
     if (p->n_subap < 1 || p->n_subap > N) return PWFS_EINVAL;
     if (p->slope_norm != 0 && p->slope_norm != 1) return PWFS_EINVAL;
     if (p->illum_thresh > 1.f || !std::isfinite(p->illum_thresh)) return PWFS_EINVAL;
@@ -403,11 +437,19 @@ int pwfs_create(const pwfs_params *p, pwfs_t **out) {
     for (size_t i = 0; i < (size_t)N * N; ++i)
         if (!(p->pupil_amp[i] >= 0.f) || !std::isfinite(p->pupil_amp[i])) return PWFS_EINVAL;
     Launcher L;
-    if (!find_launcher(M, 4 * s == M, &L)) return PWFS_EUNSUPPORTED;
+    const bool quarter = (4 * s == M) && stop_h < 0.0;
+    if (!find_launcher(M, quarter, &L)) return PWFS_EUNSUPPORTED;
 
     pwfs *h = new (std::nothrow) pwfs();
     if (!h) return PWFS_ENOMEM;
-    h->prm = *p; h->s = s; h->quarter = (4 * s == M); h->L = L; h->device = p->device;
+    h->prm = *p; h->s = s; h->quarter = quarter; h->L = L; h->device = p->device;
+    h->stop_h = stop_h;
+    if (listed)
+        for (int k = 0; k < x->n_tilts; ++k) {
+            h->list_dx.push_back((double)x->tilt_x[k]);
+            h->list_dy.push_back((double)x->tilt_y[k]);
+            h->list_w.push_back(x->tilt_w ? (double)x->tilt_w[k] : 1.0);
+        }
     int rc = PWFS_OK;
     cudaError_t e = cudaSetDevice(p->device);
     if (e != cudaSuccess) { h->last_cuda = (int)e; rc = PWFS_ECUDA; }

@@ -20,7 +20,7 @@ PWFS_OK, PWFS_EINVAL, PWFS_ENOMEM, PWFS_ECUDA, PWFS_EUNSUPPORTED = 0, -1, -2, -3
 NUM_KERNEL_CLASSES = 4
 KERNEL_CLASSES = ("xpass", "ypass", "xrebin", "slopes")
 
-EXPORTS = ("pwfs_create", "pwfs_info", "pwfs_valid_mask", "pwfs_run", "pwfs_run_host",
+EXPORTS = ("pwfs_create", "pwfs_create_ex", "pwfs_info", "pwfs_valid_mask", "pwfs_run", "pwfs_run_host",
            "pwfs_destroy", "pwfs_strerror", "pwfs_last_cuda_error", "pwfs_supported_grid",
            "pwfs_set_schedule", "pwfs_set_timing", "pwfs_get_timing", "pwfs_geometry")
 
@@ -30,6 +30,11 @@ class pwfs_params(C.Structure):
                 ("mask_shift_px", C.c_int32), ("mod_radius", C.c_float), ("mod_points", C.c_int32),
                 ("mod_angle0", C.c_float), ("n_subap", C.c_int32), ("illum_thresh", C.c_float),
                 ("slope_norm", C.c_int32), ("device", C.c_int32)]
+
+
+class pwfs_ext(C.Structure):
+    _fields_ = [("n_tilts", C.c_int32), ("tilt_x", C.POINTER(C.c_float)), ("tilt_y", C.POINTER(C.c_float)),
+                ("tilt_w", C.POINTER(C.c_float)), ("field_stop_px", C.c_float)]
 
 
 class PwfsError(RuntimeError):
@@ -54,6 +59,8 @@ def load_library() -> C.CDLL:
     vp, i32 = C.c_void_p, C.c_int32
     lib.pwfs_create.argtypes = [C.POINTER(pwfs_params), C.POINTER(vp)]
     lib.pwfs_create.restype = C.c_int
+    lib.pwfs_create_ex.argtypes = [C.POINTER(pwfs_params), C.POINTER(pwfs_ext), C.POINTER(vp)]
+    lib.pwfs_create_ex.restype = C.c_int
     lib.pwfs_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i32)]
     lib.pwfs_info.restype = C.c_int
     lib.pwfs_valid_mask.argtypes = [vp, vp]
@@ -95,7 +102,10 @@ class PWFS:
 
     def __init__(self, pupil_amp: np.ndarray, m_grid: int, mod_radius: float, mod_points: int,
                  n_subap: int, mask_shift_px: int = 0, mod_angle0: float = 0.0,
-                 illum_thresh: float = 0.5, slope_norm: int = 0, device: int = 0):
+                 illum_thresh: float = 0.5, slope_norm: int = 0, device: int = 0,
+                 tilt_list=None, field_stop_px: float = -1.0):
+        """tilt_list = (x, y[, w]) arrays in lambda/D replaces the modulation circle;
+        field_stop_px >= 0 adds the square focal-plane stop (include/pwfs.h, pwfs_ext)."""
         self._h = None
         self._lib = load_library()
         amp = np.ascontiguousarray(pupil_amp, dtype=np.float32)
@@ -105,7 +115,20 @@ class PWFS:
                           mask_shift_px, mod_radius, mod_points, mod_angle0, n_subap, illum_thresh,
                           slope_norm, device)
         h = C.c_void_p()
-        rc = self._lib.pwfs_create(C.byref(prm), C.byref(h))
+        if tilt_list is None and field_stop_px < 0:
+            rc = self._lib.pwfs_create(C.byref(prm), C.byref(h))
+        else:
+            fp = C.POINTER(C.c_float)
+            ext = pwfs_ext(0, None, None, None, field_stop_px)
+            if tilt_list is not None:
+                tl = [np.ascontiguousarray(a, dtype=np.float32).ravel() for a in tilt_list]
+                if len(tl) not in (2, 3) or any(a.size != tl[0].size for a in tl):
+                    raise ValueError("tilt_list must be (x, y) or (x, y, w) arrays of one length")
+                ext.n_tilts = tl[0].size
+                ext.tilt_x, ext.tilt_y = tl[0].ctypes.data_as(fp), tl[1].ctypes.data_as(fp)
+                ext.tilt_w = tl[2].ctypes.data_as(fp) if len(tl) == 3 else None
+                mod_points = tl[0].size
+            rc = self._lib.pwfs_create_ex(C.byref(prm), C.byref(ext), C.byref(h))
         if rc != PWFS_OK:
             raise PwfsError(rc, "pwfs_create", strerror(rc))
         self._h = h

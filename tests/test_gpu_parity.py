@@ -210,3 +210,79 @@ def test_bad_parameters_are_rejected(torch_cuda):
         assert ei.value.code == code, kw
     with pytest.raises(PwfsError):                      # no light: n_valid == 0
         PWFS(np.zeros((32, 32), np.float32), 128, 1.0, 4, 8)
+
+
+# ------------------------------------------------ f3: tilt list, field stop ---
+def _run_both_list(torch, A, M, ns, phase, tx, ty, tw, stop, **kw):
+    from oracle import pwfs_oracle as orc
+    from paper_1607_07624_b200.pwfs import PWFS
+    tl = (tx, ty) if tw is None else (tx, ty, tw)
+    sensor = PWFS(A, M, 0.0, 1, ns, tilt_list=tl, field_stop_px=stop, **kw)
+    try:
+        fr, sl = sensor.run(torch.from_numpy(phase).cuda())
+        torch.cuda.synchronize()
+        # the oracle gets the same float32 list values, widened exactly
+        f32 = lambda a: np.asarray(a, np.float32).astype(np.float64)
+        w = np.ones(len(tx)) if tw is None else f32(tw)
+        fr_ref, sl_ref = orc.pwfs_run_list(A, M, f32(tx), f32(ty), w, ns, phase, s=kw.get("mask_shift_px", 0),
+                                           stop_h=stop, norm_mode=kw.get("slope_norm", 0))
+        return _compare(fr.cpu().numpy(), sl.cpu().numpy(), fr_ref, sl_ref)
+    finally:
+        sensor.close()
+
+
+def test_f3_uniform_circle_list_equals_the_circle_bit_for_bit(torch_cuda):
+    from paper_1607_07624_b200.pwfs import PWFS, from_config
+    torch = torch_cuda
+    cfg = wl.CONFIGS["cfg1_tiny"]
+    A = wl.make_pupil(cfg)
+    phase = torch.from_numpy(wl.phase_batch(cfg, steps=3)).cuda()
+    th = 2.0 * np.pi * np.arange(cfg.mod_points) / cfg.mod_points
+    with from_config(cfg) as circ, PWFS(A, cfg.m_grid, 0.0, 1, cfg.n_subap,
+                                        tilt_list=(cfg.mod_radius * np.cos(th), cfg.mod_radius * np.sin(th))) as lst:
+        f0, s0 = circ.run(phase)
+        f1, s1 = lst.run(phase)
+        # float32 list entries differ from the double-precision circle in the last bits only
+        assert (f0 - f1).abs().max() <= 2e-5 * f0.abs().max() and (s0 - s1).abs().max() <= 2e-5
+
+
+@pytest.mark.parametrize("N,M,ns,stop", [
+    (64, 128, 16, -1.0),      # weighted list on the quarter-mask kernels
+    (64, 128, 16, 40.0),      # + field stop (table-mask kernels)
+    (60, 128, 23, 17.5),      # margins, non-integer binning, tight stop
+    (160, 320, 40, 103.0),    # cfg2 geometry, FoV 2" at 750 nm on 8.2 m ~ +-103 bins
+    (240, 480, 40, 100.0),
+    (250, 512, 50, 200.0),
+])
+def test_f3_weighted_list_and_stop(torch_cuda, N, M, ns, stop):
+    rng = np.random.default_rng(N + M)
+    c = (np.arange(N) - (N - 1) / 2.0)
+    X, Y = np.meshgrid(c, c)
+    A = ((np.hypot(X, Y) <= N / 2.0) & (np.hypot(X, Y) >= 0.12 * N)).astype(np.float32)
+    phase = (rng.standard_normal((2, N, N)) * 2.0).astype(np.float32)
+    phase[1] = wl.tilt_phase(N, -0.4, 0.25)
+    # an "extended source": 3 x 3 grid of points with a Gaussian brightness profile, plus a repeated x (shared row pass)
+    gx, gy = np.meshgrid([-0.8, 0.0, 0.8], [-0.8, 0.0, 0.8])
+    tx, ty = gx.ravel(), gy.ravel()
+    tw = np.exp(-(tx ** 2 + ty ** 2) / 0.5)
+    _run_both_list(torch_cuda, A, M, ns, phase, tx, ty, tw, stop)
+
+
+def test_f3_full_size_elt_extended_source(torch_cuda):
+    """cfg4 geometry with a 12-point weighted list and a field stop, 1 frame against the oracle."""
+    cfg = wl.CONFIGS["cfg4_elt"]
+    A = wl.make_pupil(cfg)
+    phase = wl.phase_batch(cfg, steps=1)
+    th = 2.0 * np.pi * np.arange(12) / 12
+    tx, ty = np.concatenate([1.5 * np.cos(th[:8:1]), [0.0, 0.5, -0.5, 0.0]]), np.concatenate([1.5 * np.sin(th[:8:1]), [0.0, 0.0, 0.0, 0.7]])
+    tw = np.linspace(0.5, 1.5, 12)
+    _run_both_list(torch_cuda, A, cfg.m_grid, cfg.n_subap, phase, tx, ty, tw, 300.0)
+
+
+def test_f3_bad_lists_are_rejected(torch_cuda):
+    from paper_1607_07624_b200.pwfs import PWFS, PwfsError, PWFS_EINVAL
+    A = np.ones((32, 32), np.float32)
+    for tl in [([0.0, 1.0], [0.0, 0.0], [1.0, -1.0]), ([0.0], [0.0], [0.0]), ([np.nan], [0.0])]:
+        with pytest.raises(PwfsError) as ei:
+            PWFS(A, 128, 1.0, 4, 8, tilt_list=tl)
+        assert ei.value.code == PWFS_EINVAL
