@@ -194,6 +194,28 @@ def phase_batch(cfg: WfsConfig, steps: Optional[int] = None, first_step: int = 0
     return out
 
 
+def atmosphere(cfg: WfsConfig) -> dict:
+    """Inputs of the f1 propagation step for a frozen-flow config: the
+    same seeded layers phase_batch() samples, stored as float32 [L][G][G] phase at 500 nm,
+    plus the geometry in plain numbers -- wind velocity vectors [m/s], layer heights [m],
+    tangents of the source directions, wavelength scale factors 500/lambda.  No
+    interpolation or shifting happens here (that is the method, not the input)."""
+    if cfg.independent_screens:
+        raise ValueError(f"{cfg.name} uses independent screens, not a frozen-flow atmosphere")
+    screens = np.stack([vk_screen(cfg.screen_px, cfg.pitch, cfg.r0_500 * w ** (-3.0 / 5.0), cfg.L0, cfg.seed + li)
+                        for li, w in enumerate(cfg.layer_weights)]).astype(np.float32)
+    wind = np.array([[v * math.cos(math.radians(d)), v * math.sin(math.radians(d))]
+                     for v, d in zip(cfg.wind_speed, cfg.wind_dir_deg)], dtype=np.float64)
+    tan_r = math.tan(cfg.star_radius_arcsec * ARCSEC)
+    dirs = np.array([[tan_r * math.cos(2.0 * math.pi * si / max(cfg.n_stars, 1)),
+                      tan_r * math.sin(2.0 * math.pi * si / max(cfg.n_stars, 1))]
+                     for si in range(cfg.n_stars)], dtype=np.float64)
+    return dict(screens=screens, pitch=cfg.pitch, wind_vxy=wind,
+                heights=np.array(cfg.layer_heights, dtype=np.float64), dirs_tan=dirs,
+                wl_scale=np.array([500.0 / lam for lam in cfg.wavelengths_nm], dtype=np.float64),
+                dt=cfg.dt, n_pupil=cfg.n_pupil)
+
+
 def tilt_phase(N: int, alpha_x: float, alpha_y: float = 0.0) -> np.ndarray:
     """Test input: a pure tilt of (alpha_x, alpha_y) lambda/D across the N-px
     pupil, phi = 2 pi (alpha_x (x-c) + alpha_y (y-c)) / N, float32."""
