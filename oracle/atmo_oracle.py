@@ -2,7 +2,7 @@
 wavefront propagation through phase screens.
 
 Plain numpy, float64, written from the definition; shares nothing with the CUDA
-path (paper_1607_07624_b200/csrc/atmo_kernels.cuh) and is imported only by
+path (paper_1607_07624_b200/csrc/atmo_api.cu) and is imported only by
 tests/, __graft_entry__.smoke() and bench.py's cpu_baseline leg.
 
 What it follows.  The paper names the object and its wiring only: "Wavefront

@@ -14,9 +14,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libpwfs.so")
-SOURCES = [os.path.join(CSRC, "pwfs_api.cu")]
+SOURCES = [os.path.join(CSRC, "pwfs_api.cu"), os.path.join(CSRC, "atmo_api.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, "pwfs_kernels.cuh"), os.path.join(CSRC, "pwfs_dft.cuh"),
-                  os.path.join(ROOT, "include", "pwfs.h")]
+                  os.path.join(ROOT, "include", "pwfs.h"), os.path.join(ROOT, "include", "pwfs_atmo.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--shared", "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]
 

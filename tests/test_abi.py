@@ -18,19 +18,43 @@ def lib():
     return pwfs.load_library()
 
 
-def _declared_functions():
-    src = open(os.path.join(ROOT, "include", "pwfs.h")).read()
+def _declared_functions(header):
+    src = open(os.path.join(ROOT, "include", header)).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(pwfs_[a-z_]+)\s*\(", src)))
 
 
 def test_header_symbols_are_exported(lib):
-    from paper_1607_07624_b200 import pwfs
-    names = _declared_functions()
-    assert len(names) >= 13 and "pwfs_create" in names and "pwfs_run" in names and "pwfs_destroy" in names
-    for n in names:
-        assert hasattr(lib, n), f"libpwfs.so does not export {n}"
-    assert sorted(pwfs.EXPORTS) == names             # the binding covers the whole header
+    from paper_1607_07624_b200 import atmo, pwfs
+    bindings = {"pwfs.h": pwfs.EXPORTS, "pwfs_atmo.h": atmo.EXPORTS}
+    assert sorted(os.listdir(os.path.join(ROOT, "include"))) == sorted(bindings)
+    for header, exports in bindings.items():
+        names = _declared_functions(header)
+        for n in names:
+            assert hasattr(lib, n), f"libpwfs.so does not export {n}"
+        assert sorted(exports) == names, header       # the binding covers the whole header
+    names = _declared_functions("pwfs.h")
+    assert len(names) >= 14 and "pwfs_create" in names and "pwfs_run" in names and "pwfs_destroy" in names
+
+
+def test_atmo_entry_points_reject_bad_arguments_without_a_device(lib):
+    from paper_1607_07624_b200 import atmo, pwfs
+    atmo._lib()
+    h = C.c_void_p()
+    assert lib.pwfs_atmo_create(None, C.byref(h)) == pwfs.PWFS_EINVAL
+    scr = np.zeros((1, 8, 8), np.float32)
+    z2, z1, one = np.zeros(2), np.zeros(1), np.ones(1)
+    dp, fp = C.POINTER(C.c_double), C.POINTER(C.c_float)
+    mk = lambda **kw: atmo.pwfs_atmo_params(**{**dict(
+        n_layers=1, screen_px=8, screens=scr.ctypes.data_as(fp), pitch=0.1, wind_vxy=z2.ctypes.data_as(dp),
+        heights=z1.ctypes.data_as(dp), n_dirs=1, dirs_tan=z2.ctypes.data_as(dp), n_wl=1,
+        wl_scale=one.ctypes.data_as(dp), n_pupil=8, device=0), **kw})
+    for bad in (dict(n_layers=0), dict(n_pupil=9), dict(pitch=0.0), dict(n_dirs=0), dict(n_wl=0), dict(pitch=float("nan"))):
+        prm = mk(**bad)
+        assert lib.pwfs_atmo_create(C.byref(prm), C.byref(h)) == pwfs.PWFS_EINVAL, bad
+        assert h.value is None
+    lib.pwfs_atmo_destroy(None)
+    assert lib.pwfs_atmo_propagate(None, 0, 1, 1e-3, None, None) == pwfs.PWFS_EINVAL
 
 
 def test_params_struct_layout_matches_header():
@@ -90,6 +114,7 @@ def test_product_path_does_not_touch_the_oracle():
         for fn in files:
             if fn.endswith((".py", ".cu", ".cuh", ".h")):
                 txt = open(os.path.join(dirpath, fn)).read()
-                assert "pwfs_oracle" not in txt and "from oracle" not in txt and "import oracle" not in txt, fn
-    otxt = open(os.path.join(ROOT, "oracle", "pwfs_oracle.py")).read() + open(os.path.join(ROOT, "oracle", "pwfs_oracle.c")).read()
+                assert "_oracle" not in txt and "from oracle" not in txt and "import oracle" not in txt, fn
+    otxt = "".join(open(os.path.join(ROOT, "oracle", fn)).read() for fn in os.listdir(os.path.join(ROOT, "oracle"))
+                   if fn.endswith((".py", ".c", ".h")))
     assert "import paper_1607_07624_b200" not in otxt and "from paper_1607_07624_b200" not in otxt and "libpwfs.so" not in otxt
