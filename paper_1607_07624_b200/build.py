@@ -9,16 +9,18 @@ from __future__ import annotations
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libpwfs.so")
-SOURCES = [os.path.join(CSRC, "pwfs_api.cu"), os.path.join(CSRC, "atmo_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "pwfs_kernels.cuh"), os.path.join(CSRC, "pwfs_dft.cuh"),
-                  os.path.join(ROOT, "include", "pwfs.h"), os.path.join(ROOT, "include", "pwfs_atmo.h")]
+SOURCES = [os.path.join(CSRC, n) for n in ("pwfs_api.cu", "atmo_api.cu", "chain_api.cu")]
+HEADERS = [os.path.join(CSRC, "pwfs_kernels.cuh"), os.path.join(CSRC, "pwfs_dft.cuh")] + \
+          [os.path.join(ROOT, "include", n) for n in ("pwfs.h", "pwfs_atmo.h", "pwfs_chain.h")]
+OBJDIR = os.path.join(HERE, "build")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "--shared", "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]
+              "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]
 
 
 def nvcc_path() -> str:
@@ -28,18 +30,34 @@ def nvcc_path() -> str:
     return "nvcc"
 
 
+def _newer(target: str, deps) -> bool:
+    return os.path.exists(target) and all(os.path.getmtime(target) >= os.path.getmtime(d) for d in deps)
+
+
 def up_to_date() -> bool:
-    return os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS)
+    return _newer(LIB, SOURCES + HEADERS)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and up_to_date():
-        return LIB
-    tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [nvcc_path()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
+def _compile(src: str, force: bool, verbose: bool) -> str:
+    obj = os.path.join(OBJDIR, os.path.basename(src)[:-3] + ".o")
+    if not force and _newer(obj, [src] + HEADERS):
+        return obj
+    cmd = [nvcc_path()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, src]
     if verbose:
         print(" ".join(cmd), flush=True)
     subprocess.run(cmd, check=True)
+    return obj
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    """One nvcc -c per source (in parallel; unchanged objects are kept), then one link."""
+    if not force and up_to_date():
+        return LIB
+    os.makedirs(OBJDIR, exist_ok=True)
+    with ThreadPoolExecutor(max_workers=len(SOURCES)) as pool:
+        objs = list(pool.map(lambda s: _compile(s, force, verbose), SOURCES))
+    tmp = LIB + f".tmp{os.getpid()}"
+    subprocess.run([nvcc_path(), "--shared", "-o", tmp] + objs, check=True)
     os.replace(tmp, LIB)
     return LIB
 

@@ -25,8 +25,8 @@ def _declared_functions(header):
 
 
 def test_header_symbols_are_exported(lib):
-    from paper_1607_07624_b200 import atmo, pwfs
-    bindings = {"pwfs.h": pwfs.EXPORTS, "pwfs_atmo.h": atmo.EXPORTS}
+    from paper_1607_07624_b200 import atmo, chain, pwfs
+    bindings = {"pwfs.h": pwfs.EXPORTS, "pwfs_atmo.h": atmo.EXPORTS, "pwfs_chain.h": chain.EXPORTS}
     assert sorted(os.listdir(os.path.join(ROOT, "include"))) == sorted(bindings)
     for header, exports in bindings.items():
         names = _declared_functions(header)
@@ -55,6 +55,51 @@ def test_atmo_entry_points_reject_bad_arguments_without_a_device(lib):
         assert h.value is None
     lib.pwfs_atmo_destroy(None)
     assert lib.pwfs_atmo_propagate(None, 0, 1, 1e-3, None, None) == pwfs.PWFS_EINVAL
+
+
+def test_chain_entry_points_reject_bad_arguments_without_a_device(lib):
+    from paper_1607_07624_b200 import chain, pwfs
+    chain._lib()
+    h = C.c_void_p()
+    mk = lambda **kw: chain.pwfs_ccd_params(**{**dict(det_size=8, n_inst=1, n_int=1, gain=1.0, quantum_eff=0.5,
+                                                      photon_noise=1, readout_noise=1, readout_level=1.0, seed=1,
+                                                      device=0), **kw})
+    assert lib.pwfs_ccd_create(None, C.byref(h)) == pwfs.PWFS_EINVAL
+    for bad in (dict(det_size=0), dict(n_inst=0), dict(n_int=0), dict(gain=-1.0), dict(quantum_eff=1.5),
+                dict(readout_level=float("nan")), dict(gain=float("inf"))):
+        prm = mk(**bad)
+        assert lib.pwfs_ccd_create(C.byref(prm), C.byref(h)) == pwfs.PWFS_EINVAL, bad
+        assert h.value is None
+    assert lib.pwfs_ccd_run(None, None, 1, 0, None, None) == pwfs.PWFS_EINVAL
+    v = np.zeros((4, 4), np.uint8)
+    assert lib.pwfs_slopec_create(4, C.c_void_p(v.ctypes.data), 0, None, 0, C.byref(h)) == pwfs.PWFS_EINVAL   # none valid
+    v[1, 1] = 1
+    assert lib.pwfs_slopec_create(4, C.c_void_p(v.ctypes.data), 2, None, 0, C.byref(h)) == pwfs.PWFS_EINVAL   # bad norm
+    assert lib.pwfs_slopec_create(0, C.c_void_p(v.ctypes.data), 0, None, 0, C.byref(h)) == pwfs.PWFS_EINVAL
+    assert lib.pwfs_slopec_run(None, None, 1, None, None) == pwfs.PWFS_EINVAL
+    assert lib.pwfs_rec_create(0, 4, C.c_void_p(v.ctypes.data), 0, C.byref(h)) == pwfs.PWFS_EINVAL
+    assert lib.pwfs_rec_create(4, 4, None, 0, C.byref(h)) == pwfs.PWFS_EINVAL
+    assert lib.pwfs_rec_run(None, None, 1, None, None) == pwfs.PWFS_EINVAL
+    for n in ("pwfs_ccd_destroy", "pwfs_slopec_destroy", "pwfs_rec_destroy"):
+        getattr(lib, n)(None)                                                    # NULL-safe
+    import torch
+    if not torch.cuda.is_available():                                            # no device: loud failure, no fallback
+        prm = mk()
+        assert lib.pwfs_ccd_create(C.byref(prm), C.byref(h)) == pwfs.PWFS_ECUDA
+        R = np.ones((2, 4), np.float32)
+        assert lib.pwfs_rec_create(2, 4, C.c_void_p(R.ctypes.data), 0, C.byref(h)) in (pwfs.PWFS_ECUDA, pwfs.PWFS_ENOMEM)
+        assert lib.pwfs_slopec_create(4, C.c_void_p(v.ctypes.data), 0, None, 0, C.byref(h)) in (pwfs.PWFS_ECUDA, pwfs.PWFS_ENOMEM)
+        assert h.value is None
+
+
+def test_ccd_params_struct_layout_matches_header():
+    from paper_1607_07624_b200.chain import pwfs_ccd_params
+    src = open(os.path.join(ROOT, "include", "pwfs_chain.h")).read()
+    body = src[src.index("typedef struct {"):src.index("} pwfs_ccd_params;")]
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    declared = re.findall(r"\b(?:int32_t|uint64_t|double)\s*(\w+);", body)
+    assert declared == [f[0] for f in pwfs_ccd_params._fields_]
+    assert C.sizeof(pwfs_ccd_params) == 64
 
 
 def test_params_struct_layout_matches_header():
