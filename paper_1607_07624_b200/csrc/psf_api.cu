@@ -1,0 +1,375 @@
+// psf_api.cu -- f4, PSF camera: C ABI of include/pwfs_psf.h and its kernels.
+//
+// PSF = |DFT2(A exp(i c phi))|^2 on an M x M grid, M = 32 R1 >= 2N.  Same 1-D engine as the
+// pyramid path (pwfs_kernels.cuh): one warp = one length-M transform, a zero-pad-pruned DFT of
+// size R1 in registers, one exchange through padded shared memory, a DFT of size 32 -- but
+// forward only, so the result stays in the "k1 + R1 k2" register order and is consumed there.
+//
+//   psf_row_kernel   N pupil rows per frame: phasor (phase rescaled to the imaging wavelength)
+//                    -> DFT over x -> T[f][u][y], transposed through shared memory so that the
+//                    column pass reads 128-byte lines.
+//   psf_col_kernel   one warp per NB columns u, looping over its share of the frames: DFT over
+//                    y (only the N non-zero inputs are read), |.|^2 accumulated over the frames in
+//                    registers; Strehl ratio from the (0,0) bin; one partial PSF per frame split.
+//   psf_fold_kernel  accumulator += sum of the partial PSFs (fixed order: deterministic).
+//   psf_read_kernel  long exposure = accumulator / (frames M^2 sum A^2).
+// Work per frame: (N + M) transforms of length M; HBM: phase in, T out and back, nothing else.
+#include "../../include/pwfs_psf.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <new>
+#include <vector>
+
+#include "pwfs_dft.cuh"
+
+using namespace pwk;
+
+namespace {
+
+constexpr int kPitchP = 33;                         // float2 pitch of an exchange row (conflict-free 64-bit)
+constexpr float kInv2PiHiP = 0.15915493667125702f;  // fl32(1/(2 pi))
+constexpr float kInv2PiLoP = 6.4206382e-09f;        // 1/(2 pi) - hi
+
+template <int R1_, int NB_, int WPB_>
+struct PsfCfg {
+    static constexpr int R1 = R1_, NB = NB_, WPB = WPB_;
+    static constexpr int M = 32 * R1_;
+    static constexpr int NZ = (R1_ + 1) / 2;         // M >= 2N: at most ceil(R1/2) non-zero inputs per lane
+    static constexpr int ITEMS = NB_ * R1_;          // size-32 DFTs per warp batch
+    static_assert(ITEMS <= 32, "one size-32 DFT per lane");
+    static constexpr int WARP_BUF = ITEMS * kPitchP + 1;
+    static constexpr int TAB = R1_ * kPitchP;
+    static constexpr int RPC = NB_ * WPB_;           // rows per CTA, row pass
+    static constexpr size_t smem = (size_t)(TAB + WPB_ * WARP_BUF) * sizeof(float2);
+};
+
+struct PsfDev {
+    int N, M, NP;            // NP = N rounded up to 32
+    float scale;             // phase_scale
+    float inv_sumA_sq;       // 1 / (sum A)^2
+    const float *amp;        // [N][N]
+    const float2 *tw;        // [R1][32] exp(-2 pi i k1 n2 / M)
+};
+
+template <class C>
+__device__ __forceinline__ void load_tw(float2 *s_tw, const PsfDev &t) {
+    for (int i = threadIdx.x; i < C::R1 * 32; i += blockDim.x) s_tw[(i >> 5) * kPitchP + (i & 31)] = __ldg(t.tw + i);
+}
+
+// grid (ceil(NP / RPC), F); block 32 * WPB.
+template <class C>
+__global__ void __launch_bounds__(32 * C::WPB)
+psf_row_kernel(PsfDev t, const float *__restrict__ phase, float2 *__restrict__ T) {
+    extern __shared__ float2 smem[];
+    float2 *s_tw = smem, *s_buf = smem + C::TAB;
+    const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
+    const int N = t.N, f = blockIdx.y, y0 = blockIdx.x * C::RPC;
+    float2 *buf = s_buf + wl * C::WARP_BUF;
+    load_tw<C>(s_tw, t);
+#pragma unroll
+    for (int b = 0; b < C::NB; ++b) {
+        const int y = y0 + wl * C::NB + b;
+        float2 v[C::R1];
+#pragma unroll
+        for (int n1 = 0; n1 < C::NZ; ++n1) {
+            const int x = 32 * n1 + lane;
+            const bool ok = (y < N) && (x < N);
+            const float ph = ok ? __ldg(phase + ((size_t)f * N + y) * N + x) * t.scale : 0.f;
+            const float am = ok ? __ldg(t.amp + (size_t)y * N + x) : 0.f;
+            // phase in turns, reduced with a two-term 1/(2 pi) (exact integer part, FMA keeps the low bits)
+            const float q = rintf(ph * kInv2PiHiP);
+            float tr = fmaf(ph, kInv2PiHiP, -q);
+            tr = fmaf(ph, kInv2PiLoP, tr);
+            float sn, cs;
+            __sincosf(tr * 6.283185307179586f, &sn, &cs);
+            v[n1] = make_float2(am * cs, am * sn);
+        }
+        DftP<C::R1, -1, C::NZ>::run(v);
+#pragma unroll
+        for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitchP + lane] = v[k1];
+    }
+    __syncthreads();
+    if (lane < C::ITEMS) {
+        const int k1 = lane % C::R1;
+        float2 *row = buf + lane * kPitchP;
+        const float2 *twr = s_tw + k1 * kPitchP;
+        float2 u[32];
+#pragma unroll
+        for (int n2 = 0; n2 < 32; ++n2) u[n2] = cmul(row[n2], twr[n2]);
+        Dft<32, -1>::run(u);
+#pragma unroll
+        for (int k2 = 0; k2 < 32; ++k2) row[k2] = u[k2];
+    }
+    __syncthreads();
+    // X[u = k1 + R1 k2] of CTA row r sits at s_buf[(r/NB) WARP_BUF + ((r%NB) R1 + k1) pitch + k2];
+    // adjacent threads take adjacent rows y of one u: runs of RPC * 8 bytes in T[f][u][y]
+    float2 *Tf = T + (size_t)f * C::M * t.NP;
+    for (int i = threadIdx.x; i < C::RPC * C::M; i += 32 * C::WPB) {
+        const int r = i % C::RPC, uu = i / C::RPC;
+        const int k1 = uu % C::R1, k2 = uu / C::R1;
+        if (y0 + r < t.NP)
+            Tf[(size_t)uu * t.NP + y0 + r] = s_buf[(r / C::NB) * C::WARP_BUF + ((r % C::NB) * C::R1 + k1) * kPitchP + k2];
+    }
+}
+
+// grid (ceil(M / (NB * WPB)), fsplit); block 32 * WPB.  partial: [fsplit][M][M] (fftshifted).
+template <class C>
+__global__ void __launch_bounds__(32 * C::WPB)
+psf_col_kernel(PsfDev t, const float2 *__restrict__ T, int F, int fsplit, float *__restrict__ partial,
+               float *__restrict__ sr) {
+    extern __shared__ float2 smem[];
+    float2 *s_tw = smem, *s_buf = smem + C::TAB;
+    const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
+    const int NP = t.NP, fs = blockIdx.y;
+    const int u0 = (blockIdx.x * C::WPB + wl) * C::NB;
+    float2 *buf = s_buf + wl * C::WARP_BUF;
+    load_tw<C>(s_tw, t);
+    __syncthreads();
+    if (u0 >= C::M) return;
+    const int f_lo = (int)(((long long)fs * F) / fsplit), f_hi = (int)(((long long)(fs + 1) * F) / fsplit);
+    float acc[32];
+#pragma unroll
+    for (int k2 = 0; k2 < 32; ++k2) acc[k2] = 0.f;
+    float2 pre[C::NB][C::NZ];
+    auto fetch = [&](int f) {
+        const float2 *src = T + ((size_t)f * C::M + u0) * NP + lane;
+#pragma unroll
+        for (int b = 0; b < C::NB; ++b)
+#pragma unroll
+            for (int n1 = 0; n1 < C::NZ; ++n1)
+                pre[b][n1] = (32 * n1 < NP && u0 + b < C::M) ? __ldg(src + (size_t)b * NP + 32 * n1) : make_float2(0.f, 0.f);
+    };
+    if (f_lo < f_hi) fetch(f_lo);
+    const int my_b = lane / C::R1, my_k1 = lane % C::R1;
+    for (int f = f_lo; f < f_hi; ++f) {
+#pragma unroll
+        for (int b = 0; b < C::NB; ++b) {
+            float2 v[C::R1];
+#pragma unroll
+            for (int n1 = 0; n1 < C::NZ; ++n1) v[n1] = pre[b][n1];
+            if (b == C::NB - 1 && f + 1 < f_hi) fetch(f + 1);
+            DftP<C::R1, -1, C::NZ>::run(v);
+#pragma unroll
+            for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitchP + lane] = v[k1];
+        }
+        __syncwarp();
+        if (lane < C::ITEMS) {
+            const float2 *row = buf + lane * kPitchP;
+            const float2 *twr = s_tw + my_k1 * kPitchP;
+            float2 u[32];
+#pragma unroll
+            for (int n2 = 0; n2 < 32; ++n2) u[n2] = cmul(row[n2], twr[n2]);
+            Dft<32, -1>::run(u);
+#pragma unroll
+            for (int k2 = 0; k2 < 32; ++k2) acc[k2] = fmaf(u[k2].x, u[k2].x, fmaf(u[k2].y, u[k2].y, acc[k2]));
+            if (sr && my_k1 == 0 && u0 + my_b == 0)          // F4c: the (0, 0) bin
+                sr[f] = fmaf(u[0].x, u[0].x, u[0].y * u[0].y) * t.inv_sumA_sq;
+        }
+        __syncwarp();
+    }
+    if (lane < C::ITEMS && u0 + my_b < C::M) {
+        const int uo = (u0 + my_b + C::M / 2) % C::M;
+        float *dst = partial + (size_t)fs * C::M * C::M + uo;
+#pragma unroll
+        for (int k2 = 0; k2 < 32; ++k2) {
+            const int vo = (my_k1 + C::R1 * k2 + C::M / 2) % C::M;
+            dst[(size_t)vo * C::M] = acc[k2];
+        }
+    }
+}
+
+__global__ void psf_fold_kernel(float *__restrict__ accum, const float *__restrict__ partial, int fsplit, size_t MM) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= MM) return;
+    float s = accum[i];
+    for (int k = 0; k < fsplit; ++k) s += __ldg(partial + (size_t)k * MM + i);
+    accum[i] = s;
+}
+
+__global__ void psf_read_kernel(const float *__restrict__ accum, float *__restrict__ out, float scale, size_t MM) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < MM) out[i] = accum[i] * scale;
+}
+
+struct PsfLauncher {
+    int NB, WPB, RPC;
+    size_t smem;
+    void (*row)(dim3, cudaStream_t, const PsfDev &, const float *, float2 *);
+    void (*col)(dim3, cudaStream_t, const PsfDev &, const float2 *, int, int, float *, float *);
+    cudaError_t (*prepare)();
+};
+
+template <class C>
+void row_t(dim3 g, cudaStream_t st, const PsfDev &t, const float *ph, float2 *T) {
+    psf_row_kernel<C><<<g, 32 * C::WPB, C::smem, st>>>(t, ph, T);
+}
+template <class C>
+void col_t(dim3 g, cudaStream_t st, const PsfDev &t, const float2 *T, int F, int fsplit, float *part, float *sr) {
+    psf_col_kernel<C><<<g, 32 * C::WPB, C::smem, st>>>(t, T, F, fsplit, part, sr);
+}
+template <class C>
+cudaError_t prepare_t() {
+    cudaError_t e = cudaFuncSetAttribute(psf_row_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(psf_col_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem);
+    return e;
+}
+template <class C>
+PsfLauncher make() { return PsfLauncher{C::NB, C::WPB, C::RPC, C::smem, row_t<C>, col_t<C>, prepare_t<C>}; }
+
+bool find_psf_launcher(int M, PsfLauncher *out) {
+    if (M % 32) return false;
+    switch (M / 32) {
+        case 4:  *out = make<PsfCfg<4, 8, 4>>(); return true;
+        case 8:  *out = make<PsfCfg<8, 4, 4>>(); return true;
+        case 10: *out = make<PsfCfg<10, 3, 4>>(); return true;
+        case 15: *out = make<PsfCfg<15, 2, 4>>(); return true;
+        case 16: *out = make<PsfCfg<16, 2, 4>>(); return true;
+        case 20: *out = make<PsfCfg<20, 1, 8>>(); return true;
+        case 25: *out = make<PsfCfg<25, 1, 8>>(); return true;
+        case 32: *out = make<PsfCfg<32, 1, 8>>(); return true;
+        default: return false;
+    }
+}
+
+int cuda_rc(cudaError_t e) { return e == cudaErrorMemoryAllocation ? PWFS_ENOMEM : PWFS_ECUDA; }
+
+}  // namespace
+
+struct pwfs_psf {
+    int device = 0;
+    PsfDev dev{};
+    PsfLauncher L{};
+    double sumA2 = 0.0;
+    float *d_amp = nullptr;
+    float2 *d_tw = nullptr;
+    float *d_acc = nullptr;          // [M][M] sum over frames of |X|^2, fftshifted
+    float2 *T = nullptr; size_t T_frames = 0;
+    float *partial = nullptr; int partial_split = 0;
+    long long count = 0;
+    int num_sms = 148;
+    size_t scratch_budget = (size_t)2 << 30;
+};
+
+extern "C" {
+
+int pwfs_psf_create(const pwfs_psf_params *p, pwfs_psf_t **out) {
+    if (out) *out = nullptr;
+    if (!p || !out || !p->pupil_amp) return PWFS_EINVAL;
+    const int N = p->n_pupil, M = p->m_grid;
+    if (N < 2 || M < 2 * N || !std::isfinite(p->phase_scale)) return PWFS_EINVAL;
+    PsfLauncher L;
+    if (!find_psf_launcher(M, &L)) return PWFS_EUNSUPPORTED;
+    double sumA = 0.0, sumA2 = 0.0;
+    for (size_t i = 0; i < (size_t)N * N; ++i) {
+        const double a = p->pupil_amp[i];
+        if (!(a >= 0.0) || !std::isfinite(a)) return PWFS_EINVAL;
+        sumA += a; sumA2 += a * a;
+    }
+    if (!(sumA > 0.0)) return PWFS_EINVAL;
+    const int R1 = M / 32;
+    std::vector<float2> tw((size_t)R1 * 32);
+    for (int k1 = 0; k1 < R1; ++k1)
+        for (int n2 = 0; n2 < 32; ++n2) {
+            const double a = -6.283185307179586476925286766559 * (double)((long long)k1 * n2 % M) / (double)M;
+            tw[(size_t)k1 * 32 + n2] = make_float2((float)std::cos(a), (float)std::sin(a));
+        }
+    pwfs_psf *h = new (std::nothrow) pwfs_psf();
+    if (!h) return PWFS_ENOMEM;
+    h->device = p->device; h->L = L; h->sumA2 = sumA2;
+    const size_t MM = (size_t)M * M;
+    cudaError_t e = cudaSetDevice(p->device);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_amp, (size_t)N * N * sizeof(float));
+    if (e == cudaSuccess) e = cudaMemcpy(h->d_amp, p->pupil_amp, (size_t)N * N * sizeof(float), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_tw, tw.size() * sizeof(float2));
+    if (e == cudaSuccess) e = cudaMemcpy(h->d_tw, tw.data(), tw.size() * sizeof(float2), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_acc, MM * sizeof(float));
+    if (e == cudaSuccess) e = cudaMemset(h->d_acc, 0, MM * sizeof(float));
+    if (e == cudaSuccess) e = L.prepare();
+    if (e == cudaSuccess) {
+        int sms = 0;
+        if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, p->device) == cudaSuccess && sms > 0) h->num_sms = sms;
+    }
+    if (e != cudaSuccess) { int rc = cuda_rc(e); pwfs_psf_destroy(h); return rc; }
+    PsfDev &d = h->dev;
+    d.N = N; d.M = M; d.NP = (N + 31) / 32 * 32;
+    d.scale = p->phase_scale;
+    d.inv_sumA_sq = (float)(1.0 / (sumA * sumA));
+    d.amp = h->d_amp; d.tw = h->d_tw;
+    *out = h;
+    return PWFS_OK;
+}
+
+int pwfs_psf_accumulate(pwfs_psf_t *h, const float *d_phase, int32_t B, float *d_sr, void *cuda_stream) {
+    if (!h || B < 0) return PWFS_EINVAL;
+    if (B == 0) return PWFS_OK;
+    if (!d_phase) return PWFS_EINVAL;
+    if (cudaSetDevice(h->device) != cudaSuccess) return PWFS_ECUDA;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const PsfDev &d = h->dev;
+    const PsfLauncher &L = h->L;
+    const size_t MM = (size_t)d.M * d.M, per_frame = (size_t)d.M * d.NP * sizeof(float2);
+    const int F = (int)std::min<size_t>((size_t)B, std::max<size_t>(1, h->scratch_budget / per_frame));
+    // column pass: ~32 warps per SM in flight; the frame loop is split only as far as that needs
+    const int col_ctas = (d.M + L.NB * L.WPB - 1) / (L.NB * L.WPB);
+    int fsplit = (32 * h->num_sms + col_ctas * L.WPB - 1) / (col_ctas * L.WPB);
+    fsplit = std::max(1, std::min(fsplit, F));
+    if ((size_t)F > h->T_frames) {
+        if (h->T) cudaFree(h->T);
+        h->T = nullptr; h->T_frames = 0;
+        cudaError_t e = cudaMalloc((void **)&h->T, (size_t)F * per_frame);
+        if (e != cudaSuccess) return cuda_rc(e);
+        h->T_frames = (size_t)F;
+    }
+    if (fsplit > h->partial_split) {
+        if (h->partial) cudaFree(h->partial);
+        h->partial = nullptr; h->partial_split = 0;
+        cudaError_t e = cudaMalloc((void **)&h->partial, (size_t)fsplit * MM * sizeof(float));
+        if (e != cudaSuccess) return cuda_rc(e);
+        h->partial_split = fsplit;
+    }
+    for (int f0 = 0; f0 < B; f0 += F) {
+        const int Fc = std::min(F, B - f0);
+        const int fsp = std::min(fsplit, Fc);
+        L.row(dim3((d.NP + L.RPC - 1) / L.RPC, Fc), st, d, d_phase + (size_t)f0 * d.N * d.N, h->T);
+        L.col(dim3(col_ctas, fsp), st, d, h->T, Fc, fsp, h->partial, d_sr ? d_sr + f0 : nullptr);
+        psf_fold_kernel<<<(unsigned)((MM + 255) / 256), 256, 0, st>>>(h->d_acc, h->partial, fsp, MM);
+    }
+    if (cudaGetLastError() != cudaSuccess) return PWFS_ECUDA;
+    h->count += B;
+    return PWFS_OK;
+}
+
+int pwfs_psf_read(pwfs_psf_t *h, float *d_psf, int64_t *frames_out, void *cuda_stream) {
+    if (!h || !d_psf) return PWFS_EINVAL;
+    if (cudaSetDevice(h->device) != cudaSuccess) return PWFS_ECUDA;
+    const size_t MM = (size_t)h->dev.M * h->dev.M;
+    const double scale = h->count > 0 ? 1.0 / ((double)h->count * (double)MM * h->sumA2) : 0.0;
+    psf_read_kernel<<<(unsigned)((MM + 255) / 256), 256, 0, (cudaStream_t)cuda_stream>>>(h->d_acc, d_psf, (float)scale, MM);
+    if (frames_out) *frames_out = h->count;
+    return cudaGetLastError() == cudaSuccess ? PWFS_OK : PWFS_ECUDA;
+}
+
+int pwfs_psf_reset(pwfs_psf_t *h, void *cuda_stream) {
+    if (!h) return PWFS_EINVAL;
+    if (cudaSetDevice(h->device) != cudaSuccess) return PWFS_ECUDA;
+    const size_t MM = (size_t)h->dev.M * h->dev.M;
+    if (cudaMemsetAsync(h->d_acc, 0, MM * sizeof(float), (cudaStream_t)cuda_stream) != cudaSuccess) return PWFS_ECUDA;
+    h->count = 0;
+    return PWFS_OK;
+}
+
+void pwfs_psf_destroy(pwfs_psf_t *h) {
+    if (!h) return;
+    cudaSetDevice(h->device);
+    if (h->d_amp) cudaFree(h->d_amp);
+    if (h->d_tw) cudaFree(h->d_tw);
+    if (h->d_acc) cudaFree(h->d_acc);
+    if (h->T) cudaFree(h->T);
+    if (h->partial) cudaFree(h->partial);
+    delete h;
+}
+
+}  // extern "C"

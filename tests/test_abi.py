@@ -25,8 +25,9 @@ def _declared_functions(header):
 
 
 def test_header_symbols_are_exported(lib):
-    from paper_1607_07624_b200 import atmo, chain, pwfs
-    bindings = {"pwfs.h": pwfs.EXPORTS, "pwfs_atmo.h": atmo.EXPORTS, "pwfs_chain.h": chain.EXPORTS}
+    from paper_1607_07624_b200 import atmo, chain, psf, pwfs
+    bindings = {"pwfs.h": pwfs.EXPORTS, "pwfs_atmo.h": atmo.EXPORTS, "pwfs_chain.h": chain.EXPORTS,
+                "pwfs_psf.h": psf.EXPORTS}
     assert sorted(os.listdir(os.path.join(ROOT, "include"))) == sorted(bindings)
     for header, exports in bindings.items():
         names = _declared_functions(header)
@@ -89,6 +90,32 @@ def test_chain_entry_points_reject_bad_arguments_without_a_device(lib):
         R = np.ones((2, 4), np.float32)
         assert lib.pwfs_rec_create(2, 4, C.c_void_p(R.ctypes.data), 0, C.byref(h)) in (pwfs.PWFS_ECUDA, pwfs.PWFS_ENOMEM)
         assert lib.pwfs_slopec_create(4, C.c_void_p(v.ctypes.data), 0, None, 0, C.byref(h)) in (pwfs.PWFS_ECUDA, pwfs.PWFS_ENOMEM)
+        assert h.value is None
+
+
+def test_psf_entry_points_reject_bad_arguments_without_a_device(lib):
+    from paper_1607_07624_b200 import psf, pwfs
+    psf._lib()
+    h = C.c_void_p()
+    amp = np.ones((16, 16), np.float32)
+    fp = C.POINTER(C.c_float)
+    mk = lambda **kw: psf.pwfs_psf_params(**{**dict(n_pupil=16, m_grid=128, pupil_amp=amp.ctypes.data_as(fp),
+                                                    phase_scale=1.0, device=0), **kw})
+    assert lib.pwfs_psf_create(None, C.byref(h)) == pwfs.PWFS_EINVAL
+    for bad, code in ((dict(n_pupil=1), pwfs.PWFS_EINVAL), (dict(n_pupil=100), pwfs.PWFS_EINVAL),      # M < 2N
+                      (dict(m_grid=96), pwfs.PWFS_EUNSUPPORTED), (dict(phase_scale=float("nan")), pwfs.PWFS_EINVAL),
+                      (dict(pupil_amp=(0 * amp).ctypes.data_as(fp)), pwfs.PWFS_EINVAL)):
+        prm = mk(**bad)
+        assert lib.pwfs_psf_create(C.byref(prm), C.byref(h)) == code, bad
+        assert h.value is None
+    assert lib.pwfs_psf_accumulate(None, None, 1, None, None) == pwfs.PWFS_EINVAL
+    assert lib.pwfs_psf_read(None, None, None, None) == pwfs.PWFS_EINVAL
+    assert lib.pwfs_psf_reset(None, None) == pwfs.PWFS_EINVAL
+    lib.pwfs_psf_destroy(None)
+    import torch
+    if not torch.cuda.is_available():
+        prm = mk()
+        assert lib.pwfs_psf_create(C.byref(prm), C.byref(h)) in (pwfs.PWFS_ECUDA, pwfs.PWFS_ENOMEM)
         assert h.value is None
 
 
