@@ -25,9 +25,9 @@ def _declared_functions(header):
 
 
 def test_header_symbols_are_exported(lib):
-    from paper_1607_07624_b200 import atmo, chain, psf, pwfs
+    from paper_1607_07624_b200 import atmo, chain, psf, pwfs, sh
     bindings = {"pwfs.h": pwfs.EXPORTS, "pwfs_atmo.h": atmo.EXPORTS, "pwfs_chain.h": chain.EXPORTS,
-                "pwfs_psf.h": psf.EXPORTS}
+                "pwfs_psf.h": psf.EXPORTS, "pwfs_sh.h": sh.EXPORTS}
     assert sorted(os.listdir(os.path.join(ROOT, "include"))) == sorted(bindings)
     for header, exports in bindings.items():
         names = _declared_functions(header)
@@ -116,6 +116,35 @@ def test_psf_entry_points_reject_bad_arguments_without_a_device(lib):
     if not torch.cuda.is_available():
         prm = mk()
         assert lib.pwfs_psf_create(C.byref(prm), C.byref(h)) in (pwfs.PWFS_ECUDA, pwfs.PWFS_ENOMEM)
+        assert h.value is None
+
+
+def test_sh_entry_points_reject_bad_arguments_without_a_device(lib):
+    from paper_1607_07624_b200 import pwfs, sh
+    sh._lib()
+    h = C.c_void_p()
+    amp = np.ones((16, 16), np.float32)
+    fp = C.POINTER(C.c_float)
+    mk = lambda **kw: sh.pwfs_sh_params(**{**dict(n_pupil=16, n_subap=4, pupil_amp=amp.ctypes.data_as(fp), fft_px=8,
+                                                  n_px=4, bin=2, illum_thresh=0.5, phase_scale=1.0, device=0), **kw})
+    assert lib.pwfs_sh_create(None, C.byref(h)) == pwfs.PWFS_EINVAL
+    for bad, code in ((dict(n_subap=5), pwfs.PWFS_EINVAL), (dict(fft_px=7), pwfs.PWFS_EINVAL),
+                      (dict(fft_px=2), pwfs.PWFS_EINVAL),                      # P < b
+                      (dict(n_px=5, bin=2), pwfs.PWFS_EINVAL),                 # window larger than the FFT grid
+                      (dict(n_px=3, bin=1), pwfs.PWFS_EINVAL),                 # parity
+                      (dict(fft_px=128), pwfs.PWFS_EUNSUPPORTED),
+                      (dict(pupil_amp=(0 * amp).ctypes.data_as(fp)), pwfs.PWFS_EINVAL)):
+        prm = mk(**bad)
+        assert lib.pwfs_sh_create(C.byref(prm), C.byref(h)) == code, bad
+        assert h.value is None
+    assert lib.pwfs_sh_run(None, None, 1, None, None, None) == pwfs.PWFS_EINVAL
+    assert lib.pwfs_sh_info(None, None, None) == pwfs.PWFS_EINVAL
+    assert lib.pwfs_sh_valid_mask(None, None) == pwfs.PWFS_EINVAL
+    lib.pwfs_sh_destroy(None)
+    import torch
+    if not torch.cuda.is_available():
+        prm = mk()
+        assert lib.pwfs_sh_create(C.byref(prm), C.byref(h)) in (pwfs.PWFS_ECUDA, pwfs.PWFS_ENOMEM)
         assert h.value is None
 
 
