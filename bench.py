@@ -110,6 +110,112 @@ def oracle_sample_frames(cfg) -> int:
     return max(1, min(cfg.batch, int(round(4 * ref / cost))))
 
 
+def measured_hbm_peak():
+    """HBM GB/s from the driver-written MEASURED_PEAKS.json, else the profiling guide's fallback."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
+    except Exception:
+        return 6550.0, "fallback (B200_PROFILING.md)"
+
+
+def bench_stages(cfg, dev, phase, frames, flush, reps: int = 5) -> dict:
+    """The rows of SURVEY.md 8(f) on this config's geometry, each timed alone with CUDA events on the
+    launching stream (L2 flushed before every timed call) and set against the roofline that bounds it:
+    algorithmic bytes / measured HBM copy bandwidth, or nominal flop / derived FP32 peak."""
+    import torch
+    from paper_1607_07624_b200.atmo import Atmosphere
+    from paper_1607_07624_b200.chain import CCD, Reconstructor, SlopeComputer
+    from paper_1607_07624_b200.psf import PsfCamera
+    from paper_1607_07624_b200.sh import ShackHartmann
+    from paper_1607_07624_b200.pwfs import from_config
+    hbm, hbm_src = measured_hbm_peak()
+    stream = torch.cuda.current_stream(dev)
+    B, N, M = phase.shape[0], cfg.n_pupil, cfg.m_grid
+    D = frames.shape[1]
+
+    def timed(fn):
+        for _ in range(2):
+            fn()
+        best = []
+        for _ in range(reps):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            fn()
+            b.record(stream)
+            torch.cuda.synchronize(dev)
+            best.append(a.elapsed_time(b))
+        return statistics.median(best)
+
+    def hbm_row(ms, nbytes, launches, note):
+        gbs = nbytes / (ms * 1e-3) / 1e9
+        return {"ms": ms, "bound": "hbm", "algorithmic_bytes": int(nbytes), "achieved": gbs, "peak": hbm, "unit": "GB/s",
+                "frac": gbs / hbm, "launches": launches, "note": note}
+
+    def alu_row(ms, flop, launches, note):
+        tf = flop / (ms * 1e-3) / 1e12
+        return {"ms": ms, "bound": "alu", "nominal_flop": float(flop), "achieved": tf, "peak": FP32_PEAK_TFLOPS,
+                "unit": "TFLOP/s", "frac": tf / FP32_PEAK_TFLOPS, "launches": launches, "note": note}
+
+    out = {"peak_source": {"hbm": hbm_src, "alu": "derived FP32 peak (DESIGN.md 7)"}, "frames": B}
+    # f1: propagation through phase screens (frozen-flow configs only)
+    if not cfg.independent_screens:
+        atm = wl.atmosphere(cfg)
+        L, S, W = atm["screens"].shape[0], len(atm["dirs_tan"]), len(atm["wl_scale"])
+        n_steps = B // (S * W)
+        with Atmosphere(**{k: v for k, v in atm.items() if k != "dt"}, device=dev.index) as a:
+            buf = torch.empty_like(phase)
+            ms = timed(lambda: a.propagate(0, n_steps, atm["dt"], out=buf))
+        nbytes = n_steps * S * (W * N * N * 4 + L * (N + 1) * (N + 1) * 4)
+        out["f1_atmo_propagate"] = hbm_row(ms, nbytes, 1, f"{L} layers, {S} dir x {W} wl, {n_steps} steps: N^2 floats out per "
+                                           "frame + L (N+1)^2 screen samples in per direction")
+    # f2: detector, slope computer, reconstructor
+    with from_config(cfg, device=dev.index) as sensor:
+        valid = sensor.valid_mask()
+    nv = int(valid.sum())
+    n_ph = 100.0 * D * D / 4                                       # ~100 photons per lit pixel
+    with CCD(D, gain=n_ph / float((wl.make_pupil(cfg).astype(np.float64) ** 2).sum()), quantum_eff=0.32,
+             photon_noise=True, readout_noise=True, readout_level=1.0, seed=1, device=dev.index) as ccd:
+        pix = torch.empty_like(frames)
+        ms = timed(lambda: ccd.run(frames, out=pix))
+        out["f2_ccd"] = hbm_row(ms, B * D * D * 8, 1, "photon + read noise, n_int = 1: 4 B in + 4 B out per pixel")
+    with SlopeComputer(valid, sn=np.zeros(2 * nv, np.float32), device=dev.index) as sc:
+        sl = torch.empty((B, 2 * nv), dtype=torch.float32, device=dev)
+        ms = timed(lambda: sc.run(pix, out=sl))
+        out["f2_slopec"] = hbm_row(ms, B * (4 * nv * 4 + 2 * nv * 4), 1, "4 valid pixels in + 2 slopes out per subaperture")
+    n_modes = min(4096, 2 * nv)
+    rng = np.random.default_rng(0)
+    R = rng.standard_normal((n_modes, 2 * nv), dtype=np.float32) / nv
+    with Reconstructor(R, device=dev.index) as rec:
+        modes = torch.empty((B, n_modes), dtype=torch.float32, device=dev)
+        ms = timed(lambda: rec.run(sl, out=modes))
+        out["f2_rec_batch"] = alu_row(ms, 2.0 * B * n_modes * 2 * nv, 1, f"{n_modes} modes x {2 * nv} slopes x {B} frames, FP32 FMA")
+        m1 = torch.empty((1, n_modes), dtype=torch.float32, device=dev)
+        ms = timed(lambda: rec.run(sl[:1], out=m1))
+        out["f2_rec_gemv"] = hbm_row(ms, n_modes * 2 * nv * 4, 1, "one frame: recmat streamed once")
+    del R
+    # f4: PSF camera on the same grid, Shack-Hartmann on the same pupil
+    with PsfCamera(wl.make_pupil(cfg), M, phase_scale=0.45, device=dev.index) as cam:
+        ms = timed(lambda: cam.accumulate(phase, want_sr=True))
+        chunks = -(-B * M * ((N + 31) // 32 * 32) * 8 // (2 << 30))
+        out["f4_psf"] = alu_row(ms, B * 5.0 * M * M * math.log2(M * M), 3 * chunks,
+                                "one forward 2-D transform per frame, nominal 5 M^2 log2 M^2")
+    b = next((c for c in (6, 5, 4, 8, 3, 2) if N % c == 0), 1)
+    P, n_px, bin_ = (16, 8, 2) if b <= 8 else (32, 8, 4)
+    with ShackHartmann(wl.make_pupil(cfg), N // b, P, n_px, bin_, phase_scale=0.45, device=dev.index) as sh:
+        ms = timed(lambda: sh.run(phase))
+        Dsh, Pc = sh.det_size, n_px * bin_
+        flop = B * (N // b) ** 2 * 8.0 * b * Pc * (b + Pc)
+        row_h = hbm_row(ms, B * (N * N * 4 + Dsh * Dsh * 4), 1, "")
+        row_a = alu_row(ms, flop, 1, "")
+        row = row_h if row_h["frac"] >= row_a["frac"] else row_a
+        row["note"] = (f"{N // b}^2 subapertures of {b} px, P = {P}, {n_px}^2 detector px each: phase in + frame out "
+                       f"({row_h['frac']:.3f} of HBM) vs direct-DFT FMAs ({row_a['frac']:.3f} of FP32)")
+        out["f4_shack_hartmann"] = row
+    return out
+
+
 def run_reference(args, cfg):
     """--impl reference: the CPU oracle (this tier's reference arm), rank 0 only."""
     rank = int(os.environ.get("RANK", "0"))
@@ -289,6 +395,8 @@ def run_ours(args, cfg):
             "latency_b1": latency,
             "clocks": clocks,
         }
+        if not args.no_stages:
+            line["stages"] = bench_stages(cfg, dev, phase, frames, flush)
         if not args.no_cpu_baseline:
             nfr = oracle_sample_frames(cfg)
             dt, cores = time_oracle(cfg, nfr)
@@ -309,6 +417,7 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--config", default="cfg4_elt", choices=wl.CONFIG_ORDER)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-stages", action="store_true", help="skip the per-stage timings of the 8(f) rows")
     args = ap.parse_args()
     if args.steps < 1 or args.warmup < 0:
         raise SystemExit("bench.py: need --steps >= 1 and --warmup >= 0")
