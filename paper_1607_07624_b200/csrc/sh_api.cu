@@ -1,14 +1,24 @@
 // sh_api.cu -- f4, Shack-Hartmann: C ABI of include/pwfs_sh.h and its kernel.
 //
-// One warp = one subaperture of one frame, everything in shared memory:
-//   1. phasor of the b x b pupil pixels (range-reduced MUFU sincos),
-//   2. DFT along x to the Pc = n_px * bin kept columns only (b inputs each: direct sums against
-//      a 2P-entry twiddle table that carries the half-pixel centring),
-//   3. DFT along y to the Pc kept rows, |.|^2 / P^2,
-//   4. bin x bin sums -> the subaperture's detector window, centre of gravity -> slopes.
-// b <= 16 and P <= 64, so a transform is at most 16 terms: direct sums beat any FFT staging, and
-// the whole subaperture costs b Pc (b + Pc) complex FMAs.  HBM sees the phase once and the frame
-// once; the kernel is bound by those bytes for small P and by FP32 FMAs for large P.
+// Both DFTs of a subaperture are b-term direct sums against one table W[t][c] =
+// exp(-2 pi i (c - Pc/2 + 1/2) t / P), t < b, c < Pc = n_px * bin (the kept, fftshifted columns with the
+// half-pixel centring folded in): H = g W along x, spot = |W^T H|^2 along y.  b <= 16 and P <= 64, so
+// direct sums beat any FFT staging; the whole subaperture costs b Pc (b + Pc) complex FMAs.
+//
+// sh_kernel<B, NC>: LPS = 2^k lanes own one subaperture, each lane NC adjacent columns c, so a warp
+// works on 32 / LPS neighbouring subapertures of one lenslet row (coalesced phase rows in, coalesced
+// detector rows out).
+//   1. phasor of the b x b pupil pixels (range-reduced MUFU sincos) -> shared memory, stored as
+//      (re, re, im, im) so that one LDS.128 feeds two FFMA2;
+//   2. along x: the lane keeps its NC columns of W in registers and accumulates H[y][c] for all y
+//      in registers: one g load per 2 NC FFMA2;
+//   3. along y: for each kept row v the b table entries W[y][v] are warp-uniform loads, again one per
+//      2 NC FFMA2; |.|^2 / P^2 falls out in the lane that owns the column;
+//   4. bin x bin sums (rows in the lane, columns through a per-warp row buffer), detector window
+//      written from registers, centre of gravity reduced over the LPS lanes by shuffles.
+// A complex sum  sum a w  is kept as two packed accumulators P = sum re(a) w, Q = sum im(a) w and
+// folded once at the end (P.x - Q.y, P.y + Q.x): two FFMA2 per complex FMA, no operand shuffling.
+// HBM sees the phase once and the frame once.
 #include "../../include/pwfs_sh.h"
 
 #include <cuda_runtime.h>
@@ -23,121 +33,199 @@ namespace {
 
 constexpr int kShWarps = 4;
 constexpr int kMaxB = 16, kMaxP = 64;
+constexpr size_t kShSmemBudget = 160 * 1024;
 constexpr float kInv2PiHiS = 0.15915493667125702f;
 constexpr float kInv2PiLoS = 6.4206382e-09f;
 
 struct ShDev {
     int N, n_sub, b, P, n_px, bin, Pc;
+    int lg_lps;              // log2 of the lanes that share one subaperture
+    int gpitch;              // float4 per subaperture in the phasor buffer (b*b padded to 1 mod 8)
+    int gpr;                 // warp tasks per lenslet row = ceil(n_sub / (32 >> lg_lps))
+    int vec;                 // 1: detector rows may be stored NC-wide (alignment holds)
     float scale, invP2;
     const float *amp;        // [N][N]
-    const float2 *tw;        // [2P] exp(-2 pi i m / (2P))
+    const float4 *wtab;      // [b][Pc] (re, re, im, im) of W[t][c]
     const int *vslot;        // [n_sub^2] slope slot of a valid subaperture, -1 otherwise
     int n_valid;
 };
 
-__host__ __device__ inline size_t sh_warp_floats(int b, int Pc) {
-    return (size_t)2 * b * b + (size_t)2 * b * Pc + (size_t)Pc * Pc;
-}
+__device__ __forceinline__ float2 lo2(float4 v) { return make_float2(v.x, v.y); }
+__device__ __forceinline__ float2 hi2(float4 v) { return make_float2(v.z, v.w); }
 
-__device__ __forceinline__ float2 cfma(float2 a, float2 w, float2 acc) {   // acc + a * w
-    acc.x = fmaf(a.x, w.x, acc.x); acc.x = fmaf(-a.y, w.y, acc.x);
-    acc.y = fmaf(a.x, w.y, acc.y); acc.y = fmaf(a.y, w.x, acc.y);
-    return acc;
-}
-
-// grid (ceil(n_sub^2 / kShWarps), F); block 32 * kShWarps; dynamic smem: tw[2P] + per-warp buffers.
+// grid (ceil(n_sub * gpr / kShWarps), F); block 32 * kShWarps;
+// dynamic smem: W[B][Pc] float4, then per warp the phasor buffer [SPW][gpitch] float4 and a row buffer [32 NC] float.
+template <int B, int NC>
 __global__ void __launch_bounds__(32 * kShWarps)
 sh_kernel(ShDev t, const float *__restrict__ phase, float *__restrict__ frames, float *__restrict__ slopes) {
-    extern __shared__ float2 sh_smem[];
-    float2 *s_tw = sh_smem;
+    extern __shared__ float4 sh_smem[];
     const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
-    const int b = t.b, P = t.P, Pc = t.Pc, P2 = 2 * t.P;
-    float *wbase = reinterpret_cast<float *>(sh_smem + P2) + (size_t)wl * sh_warp_floats(b, Pc);
-    float2 *g = reinterpret_cast<float2 *>(wbase);                 // [b][b]
-    float2 *H = g + b * b;                                         // [b][Pc]
-    float *spot = reinterpret_cast<float *>(H + b * Pc);           // [Pc][Pc]
-    for (int i = threadIdx.x; i < P2; i += blockDim.x) s_tw[i] = __ldg(t.tw + i);
+    const int Pc = t.Pc, lgL = t.lg_lps, lgS = 5 - lgL, LPS = 1 << lgL, SPW = 1 << lgS;
+    float4 *s_w = sh_smem;                                                    // [B][Pc]
+    float4 *g = s_w + B * Pc + (size_t)wl * ((size_t)SPW * t.gpitch + 8 * NC); // [SPW][gpitch]
+    float *rowbuf = reinterpret_cast<float *>(g + (size_t)SPW * t.gpitch);    // [32 NC]
+    for (int i = threadIdx.x; i < B * Pc; i += blockDim.x) s_w[i] = __ldg(t.wtab + i);
     __syncthreads();
-    const int sub = blockIdx.x * kShWarps + wl, f = blockIdx.y;
-    if (sub >= t.n_sub * t.n_sub) return;
-    const int sj = sub / t.n_sub, si = sub - sj * t.n_sub;
+    const int task = blockIdx.x * kShWarps + wl, f = blockIdx.y;
+    if (task >= t.n_sub * t.gpr) return;                                      // warp-uniform
+    const int sj = task / t.gpr, si0 = (task - sj * t.gpr) << lgS;
+    const int s = lane >> lgL, col = lane & (LPS - 1), si = si0 + s;
 
-    // 1. phasor (F4f)
-    const float *ph0 = phase + ((size_t)f * t.N + (size_t)sj * b) * t.N + (size_t)si * b;
-    const float *am0 = t.amp + ((size_t)sj * b) * t.N + (size_t)si * b;
-    for (int e = lane; e < b * b; e += 32) {
-        const int y = e / b, x = e - y * b;
-        const float ph = __ldg(ph0 + (size_t)y * t.N + x) * t.scale;
-        const float am = __ldg(am0 + (size_t)y * t.N + x);
-        const float q = rintf(ph * kInv2PiHiS);
-        float tr = fmaf(ph, kInv2PiHiS, -q);
-        tr = fmaf(ph, kInv2PiLoS, tr);
-        float sn, cs;
-        __sincosf(tr * 6.283185307179586f, &sn, &cs);
-        g[e] = make_float2(am * cs, am * sn);
-    }
-    __syncwarp();
-    // 2. along x: H[y][uc] = sum_x g[y][x] exp(-2 pi i (u~ + 1/2) x / P), u~ = uc - Pc/2 (fftshifted crop)
-    for (int e = lane; e < b * Pc; e += 32) {
-        const int y = e / Pc, uc = e - y * Pc;
-        int step = (2 * (uc - Pc / 2) + 1) % P2;
-        if (step < 0) step += P2;
-        float2 acc = make_float2(0.f, 0.f);
-        int m = 0;
-        for (int x = 0; x < b; ++x) {
-            acc = cfma(g[y * b + x], s_tw[m], acc);
-            m += step;
-            if (m >= P2) m -= P2;
+    // 1. phasor (F4f): rows of SPW * B contiguous pupil pixels
+    {
+        const int rowlen = B << lgS;
+        const float *ph0 = phase + ((size_t)f * t.N + (size_t)sj * B) * t.N + (size_t)si0 * B;
+        const float *am0 = t.amp + ((size_t)sj * B) * t.N + (size_t)si0 * B;
+        const int xmax = t.N - si0 * B;                                       // pixels left in this pupil row
+        for (int e = lane; e < B * rowlen; e += 32) {
+            const int y = (e >> lgS) / B, sx = e - y * rowlen;
+            const int ss = sx / B, x = sx - ss * B;
+            float re = 0.f, im = 0.f;
+            if (sx < xmax) {
+                const float ph = __ldg(ph0 + (size_t)y * t.N + sx) * t.scale;
+                const float am = __ldg(am0 + (size_t)y * t.N + sx);
+                const float q = rintf(ph * kInv2PiHiS);
+                float tr = fmaf(ph, kInv2PiHiS, -q);
+                tr = fmaf(ph, kInv2PiLoS, tr);
+                float sn, cs;
+                __sincosf(tr * 6.283185307179586f, &sn, &cs);
+                re = am * cs; im = am * sn;
+            }
+            g[ss * t.gpitch + y * B + x] = make_float4(re, re, im, im);
         }
-        H[e] = acc;
+    }
+    // the lane's NC columns of W
+    float2 Wl[NC][B];
+#pragma unroll
+    for (int j = 0; j < NC; ++j) {
+        const int uc = min(col * NC + j, Pc - 1);
+#pragma unroll
+        for (int x = 0; x < B; ++x) { const float4 w = s_w[x * Pc + uc]; Wl[j][x] = make_float2(w.x, w.z); }
     }
     __syncwarp();
-    // 3. along y, |.|^2 / P^2
-    for (int e = lane; e < Pc * Pc; e += 32) {
-        const int vc = e / Pc, uc = e - vc * Pc;
-        int step = (2 * (vc - Pc / 2) + 1) % P2;
-        if (step < 0) step += P2;
-        float2 acc = make_float2(0.f, 0.f);
-        int m = 0;
-        for (int y = 0; y < b; ++y) {
-            acc = cfma(H[y * Pc + uc], s_tw[m], acc);
-            m += step;
-            if (m >= P2) m -= P2;
+    // 2. along x: H[y][c] = sum_x g[y][x] W[x][c]
+    float2 H[NC][B];
+    {
+        const float4 *gs = g + s * t.gpitch;
+#pragma unroll
+        for (int y = 0; y < B; ++y) {
+            float2 Pa[NC], Qa[NC];
+#pragma unroll
+            for (int j = 0; j < NC; ++j) Pa[j] = Qa[j] = make_float2(0.f, 0.f);
+#pragma unroll
+            for (int x = 0; x < B; ++x) {
+                const float4 a = gs[y * B + x];
+#pragma unroll
+                for (int j = 0; j < NC; ++j) {
+                    Pa[j] = __ffma2_rn(lo2(a), Wl[j][x], Pa[j]);
+                    Qa[j] = __ffma2_rn(hi2(a), Wl[j][x], Qa[j]);
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < NC; ++j) H[j][y] = make_float2(Pa[j].x - Qa[j].y, Pa[j].y + Qa[j].x);
         }
-        spot[e] = fmaf(acc.x, acc.x, acc.y * acc.y) * t.invP2;
     }
-    __syncwarp();
-    // 4. detector window (F4g) and centre of gravity (F4i)
+    // 3./4. along y, |.|^2 / P^2, detector window (F4g), centre of gravity (F4i)
     const int n_px = t.n_px, bin = t.bin, D = t.n_sub * n_px;
-    float *win = frames + ((size_t)f * D + (size_t)sj * n_px) * D + (size_t)si * n_px;
+    const bool live = si < t.n_sub;
+    float *win = frames + ((size_t)f * D + (size_t)sj * n_px) * D + (size_t)min(si, t.n_sub - 1) * n_px;
     const float c0 = 0.5f * (float)(n_px - 1);
     float tot = 0.f, mx = 0.f, my = 0.f;
-    for (int e = lane; e < n_px * n_px; e += 32) {
-        const int py = e / n_px, px = e - py * n_px;
-        float s = 0.f;
-        for (int yy = 0; yy < bin; ++yy)
-            for (int xx = 0; xx < bin; ++xx) s += spot[(py * bin + yy) * Pc + px * bin + xx];
-        win[(size_t)py * D + px] = s;
-        tot += s;
-        mx = fmaf((float)px - c0, s, mx);
-        my = fmaf((float)py - c0, s, my);
+    float racc[NC];
+#pragma unroll
+    for (int j = 0; j < NC; ++j) racc[j] = 0.f;
+    int cnt = 0, py = 0;
+    for (int vc = 0; vc < Pc; ++vc) {
+        float2 Pa[NC], Qa[NC];
+#pragma unroll
+        for (int j = 0; j < NC; ++j) Pa[j] = Qa[j] = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int y = 0; y < B; ++y) {
+            const float4 w = s_w[y * Pc + vc];
+#pragma unroll
+            for (int j = 0; j < NC; ++j) {
+                Pa[j] = __ffma2_rn(lo2(w), H[j][y], Pa[j]);
+                Qa[j] = __ffma2_rn(hi2(w), H[j][y], Qa[j]);
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < NC; ++j) {
+            const float er = Pa[j].x - Qa[j].y, ei = Pa[j].y + Qa[j].x;
+            racc[j] += fmaf(er, er, ei * ei) * t.invP2;
+        }
+        if (++cnt < bin) continue;
+        cnt = 0;
+        const float fy = (float)py - c0;
+        if (bin == 1) {                                                       // detector pixel = FFT pixel
+            float *row = win + (size_t)py * D + col * NC;
+            if (live) {
+                if (NC == 4 && t.vec && col * NC + NC <= Pc) {
+                    *reinterpret_cast<float4 *>(row) = make_float4(racc[0], racc[1], racc[2], racc[3]);
+                } else if (NC == 2 && t.vec && col * NC + NC <= Pc) {
+                    *reinterpret_cast<float2 *>(row) = make_float2(racc[0], racc[1]);
+                } else {
+#pragma unroll
+                    for (int j = 0; j < NC; ++j) if (col * NC + j < Pc) row[j] = racc[j];
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < NC; ++j) {
+                const float v = col * NC + j < Pc ? racc[j] : 0.f;
+                tot += v;
+                mx = fmaf((float)(col * NC + j) - c0, v, mx);
+                my = fmaf(fy, v, my);
+                racc[j] = 0.f;
+            }
+        } else {                                                              // columns through the row buffer
+            float *rb = rowbuf + s * (LPS * NC);
+#pragma unroll
+            for (int j = 0; j < NC; ++j) { rb[col * NC + j] = racc[j]; racc[j] = 0.f; }
+            __syncwarp();
+            for (int px = col; px < n_px; px += LPS) {
+                float v = 0.f;
+                for (int xx = 0; xx < bin; ++xx) v += rb[px * bin + xx];
+                if (live) win[(size_t)py * D + px] = v;
+                tot += v;
+                mx = fmaf((float)px - c0, v, mx);
+                my = fmaf(fy, v, my);
+            }
+            __syncwarp();
+        }
+        ++py;
     }
     if (slopes) {
-        const int slot = __ldg(t.vslot + sub);
-        if (slot >= 0) {                                           // warp-uniform
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                tot += __shfl_xor_sync(0xffffffffu, tot, o);
-                mx += __shfl_xor_sync(0xffffffffu, mx, o);
-                my += __shfl_xor_sync(0xffffffffu, my, o);
-            }
-            if (lane == 0) {
+        for (int o = LPS >> 1; o > 0; o >>= 1) {
+            tot += __shfl_xor_sync(0xffffffffu, tot, o);
+            mx += __shfl_xor_sync(0xffffffffu, mx, o);
+            my += __shfl_xor_sync(0xffffffffu, my, o);
+        }
+        if (live && col == 0) {
+            const int slot = __ldg(t.vslot + sj * t.n_sub + si);
+            if (slot >= 0) {
                 float *out = slopes + (size_t)f * 2 * t.n_valid;
                 out[slot] = mx / tot;
                 out[t.n_valid + slot] = my / tot;
             }
         }
     }
+}
+
+using ShKernel = void (*)(ShDev, const float *, float *, float *);
+
+template <int B>
+ShKernel sh_pick_nc(int nc) {
+    if constexpr (B <= 8) { if (nc == 4) return sh_kernel<B, 4>; }
+    return nc >= 2 ? sh_kernel<B, 2> : sh_kernel<B, 1>;
+}
+
+ShKernel sh_pick(int b, int nc) {
+    switch (b) {
+#define SH_CASE(B_) case B_: return sh_pick_nc<B_>(nc);
+        SH_CASE(1) SH_CASE(2) SH_CASE(3) SH_CASE(4) SH_CASE(5) SH_CASE(6) SH_CASE(7) SH_CASE(8)
+        SH_CASE(9) SH_CASE(10) SH_CASE(11) SH_CASE(12) SH_CASE(13) SH_CASE(14) SH_CASE(15) SH_CASE(16)
+#undef SH_CASE
+    }
+    return nullptr;
 }
 
 int cuda_rc(cudaError_t e) { return e == cudaErrorMemoryAllocation ? PWFS_ENOMEM : PWFS_ECUDA; }
@@ -147,10 +235,12 @@ int cuda_rc(cudaError_t e) { return e == cudaErrorMemoryAllocation ? PWFS_ENOMEM
 struct pwfs_sh {
     int device = 0;
     ShDev dev{};
+    ShKernel kernel = nullptr;
+    int nc = 1;
     size_t smem = 0;
     std::vector<uint8_t> valid;
     float *d_amp = nullptr;
-    float2 *d_tw = nullptr;
+    float4 *d_wtab = nullptr;
     int *d_vslot = nullptr;
 };
 
@@ -189,29 +279,47 @@ int pwfs_sh_create(const pwfs_sh_params *p, pwfs_sh_t **out) {
             if (lit >= thresh * b * b * amax2) { valid[(size_t)j * ns + i] = 1; vslot[(size_t)j * ns + i] = nv++; }
         }
     if (nv == 0) return PWFS_EINVAL;
-    std::vector<float2> tw((size_t)2 * P);
-    for (int m = 0; m < 2 * P; ++m) {
-        const double a = -3.14159265358979323846264338327950288 * (double)m / (double)P;
-        tw[m] = make_float2((float)std::cos(a), (float)std::sin(a));
-    }
+    // W[t][c] = exp(-2 pi i (2 (c - Pc/2) + 1) t / (2P)), argument reduced in integers
+    std::vector<float4> wtab((size_t)b * Pc);
+    for (int tt = 0; tt < b; ++tt)
+        for (int c = 0; c < (int)Pc; ++c) {
+            long long m = ((2LL * (c - Pc / 2) + 1) * tt) % (2LL * P);
+            if (m < 0) m += 2LL * P;
+            const double a = -3.14159265358979323846264338327950288 * (double)m / (double)P;
+            const float wr = (float)std::cos(a), wi = (float)std::sin(a);
+            wtab[(size_t)tt * Pc + c] = make_float4(wr, wr, wi, wi);
+        }
+    // columns per lane, lanes per subaperture (a power of two), subapertures per warp
+    const int nc = (b <= 8 && Pc >= 16) ? 4 : (Pc >= 4 ? 2 : 1);
+    int lg = 0;
+    while ((nc << lg) < Pc) ++lg;                                  // Pc <= 64 = 2 * 32 -> lg <= 5
+    const int gpitch = ((b * b + 6) / 8) * 8 + 1;                  // = 1 mod 8: subapertures land on distinct banks
+    auto smem_of = [&](int l) {
+        return ((size_t)b * Pc + (size_t)kShWarps * ((size_t)(32 >> l) * gpitch + 8 * nc)) * sizeof(float4);
+    };
+    while (lg < 5 && smem_of(lg) > kShSmemBudget) ++lg;            // large b with a tiny window: fewer subapertures per warp
     pwfs_sh *h = new (std::nothrow) pwfs_sh();
     if (!h) return PWFS_ENOMEM;
     h->device = p->device;
     h->valid = valid;
-    h->smem = (size_t)2 * P * sizeof(float2) + kShWarps * sh_warp_floats(b, (int)Pc) * sizeof(float);
+    h->nc = nc;
+    h->kernel = sh_pick(b, nc);
+    h->smem = smem_of(lg);
     cudaError_t e = cudaSetDevice(p->device);
     if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_amp, (size_t)N * N * sizeof(float));
     if (e == cudaSuccess) e = cudaMemcpy(h->d_amp, p->pupil_amp, (size_t)N * N * sizeof(float), cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_tw, tw.size() * sizeof(float2));
-    if (e == cudaSuccess) e = cudaMemcpy(h->d_tw, tw.data(), tw.size() * sizeof(float2), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_wtab, wtab.size() * sizeof(float4));
+    if (e == cudaSuccess) e = cudaMemcpy(h->d_wtab, wtab.data(), wtab.size() * sizeof(float4), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_vslot, vslot.size() * sizeof(int));
     if (e == cudaSuccess) e = cudaMemcpy(h->d_vslot, vslot.data(), vslot.size() * sizeof(int), cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sh_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute((const void *)h->kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem);
     if (e != cudaSuccess) { int rc = cuda_rc(e); pwfs_sh_destroy(h); return rc; }
     ShDev &d = h->dev;
     d.N = N; d.n_sub = ns; d.b = b; d.P = P; d.n_px = p->n_px; d.bin = p->bin; d.Pc = (int)Pc;
+    d.lg_lps = lg; d.gpitch = gpitch; d.gpr = (ns + (32 >> lg) - 1) / (32 >> lg);
+    d.vec = (p->n_px % nc == 0) ? 1 : 0;
     d.scale = p->phase_scale; d.invP2 = (float)(1.0 / ((double)P * P));
-    d.amp = h->d_amp; d.tw = h->d_tw; d.vslot = h->d_vslot; d.n_valid = nv;
+    d.amp = h->d_amp; d.wtab = h->d_wtab; d.vslot = h->d_vslot; d.n_valid = nv;
     *out = h;
     return PWFS_OK;
 }
@@ -234,12 +342,13 @@ int pwfs_sh_run(pwfs_sh_t *h, const float *d_phase, int32_t B, float *d_frames, 
     if (B == 0) return PWFS_OK;
     if (!d_phase || !d_frames) return PWFS_EINVAL;
     if (cudaSetDevice(h->device) != cudaSuccess) return PWFS_ECUDA;
-    const ShDev &d = h->dev;
-    const int subs = d.n_sub * d.n_sub, D = d.n_sub * d.n_px;
+    ShDev d = h->dev;
+    const int tasks = d.n_sub * d.gpr, D = d.n_sub * d.n_px;
     const size_t NN = (size_t)d.N * d.N, DD = (size_t)D * D;
+    if ((uintptr_t)d_frames % 16 != 0) d.vec = 0;                  // NC-wide stores need the caller's buffer aligned
     for (int f0 = 0; f0 < B; f0 += 65535) {
         const int Fc = B - f0 < 65535 ? B - f0 : 65535;
-        sh_kernel<<<dim3((subs + kShWarps - 1) / kShWarps, Fc), 32 * kShWarps, h->smem, (cudaStream_t)cuda_stream>>>(
+        h->kernel<<<dim3((tasks + kShWarps - 1) / kShWarps, Fc), 32 * kShWarps, h->smem, (cudaStream_t)cuda_stream>>>(
             d, d_phase + (size_t)f0 * NN, d_frames + (size_t)f0 * DD,
             d_slopes ? d_slopes + (size_t)f0 * 2 * d.n_valid : nullptr);
     }
@@ -250,7 +359,7 @@ void pwfs_sh_destroy(pwfs_sh_t *h) {
     if (!h) return;
     cudaSetDevice(h->device);
     if (h->d_amp) cudaFree(h->d_amp);
-    if (h->d_tw) cudaFree(h->d_tw);
+    if (h->d_wtab) cudaFree(h->d_wtab);
     if (h->d_vslot) cudaFree(h->d_vslot);
     delete h;
 }
