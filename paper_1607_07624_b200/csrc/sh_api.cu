@@ -53,10 +53,46 @@ struct ShDev {
 __device__ __forceinline__ float2 lo2(float4 v) { return make_float2(v.x, v.y); }
 __device__ __forceinline__ float2 hi2(float4 v) { return make_float2(v.z, v.w); }
 
+// One detector row of one subaperture from the lane's NC adjacent FFT columns when BIN divides NC:
+// NO = NC / BIN detector pixels starting at col * NO, stored NO-wide when `vec` says the alignment holds.
+template <int NC, int BIN>
+__device__ __forceinline__ void emit_row(float (&racc)[NC], float *row, int col, int n_px, bool live, int vec,
+                                         float c0, float fy, float &tot, float &mx, float &my) {
+    if constexpr (NC % BIN == 0) {
+        constexpr int NO = NC / BIN;
+        float v[NO];
+#pragma unroll
+        for (int k = 0; k < NO; ++k) {
+            float a = 0.f;
+#pragma unroll
+            for (int x = 0; x < BIN; ++x) a += racc[k * BIN + x];
+            v[k] = col * NO + k < n_px ? a : 0.f;
+        }
+#pragma unroll
+        for (int j = 0; j < NC; ++j) racc[j] = 0.f;
+        if (live) {
+            if (NO == 4 && vec && col * NO + NO <= n_px) {
+                *reinterpret_cast<float4 *>(row + col * NO) = make_float4(v[0], v[1], v[2], v[3]);
+            } else if (NO == 2 && vec && col * NO + NO <= n_px) {
+                *reinterpret_cast<float2 *>(row + col * NO) = make_float2(v[0], v[1]);
+            } else {
+#pragma unroll
+                for (int k = 0; k < NO; ++k) if (col * NO + k < n_px) row[col * NO + k] = v[k];
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < NO; ++k) {
+            tot += v[k];
+            mx = fmaf((float)(col * NO + k) - c0, v[k], mx);
+            my = fmaf(fy, v[k], my);
+        }
+    }
+}
+
 // grid (ceil(n_sub * gpr / kShWarps), F); block 32 * kShWarps;
 // dynamic smem: W[B][Pc] float4, then per warp the phasor buffer [SPW][gpitch] float4 and a row buffer [32 NC] float.
 template <int B, int NC>
-__global__ void __launch_bounds__(32 * kShWarps)
+__global__ void __launch_bounds__(32 * kShWarps, (B * NC <= 24) ? 4 : 2)
 sh_kernel(ShDev t, const float *__restrict__ phase, float *__restrict__ frames, float *__restrict__ slopes) {
     extern __shared__ float4 sh_smem[];
     const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
@@ -77,21 +113,31 @@ sh_kernel(ShDev t, const float *__restrict__ phase, float *__restrict__ frames, 
         const float *ph0 = phase + ((size_t)f * t.N + (size_t)sj * B) * t.N + (size_t)si0 * B;
         const float *am0 = t.amp + ((size_t)sj * B) * t.N + (size_t)si0 * B;
         const int xmax = t.N - si0 * B;                                       // pixels left in this pupil row
-        for (int e = lane; e < B * rowlen; e += 32) {
-            const int y = (e >> lgS) / B, sx = e - y * rowlen;
-            const int ss = sx / B, x = sx - ss * B;
-            float re = 0.f, im = 0.f;
-            if (sx < xmax) {
-                const float ph = __ldg(ph0 + (size_t)y * t.N + sx) * t.scale;
-                const float am = __ldg(am0 + (size_t)y * t.N + sx);
-                const float q = rintf(ph * kInv2PiHiS);
-                float tr = fmaf(ph, kInv2PiHiS, -q);
-                tr = fmaf(ph, kInv2PiLoS, tr);
+        constexpr int U = 4;                                                  // loads of U rounds in flight
+        for (int e0 = lane; e0 < B * rowlen; e0 += 32 * U) {
+            float ph[U], am[U];
+            int dst[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int e = e0 + 32 * u;
+                const int y = (e >> lgS) / B, sx = e - y * rowlen;
+                const int ss = sx / B, x = sx - ss * B;
+                const bool in = e < B * rowlen && sx < xmax;
+                dst[u] = e < B * rowlen ? ss * t.gpitch + y * B + x : -1;
+                ph[u] = in ? __ldg(ph0 + (size_t)y * t.N + sx) : 0.f;
+                am[u] = in ? __ldg(am0 + (size_t)y * t.N + sx) : 0.f;
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const float p = ph[u] * t.scale;
+                const float q = rintf(p * kInv2PiHiS);
+                float tr = fmaf(p, kInv2PiHiS, -q);
+                tr = fmaf(p, kInv2PiLoS, tr);
                 float sn, cs;
                 __sincosf(tr * 6.283185307179586f, &sn, &cs);
-                re = am * cs; im = am * sn;
+                const float re = am[u] * cs, im = am[u] * sn;
+                if (dst[u] >= 0) g[dst[u]] = make_float4(re, re, im, im);
             }
-            g[ss * t.gpitch + y * B + x] = make_float4(re, re, im, im);
         }
     }
     // the lane's NC columns of W
@@ -157,25 +203,11 @@ sh_kernel(ShDev t, const float *__restrict__ phase, float *__restrict__ frames, 
         cnt = 0;
         const float fy = (float)py - c0;
         if (bin == 1) {                                                       // detector pixel = FFT pixel
-            float *row = win + (size_t)py * D + col * NC;
-            if (live) {
-                if (NC == 4 && t.vec && col * NC + NC <= Pc) {
-                    *reinterpret_cast<float4 *>(row) = make_float4(racc[0], racc[1], racc[2], racc[3]);
-                } else if (NC == 2 && t.vec && col * NC + NC <= Pc) {
-                    *reinterpret_cast<float2 *>(row) = make_float2(racc[0], racc[1]);
-                } else {
-#pragma unroll
-                    for (int j = 0; j < NC; ++j) if (col * NC + j < Pc) row[j] = racc[j];
-                }
-            }
-#pragma unroll
-            for (int j = 0; j < NC; ++j) {
-                const float v = col * NC + j < Pc ? racc[j] : 0.f;
-                tot += v;
-                mx = fmaf((float)(col * NC + j) - c0, v, mx);
-                my = fmaf(fy, v, my);
-                racc[j] = 0.f;
-            }
+            emit_row<NC, 1>(racc, win + (size_t)py * D, col, n_px, live, t.vec, c0, fy, tot, mx, my);
+        } else if (bin == 2 && NC % 2 == 0) {                                 // column pairs live in one lane
+            emit_row<NC, 2>(racc, win + (size_t)py * D, col, n_px, live, t.vec, c0, fy, tot, mx, my);
+        } else if (bin == 4 && NC == 4) {
+            emit_row<NC, 4>(racc, win + (size_t)py * D, col, n_px, live, t.vec, c0, fy, tot, mx, my);
         } else {                                                              // columns through the row buffer
             float *rb = rowbuf + s * (LPS * NC);
 #pragma unroll
@@ -317,7 +349,7 @@ int pwfs_sh_create(const pwfs_sh_params *p, pwfs_sh_t **out) {
     ShDev &d = h->dev;
     d.N = N; d.n_sub = ns; d.b = b; d.P = P; d.n_px = p->n_px; d.bin = p->bin; d.Pc = (int)Pc;
     d.lg_lps = lg; d.gpitch = gpitch; d.gpr = (ns + (32 >> lg) - 1) / (32 >> lg);
-    d.vec = (p->n_px % nc == 0) ? 1 : 0;
+    d.vec = (nc % p->bin == 0 && p->n_px % (nc / p->bin) == 0) ? 1 : 0;   // NO-wide stores stay aligned
     d.scale = p->phase_scale; d.invP2 = (float)(1.0 / ((double)P * P));
     d.amp = h->d_amp; d.wtab = h->d_wtab; d.vslot = h->d_vslot; d.n_valid = nv;
     *out = h;
