@@ -15,8 +15,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libpwfs.so")
-SOURCES = [os.path.join(CSRC, n) for n in ("pwfs_api.cu", "atmo_api.cu", "chain_api.cu", "psf_api.cu", "sh_api.cu")]
-HEADERS = [os.path.join(CSRC, "pwfs_kernels.cuh"), os.path.join(CSRC, "pwfs_dft.cuh")] + \
+SOURCES = [os.path.join(CSRC, n) for n in ("pwfs_api.cu", "atmo_api.cu", "chain_api.cu", "rec_tc.cu", "psf_api.cu", "sh_api.cu")]
+HEADERS = [os.path.join(CSRC, n) for n in ("pwfs_kernels.cuh", "pwfs_dft.cuh", "rec_tc.cuh")] + \
           [os.path.join(ROOT, "include", n) for n in ("pwfs.h", "pwfs_atmo.h", "pwfs_chain.h", "pwfs_psf.h", "pwfs_sh.h")]
 OBJDIR = os.path.join(HERE, "build")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

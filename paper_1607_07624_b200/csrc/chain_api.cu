@@ -11,10 +11,12 @@
 //                   B = 1 is a GEMV streaming recmat once from HBM; larger batches re-use each
 //                   recmat line for FB frames out of registers.
 #include "../../include/pwfs_chain.h"
+#include "rec_tc.cuh"
 
 #include <cuda_runtime.h>
 
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -202,6 +204,9 @@ rec_kernel(const float *__restrict__ R, int n_modes, int ldk, const float *__res
         }
 }
 
+constexpr int kRecTcMinBatch = 24;              // below this the FP32 kernel's register tiles win
+constexpr long long kRecTcMinElems = 1 << 16;   // recmat elements
+
 template <int MR, int FB>
 void launch_rec(bool vec, dim3 grid, cudaStream_t st, const float *R, int n_modes, int ldk, const float *S, int ns,
                 int B, float *out) {
@@ -243,6 +248,8 @@ struct pwfs_rec {
     int n_modes = 0, n_slopes = 0, ldk = 0;
     float *d_R = nullptr;
     int num_sms = 148;
+    RecTc *tc = nullptr;       // tensor-core path for batches, built on the first batched call
+    bool tc_off = false;       // PWFS_REC_TC=0, or the driver lacks cuTensorMapEncodeTiled
 };
 
 extern "C" {
@@ -364,6 +371,8 @@ int pwfs_rec_create(int32_t n_modes, int32_t n_slopes, const float *h_recmat, in
         if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) == cudaSuccess && sms > 0) h->num_sms = sms;
     }
     if (e != cudaSuccess) { int rc = cuda_rc(e); pwfs_rec_destroy(h); return rc; }
+    const char *env = std::getenv("PWFS_REC_TC");
+    h->tc_off = env && env[0] == '0';
     *out = h;
     return PWFS_OK;
 }
@@ -373,6 +382,15 @@ int pwfs_rec_run(pwfs_rec_t *h, const float *d_slopes, int32_t B, float *d_modes
     if (B == 0) return PWFS_OK;
     if (!d_slopes || !d_modes) return PWFS_EINVAL;
     if (cudaSetDevice(h->device) != cudaSuccess) return PWFS_ECUDA;
+    // batches: TF32x3 on the tensor cores (rec_tc.cu); single frames and small problems: FP32 FMA below
+    if (!h->tc_off && B >= kRecTcMinBatch && (long long)h->n_modes * h->n_slopes >= kRecTcMinElems) {
+        if (!h->tc) {
+            const int rc = rec_tc_create(&h->tc, h->d_R, h->n_modes, h->n_slopes, h->ldk, h->device, h->num_sms);
+            if (rc == PWFS_EUNSUPPORTED) h->tc_off = true;
+            else if (rc != PWFS_OK) return rc;
+        }
+        if (h->tc) return rec_tc_run(h->tc, d_slopes, B, d_modes, (cudaStream_t)cuda_stream);
+    }
     // frames per warp tile: the whole batch when it is small, else 16 or 8, whichever pads less
     int FB = 1;
     while (FB < B && FB < 16) FB *= 2;
@@ -390,6 +408,7 @@ void pwfs_rec_destroy(pwfs_rec_t *h) {
     if (!h) return;
     cudaSetDevice(h->device);
     if (h->d_R) cudaFree(h->d_R);
+    rec_tc_destroy(h->tc);
     delete h;
 }
 

@@ -1,0 +1,323 @@
+// rec_tc.cu -- f2, modal reconstructor for a BATCH of frames on the 5th-generation
+// tensor cores: modes[b][m] = sum_j recmat[m][j] slopes[b][j] (reading F2g).
+//
+// This is the one dense contraction of the chain (n_modes x n_slopes x B).  The FP32 bar of the
+// parity tests (|d| <= 1e-5 sum |R||s|) rules out single-pass TF32 (2^-11 per operand), so every
+// operand is split into two TF32-representable planes, x = hi + lo + O(2^-22 |x|), and the product is
+//   R S^T ~= Rhi Shi^T + Rhi Slo^T + Rlo Shi^T        (dropped terms <= 3 * 2^-22 |R||S| = 7e-7)
+// accumulated in FP32 in tensor memory: three tcgen05.mma.kind::tf32 per K step, same accumulator.
+// recmat's planes are built once at create (it is static calibration data); the slope planes are
+// written by a small split kernel per call.
+//
+// Kernel (one 128 x 128 output tile of one K split per CTA, 192 threads):
+//   warp 0 (one lane)  TMA producer: four 128 x 32 FP32 boxes (Rhi, Rlo, Shi, Slo; 128-byte swizzle)
+//                      per stage into a 3-stage ring, completion on the stage's "full" mbarrier;
+//   warp 1 (one lane)  MMA issuer: per stage 4 K steps x 3 UMMAs (M 128, N 128, K 8) from shared-memory
+//                      descriptors into 128 TMEM columns; tcgen05.commit releases the stage ("empty")
+//                      and, after the last one, signals the epilogue;
+//   warps 2-5          epilogue: tcgen05.ld 32 lanes x 32 columns at a time, rows = modes so that a
+//                      column store is one coalesced 128-byte line of modes[b][m0..m0+32).
+// Tiles x K splits ~ number of SMs; the split-K partial sums are added in a fixed order by a second
+// kernel (deterministic, no atomics).  HBM-bound by design: 8 bytes of recmat planes per matrix
+// element per call, against 3 x 2 M N K TF32 flop.
+#include "rec_tc.cuh"
+
+#include <cuda.h>
+
+#include <cstdint>
+#include <new>
+
+#include "../../include/pwfs.h"
+
+namespace {
+
+constexpr int BM = 128, BN = 128, BK = 32, UK = 8, STAGES = 3;
+constexpr int kTileBytes = BM * BK * 4;               // 16 KB, one operand plane of one stage
+constexpr int kStageBytes = 4 * kTileBytes;           // Rhi, Rlo, Shi, Slo
+constexpr int kThreads = 192;
+constexpr uint32_t kTmemCols = 128;
+constexpr size_t kSmemBytes = (size_t)STAGES * kStageBytes + 1024 /* alignment slack */ + 256 /* barriers */;
+static_assert(BK * 4 == 128, "one K block is one 128-byte swizzle row");
+
+// tcgen05 instruction descriptor, kind::tf32: D = F32 (bits 4-5 = 1), A = B = TF32 (bits 7-9, 10-12 = 2),
+// both K-major (bits 15, 16 = 0), N >> 3 at bits 17-22, M >> 4 at bits 24-28.
+constexpr uint32_t kIdesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n" : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map, uint32_t bar, int c0, int c1) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+        ::"r"(dst), "l"((uint64_t)map), "r"(bar), "r"(c0), "r"(c1) : "memory");
+}
+// Shared-memory matrix descriptor, K-major operand in the canonical 128-byte-swizzle layout (what TMA
+// SWIZZLE_128B writes for a box of 32 floats x rows): start >> 4 at bits 0-13, leading offset unused for
+// swizzled K-major (1), stride offset = 8 rows x 128 B = 1024 >> 4 at bits 32-45, descriptor version 1
+// at bit 46, layout type SWIZZLE_128B = 2 at bits 61-63.
+__device__ __forceinline__ uint64_t smem_desc(uint32_t saddr) {
+    return (uint64_t)((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
+}
+__device__ __forceinline__ void umma_tf32(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n"
+        "}\n" ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(kIdesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tmem_ld_32x32(uint32_t taddr, uint32_t (&r)[32]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
+          "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
+          "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+        : "r"(taddr));
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+// grid (m_tiles, ksplit, n_tiles); block 192; dynamic smem kSmemBytes.
+// dst: modes [B][n_modes] when ksplit == 1, else partials [ksplit][B][n_modes].
+__global__ void __launch_bounds__(kThreads, 1)
+rec_tc_kernel(const __grid_constant__ CUtensorMap mRhi, const __grid_constant__ CUtensorMap mRlo,
+              const __grid_constant__ CUtensorMap mShi, const __grid_constant__ CUtensorMap mSlo,
+              float *__restrict__ dst, int n_modes, int B, int nkb, int ksplit) {
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;          // 128-byte swizzle needs 1024-byte tiles
+    const uint32_t bars = base + STAGES * kStageBytes;
+    // barriers: full[s] at +8 s, empty[s] at +8 (STAGES + s), accumulator-ready at +8 (2 STAGES); then the TMEM address
+    const uint32_t bar_acc = bars + 8 * (2 * STAGES);
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem_raw + (bars - smem_u32(smem_raw)) + 8 * (2 * STAGES + 1));
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int m_tile = blockIdx.x, ks = blockIdx.y, n_tile = blockIdx.z;
+    const int kb_lo = (int)(((long long)ks * nkb) / ksplit), kb_hi = (int)(((long long)(ks + 1) * nkb) / ksplit);
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < STAGES; ++s) { mbar_init(bars + 8 * s, 1); mbar_init(bars + 8 * (STAGES + s), 1); }
+        mbar_init(bar_acc, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 2) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "n"(kTmemCols) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem = *tmem_slot;
+
+    if (warp == 0) {
+        if (lane == 0) {                                                  // ---- TMA producer
+            int it = 0;
+            for (int kb = kb_lo; kb < kb_hi; ++kb, ++it) {
+                const int s = it % STAGES;
+                const uint32_t full = bars + 8 * s, empty = bars + 8 * (STAGES + s), st = base + s * kStageBytes;
+                mbar_wait(empty, ((it / STAGES) & 1) ^ 1);
+                mbar_expect_tx(full, kStageBytes);
+                tma_load_2d(st + 0 * kTileBytes, &mRhi, full, kb * BK, m_tile * BM);
+                tma_load_2d(st + 1 * kTileBytes, &mRlo, full, kb * BK, m_tile * BM);
+                tma_load_2d(st + 2 * kTileBytes, &mShi, full, kb * BK, n_tile * BN);
+                tma_load_2d(st + 3 * kTileBytes, &mSlo, full, kb * BK, n_tile * BN);
+            }
+        }
+    } else if (warp == 1) {
+        if (lane == 0) {                                                  // ---- MMA issuer
+            int it = 0;
+            for (int kb = kb_lo; kb < kb_hi; ++kb, ++it) {
+                const int s = it % STAGES;
+                const uint32_t full = bars + 8 * s, empty = bars + 8 * (STAGES + s), st = base + s * kStageBytes;
+                mbar_wait(full, (it / STAGES) & 1);
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll
+                for (int k = 0; k < BK / UK; ++k) {
+                    const uint32_t ko = k * UK * 4;                      // 32 bytes along the swizzled row
+                    const uint64_t rhi = smem_desc(st + 0 * kTileBytes + ko), rlo = smem_desc(st + 1 * kTileBytes + ko);
+                    const uint64_t shi = smem_desc(st + 2 * kTileBytes + ko), slo = smem_desc(st + 3 * kTileBytes + ko);
+                    umma_tf32(tmem, rlo, shi, (it > 0 || k > 0) ? 1u : 0u);   // small terms first
+                    umma_tf32(tmem, rhi, slo, 1u);
+                    umma_tf32(tmem, rhi, shi, 1u);
+                }
+                umma_commit(empty);                                       // frees the stage when these UMMAs retire
+            }
+            umma_commit(bar_acc);
+        }
+    } else {                                                              // ---- epilogue, warps 2..5
+        const int q = warp & 3;                                           // TMEM lane quarter this warp may read
+        mbar_wait(bar_acc, 0);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        const int m = m_tile * BM + q * 32 + lane;
+        float *out = dst + (size_t)ks * B * n_modes;
+        for (int c0 = 0; c0 < BN; c0 += 32) {
+            const int n0 = n_tile * BN + c0;
+            if (n0 >= B) break;                                           // warp-uniform
+            uint32_t r[32];
+            tmem_ld_32x32(tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)c0, r);
+            if (m < n_modes) {
+#pragma unroll
+                for (int j = 0; j < 32; ++j)
+                    if (n0 + j < B) out[(size_t)(n0 + j) * n_modes + m] = __uint_as_float(r[j]);
+            }
+        }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 2)
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(kTmemCols) : "memory");
+}
+
+// x -> hi = tf32(x), lo = tf32(x - hi) (round to nearest, low 13 mantissa bits zero), zero beyond `cols`.
+// grid (ceil(ldp / 256), rows)
+__global__ void split_tf32_kernel(const float *__restrict__ src, size_t src_pitch, int cols, int ldp,
+                                  float *__restrict__ hi, float *__restrict__ lo) {
+    const int c = blockIdx.x * blockDim.x + threadIdx.x, r = blockIdx.y;
+    if (c >= ldp) return;
+    const float x = c < cols ? __ldg(src + (size_t)r * src_pitch + c) : 0.f;
+    uint32_t h, l;
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(h) : "f"(x));
+    const float rest = x - __uint_as_float(h);
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(l) : "f"(rest));
+    hi[(size_t)r * ldp + c] = __uint_as_float(h);
+    lo[(size_t)r * ldp + c] = __uint_as_float(l);
+}
+
+// out[i] = sum_ks part[ks][i], fixed order
+__global__ void splitk_sum_kernel(const float *__restrict__ part, size_t n, int ksplit, float *__restrict__ out) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float s = 0.f;
+    for (int ks = 0; ks < ksplit; ++ks) s += __ldg(part + (size_t)ks * n + i);
+    out[i] = s;
+}
+
+using EncodeTiledFn = CUresult (*)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_tiled_fn() {
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+        return nullptr;
+    return reinterpret_cast<EncodeTiledFn>(fn);
+}
+
+// [rows][ldp] FP32 plane, box 32 (K) x 128 (rows), 128-byte swizzle; rows beyond `rows` read as zero
+bool make_map(EncodeTiledFn enc, CUtensorMap *map, const float *plane, int rows, int ldp) {
+    const cuuint64_t dims[2] = {(cuuint64_t)ldp, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)ldp * sizeof(float)};
+    const cuuint32_t box[2] = {(cuuint32_t)BK, (cuuint32_t)BM};
+    const cuuint32_t estr[2] = {1, 1};
+    return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float *>(plane), dims, strides, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+int cuda_rc(cudaError_t e) { return e == cudaErrorMemoryAllocation ? PWFS_ENOMEM : PWFS_ECUDA; }
+
+}  // namespace
+
+struct RecTc {
+    int device = 0, n_modes = 0, n_slopes = 0, ldp = 0, num_sms = 148;
+    EncodeTiledFn enc = nullptr;
+    float *d_Rhi = nullptr, *d_Rlo = nullptr;
+    float *d_Shi = nullptr, *d_Slo = nullptr, *d_part = nullptr;
+    int b_cap = 0;                  // frames the slope planes / partials are sized for
+    size_t part_cap = 0;            // floats in d_part
+    CUtensorMap mRhi, mRlo, mShi, mSlo;
+};
+
+int rec_tc_create(RecTc **out, const float *d_R, int n_modes, int n_slopes, int ldk, int device, int num_sms) {
+    *out = nullptr;
+    RecTc *h = new (std::nothrow) RecTc();
+    if (!h) return PWFS_ENOMEM;
+    h->device = device; h->n_modes = n_modes; h->n_slopes = n_slopes; h->num_sms = num_sms;
+    h->ldp = (n_slopes + BK - 1) / BK * BK;
+    h->enc = encode_tiled_fn();
+    if (!h->enc) { delete h; return PWFS_EUNSUPPORTED; }
+    const size_t bytes = (size_t)n_modes * h->ldp * sizeof(float);
+    cudaError_t e = cudaMalloc((void **)&h->d_Rhi, bytes);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_Rlo, bytes);
+    if (e == cudaSuccess) {
+        split_tf32_kernel<<<dim3((h->ldp + 255) / 256, n_modes), 256>>>(d_R, (size_t)ldk, n_slopes, h->ldp, h->d_Rhi, h->d_Rlo);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(rec_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+    if (e != cudaSuccess) { int rc = cuda_rc(e); rec_tc_destroy(h); return rc; }
+    if (!make_map(h->enc, &h->mRhi, h->d_Rhi, n_modes, h->ldp) || !make_map(h->enc, &h->mRlo, h->d_Rlo, n_modes, h->ldp)) {
+        rec_tc_destroy(h);
+        return PWFS_ECUDA;
+    }
+    *out = h;
+    return PWFS_OK;
+}
+
+int rec_tc_run(RecTc *h, const float *d_slopes, int B, float *d_modes, cudaStream_t st) {
+    const int m_tiles = (h->n_modes + BM - 1) / BM, n_tiles = (B + BN - 1) / BN, nkb = h->ldp / BK;
+    int ksplit = h->num_sms / (m_tiles * n_tiles);
+    if (ksplit > nkb / 4) ksplit = nkb / 4;                               // at least 4 K blocks per split
+    if (ksplit < 1) ksplit = 1;
+    const size_t part_need = ksplit > 1 ? (size_t)ksplit * B * h->n_modes : 0;
+    if (B > h->b_cap || part_need > h->part_cap) {                        // first call at this batch size: grow
+        if (cudaStreamSynchronize(st) != cudaSuccess) return PWFS_ECUDA;
+        if (B > h->b_cap) {
+            const int cap = (B + BN - 1) / BN * BN;
+            cudaFree(h->d_Shi); cudaFree(h->d_Slo);
+            h->d_Shi = h->d_Slo = nullptr; h->b_cap = 0;
+            const size_t bytes = (size_t)cap * h->ldp * sizeof(float);
+            cudaError_t e = cudaMalloc((void **)&h->d_Shi, bytes);
+            if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_Slo, bytes);
+            if (e == cudaSuccess) e = cudaMemset(h->d_Shi, 0, bytes);
+            if (e == cudaSuccess) e = cudaMemset(h->d_Slo, 0, bytes);
+            if (e != cudaSuccess) return cuda_rc(e);
+            if (!make_map(h->enc, &h->mShi, h->d_Shi, cap, h->ldp) || !make_map(h->enc, &h->mSlo, h->d_Slo, cap, h->ldp))
+                return PWFS_ECUDA;
+            h->b_cap = cap;
+        }
+        if (part_need > h->part_cap) {
+            cudaFree(h->d_part);
+            h->d_part = nullptr; h->part_cap = 0;
+            cudaError_t e = cudaMalloc((void **)&h->d_part, part_need * sizeof(float));
+            if (e != cudaSuccess) return cuda_rc(e);
+            h->part_cap = part_need;
+        }
+    }
+    split_tf32_kernel<<<dim3((h->ldp + 255) / 256, B), 256, 0, st>>>(d_slopes, (size_t)h->n_slopes, h->n_slopes, h->ldp,
+                                                                    h->d_Shi, h->d_Slo);
+    rec_tc_kernel<<<dim3(m_tiles, ksplit, n_tiles), kThreads, kSmemBytes, st>>>(
+        h->mRhi, h->mRlo, h->mShi, h->mSlo, ksplit > 1 ? h->d_part : d_modes, h->n_modes, B, nkb, ksplit);
+    if (ksplit > 1) {
+        const size_t n = (size_t)B * h->n_modes;
+        splitk_sum_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(h->d_part, n, ksplit, d_modes);
+    }
+    return cudaGetLastError() == cudaSuccess ? PWFS_OK : PWFS_ECUDA;
+}
+
+void rec_tc_destroy(RecTc *h) {
+    if (!h) return;
+    cudaFree(h->d_Rhi); cudaFree(h->d_Rlo); cudaFree(h->d_Shi); cudaFree(h->d_Slo); cudaFree(h->d_part);
+    delete h;
+}

@@ -156,7 +156,11 @@ def test_slopec_agrees_with_the_hot_path_slopes(torch_cuda):
 
 # ------------------------------------------------------------ reconstructor ---
 @pytest.mark.parametrize("n_modes,ns,B", [(54, 2512, 1), (5, 416, 3), (37, 1030, 17), (1, 1, 1), (33, 7, 2),
-                                          (300, 2528, 40), (1200, 416, 9), (4096, 11712, 1)])
+                                          (300, 2528, 40), (1200, 416, 9), (4096, 11712, 1),
+                                          # batches >= 24 frames run on the tensor cores (rec_tc.cu): ragged tiles in
+                                          # every dimension, K not a multiple of 32, two frame tiles, one K block
+                                          (130, 1000, 24), (257, 515, 130), (128, 2048, 128), (2100, 31, 33),
+                                          (64, 4100, 300)])
 def test_reconstructor_matches_matrix_product(torch_cuda, n_modes, ns, B):
     from oracle import chain_oracle as co
     from paper_1607_07624_b200.chain import Reconstructor
