@@ -190,7 +190,19 @@ def bench_stages(cfg, dev, phase, frames, flush, reps: int = 5) -> dict:
     with Reconstructor(R, device=dev.index) as rec:
         modes = torch.empty((B, n_modes), dtype=torch.float32, device=dev)
         ms = timed(lambda: rec.run(sl, out=modes))
-        out["f2_rec_batch"] = alu_row(ms, 2.0 * B * n_modes * 2 * nv, 1, f"{n_modes} modes x {2 * nv} slopes x {B} frames, FP32 FMA")
+        ns = 2 * nv
+        if B >= 24 and os.environ.get("PWFS_REC_TC", "1") != "0":   # chain_api.cu: batches run the tcgen05 TF32x3 kernel
+            row = hbm_row(ms, n_modes * ns * 4 + B * ns * 4 + B * n_modes * 4, 3,
+                          f"{n_modes} modes x {ns} slopes x {B} frames, tcgen05 TF32x3 (FP32 bar): algorithmic bytes = "
+                          "recmat once + slopes in + modes out; the kernel streams the two TF32 planes of recmat "
+                          "(8 B per element), see plane_frac")
+            ldp = -(-ns // 32) * 32
+            row["plane_bytes"] = int(2 * n_modes * ldp * 4)
+            row["plane_frac"] = row["plane_bytes"] / (ms * 1e-3) / 1e9 / hbm
+            row["tf32_tflops"] = 3 * 2.0 * B * n_modes * ns / (ms * 1e-3) / 1e12
+            out["f2_rec_batch"] = row
+        else:
+            out["f2_rec_batch"] = alu_row(ms, 2.0 * B * n_modes * ns, 1, f"{n_modes} modes x {ns} slopes x {B} frames, FP32 FMA")
         m1 = torch.empty((1, n_modes), dtype=torch.float32, device=dev)
         ms = timed(lambda: rec.run(sl[:1], out=m1))
         out["f2_rec_gemv"] = hbm_row(ms, n_modes * 2 * nv * 4, 1, "one frame: recmat streamed once")

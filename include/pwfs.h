@@ -130,9 +130,10 @@ int pwfs_run(pwfs_t *h, const float *d_phase, int32_t B, float *d_frames, float 
              void *cuda_stream);
 
 /* Same computation with HOST buffers (h_slopes may be NULL): copies the phase
- * batch host->device, runs, copies frames and slopes device->host on an
- * internal stream and returns after they have arrived (synchronous).  Pinned
- * host memory makes the copies asynchronous to the kernels of the previous
+ * batch host->device, runs, copies frames and slopes device->host and returns
+ * after they have arrived (synchronous).  Works chunk by chunk on three
+ * internal streams, so with pinned host memory the copy-in of the next chunk
+ * and the copy-out of the previous one run under the kernels of the current
  * chunk; pageable memory works but is slower. */
 int pwfs_run_host(pwfs_t *h, const float *h_phase, int32_t B, float *h_frames, float *h_slopes);
 

@@ -119,7 +119,8 @@ struct pwfs {
     float2 *T = nullptr; size_t T_elems = 0;
     float *colbin = nullptr; size_t colbin_elems = 0;
     // host-buffer path
-    cudaStream_t hstream = nullptr;
+    cudaStream_t hstream = nullptr, in_stream = nullptr, out_stream = nullptr;   // compute, H2D, D2H
+    std::vector<cudaEvent_t> in_ev, done_ev;                                     // per chunk
     float *d_phase = nullptr, *d_frames = nullptr, *d_slopes = nullptr;
     size_t d_cap_frames = 0;
     // schedule
@@ -488,6 +489,10 @@ void pwfs_destroy(pwfs_t *h) {
     if (h->d_frames) cudaFree(h->d_frames);
     if (h->d_slopes) cudaFree(h->d_slopes);
     if (h->hstream) cudaStreamDestroy(h->hstream);
+    if (h->in_stream) cudaStreamDestroy(h->in_stream);
+    if (h->out_stream) cudaStreamDestroy(h->out_stream);
+    for (auto ev : h->in_ev) cudaEventDestroy(ev);
+    for (auto ev : h->done_ev) cudaEventDestroy(ev);
     for (auto &sp : h->spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
     for (auto ev : h->event_pool) cudaEventDestroy(ev);
     delete h;
@@ -553,6 +558,39 @@ int pwfs_get_timing(pwfs_t *h, float ms[PWFS_NUM_KERNEL_CLASSES], int64_t launch
     return PWFS_OK;
 }
 
+// One chunk of Fc <= F frames: the four kernels of the path on `st`.
+static int run_chunk(pwfs_t *h, const float *d_phase, int Fc, float *d_frames, float *d_slopes, int ks, cudaStream_t st) {
+    const DevTables &t = h->tab;
+    const Launcher &L = h->L;
+    {   // K1: phasor + x-convolution (a1, a3, a4, a5 along x)
+        SpanGuard g(h, st, 0);
+        // split the x-tilt loop only as far as needed to fill the machine (>= 8 waves of 2 CTAs/SM),
+        // keeping >= 3 tilts per CTA so the one-off phasor stays amortised
+        const int row_ctas = (t.NP + L.RPC - 1) / L.RPC;
+        int jsplit = 1;
+        while ((long long)row_ctas * Fc * jsplit < 16LL * h->num_sms && t.KX / (jsplit + 1) >= 3) ++jsplit;
+        L.launch_x(dim3(row_ctas, jsplit, Fc), st, t, d_phase, h->T, jsplit);
+    }
+    {   // K2: y-convolution + |E|^2 over k + y-rebin (a3, a4, a5 along y, a6, a7)
+        SpanGuard g(h, st, 1);
+        const int per_cta = L.NB * L.WPB_Y;
+        L.launch_y(dim3((t.ncols + per_cta - 1) / per_cta, ks, Fc), st, t, h->T, h->colbin, ks);
+    }
+    {   // K3a: x-rebin (a7)
+        SpanGuard g(h, st, 2);
+        const int threads = std::min(256, (t.D + 31) / 32 * 32);
+        // 1/K of O6; the quarter-mask kernels leave O5's 1/M per axis (1/M^4 on |E|^2) to this scale
+        const double m4 = h->quarter ? std::pow((double)t.M, 4.0) : 1.0;
+        xrebin_kernel<<<dim3(t.D, Fc), threads, 0, st>>>(t, h->colbin, d_frames, ks, (float)(1.0 / ((double)t.K * m4)));
+    }
+    if (d_slopes) {   // K3b: slopes (a8)
+        SpanGuard g(h, st, 3);
+        slopes_kernel<<<Fc, 256, 0, st>>>(t, d_frames, d_slopes);
+    }
+    PWFS_CUDA(h, cudaGetLastError());
+    return PWFS_OK;
+}
+
 int pwfs_run(pwfs_t *h, const float *d_phase, int32_t B, float *d_frames, float *d_slopes, void *cuda_stream) {
     if (!h || B < 0) return PWFS_EINVAL;
     if (B == 0) return PWFS_OK;
@@ -564,37 +602,11 @@ int pwfs_run(pwfs_t *h, const float *d_phase, int32_t B, float *d_frames, float 
     schedule(h, B, &F, &ks);
     int rc = ensure_scratch(h, F, ks);
     if (rc) return rc;
-    const Launcher &L = h->L;
     const size_t NN = (size_t)t.N * t.N, DD = (size_t)t.D * t.D;
     for (int f0 = 0; f0 < B; f0 += F) {
-        const int Fc = std::min(F, B - f0);
-        {   // K1: phasor + x-convolution (a1, a3, a4, a5 along x)
-            SpanGuard g(h, st, 0);
-            // split the x-tilt loop only as far as needed to fill the machine (>= 8 waves of 2 CTAs/SM),
-            // keeping >= 3 tilts per CTA so the one-off phasor stays amortised
-            const int row_ctas = (t.NP + L.RPC - 1) / L.RPC;
-            int jsplit = 1;
-            while ((long long)row_ctas * Fc * jsplit < 16LL * h->num_sms && t.KX / (jsplit + 1) >= 3) ++jsplit;
-            L.launch_x(dim3(row_ctas, jsplit, Fc), st, t, d_phase + (size_t)f0 * NN, h->T, jsplit);
-        }
-        {   // K2: y-convolution + |E|^2 over k + y-rebin (a3, a4, a5 along y, a6, a7)
-            SpanGuard g(h, st, 1);
-            const int per_cta = L.NB * L.WPB_Y;
-            L.launch_y(dim3((t.ncols + per_cta - 1) / per_cta, ks, Fc), st, t, h->T, h->colbin, ks);
-        }
-        {   // K3a: x-rebin (a7)
-            SpanGuard g(h, st, 2);
-            const int threads = std::min(256, (t.D + 31) / 32 * 32);
-            // 1/K of O6; the quarter-mask kernels leave O5's 1/M per axis (1/M^4 on |E|^2) to this scale
-            const double m4 = h->quarter ? std::pow((double)t.M, 4.0) : 1.0;
-            xrebin_kernel<<<dim3(t.D, Fc), threads, 0, st>>>(t, h->colbin, d_frames + (size_t)f0 * DD, ks,
-                                                             (float)(1.0 / ((double)t.K * m4)));
-        }
-        if (d_slopes) {   // K3b: slopes (a8)
-            SpanGuard g(h, st, 3);
-            slopes_kernel<<<Fc, 256, 0, st>>>(t, d_frames + (size_t)f0 * DD, d_slopes + (size_t)f0 * 2 * t.n_valid);
-        }
-        PWFS_CUDA(h, cudaGetLastError());
+        rc = run_chunk(h, d_phase + (size_t)f0 * NN, std::min(F, B - f0), d_frames + (size_t)f0 * DD,
+                       d_slopes ? d_slopes + (size_t)f0 * 2 * t.n_valid : nullptr, ks, st);
+        if (rc) return rc;
     }
     return PWFS_OK;
 }
@@ -618,12 +630,38 @@ int pwfs_run_host(pwfs_t *h, const float *h_phase, int32_t B, float *h_frames, f
         if (e != cudaSuccess) { h->last_cuda = (int)e; return e == cudaErrorMemoryAllocation ? PWFS_ENOMEM : PWFS_ECUDA; }
         h->d_cap_frames = (size_t)B;
     }
-    PWFS_CUDA(h, cudaMemcpyAsync(h->d_phase, h_phase, (size_t)B * NN * sizeof(float), cudaMemcpyHostToDevice, h->hstream));
-    int rc = pwfs_run(h, h->d_phase, B, h->d_frames, h_slopes ? h->d_slopes : nullptr, h->hstream);
+    if (!h->in_stream) PWFS_CUDA(h, cudaStreamCreateWithFlags(&h->in_stream, cudaStreamNonBlocking));
+    if (!h->out_stream) PWFS_CUDA(h, cudaStreamCreateWithFlags(&h->out_stream, cudaStreamNonBlocking));
+    int F, ks;
+    schedule(h, B, &F, &ks);
+    int rc = ensure_scratch(h, F, ks);
     if (rc) return rc;
-    PWFS_CUDA(h, cudaMemcpyAsync(h_frames, h->d_frames, (size_t)B * DD * sizeof(float), cudaMemcpyDeviceToHost, h->hstream));
-    if (h_slopes)
-        PWFS_CUDA(h, cudaMemcpyAsync(h_slopes, h->d_slopes, (size_t)B * SS * sizeof(float), cudaMemcpyDeviceToHost, h->hstream));
+    const size_t n_chunks = ((size_t)B + F - 1) / F;
+    while (h->in_ev.size() < n_chunks) {
+        cudaEvent_t a, b;
+        PWFS_CUDA(h, cudaEventCreateWithFlags(&a, cudaEventDisableTiming));
+        h->in_ev.push_back(a);
+        PWFS_CUDA(h, cudaEventCreateWithFlags(&b, cudaEventDisableTiming));
+        h->done_ev.push_back(b);
+    }
+    // three streams, chunk by chunk: the copy-in of chunk c+1 and the copy-out of chunk c-1 run under
+    // the kernels of chunk c (pinned host memory; pageable memory degrades to staged copies)
+    size_t c = 0;
+    for (int f0 = 0; f0 < B; f0 += F, ++c) {
+        const int Fc = std::min(F, B - f0);
+        float *dp = h->d_phase + (size_t)f0 * NN, *df = h->d_frames + (size_t)f0 * DD, *ds = h->d_slopes + (size_t)f0 * SS;
+        PWFS_CUDA(h, cudaMemcpyAsync(dp, h_phase + (size_t)f0 * NN, (size_t)Fc * NN * sizeof(float), cudaMemcpyHostToDevice, h->in_stream));
+        PWFS_CUDA(h, cudaEventRecord(h->in_ev[c], h->in_stream));
+        PWFS_CUDA(h, cudaStreamWaitEvent(h->hstream, h->in_ev[c], 0));
+        rc = run_chunk(h, dp, Fc, df, h_slopes ? ds : nullptr, ks, h->hstream);
+        if (rc) return rc;
+        PWFS_CUDA(h, cudaEventRecord(h->done_ev[c], h->hstream));
+        PWFS_CUDA(h, cudaStreamWaitEvent(h->out_stream, h->done_ev[c], 0));
+        PWFS_CUDA(h, cudaMemcpyAsync(h_frames + (size_t)f0 * DD, df, (size_t)Fc * DD * sizeof(float), cudaMemcpyDeviceToHost, h->out_stream));
+        if (h_slopes)
+            PWFS_CUDA(h, cudaMemcpyAsync(h_slopes + (size_t)f0 * SS, ds, (size_t)Fc * SS * sizeof(float), cudaMemcpyDeviceToHost, h->out_stream));
+    }
+    PWFS_CUDA(h, cudaStreamSynchronize(h->out_stream));
     PWFS_CUDA(h, cudaStreamSynchronize(h->hstream));
     return PWFS_OK;
 }
