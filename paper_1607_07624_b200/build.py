@@ -15,8 +15,13 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libpwfs.so")
-SOURCES = [os.path.join(CSRC, n) for n in ("pwfs_api.cu", "atmo_api.cu", "chain_api.cu", "rec_tc.cu", "psf_api.cu", "sh_api.cu")]
-HEADERS = [os.path.join(CSRC, n) for n in ("pwfs_kernels.cuh", "pwfs_dft.cuh", "rec_tc.cuh")] + \
+GRID_R1 = (4, 5, 6, 8, 9, 10, 12, 15, 16, 18, 20, 24, 25, 27, 30, 32)   # PWFS_FOR_EACH_R1 of csrc/pwfs_launch.cuh
+# (source, extra flags, object name): the FFT kernels of each grid size M = 32 R1 are their own translation unit
+UNITS = [(os.path.join(CSRC, n), [], n[:-3] + ".o")
+         for n in ("pwfs_api.cu", "atmo_api.cu", "chain_api.cu", "rec_tc.cu", "psf_api.cu", "sh_api.cu")] + \
+        [(os.path.join(CSRC, "pwfs_inst.cu"), [f"-DPWFS_INST_R1={r}"], f"pwfs_inst_r{r}.o") for r in GRID_R1]
+SOURCES = sorted({u[0] for u in UNITS})
+HEADERS = [os.path.join(CSRC, n) for n in ("pwfs_kernels.cuh", "pwfs_dft.cuh", "pwfs_launch.cuh", "rec_tc.cuh")] + \
           [os.path.join(ROOT, "include", n) for n in ("pwfs.h", "pwfs_atmo.h", "pwfs_chain.h", "pwfs_psf.h", "pwfs_sh.h")]
 OBJDIR = os.path.join(HERE, "build")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
@@ -38,11 +43,12 @@ def up_to_date() -> bool:
     return _newer(LIB, SOURCES + HEADERS)
 
 
-def _compile(src: str, force: bool, verbose: bool) -> str:
-    obj = os.path.join(OBJDIR, os.path.basename(src)[:-3] + ".o")
+def _compile(unit, force: bool, verbose: bool) -> str:
+    src, extra, name = unit
+    obj = os.path.join(OBJDIR, name)
     if not force and _newer(obj, [src] + HEADERS):
         return obj
-    cmd = [nvcc_path()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, src]
+    cmd = [nvcc_path()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, src]
     if verbose:
         print(" ".join(cmd), flush=True)
     subprocess.run(cmd, check=True)
@@ -54,8 +60,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and up_to_date():
         return LIB
     os.makedirs(OBJDIR, exist_ok=True)
-    with ThreadPoolExecutor(max_workers=len(SOURCES)) as pool:
-        objs = list(pool.map(lambda s: _compile(s, force, verbose), SOURCES))
+    with ThreadPoolExecutor(max_workers=min(len(UNITS), os.cpu_count() or 4)) as pool:
+        objs = list(pool.map(lambda u: _compile(u, force, verbose), UNITS))
     tmp = LIB + f".tmp{os.getpid()}"
     subprocess.run([nvcc_path(), "--shared", "-o", tmp] + objs, check=True)
     os.replace(tmp, LIB)

@@ -223,12 +223,20 @@ bool find_psf_launcher(int M, PsfLauncher *out) {
     if (M % 32) return false;
     switch (M / 32) {
         case 4:  *out = make<PsfCfg<4, 8, 4>>(); return true;
+        case 5:  *out = make<PsfCfg<5, 6, 4>>(); return true;
+        case 6:  *out = make<PsfCfg<6, 5, 4>>(); return true;
         case 8:  *out = make<PsfCfg<8, 4, 4>>(); return true;
+        case 9:  *out = make<PsfCfg<9, 3, 4>>(); return true;
         case 10: *out = make<PsfCfg<10, 3, 4>>(); return true;
+        case 12: *out = make<PsfCfg<12, 2, 4>>(); return true;
         case 15: *out = make<PsfCfg<15, 2, 4>>(); return true;
         case 16: *out = make<PsfCfg<16, 2, 4>>(); return true;
+        case 18: *out = make<PsfCfg<18, 1, 8>>(); return true;
         case 20: *out = make<PsfCfg<20, 1, 8>>(); return true;
+        case 24: *out = make<PsfCfg<24, 1, 8>>(); return true;
         case 25: *out = make<PsfCfg<25, 1, 8>>(); return true;
+        case 27: *out = make<PsfCfg<27, 1, 8>>(); return true;
+        case 30: *out = make<PsfCfg<30, 1, 8>>(); return true;
         case 32: *out = make<PsfCfg<32, 1, 8>>(); return true;
         default: return false;
     }

@@ -14,7 +14,7 @@
 #include <new>
 #include <vector>
 
-#include "pwfs_kernels.cuh"
+#include "pwfs_launch.cuh"
 
 using namespace pwk;
 
@@ -22,80 +22,14 @@ namespace {
 
 constexpr double kTwoPi = 6.283185307179586476925286766559;
 
-// ---- per-grid kernel configurations (R1 = M/32, NB, warps/CTA row pass, column pass)
-using Cfg4 = PassCfg<4, 8, 4, 4>;     // M = 128
-using Cfg8 = PassCfg<8, 4, 4, 4>;     // M = 256
-using Cfg10 = PassCfg<10, 3, 8, 4, 2, 1>;  // M = 320
-using Cfg15 = PassCfg<15, 2, 8, 4, 2, 1>;   // M = 480
-using Cfg16 = PassCfg<16, 2, 8, 4, 2, 1>;   // M = 512
-using Cfg20 = PassCfg<20, 1, 8, 4, 2, 1>;  // M = 640
-using Cfg25 = PassCfg<25, 1, 8, 4, 2, 1>;  // M = 800
-#ifndef PWFS_C32_WX
-#define PWFS_C32_WX 8
-#define PWFS_C32_WY 4
-#define PWFS_C32_MX 2
-#define PWFS_C32_MY 2
-#endif
-using Cfg32 = PassCfg<32, 1, PWFS_C32_WX, PWFS_C32_WY, PWFS_C32_MX, PWFS_C32_MY>;  // M = 1024
-
-struct Launcher {
-    int R1, NB, WPB_X, WPB_Y, RPC;
-    size_t smem_x, smem_y;
-    const void *xfn, *yfn;
-    void (*launch_x)(dim3, cudaStream_t, const DevTables &, const float *, float2 *, int);
-    void (*launch_y)(dim3, cudaStream_t, const DevTables &, const float2 *, float *, int);
-};
-
-template <class C, bool QM>
-void launch_x_t(dim3 grid, cudaStream_t st, const DevTables &t, const float *phase, float2 *T, int jsplit) {
-    xpass_kernel<C, QM><<<grid, 32 * C::WPB_X, QM ? C::smem_x_q : C::smem_x_t, st>>>(t, phase, T, jsplit);
-}
-template <class C, bool QM>
-void launch_y_t(dim3 grid, cudaStream_t st, const DevTables &t, const float2 *T, float *colbin, int ksplit) {
-    ypass_kernel<C, QM><<<grid, 32 * C::WPB_Y, C::smem_y, st>>>(t, T, colbin, ksplit);
-}
-template <class C, bool QM>
-Launcher make_launcher_q() {
-    Launcher l;
-    l.R1 = C::R1; l.NB = C::NB; l.WPB_X = C::WPB_X; l.WPB_Y = C::WPB_Y; l.RPC = C::RPC;
-    l.smem_x = QM ? C::smem_x_q : C::smem_x_t; l.smem_y = C::smem_y;
-    l.xfn = (const void *)xpass_kernel<C, QM>;
-    l.yfn = (const void *)ypass_kernel<C, QM>;
-    l.launch_x = launch_x_t<C, QM>;
-    l.launch_y = launch_y_t<C, QM>;
-    return l;
-}
-// quarter = the mask shift is exactly M/4: kernels with the table-free power-of-i mask
-template <class C>
-Launcher make_launcher(bool quarter) { return quarter ? make_launcher_q<C, true>() : make_launcher_q<C, false>(); }
-
+// One kernel family per grid size M = 32 R1 (pwfs_launch.cuh); each is instantiated in its own
+// translation unit (pwfs_inst.cu compiled with -DPWFS_INST_R1=<R1>) so that the build runs in parallel.
 bool find_launcher(int M, bool quarter, Launcher *out) {
     if (M % 32) return false;
     switch (M / 32) {
-#if !defined(PWFS_ONLY_R1) || PWFS_ONLY_R1 == 4
-        case 4: *out = make_launcher<Cfg4>(quarter); return true;
-#endif
-#if !defined(PWFS_ONLY_R1) || PWFS_ONLY_R1 == 8
-        case 8: *out = make_launcher<Cfg8>(quarter); return true;
-#endif
-#if !defined(PWFS_ONLY_R1) || PWFS_ONLY_R1 == 10
-        case 10: *out = make_launcher<Cfg10>(quarter); return true;
-#endif
-#if !defined(PWFS_ONLY_R1) || PWFS_ONLY_R1 == 15
-        case 15: *out = make_launcher<Cfg15>(quarter); return true;
-#endif
-#if !defined(PWFS_ONLY_R1) || PWFS_ONLY_R1 == 16
-        case 16: *out = make_launcher<Cfg16>(quarter); return true;
-#endif
-#if !defined(PWFS_ONLY_R1) || PWFS_ONLY_R1 == 20
-        case 20: *out = make_launcher<Cfg20>(quarter); return true;
-#endif
-#if !defined(PWFS_ONLY_R1) || PWFS_ONLY_R1 == 25
-        case 25: *out = make_launcher<Cfg25>(quarter); return true;
-#endif
-#if !defined(PWFS_ONLY_R1) || PWFS_ONLY_R1 == 32
-        case 32: *out = make_launcher<Cfg32>(quarter); return true;
-#endif
+#define PWFS_CASE(R) case R: *out = launcher_for<R>(quarter); return true;
+        PWFS_FOR_EACH_R1(PWFS_CASE)
+#undef PWFS_CASE
         default: return false;
     }
 }

@@ -1,0 +1,39 @@
+// pwfs_inst.cu -- the row-pass / column-pass kernels of ONE grid size, M = 32 * PWFS_INST_R1, both
+// mask variants.  build.py compiles this file once per R1 of PWFS_FOR_EACH_R1 (pwfs_launch.cuh).
+#include "pwfs_launch.cuh"
+
+#ifndef PWFS_INST_R1
+#define PWFS_INST_R1 4   // a bare `nvcc -c` of this file still gives a valid object
+#endif
+
+namespace pwk {
+namespace {
+
+using C = CfgFor<PWFS_INST_R1>::type;
+
+template <bool QM>
+void launch_x_t(dim3 grid, cudaStream_t st, const DevTables &t, const float *phase, float2 *T, int jsplit) {
+    xpass_kernel<C, QM><<<grid, 32 * C::WPB_X, QM ? C::smem_x_q : C::smem_x_t, st>>>(t, phase, T, jsplit);
+}
+template <bool QM>
+void launch_y_t(dim3 grid, cudaStream_t st, const DevTables &t, const float2 *T, float *colbin, int ksplit) {
+    ypass_kernel<C, QM><<<grid, 32 * C::WPB_Y, C::smem_y, st>>>(t, T, colbin, ksplit);
+}
+template <bool QM>
+Launcher make() {
+    Launcher l;
+    l.R1 = C::R1; l.NB = C::NB; l.WPB_X = C::WPB_X; l.WPB_Y = C::WPB_Y; l.RPC = C::RPC;
+    l.smem_x = QM ? C::smem_x_q : C::smem_x_t; l.smem_y = C::smem_y;
+    l.xfn = (const void *)xpass_kernel<C, QM>;
+    l.yfn = (const void *)ypass_kernel<C, QM>;
+    l.launch_x = launch_x_t<QM>;
+    l.launch_y = launch_y_t<QM>;
+    return l;
+}
+
+}  // namespace
+
+template <>
+Launcher launcher_for<PWFS_INST_R1>(bool quarter) { return quarter ? make<true>() : make<false>(); }
+
+}  // namespace pwk

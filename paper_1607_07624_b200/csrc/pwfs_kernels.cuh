@@ -390,7 +390,7 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
 // ------------------------------------------------------------------ K3a -----
 // frame[f][jy][jx] = (1/K) sum_ks sum_c wx[jx][c] colbin[f][ks][xc(jx,c)][jy]
 // grid (D (jx), F); block covers jy.
-__global__ void xrebin_kernel(DevTables t, const float *__restrict__ colbin, float *__restrict__ frames,
+static __global__ void xrebin_kernel(DevTables t, const float *__restrict__ colbin, float *__restrict__ frames,
                               int ksplit, float scale) {
     const int jx = blockIdx.x, f = blockIdx.y;
     const int D = t.D;
@@ -413,7 +413,7 @@ __global__ void xrebin_kernel(DevTables t, const float *__restrict__ colbin, flo
 
 // ------------------------------------------------------------------ K3b -----
 // One CTA per frame: nbar = mean over valid subaps of a+b+c+d, then slopes.
-__global__ void slopes_kernel(DevTables t, const float *__restrict__ frames, float *__restrict__ slopes) {
+static __global__ void slopes_kernel(DevTables t, const float *__restrict__ frames, float *__restrict__ slopes) {
     __shared__ float red[32];
     __shared__ float s_nbar;
     const int f = blockIdx.x, D = t.D, ns = t.n_sub, nv = t.n_valid;

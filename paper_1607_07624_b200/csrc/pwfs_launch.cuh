@@ -1,0 +1,49 @@
+// pwfs_launch.cuh -- the kernel configuration of every supported grid size M = 32 R1 and the
+// launcher record pwfs_api.cu dispatches through.  launcher_for<R1>() is defined once per R1 in
+// pwfs_inst.cu (one translation unit per grid size).
+#pragma once
+#include "pwfs_kernels.cuh"
+
+namespace pwk {
+
+// R1 = M / 32 of the built grids: M = 128 ... 1024, every 2/3/5-smooth multiple of 32 in that range
+// except 32 * {1, 2, 3}  (M >= 128 keeps at least four register points per lane)
+#define PWFS_FOR_EACH_R1(X) X(4) X(5) X(6) X(8) X(9) X(10) X(12) X(15) X(16) X(18) X(20) X(24) X(25) X(27) X(30) X(32)
+
+// PassCfg<R1, NB, warps/CTA row pass, warps/CTA column pass, min CTAs/SM row pass, column pass>:
+// NB transforms per warp so that NB * R1 fills whole rounds of 32 lanes in the size-32 stage as far as
+// the register file allows (accumulators NB * R1, prefetch NB * ceil(R1/2) complex).
+template <int R1> struct CfgFor;
+template <> struct CfgFor<4>  { using type = PassCfg<4, 8, 4, 4>; };          // M = 128
+template <> struct CfgFor<5>  { using type = PassCfg<5, 6, 4, 4>; };          // M = 160
+template <> struct CfgFor<6>  { using type = PassCfg<6, 5, 8, 4>; };          // M = 192
+template <> struct CfgFor<8>  { using type = PassCfg<8, 4, 4, 4>; };          // M = 256
+template <> struct CfgFor<9>  { using type = PassCfg<9, 3, 8, 4>; };          // M = 288
+template <> struct CfgFor<10> { using type = PassCfg<10, 3, 8, 4, 2, 1>; };   // M = 320
+template <> struct CfgFor<12> { using type = PassCfg<12, 5, 8, 4>; };         // M = 384
+template <> struct CfgFor<15> { using type = PassCfg<15, 2, 8, 4, 2, 1>; };   // M = 480
+template <> struct CfgFor<16> { using type = PassCfg<16, 2, 8, 4, 2, 1>; };   // M = 512
+template <> struct CfgFor<18> { using type = PassCfg<18, 3, 8, 4, 2, 1>; };   // M = 576
+template <> struct CfgFor<20> { using type = PassCfg<20, 1, 8, 4, 2, 1>; };   // M = 640
+template <> struct CfgFor<24> { using type = PassCfg<24, 1, 8, 4, 2, 1>; };   // M = 768
+template <> struct CfgFor<25> { using type = PassCfg<25, 1, 8, 4, 2, 1>; };   // M = 800
+template <> struct CfgFor<27> { using type = PassCfg<27, 1, 8, 4, 2, 1>; };   // M = 864
+template <> struct CfgFor<30> { using type = PassCfg<30, 1, 8, 4, 2, 1>; };   // M = 960
+template <> struct CfgFor<32> { using type = PassCfg<32, 1, 8, 4, 2, 2>; };   // M = 1024
+
+struct Launcher {
+    int R1, NB, WPB_X, WPB_Y, RPC;
+    size_t smem_x, smem_y;
+    const void *xfn, *yfn;
+    void (*launch_x)(dim3, cudaStream_t, const DevTables &, const float *, float2 *, int);
+    void (*launch_y)(dim3, cudaStream_t, const DevTables &, const float2 *, float *, int);
+};
+
+// quarter = the mask shift is exactly M/4 and there is no field stop: kernels with the table-free
+// power-of-i mask; otherwise the table-mask kernels
+template <int R1> Launcher launcher_for(bool quarter);
+#define PWFS_DECL(R) template <> Launcher launcher_for<R>(bool quarter);
+PWFS_FOR_EACH_R1(PWFS_DECL)
+#undef PWFS_DECL
+
+}  // namespace pwk

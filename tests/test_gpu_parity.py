@@ -106,6 +106,15 @@ def test_full_size_configs_sampled_frames(torch_cuda, name, frames):
     (250, 512, 50, 6, 2.5),      # M = 512, ragged N
     (300, 640, 30, 4, 1.0),      # M = 640
     (37, 320, 37, 3, 0.7),       # tiny pupil in a large grid, b = 1
+    # the other grids M = 32 R1 (radix-3/5/9/27 register stages, odd warp batches NB = 3, 5, 6)
+    (80, 160, 20, 4, 1.0),       # R1 = 5
+    (90, 192, 18, 6, 1.5),       # R1 = 6, margins
+    (144, 288, 24, 4, 2.0),      # R1 = 9
+    (190, 384, 38, 3, 1.0),      # R1 = 12
+    (288, 576, 36, 4, 2.0),      # R1 = 18
+    (380, 768, 76, 3, 1.0),      # R1 = 24
+    (432, 864, 54, 2, 1.0),      # R1 = 27
+    (470, 960, 47, 2, 1.5),      # R1 = 30, ragged N
 ])
 def test_geometries(torch_cuda, N, M, ns, K, r):
     rng = np.random.default_rng(N * 7 + M)

@@ -55,7 +55,9 @@ def _check(torch, A, phase, M, scale=1.0):
 @pytest.mark.parametrize("N,M,B,rms", [(64, 128, 3, 1.0), (37, 128, 2, 0.5), (100, 256, 3, 2.0), (160, 320, 3, 3.0),
                                        (150, 320, 2, 1.0), (240, 480, 2, 2.0), (120, 512, 2, 1.0), (256, 512, 2, 4.0),
                                        (60, 640, 1, 1.0), (320, 640, 2, 2.0), (400, 800, 2, 3.0), (480, 1024, 2, 5.0),
-                                       (500, 1024, 1, 1.0)])
+                                       (500, 1024, 1, 1.0),
+                                       (80, 160, 2, 1.0), (96, 192, 2, 2.0), (140, 288, 2, 1.0), (192, 384, 2, 3.0),
+                                       (288, 576, 2, 2.0), (384, 768, 1, 2.0), (430, 864, 1, 1.0), (480, 960, 1, 3.0)])
 def test_psf_matches_oracle_on_every_grid(torch_cuda, N, M, B, rms):
     rng = np.random.default_rng(N * 7 + M)
     _check(torch_cuda, _disc(N, 0.15), _smooth_phase(rng, B, N, rms), M)
