@@ -26,6 +26,8 @@
 #pragma once
 #include "pwfs_dft.cuh"
 
+#include <type_traits>
+
 namespace pwk {
 
 constexpr float kInv2PiHi = 0.15915493667125702f;   // fl32(1/(2 pi))
@@ -45,6 +47,9 @@ struct PassCfg {
     // columns per instruction: a warp stride of 2 (mod 16) 64-bit banks keeps those reads conflict-free.
     static constexpr int WARP_BUF = (ITEMS * kPitch + 15) / 16 * 16 + 2;
     static constexpr int TAB = R1_ * kPitch;              // float2 per table (twiddle, mask)
+    // M = 2048: the row pass's shared memory is full, the general-mask table a(u)/M is read through L1 instead
+    static constexpr bool AM_GLOBAL = R1_ > 32;
+    static constexpr int AM_PITCH = AM_GLOBAL ? 32 : kPitch;
     static constexpr int WPB_X = WPB_X_;     // warps per CTA, row pass
     static constexpr int WPB_Y = WPB_Y_;     // warps per CTA, column pass
     static constexpr int MINB_X = MINB_X_;   // CTAs per SM the register allocation must allow
@@ -53,7 +58,7 @@ struct PassCfg {
     static_assert(RPC % kTB == 0, "row pass: rows per CTA must be whole y-blocks of T");
     // row pass: tables (no mask table for the quarter mask) + exchange buffers + base phasor [RPC][NZ][32]
     static constexpr size_t smem_x_q = (size_t)(WPB_X_ * WARP_BUF + 1 * TAB + RPC * NZ * 32) * sizeof(float2);
-    static constexpr size_t smem_x_t = (size_t)(WPB_X_ * WARP_BUF + 2 * TAB + RPC * NZ * 32) * sizeof(float2);
+    static constexpr size_t smem_x_t = (size_t)(WPB_X_ * WARP_BUF + (AM_GLOBAL ? 1 : 2) * TAB + RPC * NZ * 32) * sizeof(float2);
     static constexpr size_t smem_y = (size_t)(WPB_Y_ * WARP_BUF + 2 * TAB) * sizeof(float2);
 };
 
@@ -79,12 +84,12 @@ struct DevTables {
     const int *vidx;          // [n_valid] j*n_sub + i of valid subapertures, row-major
 };
 
-template <bool QM>
+template <bool QM, bool AM_GLOBAL = false>
 __device__ __forceinline__ void load_tables(float2 *s_tw, float2 *s_am, const DevTables &t, int R1) {
     for (int i = threadIdx.x; i < R1 * 32; i += blockDim.x) {
         int k1 = i >> 5, n2 = i & 31;
         s_tw[k1 * kPitch + n2] = t.tw[i];
-        if constexpr (!QM) s_am[k1 * kPitch + n2] = t.am[i];
+        if constexpr (!QM && !AM_GLOBAL) s_am[k1 * kPitch + n2] = t.am[i];
     }
 }
 
@@ -141,7 +146,7 @@ __device__ __forceinline__ void stage32(float2 *buf, const float2 *s_tw, const f
                 const float sg = (k1 & 1) ? -1.f : 1.f;
                 idft32_signed_upper(u, make_float2(sg, sg));
             } else {
-                const float2 *amr = s_am + k1 * kPitch;
+                const float2 *amr = s_am + k1 * C::AM_PITCH;      // shared memory, or t.am itself (AM_GLOBAL)
 #pragma unroll
                 for (int k2 = 0; k2 < 32; ++k2) u[k2] = cmul(u[k2], amr[k2]);
                 Dft<32, +1>::run(u);
@@ -181,8 +186,8 @@ __global__ void __launch_bounds__(32 * C::WPB_X, C::MINB_X)
 xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ T, int jsplit) {
     extern __shared__ float2 smem[];
     float2 *s_tw = smem;
-    float2 *s_am = smem + C::TAB;                              // unused (zero-sized) when QM
-    float2 *s_buf = smem + (QM ? 1 : 2) * C::TAB;
+    const float2 *s_am = C::AM_GLOBAL ? t.am : smem + C::TAB;  // unused (zero-sized) when QM
+    float2 *s_buf = smem + ((QM || C::AM_GLOBAL) ? 1 : 2) * C::TAB;
     float2 *s_p = s_buf + C::WPB_X * C::WARP_BUF;              // [RPC][NZ][32] base phasor
     const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
     const int N = t.N;
@@ -191,7 +196,7 @@ xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ 
     float2 *buf = s_buf + wl * C::WARP_BUF;
     float2 *pw = s_p + (size_t)wl * C::NB * C::NZ * 32 + lane;
 
-    load_tables<QM>(s_tw, s_am, t, C::R1);
+    load_tables<QM, C::AM_GLOBAL>(s_tw, smem + C::TAB, t, C::R1);
 
     // a1: base phasor of this warp's rows, x = 32 n1 + lane
 #pragma unroll
@@ -223,16 +228,17 @@ xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ 
     // x = 32 n1 + n2 lie inside a pupil-image window (bit n1 of wmask[it])
     int item_src[C::NB];          // exchange-buffer offset of (row r, k1 = 0, n2)
     int item_dst[C::NB];          // T offset of (x = n2, y = y0 + r) within the (f, j) slab
-    unsigned wmask[C::NB];
+    using wmask_t = std::conditional_t<(C::R1 > 32), unsigned long long, unsigned>;
+    wmask_t wmask[C::NB];
 #pragma unroll
     for (int it = 0; it < C::NB; ++it) {
         const int i = threadIdx.x + it * 32 * C::WPB_X;
         const int r = i % C::RPC, n2 = i / C::RPC;
         item_src[it] = (r / C::NB) * C::WARP_BUF + (r % C::NB) * C::R1 * kPitch + n2;
         item_dst[it] = n2 * t.NP + y0 + r;
-        unsigned m = 0;
+        wmask_t m = 0;
         if (y0 + r < t.NP)
-            for (int n1 = 0; n1 < C::R1; ++n1) m |= (__ldg(t.xc_of_x + 32 * n1 + n2) >= 0 ? 1u : 0u) << n1;
+            for (int n1 = 0; n1 < C::R1; ++n1) m |= (wmask_t)(__ldg(t.xc_of_x + 32 * n1 + n2) >= 0 ? 1u : 0u) << n1;
         wmask[it] = m;
     }
 
@@ -274,7 +280,7 @@ xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ 
             apply_ipow_k1<C::R1, QM>(v);
             Dft<C::R1, +1>::run(v);
             float2 *dst = Tj + item_dst[it];
-            const unsigned m = wmask[it];
+            const wmask_t m = wmask[it];
 #pragma unroll
             for (int n1 = 0; n1 < C::R1; ++n1)
                 if ((m >> n1) & 1u) dst[n1 * n1_stride] = v[n1];
@@ -293,7 +299,7 @@ __global__ void __launch_bounds__(32 * C::WPB_Y, C::MINB_Y)
 ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colbin, int ksplit) {
     extern __shared__ float2 smem[];
     float2 *s_tw = smem;
-    float2 *s_am = smem + C::TAB;
+    const float2 *s_am = C::AM_GLOBAL ? t.am : smem + C::TAB;
     float2 *s_buf = smem + 2 * C::TAB;
     const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
     const int NP = t.NP;
@@ -301,7 +307,7 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
     const int xc0 = (blockIdx.x * C::WPB_Y + wl) * C::NB;
     float2 *buf = s_buf + wl * C::WARP_BUF;
 
-    load_tables<QM>(s_tw, s_am, t, C::R1);
+    load_tables<QM, C::AM_GLOBAL>(s_tw, smem + C::TAB, t, C::R1);
     __syncthreads();
     if (xc0 >= t.ncols) return;
 

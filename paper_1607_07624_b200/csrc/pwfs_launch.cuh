@@ -8,7 +8,7 @@ namespace pwk {
 
 // R1 = M / 32 of the built grids: M = 128 ... 1024, every 2/3/5-smooth multiple of 32 in that range
 // except 32 * {1, 2, 3}  (M >= 128 keeps at least four register points per lane)
-#define PWFS_FOR_EACH_R1(X) X(4) X(5) X(6) X(8) X(9) X(10) X(12) X(15) X(16) X(18) X(20) X(24) X(25) X(27) X(30) X(32)
+#define PWFS_FOR_EACH_R1(X) X(4) X(5) X(6) X(8) X(9) X(10) X(12) X(15) X(16) X(18) X(20) X(24) X(25) X(27) X(30) X(32) X(64)
 
 // PassCfg<R1, NB, warps/CTA row pass, warps/CTA column pass, min CTAs/SM row pass, column pass>:
 // NB transforms per warp so that NB * R1 fills whole rounds of 32 lanes in the size-32 stage as far as
@@ -30,6 +30,7 @@ template <> struct CfgFor<25> { using type = PassCfg<25, 1, 8, 4, 2, 1>; };   //
 template <> struct CfgFor<27> { using type = PassCfg<27, 1, 8, 4, 2, 1>; };   // M = 864
 template <> struct CfgFor<30> { using type = PassCfg<30, 1, 8, 4, 2, 1>; };   // M = 960
 template <> struct CfgFor<32> { using type = PassCfg<32, 1, 8, 4, 2, 2>; };   // M = 1024
+template <> struct CfgFor<64> { using type = PassCfg<64, 1, 8, 4, 1, 1>; };   // M = 2048
 
 struct Launcher {
     int R1, NB, WPB_X, WPB_Y, RPC;

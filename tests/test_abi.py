@@ -176,9 +176,9 @@ def test_strerror_and_supported_grid(lib):
     assert "memory" in pwfs.strerror(pwfs.PWFS_ENOMEM)
     assert "CUDA" in pwfs.strerror(pwfs.PWFS_ECUDA)
     assert "unknown" in pwfs.strerror(-99)
-    for m in (128, 160, 192, 256, 288, 320, 384, 480, 512, 576, 640, 768, 800, 864, 960, 1024):
+    for m in (128, 160, 192, 256, 288, 320, 384, 480, 512, 576, 640, 768, 800, 864, 960, 1024, 2048):
         assert pwfs.supported_grid(m)
-    for m in (0, 96, 100, 2048, 1000, 224, 352, 416, 448, 1056):
+    for m in (0, 96, 100, 4096, 1000, 224, 352, 416, 448, 1056):
         assert not pwfs.supported_grid(m)
 
 

@@ -115,6 +115,7 @@ def test_full_size_configs_sampled_frames(torch_cuda, name, frames):
     (380, 768, 76, 3, 1.0),      # R1 = 24
     (432, 864, 54, 2, 1.0),      # R1 = 27
     (470, 960, 47, 2, 1.5),      # R1 = 30, ragged N
+    (1000, 2048, 100, 2, 2.0),   # R1 = 64: 64 register points per lane, two rounds of size-32 transforms
 ])
 def test_geometries(torch_cuda, N, M, ns, K, r):
     rng = np.random.default_rng(N * 7 + M)
@@ -262,6 +263,8 @@ def test_f3_uniform_circle_list_equals_the_circle_bit_for_bit(torch_cuda):
     (160, 320, 40, 103.0),    # cfg2 geometry, FoV 2" at 750 nm on 8.2 m ~ +-103 bins
     (240, 480, 40, 100.0),
     (250, 512, 50, 200.0),
+    (288, 576, 36, 150.0),    # R1 = 18 on the table-mask kernels
+    (900, 2048, 90, 500.0),   # M = 2048: mask table read through L1 (AM_GLOBAL)
 ])
 def test_f3_weighted_list_and_stop(torch_cuda, N, M, ns, stop):
     rng = np.random.default_rng(N + M)
