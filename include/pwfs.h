@@ -57,7 +57,8 @@ typedef enum {
 typedef struct {
     int32_t n_pupil;        /* N >= 2 : pupil sampling, D spans exactly N px                  */
     int32_t m_grid;         /* M : FFT grid.  M >= 2N, M = 32*R with R in the built set: every
-                               2/3/5-smooth R in 4..32, i.e. M = 128 ... 1024 (pwfs_supported_grid) */
+                               2/3/5-smooth R in 4..64, i.e. 24 grids from M = 128 to 2048
+                               (pwfs_supported_grid)                                          */
     const float *pupil_amp; /* HOST ptr, N*N floats row-major [y][x]; amplitude A >= 0; copied */
     int32_t mask_shift_px;  /* s : pupil-image offset in px (mask phase 2 pi s (|u~|+|v~|)/M).
                                <= 0 selects the default M/4 (needs M % 4 == 0).

@@ -6,9 +6,10 @@
 
 namespace pwk {
 
-// R1 = M / 32 of the built grids: M = 128 ... 1024, every 2/3/5-smooth multiple of 32 in that range
-// except 32 * {1, 2, 3}  (M >= 128 keeps at least four register points per lane)
-#define PWFS_FOR_EACH_R1(X) X(4) X(5) X(6) X(8) X(9) X(10) X(12) X(15) X(16) X(18) X(20) X(24) X(25) X(27) X(30) X(32) X(64)
+// R1 = M / 32 of the built grids: every 2/3/5-smooth multiple of 32 from M = 128 to M = 2048
+// (M >= 128 keeps at least four register points per lane; 64 is the most a lane's registers hold)
+#define PWFS_FOR_EACH_R1(X) X(4) X(5) X(6) X(8) X(9) X(10) X(12) X(15) X(16) X(18) X(20) X(24) X(25) X(27) X(30) X(32) \
+    X(36) X(40) X(45) X(48) X(50) X(54) X(60) X(64)
 
 // PassCfg<R1, NB, warps/CTA row pass, warps/CTA column pass, min CTAs/SM row pass, column pass>:
 // NB transforms per warp so that NB * R1 fills whole rounds of 32 lanes in the size-32 stage as far as
@@ -30,6 +31,14 @@ template <> struct CfgFor<25> { using type = PassCfg<25, 1, 8, 4, 2, 1>; };   //
 template <> struct CfgFor<27> { using type = PassCfg<27, 1, 8, 4, 2, 1>; };   // M = 864
 template <> struct CfgFor<30> { using type = PassCfg<30, 1, 8, 4, 2, 1>; };   // M = 960
 template <> struct CfgFor<32> { using type = PassCfg<32, 1, 8, 4, 2, 2>; };   // M = 1024
+// R1 > 32: the size-32 stage runs in two rounds (the second with R1 - 32 lanes), one CTA per SM in both passes
+template <> struct CfgFor<36> { using type = PassCfg<36, 1, 8, 4, 1, 1>; };   // M = 1152
+template <> struct CfgFor<40> { using type = PassCfg<40, 1, 8, 4, 1, 1>; };   // M = 1280
+template <> struct CfgFor<45> { using type = PassCfg<45, 1, 8, 4, 1, 1>; };   // M = 1440
+template <> struct CfgFor<48> { using type = PassCfg<48, 1, 8, 4, 1, 1>; };   // M = 1536
+template <> struct CfgFor<50> { using type = PassCfg<50, 1, 8, 4, 1, 1>; };   // M = 1600
+template <> struct CfgFor<54> { using type = PassCfg<54, 1, 8, 4, 1, 1>; };   // M = 1728
+template <> struct CfgFor<60> { using type = PassCfg<60, 1, 8, 4, 1, 1>; };   // M = 1920
 template <> struct CfgFor<64> { using type = PassCfg<64, 1, 8, 4, 1, 1>; };   // M = 2048
 
 struct Launcher {

@@ -176,9 +176,10 @@ def test_strerror_and_supported_grid(lib):
     assert "memory" in pwfs.strerror(pwfs.PWFS_ENOMEM)
     assert "CUDA" in pwfs.strerror(pwfs.PWFS_ECUDA)
     assert "unknown" in pwfs.strerror(-99)
-    for m in (128, 160, 192, 256, 288, 320, 384, 480, 512, 576, 640, 768, 800, 864, 960, 1024, 2048):
+    for m in (128, 160, 192, 256, 288, 320, 384, 480, 512, 576, 640, 768, 800, 864, 960, 1024, 1152, 1280, 1440, 1536, 1600, 1728, 1920,
+              2048):
         assert pwfs.supported_grid(m)
-    for m in (0, 96, 100, 4096, 1000, 224, 352, 416, 448, 1056):
+    for m in (0, 96, 100, 4096, 1000, 224, 352, 416, 448, 1056, 1088, 1664, 1792, 2016):
         assert not pwfs.supported_grid(m)
 
 

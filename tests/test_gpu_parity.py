@@ -116,6 +116,9 @@ def test_full_size_configs_sampled_frames(torch_cuda, name, frames):
     (432, 864, 54, 2, 1.0),      # R1 = 27
     (470, 960, 47, 2, 1.5),      # R1 = 30, ragged N
     (1000, 2048, 100, 2, 2.0),   # R1 = 64: 64 register points per lane, two rounds of size-32 transforms
+    # R1 = 36 ... 60: second round of the size-32 stage with R1 - 32 lanes
+    (570, 1152, 57, 2, 1.0), (640, 1280, 64, 2, 1.5), (700, 1440, 70, 2, 1.0), (768, 1536, 96, 2, 2.0),
+    (800, 1600, 80, 2, 1.0), (860, 1728, 86, 2, 1.0), (960, 1920, 96, 2, 1.5),
 ])
 def test_geometries(torch_cuda, N, M, ns, K, r):
     rng = np.random.default_rng(N * 7 + M)
@@ -265,6 +268,7 @@ def test_f3_uniform_circle_list_equals_the_circle_bit_for_bit(torch_cuda):
     (250, 512, 50, 200.0),
     (288, 576, 36, 150.0),    # R1 = 18 on the table-mask kernels
     (900, 2048, 90, 500.0),   # M = 2048: mask table read through L1 (AM_GLOBAL)
+    (720, 1440, 72, 300.0),   # R1 = 45, table-mask kernels
 ])
 def test_f3_weighted_list_and_stop(torch_cuda, N, M, ns, stop):
     rng = np.random.default_rng(N + M)
