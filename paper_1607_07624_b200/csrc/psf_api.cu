@@ -39,7 +39,9 @@ struct PsfCfg {
     static constexpr int M = 32 * R1_;
     static constexpr int NZ = (R1_ + 1) / 2;         // M >= 2N: at most ceil(R1/2) non-zero inputs per lane
     static constexpr int ITEMS = NB_ * R1_;          // size-32 DFTs per warp batch
-    static_assert(ITEMS <= 32, "one size-32 DFT per lane");
+    static constexpr int ROUNDS = (ITEMS + 31) / 32; // lanes take them in rounds (R1 > 32: two)
+    static constexpr bool PREFETCH = R1_ <= 32;      // column pass: next frame's inputs in registers while this one runs
+    static_assert(ITEMS <= 32 || NB_ == 1, "more than one round only for a single transform per warp");
     static constexpr int WARP_BUF = ITEMS * kPitchP + 1;
     static constexpr int TAB = R1_ * kPitchP;
     static constexpr int RPC = NB_ * WPB_;           // rows per CTA, row pass
@@ -92,16 +94,20 @@ psf_row_kernel(PsfDev t, const float *__restrict__ phase, float2 *__restrict__ T
         for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitchP + lane] = v[k1];
     }
     __syncthreads();
-    if (lane < C::ITEMS) {
-        const int k1 = lane % C::R1;
-        float2 *row = buf + lane * kPitchP;
-        const float2 *twr = s_tw + k1 * kPitchP;
-        float2 u[32];
 #pragma unroll
-        for (int n2 = 0; n2 < 32; ++n2) u[n2] = cmul(row[n2], twr[n2]);
-        Dft<32, -1>::run(u);
+    for (int rd = 0; rd < C::ROUNDS; ++rd) {
+        const int w = rd * 32 + lane;
+        if (w < C::ITEMS) {
+            const int k1 = w % C::R1;
+            float2 *row = buf + w * kPitchP;
+            const float2 *twr = s_tw + k1 * kPitchP;
+            float2 u[32];
 #pragma unroll
-        for (int k2 = 0; k2 < 32; ++k2) row[k2] = u[k2];
+            for (int n2 = 0; n2 < 32; ++n2) u[n2] = cmul(row[n2], twr[n2]);
+            Dft<32, -1>::run(u);
+#pragma unroll
+            for (int k2 = 0; k2 < 32; ++k2) row[k2] = u[k2];
+        }
     }
     __syncthreads();
     // X[u = k1 + R1 k2] of CTA row r sits at s_buf[(r/NB) WARP_BUF + ((r%NB) R1 + k1) pitch + k2];
@@ -130,9 +136,11 @@ psf_col_kernel(PsfDev t, const float2 *__restrict__ T, int F, int fsplit, float 
     __syncthreads();
     if (u0 >= C::M) return;
     const int f_lo = (int)(((long long)fs * F) / fsplit), f_hi = (int)(((long long)(fs + 1) * F) / fsplit);
-    float acc[32];
+    float acc[C::ROUNDS][32];
 #pragma unroll
-    for (int k2 = 0; k2 < 32; ++k2) acc[k2] = 0.f;
+    for (int rd = 0; rd < C::ROUNDS; ++rd)
+#pragma unroll
+        for (int k2 = 0; k2 < 32; ++k2) acc[rd][k2] = 0.f;
     float2 pre[C::NB][C::NZ];
     auto fetch = [&](int f) {
         const float2 *src = T + ((size_t)f * C::M + u0) * NP + lane;
@@ -142,41 +150,51 @@ psf_col_kernel(PsfDev t, const float2 *__restrict__ T, int F, int fsplit, float 
             for (int n1 = 0; n1 < C::NZ; ++n1)
                 pre[b][n1] = (32 * n1 < NP && u0 + b < C::M) ? __ldg(src + (size_t)b * NP + 32 * n1) : make_float2(0.f, 0.f);
     };
-    if (f_lo < f_hi) fetch(f_lo);
-    const int my_b = lane / C::R1, my_k1 = lane % C::R1;
+    if (C::PREFETCH && f_lo < f_hi) fetch(f_lo);
     for (int f = f_lo; f < f_hi; ++f) {
+        if (!C::PREFETCH) fetch(f);
 #pragma unroll
         for (int b = 0; b < C::NB; ++b) {
             float2 v[C::R1];
 #pragma unroll
             for (int n1 = 0; n1 < C::NZ; ++n1) v[n1] = pre[b][n1];
-            if (b == C::NB - 1 && f + 1 < f_hi) fetch(f + 1);
+            if (C::PREFETCH && b == C::NB - 1 && f + 1 < f_hi) fetch(f + 1);
             DftP<C::R1, -1, C::NZ>::run(v);
 #pragma unroll
             for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitchP + lane] = v[k1];
         }
         __syncwarp();
-        if (lane < C::ITEMS) {
-            const float2 *row = buf + lane * kPitchP;
-            const float2 *twr = s_tw + my_k1 * kPitchP;
-            float2 u[32];
 #pragma unroll
-            for (int n2 = 0; n2 < 32; ++n2) u[n2] = cmul(row[n2], twr[n2]);
-            Dft<32, -1>::run(u);
+        for (int rd = 0; rd < C::ROUNDS; ++rd) {
+            const int w = rd * 32 + lane;
+            if (w < C::ITEMS) {
+                const int my_b = w / C::R1, my_k1 = w % C::R1;
+                const float2 *row = buf + w * kPitchP;
+                const float2 *twr = s_tw + my_k1 * kPitchP;
+                float2 u[32];
 #pragma unroll
-            for (int k2 = 0; k2 < 32; ++k2) acc[k2] = fmaf(u[k2].x, u[k2].x, fmaf(u[k2].y, u[k2].y, acc[k2]));
-            if (sr && my_k1 == 0 && u0 + my_b == 0)          // F4c: the (0, 0) bin
-                sr[f] = fmaf(u[0].x, u[0].x, u[0].y * u[0].y) * t.inv_sumA_sq;
+                for (int n2 = 0; n2 < 32; ++n2) u[n2] = cmul(row[n2], twr[n2]);
+                Dft<32, -1>::run(u);
+#pragma unroll
+                for (int k2 = 0; k2 < 32; ++k2) acc[rd][k2] = fmaf(u[k2].x, u[k2].x, fmaf(u[k2].y, u[k2].y, acc[rd][k2]));
+                if (sr && my_k1 == 0 && u0 + my_b == 0)          // F4c: the (0, 0) bin
+                    sr[f] = fmaf(u[0].x, u[0].x, u[0].y * u[0].y) * t.inv_sumA_sq;
+            }
         }
         __syncwarp();
     }
-    if (lane < C::ITEMS && u0 + my_b < C::M) {
-        const int uo = (u0 + my_b + C::M / 2) % C::M;
-        float *dst = partial + (size_t)fs * C::M * C::M + uo;
 #pragma unroll
-        for (int k2 = 0; k2 < 32; ++k2) {
-            const int vo = (my_k1 + C::R1 * k2 + C::M / 2) % C::M;
-            dst[(size_t)vo * C::M] = acc[k2];
+    for (int rd = 0; rd < C::ROUNDS; ++rd) {
+        const int w = rd * 32 + lane;
+        const int my_b = w / C::R1, my_k1 = w % C::R1;
+        if (w < C::ITEMS && u0 + my_b < C::M) {
+            const int uo = (u0 + my_b + C::M / 2) % C::M;
+            float *dst = partial + (size_t)fs * C::M * C::M + uo;
+#pragma unroll
+            for (int k2 = 0; k2 < 32; ++k2) {
+                const int vo = (my_k1 + C::R1 * k2 + C::M / 2) % C::M;
+                dst[(size_t)vo * C::M] = acc[rd][k2];
+            }
         }
     }
 }
@@ -238,6 +256,14 @@ bool find_psf_launcher(int M, PsfLauncher *out) {
         case 27: *out = make<PsfCfg<27, 1, 8>>(); return true;
         case 30: *out = make<PsfCfg<30, 1, 8>>(); return true;
         case 32: *out = make<PsfCfg<32, 1, 8>>(); return true;
+        case 36: *out = make<PsfCfg<36, 1, 8>>(); return true;
+        case 40: *out = make<PsfCfg<40, 1, 8>>(); return true;
+        case 45: *out = make<PsfCfg<45, 1, 8>>(); return true;
+        case 48: *out = make<PsfCfg<48, 1, 8>>(); return true;
+        case 50: *out = make<PsfCfg<50, 1, 8>>(); return true;
+        case 54: *out = make<PsfCfg<54, 1, 8>>(); return true;
+        case 60: *out = make<PsfCfg<60, 1, 8>>(); return true;
+        case 64: *out = make<PsfCfg<64, 1, 8>>(); return true;
         default: return false;
     }
 }

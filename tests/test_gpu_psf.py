@@ -57,7 +57,10 @@ def _check(torch, A, phase, M, scale=1.0):
                                        (60, 640, 1, 1.0), (320, 640, 2, 2.0), (400, 800, 2, 3.0), (480, 1024, 2, 5.0),
                                        (500, 1024, 1, 1.0),
                                        (80, 160, 2, 1.0), (96, 192, 2, 2.0), (140, 288, 2, 1.0), (192, 384, 2, 3.0),
-                                       (288, 576, 2, 2.0), (384, 768, 1, 2.0), (430, 864, 1, 1.0), (480, 960, 1, 3.0)])
+                                       (288, 576, 2, 2.0), (384, 768, 1, 2.0), (430, 864, 1, 1.0), (480, 960, 1, 3.0),
+                                       # R1 > 32: two rounds of size-32 transforms per warp, no register prefetch
+                                       (570, 1152, 1, 1.0), (600, 1280, 2, 2.0), (720, 1440, 1, 1.0), (768, 1536, 1, 2.0),
+                                       (790, 1600, 1, 1.0), (860, 1728, 1, 1.0), (960, 1920, 1, 2.0), (1000, 2048, 2, 3.0)])
 def test_psf_matches_oracle_on_every_grid(torch_cuda, N, M, B, rms):
     rng = np.random.default_rng(N * 7 + M)
     _check(torch_cuda, _disc(N, 0.15), _smooth_phase(rng, B, N, rms), M)
