@@ -114,7 +114,16 @@ int pwfs_rec_create(int32_t n_modes, int32_t n_slopes, const float *h_recmat, in
 
 /* d_slopes: DEVICE float [B][n_slopes]; d_modes: DEVICE float [B][n_modes],
  * modes[b][m] = sum_j recmat[m][j] * slopes[b][j] (F2g), FP32 accumulation in a
- * fixed order (deterministic).  B = 0 is a no-op. */
+ * fixed order (deterministic).  B = 0 is a no-op.
+ * Single frames and small problems run an FP32-FMA kernel.  Batches (B >= 24
+ * and n_modes * n_slopes >= 65536) run on the tensor cores: recmat and the
+ * slopes are each split into two TF32 planes and three tcgen05 products are
+ * accumulated in FP32, which keeps the FP32 bar (error <= 7e-7 sum |R||s| from
+ * the split, plus FP32 accumulation).  The first batched call builds the
+ * planes of recmat (2 x the matrix in device memory) and sizes its scratch for
+ * that B: it synchronises the stream and allocates; later calls with B no
+ * larger do neither.  Environment PWFS_REC_TC=0 at create keeps every call on
+ * the FP32 kernel. */
 int pwfs_rec_run(pwfs_rec_t *h, const float *d_slopes, int32_t B, float *d_modes, void *cuda_stream);
 
 void pwfs_rec_destroy(pwfs_rec_t *h); /* NULL-safe */
