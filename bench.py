@@ -206,6 +206,36 @@ def bench_stages(cfg, dev, phase, frames, flush, reps: int = 5) -> dict:
         m1 = torch.empty((1, n_modes), dtype=torch.float32, device=dev)
         ms = timed(lambda: rec.run(sl[:1], out=m1))
         out["f2_rec_gemv"] = hbm_row(ms, n_modes * 2 * nv * 4, 1, "one frame: recmat streamed once")
+    # the whole device chain as a loop runs it: one simulation step per iteration (f1 -> a1-a8 -> f2), n_inst frames
+    if not cfg.independent_screens:
+        atm = wl.atmosphere(cfg)
+        n_inst = len(atm["dirs_tan"]) * len(atm["wl_scale"])
+        with Atmosphere(**{k: v for k, v in atm.items() if k != "dt"}, device=dev.index) as a, \
+                from_config(cfg, device=dev.index) as sensor, \
+                CCD(D, n_inst=n_inst, gain=n_ph / float((wl.make_pupil(cfg).astype(np.float64) ** 2).sum()), quantum_eff=0.32,
+                    photon_noise=True, readout_noise=True, readout_level=1.0, seed=1, device=dev.index) as ccd, \
+                SlopeComputer(valid, sn=np.zeros(2 * nv, np.float32), device=dev.index) as sc, \
+                Reconstructor(R, device=dev.index) as rec:
+            ph = torch.empty((n_inst, N, N), dtype=torch.float32, device=dev)
+            fr = torch.empty((n_inst, D, D), dtype=torch.float32, device=dev)
+            px, s1 = torch.empty_like(fr), torch.empty((n_inst, 2 * nv), dtype=torch.float32, device=dev)
+            md = torch.empty((n_inst, n_modes), dtype=torch.float32, device=dev)
+            n_loop = 50
+            step = [0]
+
+            def loop():
+                for _ in range(n_loop):
+                    a.propagate(step[0], 1, atm["dt"], out=ph)
+                    sensor.run(ph, fr, want_slopes=False)
+                    ccd.run(fr, first_out_frame=step[0] * n_inst, out=px)
+                    sc.run(px, out=s1)
+                    rec.run(s1, out=md)
+                    step[0] += 1
+            ms = timed(loop) / n_loop
+            out["chain_loop_step"] = {"ms": ms, "steps_per_s": 1e3 / ms, "frames_per_step": n_inst, "launches": 8,
+                                      "note": "closed-loop order, one step per iteration, all on the device: propagate -> "
+                                              "pyramid (4 kernels) -> CCD -> slopes - reference -> modes (GEMV); eager "
+                                              "launches, device time per step over 50 consecutive steps"}
     del R
     # f4: PSF camera on the same grid, Shack-Hartmann on the same pupil
     with PsfCamera(wl.make_pupil(cfg), M, phase_scale=0.45, device=dev.index) as cam:
