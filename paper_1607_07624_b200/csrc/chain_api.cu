@@ -5,7 +5,8 @@
 //                   Philox4x32-10 -> Poisson / normal photon noise, read noise.  All decisions
 //                   in double (B200 keeps full-rate FP64 units; the detector is <= 184^2 px).
 //                   HBM-bound: 4 n_int bytes in, 4 bytes out per pixel.
-//   slopec_kernel   one CTA per frame: normalisation sum over valid subapertures, slopes - sn.
+//   slopec_kernel   one cluster of 8 CTAs per frame: normalisation sum over valid subapertures through
+//                   distributed shared memory, slopes - sn.
 //   rec_kernel      modes = slopes x recmat^T.  One warp = MR rows of recmat x FB frames, lanes
 //                   stride over the slope index with 128-bit loads, FP32 FMA, shuffle reduction.
 //                   B = 1 is a GEMV streaming recmat once from HBM; larger batches re-use each
@@ -13,6 +14,7 @@
 #include "../../include/pwfs_chain.h"
 #include "rec_tc.cuh"
 
+#include <cooperative_groups.h>
 #include <cuda_runtime.h>
 
 #include <cmath>
@@ -108,14 +110,24 @@ struct SlopecDev {
     const float *sn;      // [2 n_valid] or nullptr
 };
 
-__global__ void __launch_bounds__(256)
+// One thread-block CLUSTER of kSlopecCluster CTAs per frame (grid (kSlopecCluster, B)): each CTA takes a contiguous
+// share of the valid subapertures, the partial normalisation sums meet through distributed shared memory and every CTA
+// adds them in rank order (same value in all of them, deterministic), then writes the slopes of its share.  One
+// launch, no second pass through global memory, and a single frame (closed loop) is spread over 8 SMs.
+constexpr int kSlopecCluster = 8;
+
+__global__ void __cluster_dims__(kSlopecCluster, 1, 1) __launch_bounds__(256)
 slopec_kernel(SlopecDev t, const float *__restrict__ pixels, float *__restrict__ slopes) {
+    namespace cg = cooperative_groups;
+    cg::cluster_group cluster = cg::this_cluster();
     __shared__ float red[8];
-    __shared__ float s_nbar;
+    __shared__ float s_part;
     const int ns = t.n_sub, D = 2 * ns, nv = t.n_valid;
-    const float *fr = pixels + (size_t)blockIdx.x * D * D;
+    const int rank = (int)cluster.block_rank(), share = (nv + kSlopecCluster - 1) / kSlopecCluster;
+    const int i_lo = rank * share, i_hi = min(nv, i_lo + share);
+    const float *fr = pixels + (size_t)blockIdx.y * D * D;
     float part = 0.f;
-    for (int i = threadIdx.x; i < nv; i += blockDim.x) {
+    for (int i = i_lo + threadIdx.x; i < i_hi; i += blockDim.x) {
         const int id = __ldg(t.vidx + i), jj = id / ns, ii = id - jj * ns;
         part += (fr[jj * D + ii] + fr[jj * D + ns + ii]) + (fr[(ns + jj) * D + ii] + fr[(ns + jj) * D + ns + ii]);
     }
@@ -126,12 +138,15 @@ slopec_kernel(SlopecDev t, const float *__restrict__ pixels, float *__restrict__
     if (threadIdx.x == 0) {
         float v = 0.f;
         for (int w = 0; w < (int)(blockDim.x >> 5); ++w) v += red[w];
-        s_nbar = v / (float)nv;
+        s_part = v;
     }
-    __syncthreads();
-    const float nbar = s_nbar;
-    float *out = slopes + (size_t)blockIdx.x * 2 * nv;
-    for (int i = threadIdx.x; i < nv; i += blockDim.x) {
+    cluster.sync();                                                    // every CTA's partial is in its shared memory
+    float nbar = 0.f;
+    for (int r = 0; r < kSlopecCluster; ++r) nbar += *cluster.map_shared_rank(&s_part, r);
+    nbar /= (float)nv;
+    cluster.sync();                                                    // nobody leaves while its partial may still be read
+    float *out = slopes + (size_t)blockIdx.y * 2 * nv;
+    for (int i = i_lo + threadIdx.x; i < i_hi; i += blockDim.x) {
         const int id = __ldg(t.vidx + i), jj = id / ns, ii = id - jj * ns;
         const float a = fr[jj * D + ii], b = fr[jj * D + ns + ii];
         const float c = fr[(ns + jj) * D + ii], d = fr[(ns + jj) * D + ns + ii];
@@ -340,7 +355,11 @@ int pwfs_slopec_run(pwfs_slopec_t *h, const float *d_pixels, int32_t B, float *d
     if (B == 0) return PWFS_OK;
     if (!d_pixels || !d_slopes) return PWFS_EINVAL;
     if (cudaSetDevice(h->device) != cudaSuccess) return PWFS_ECUDA;
-    slopec_kernel<<<B, 256, 0, (cudaStream_t)cuda_stream>>>(h->dev, d_pixels, d_slopes);
+    for (int b0 = 0; b0 < B; b0 += 65535) {                      // grid.y limit
+        const int Bc = B - b0 < 65535 ? B - b0 : 65535;
+        slopec_kernel<<<dim3(kSlopecCluster, Bc), 256, 0, (cudaStream_t)cuda_stream>>>(
+            h->dev, d_pixels + (size_t)b0 * 4 * h->dev.n_sub * h->dev.n_sub, d_slopes + (size_t)b0 * 2 * h->dev.n_valid);
+    }
     return cudaGetLastError() == cudaSuccess ? PWFS_OK : PWFS_ECUDA;
 }
 

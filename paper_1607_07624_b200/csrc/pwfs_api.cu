@@ -52,6 +52,7 @@ struct pwfs {
     // scratch
     float2 *T = nullptr; size_t T_elems = 0;
     float *colbin = nullptr; size_t colbin_elems = 0;
+    float *nsum = nullptr; size_t nsum_elems = 0;      // [F][D] per-column sums over valid detector pixels
     // host-buffer path
     cudaStream_t hstream = nullptr, in_stream = nullptr, out_stream = nullptr;   // compute, H2D, D2H
     std::vector<cudaEvent_t> in_ev, done_ev;                                     // per chunk
@@ -60,6 +61,7 @@ struct pwfs {
     // schedule
     int user_fpc = 0, user_ksplit = 0;
     int num_sms = 148;
+    int x_resident_ctas = 296, y_resident_warps = 1184;   // what the device holds at once (occupancy query at create)
     size_t scratch_budget = (size_t)4 << 30;
     // instrumentation
     int timing = 0;
@@ -256,6 +258,7 @@ int build_tables(pwfs *h) {
     if ((rc = upload(h, rb_cnt, &t.rb_cnt))) return rc;
     if ((rc = upload(h, rb_w, &t.rb_w))) return rc;
     if ((rc = upload(h, vidx, &t.vidx))) return rc;
+    if ((rc = upload(h, h->valid, &t.vmask))) return rc;
     return PWFS_OK;
 }
 
@@ -270,9 +273,17 @@ void schedule(const pwfs *h, int B, int *fpc, int *ksplit) {
     F = (int)std::min<size_t>((size_t)F, maxF);
     F = std::max(1, std::min(F, std::max(B, 1)));
     int ks = h->user_ksplit > 0 ? h->user_ksplit : 1;
-    if (h->user_ksplit <= 0) {
-        // too few warps for the machine: split the modulation loop, keeping >= 4 points per warp
-        while ((long long)F * col_warps * ks < 2LL * slots && t.K / (ks * 2) >= 4) ks *= 2;
+    if (h->user_ksplit <= 0 && (long long)F * col_warps < 2LL * slots) {
+        // too few warps for the machine (small batches, B = 1 in a closed loop): split the modulation loop, >= 4
+        // points per warp, choosing the split that minimises (waves of resident warps) x (points per warp + 1);
+        // the + 1 stands for a warp's prologue and its y-rebin
+        double best = 1e300;
+        for (int c = 1; c <= std::max(1, t.K / 4); ++c) {
+            const long long warps = (long long)F * col_warps * c;
+            const double waves = (double)((warps + h->y_resident_warps - 1) / h->y_resident_warps);
+            const double cost = waves * ((t.K + c - 1) / c + 1.0);
+            if (cost < best * (1.0 - 1e-9)) { best = cost; ks = c; }
+        }
     }
     ks = std::max(1, std::min(ks, t.K));
     *fpc = F; *ksplit = ks;
@@ -288,6 +299,14 @@ int ensure_scratch(pwfs *h, int F, int ksplit) {
         cudaError_t e = cudaMalloc((void **)&h->T, needT * sizeof(float2));
         if (e != cudaSuccess) { h->last_cuda = (int)e; return e == cudaErrorMemoryAllocation ? PWFS_ENOMEM : PWFS_ECUDA; }
         h->T_elems = needT;
+    }
+    const size_t needN = (size_t)F * t.D;
+    if (needN > h->nsum_elems) {
+        if (h->nsum) cudaFree(h->nsum);
+        h->nsum = nullptr; h->nsum_elems = 0;
+        cudaError_t e = cudaMalloc((void **)&h->nsum, needN * sizeof(float));
+        if (e != cudaSuccess) { h->last_cuda = (int)e; return e == cudaErrorMemoryAllocation ? PWFS_ENOMEM : PWFS_ECUDA; }
+        h->nsum_elems = needN;
     }
     if (needC > h->colbin_elems) {
         if (h->colbin) cudaFree(h->colbin);
@@ -400,7 +419,12 @@ int pwfs_create_ex(const pwfs_params *p, const pwfs_ext *x, pwfs_t **out) {
     if (!rc) {
         e = cudaFuncSetAttribute(L.xfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem_x);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(L.yfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem_y);
+        int nx = 0, ny = 0;
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nx, L.xfn, 32 * L.WPB_X, L.smem_x);
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ny, L.yfn, 32 * L.WPB_Y, L.smem_y);
         if (e != cudaSuccess) { h->last_cuda = (int)e; rc = PWFS_ECUDA; }
+        h->x_resident_ctas = h->num_sms * std::max(1, nx);
+        h->y_resident_warps = h->num_sms * std::max(1, ny) * L.WPB_Y;
     }
     if (!rc) {
         const char *env = std::getenv("PWFS_SCRATCH_MB");
@@ -419,6 +443,7 @@ void pwfs_destroy(pwfs_t *h) {
     for (void *d : h->dev_allocs) cudaFree(d);
     if (h->T) cudaFree(h->T);
     if (h->colbin) cudaFree(h->colbin);
+    if (h->nsum) cudaFree(h->nsum);
     if (h->d_phase) cudaFree(h->d_phase);
     if (h->d_frames) cudaFree(h->d_frames);
     if (h->d_slopes) cudaFree(h->d_slopes);
@@ -502,7 +527,18 @@ static int run_chunk(pwfs_t *h, const float *d_phase, int Fc, float *d_frames, f
         // keeping >= 3 tilts per CTA so the one-off phasor stays amortised
         const int row_ctas = (t.NP + L.RPC - 1) / L.RPC;
         int jsplit = 1;
-        while ((long long)row_ctas * Fc * jsplit < 16LL * h->num_sms && t.KX / (jsplit + 1) >= 3) ++jsplit;
+        if ((long long)row_ctas * Fc >= 2LL * h->x_resident_ctas || t.KX < 6) {
+            // split the x-tilt loop only as far as needed to fill the machine (>= 8 waves of 2 CTAs/SM)
+            while ((long long)row_ctas * Fc * jsplit < 16LL * h->num_sms && t.KX / (jsplit + 1) >= 3) ++jsplit;
+        } else {   // small batch: (waves of resident CTAs) x (x-tilts per CTA + 1 for the phasor), >= 3 tilts per CTA
+            double best = 1e300;
+            for (int c = 1; c <= t.KX / 3; ++c) {
+                const long long ctas = (long long)row_ctas * Fc * c;
+                const double waves = (double)((ctas + h->x_resident_ctas - 1) / h->x_resident_ctas);
+                const double cost = waves * ((t.KX + c - 1) / c + 1.0);
+                if (cost < best * (1.0 - 1e-9)) { best = cost; jsplit = c; }
+            }
+        }
         L.launch_x(dim3(row_ctas, jsplit, Fc), st, t, d_phase, h->T, jsplit);
     }
     {   // K2: y-convolution + |E|^2 over k + y-rebin (a3, a4, a5 along y, a6, a7)
@@ -515,11 +551,11 @@ static int run_chunk(pwfs_t *h, const float *d_phase, int Fc, float *d_frames, f
         const int threads = std::min(256, (t.D + 31) / 32 * 32);
         // 1/K of O6; the quarter-mask kernels leave O5's 1/M per axis (1/M^4 on |E|^2) to this scale
         const double m4 = h->quarter ? std::pow((double)t.M, 4.0) : 1.0;
-        xrebin_kernel<<<dim3(t.D, Fc), threads, 0, st>>>(t, h->colbin, d_frames, ks, (float)(1.0 / ((double)t.K * m4)));
+        xrebin_kernel<<<dim3(t.D, Fc), threads, 0, st>>>(t, h->colbin, d_frames, h->nsum, ks, (float)(1.0 / ((double)t.K * m4)));
     }
     if (d_slopes) {   // K3b: slopes (a8)
         SpanGuard g(h, st, 3);
-        slopes_kernel<<<Fc, 256, 0, st>>>(t, d_frames, d_slopes);
+        slopes_kernel<<<dim3((t.n_valid + 255) / 256, Fc), 256, 0, st>>>(t, d_frames, h->nsum, d_slopes);
     }
     PWFS_CUDA(h, cudaGetLastError());
     return PWFS_OK;

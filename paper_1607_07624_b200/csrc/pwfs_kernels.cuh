@@ -82,6 +82,7 @@ struct DevTables {
     const int *rb_cnt;        // [D]
     const float *rb_w;        // [D][cmax] area weights
     const int *vidx;          // [n_valid] j*n_sub + i of valid subapertures, row-major
+    const unsigned char *vmask;   // [n_sub][n_sub] 1 = valid subaperture
 };
 
 template <bool QM, bool AM_GLOBAL = false>
@@ -394,62 +395,84 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
 }
 
 // ------------------------------------------------------------------ K3a -----
-// frame[f][jy][jx] = (1/K) sum_ks sum_c wx[jx][c] colbin[f][ks][xc(jx,c)][jy]
-// grid (D (jx), F); block covers jy.
+// frame[f][jy][jx] = (1/K) sum_ks sum_c wx[jx][c] colbin[f][ks][xc(jx,c)][jy], and this detector column's share of
+// the slope normalisation: nsum[f][jx] = sum over jy of the pixels that belong to valid subapertures.
+// grid (D (jx), F); block covers jy.  Source columns are taken four at a time so that their loads are in flight
+// together (a single frame in a closed loop is latency-bound here).
 static __global__ void xrebin_kernel(DevTables t, const float *__restrict__ colbin, float *__restrict__ frames,
-                              int ksplit, float scale) {
+                                     float *__restrict__ nsum, int ksplit, float scale) {
+    __shared__ float red[8];
     const int jx = blockIdx.x, f = blockIdx.y;
-    const int D = t.D;
-    int x = __ldg(t.rb_start + jx);
+    const int D = t.D, ns = t.n_sub;
+    const int x = __ldg(t.rb_start + jx);
     const int cnt = __ldg(t.rb_cnt + jx);
     const float *w = t.rb_w + (size_t)jx * t.cmax;
+    const int ix = jx >= ns ? jx - ns : jx;
+    float part = 0.f;
     for (int jy = threadIdx.x; jy < D; jy += blockDim.x) {
         float s = 0.f;
-        int xx = x;
-        for (int c = 0; c < cnt; ++c) {
-            const int xc = __ldg(t.xc_of_x + xx);
-            const float wc = __ldg(w + c);
-            for (int ks = 0; ks < ksplit; ++ks)
-                s = fmaf(wc, __ldg(colbin + (((size_t)f * ksplit + ks) * t.ncols + xc) * D + jy), s);
-            if (++xx == t.M) xx = 0;
+        for (int c0 = 0; c0 < cnt; c0 += 4) {
+            int xc[4];
+            float wc[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const bool ok = c0 + u < cnt;
+                int xx = x + c0 + u;
+                if (xx >= t.M) xx -= t.M;
+                xc[u] = ok ? __ldg(t.xc_of_x + xx) : 0;
+                wc[u] = ok ? __ldg(w + c0 + u) : 0.f;
+            }
+            for (int ks = 0; ks < ksplit; ++ks) {
+                const float *src = colbin + ((size_t)f * ksplit + ks) * t.ncols * D + jy;
+                float v[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) v[u] = c0 + u < cnt ? __ldg(src + (size_t)xc[u] * D) : 0.f;
+#pragma unroll
+                for (int u = 0; u < 4; ++u) s = fmaf(wc[u], v[u], s);
+            }
         }
-        frames[((size_t)f * D + jy) * D + jx] = s * scale;
-    }
-}
-
-// ------------------------------------------------------------------ K3b -----
-// One CTA per frame: nbar = mean over valid subaps of a+b+c+d, then slopes.
-static __global__ void slopes_kernel(DevTables t, const float *__restrict__ frames, float *__restrict__ slopes) {
-    __shared__ float red[32];
-    __shared__ float s_nbar;
-    const int f = blockIdx.x, D = t.D, ns = t.n_sub, nv = t.n_valid;
-    const float *fr = frames + (size_t)f * D * D;
-    float part = 0.f;
-    for (int i = threadIdx.x; i < nv; i += blockDim.x) {
-        const int id = __ldg(t.vidx + i), jj = id / ns, ii = id % ns;
-        part += (fr[jj * D + ii] + fr[jj * D + ns + ii]) + (fr[(ns + jj) * D + ii] + fr[(ns + jj) * D + ns + ii]);
+        s *= scale;
+        frames[((size_t)f * D + jy) * D + jx] = s;
+        const int iy = jy >= ns ? jy - ns : jy;
+        if (__ldg(t.vmask + iy * ns + ix)) part += s;
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
     if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = part;
     __syncthreads();
+    if (threadIdx.x == 0) {
+        float v = 0.f;
+        for (int i = 0; i < (int)((blockDim.x + 31) >> 5); ++i) v += red[i];
+        nsum[(size_t)f * D + jx] = v;
+    }
+}
+
+// ------------------------------------------------------------------ K3b -----
+// grid (ceil(n_valid / 256), F); block 256.  nbar = (1 / n_valid) sum_jx nsum[f][jx], added in one fixed order by
+// every CTA of the frame (same value everywhere, no second pass over the frame), then the slopes of 256 subapertures.
+static __global__ void slopes_kernel(DevTables t, const float *__restrict__ frames, const float *__restrict__ nsum,
+                                     float *__restrict__ slopes) {
+    __shared__ float s_nbar;
+    const int f = blockIdx.y, D = t.D, ns = t.n_sub, nv = t.n_valid;
     if (threadIdx.x < 32) {
-        float v = (threadIdx.x < (blockDim.x >> 5)) ? red[threadIdx.x] : 0.f;
+        float v = 0.f;
+        for (int j = threadIdx.x; j < D; j += 32) v += __ldg(nsum + (size_t)f * D + j);
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
         if (threadIdx.x == 0) s_nbar = v / (float)nv;
     }
     __syncthreads();
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nv) return;
     const float nbar = s_nbar;
+    const float *fr = frames + (size_t)f * D * D;
+    const int id = __ldg(t.vidx + i), jj = id / ns, ii = id - jj * ns;
+    const float a = fr[jj * D + ii], b = fr[jj * D + ns + ii];
+    const float c = fr[(ns + jj) * D + ii], d = fr[(ns + jj) * D + ns + ii];
+    const float den = t.slope_norm == 1 ? ((a + b) + (c + d)) : nbar;
     float *out = slopes + (size_t)f * 2 * nv;
-    for (int i = threadIdx.x; i < nv; i += blockDim.x) {
-        const int id = __ldg(t.vidx + i), jj = id / ns, ii = id % ns;
-        const float a = fr[jj * D + ii], b = fr[jj * D + ns + ii];
-        const float c = fr[(ns + jj) * D + ii], d = fr[(ns + jj) * D + ns + ii];
-        const float den = t.slope_norm == 1 ? ((a + b) + (c + d)) : nbar;
-        out[i] = ((a + c) - (b + d)) / den;
-        out[nv + i] = ((a + b) - (c + d)) / den;
-    }
+    out[i] = ((a + c) - (b + d)) / den;
+    out[nv + i] = ((a + b) - (c + d)) / den;
 }
 
 }  // namespace pwk
