@@ -46,6 +46,7 @@ struct ShDev {
     float scale, invP2;
     const float *amp;        // [N][N]
     const float4 *wtab;      // [b][Pc] (re, re, im, im) of W[t][c]
+    const int2 *pix;         // [b * b * SPW] pixel map of a warp task (see sh_kernel, step 1)
     const int *vslot;        // [n_sub^2] slope slot of a valid subaperture, -1 otherwise
     int n_valid;
 };
@@ -114,18 +115,19 @@ sh_kernel(ShDev t, const float *__restrict__ phase, float *__restrict__ frames, 
         const float *am0 = t.amp + ((size_t)sj * B) * t.N + (size_t)si0 * B;
         const int xmax = t.N - si0 * B;                                       // pixels left in this pupil row
         constexpr int U = 4;                                                  // loads of U rounds in flight
-        for (int e0 = lane; e0 < B * rowlen; e0 += 32 * U) {
+        const int rawlen = B * rowlen;
+        for (int e0 = lane; e0 < rawlen; e0 += 32 * U) {
             float ph[U], am[U];
             int dst[U];
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 const int e = e0 + 32 * u;
-                const int y = (e >> lgS) / B, sx = e - y * rowlen;
-                const int ss = sx / B, x = sx - ss * B;
-                const bool in = e < B * rowlen && sx < xmax;
-                dst[u] = e < B * rowlen ? ss * t.gpitch + y * B + x : -1;
-                ph[u] = in ? __ldg(ph0 + (size_t)y * t.N + sx) : 0.f;
-                am[u] = in ? __ldg(am0 + (size_t)y * t.N + sx) : 0.f;
+                // pixel e of the task: .x = y * N + sx (offset in the pupil), .y = sx << 16 | slot in the phasor buffer
+                const int2 m = e < rawlen ? __ldg(t.pix + e) : make_int2(0, 0x7fff0000);
+                const bool in = (m.y >> 16) < xmax;
+                dst[u] = e < rawlen ? (m.y & 0xffff) : -1;
+                ph[u] = in ? __ldg(ph0 + m.x) : 0.f;
+                am[u] = in ? __ldg(am0 + m.x) : 0.f;
             }
 #pragma unroll
             for (int u = 0; u < U; ++u) {
@@ -273,6 +275,7 @@ struct pwfs_sh {
     std::vector<uint8_t> valid;
     float *d_amp = nullptr;
     float4 *d_wtab = nullptr;
+    int2 *d_pix = nullptr;
     int *d_vslot = nullptr;
 };
 
@@ -342,6 +345,16 @@ int pwfs_sh_create(const pwfs_sh_params *p, pwfs_sh_t **out) {
     if (e == cudaSuccess) e = cudaMemcpy(h->d_amp, p->pupil_amp, (size_t)N * N * sizeof(float), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_wtab, wtab.size() * sizeof(float4));
     if (e == cudaSuccess) e = cudaMemcpy(h->d_wtab, wtab.data(), wtab.size() * sizeof(float4), cudaMemcpyHostToDevice);
+    // pixel map of a warp task: element e = y * (SPW b) + sx of its SPW b x b pixels -> pupil offset and buffer slot
+    const int spw = 32 >> lg, rowlen = b * spw;
+    std::vector<int2> pix((size_t)b * rowlen);
+    for (int y = 0; y < b; ++y)
+        for (int sx = 0; sx < rowlen; ++sx) {
+            const int ss = sx / b, x = sx - ss * b;
+            pix[(size_t)y * rowlen + sx] = make_int2(y * N + sx, (sx << 16) | (ss * gpitch + y * b + x));
+        }
+    if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_pix, pix.size() * sizeof(int2));
+    if (e == cudaSuccess) e = cudaMemcpy(h->d_pix, pix.data(), pix.size() * sizeof(int2), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_vslot, vslot.size() * sizeof(int));
     if (e == cudaSuccess) e = cudaMemcpy(h->d_vslot, vslot.data(), vslot.size() * sizeof(int), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaFuncSetAttribute((const void *)h->kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem);
@@ -351,7 +364,7 @@ int pwfs_sh_create(const pwfs_sh_params *p, pwfs_sh_t **out) {
     d.lg_lps = lg; d.gpitch = gpitch; d.gpr = (ns + (32 >> lg) - 1) / (32 >> lg);
     d.vec = (nc % p->bin == 0 && p->n_px % (nc / p->bin) == 0) ? 1 : 0;   // NO-wide stores stay aligned
     d.scale = p->phase_scale; d.invP2 = (float)(1.0 / ((double)P * P));
-    d.amp = h->d_amp; d.wtab = h->d_wtab; d.vslot = h->d_vslot; d.n_valid = nv;
+    d.amp = h->d_amp; d.wtab = h->d_wtab; d.pix = h->d_pix; d.vslot = h->d_vslot; d.n_valid = nv;
     *out = h;
     return PWFS_OK;
 }
@@ -392,6 +405,7 @@ void pwfs_sh_destroy(pwfs_sh_t *h) {
     cudaSetDevice(h->device);
     if (h->d_amp) cudaFree(h->d_amp);
     if (h->d_wtab) cudaFree(h->d_wtab);
+    if (h->d_pix) cudaFree(h->d_pix);
     if (h->d_vslot) cudaFree(h->d_vslot);
     delete h;
 }
