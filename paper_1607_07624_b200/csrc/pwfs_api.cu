@@ -250,6 +250,11 @@ int build_tables(pwfs *h) {
     if ((rc = upload(h, txc, &t.txc))) return rc;
     if ((rc = upload(h, tyt, &t.tyt))) return rc;
     if ((rc = upload(h, jx, &t.jx))) return rc;
+    // modulation points ordered by x-tilt: consecutive points of one slab T[f][j] re-use the column in registers
+    std::vector<int> korder(K);
+    for (int k = 0; k < K; ++k) korder[k] = k;
+    std::stable_sort(korder.begin(), korder.end(), [&](int a, int b) { return jx[a] < jx[b]; });
+    if ((rc = upload(h, korder, &t.korder))) return rc;
     if ((rc = upload(h, tw, &t.tw))) return rc;
     if ((rc = upload(h, am, &t.am))) return rc;
     if ((rc = upload(h, colx, &t.colx))) return rc;

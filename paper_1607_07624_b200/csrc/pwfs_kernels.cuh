@@ -74,6 +74,7 @@ struct DevTables {
     const float2 *txc;        // [KX][NXP] exp(i tilt_x,j(x)), zero for x >= N
     const float2 *tyt;        // [K][NP]  exp(i tilt_y,k(y)), zero for y >= N
     const int *jx;            // [K]      x-tilt index of modulation point k
+    const int *korder;        // [K]      the modulation points sorted by x-tilt index
     const float2 *tw;         // [R1][32] exp(-2 pi i k1 n2 / M)
     const float2 *am;         // [R1][32] a(k1 + R1 k2) / M
     const int *colx;          // [ncols]  grid x of compact column xc
@@ -326,9 +327,11 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
 #pragma unroll
     for (int b = 0; b < C::NB; ++b) colofs[b] = (xc0 + b < t.ncols) ? __ldg(t.colx + xc0 + b) * NP : 0;
 
+    // The warp walks its share of the modulation points in x-tilt order (korder): points that share a slab
+    // T[f][j] come one after the other and the column is fetched once for them.
     float2 pre[C::NB][C::NZ];
-    auto fetch = [&](int k) {
-        const float2 *src = Tf + (size_t)__ldg(t.jx + k) * frame_stride;
+    auto fetch = [&](int j) {
+        const float2 *src = Tf + (size_t)j * frame_stride;
 #pragma unroll
         for (int b = 0; b < C::NB; ++b)
 #pragma unroll
@@ -336,8 +339,18 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
                 pre[b][n1] = (32 * n1 < NP && xc0 + b < t.ncols) ? __ldg(src + colofs[b] + 32 * n1)
                                                                  : make_float2(0.f, 0.f);
     };
-    if (k_lo < k_hi) fetch(k_lo);
-    for (int k = k_lo; k < k_hi; ++k) {
+    int k = 0, j = -1, k_next = 0, j_next = -1;
+    if (k_lo < k_hi) {
+        k_next = __ldg(t.korder + k_lo);
+        j_next = __ldg(t.jx + k_next);
+        fetch(j_next);
+    }
+    for (int idx = k_lo; idx < k_hi; ++idx) {
+        k = k_next; j = j_next;
+        if (idx + 1 < k_hi) {
+            k_next = __ldg(t.korder + idx + 1);
+            j_next = __ldg(t.jx + k_next);
+        }
         const float2 *ty = t.tyt + (size_t)k * NP + lane;
         float2 tyv[C::NZ];
 #pragma unroll
@@ -347,7 +360,7 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
             float2 v[C::R1];
 #pragma unroll
             for (int n1 = 0; n1 < C::NZ; ++n1) v[n1] = cmul(pre[b][n1], tyv[n1]);
-            if (b == C::NB - 1 && k + 1 < k_hi) fetch(k + 1);
+            if (b == C::NB - 1 && idx + 1 < k_hi && j_next != j) fetch(j_next);
             DftP<C::R1, -1, C::NZ>::run(v);
 #pragma unroll
             for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitch + lane] = v[k1];
