@@ -55,7 +55,7 @@ struct pwfs {
     float *nsum = nullptr; size_t nsum_elems = 0;      // [F][D] per-column sums over valid detector pixels
     // host-buffer path
     cudaStream_t hstream = nullptr, in_stream = nullptr, out_stream = nullptr;   // compute, H2D, D2H
-    std::vector<cudaEvent_t> in_ev, done_ev;                                     // per chunk
+    std::vector<cudaEvent_t> in_ev, done_ev, tail_ev;                            // per chunk
     float *d_phase = nullptr, *d_frames = nullptr, *d_slopes = nullptr;
     size_t d_cap_frames = 0;
     // schedule
@@ -457,6 +457,7 @@ void pwfs_destroy(pwfs_t *h) {
     if (h->out_stream) cudaStreamDestroy(h->out_stream);
     for (auto ev : h->in_ev) cudaEventDestroy(ev);
     for (auto ev : h->done_ev) cudaEventDestroy(ev);
+    for (auto ev : h->tail_ev) cudaEventDestroy(ev);
     for (auto &sp : h->spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
     for (auto ev : h->event_pool) cudaEventDestroy(ev);
     delete h;
@@ -522,35 +523,41 @@ int pwfs_get_timing(pwfs_t *h, float ms[PWFS_NUM_KERNEL_CLASSES], int64_t launch
     return PWFS_OK;
 }
 
-// One chunk of Fc <= F frames: the four kernels of the path on `st`.
-static int run_chunk(pwfs_t *h, const float *d_phase, int Fc, float *d_frames, float *d_slopes, int ks, cudaStream_t st) {
+// One chunk of Fc <= F frames is three enqueue steps: K1 (row pass), K2 (column pass), tail (x-rebin + slopes).
+static int launch_k1(pwfs_t *h, const float *d_phase, int Fc, cudaStream_t st) {
     const DevTables &t = h->tab;
     const Launcher &L = h->L;
-    {   // K1: phasor + x-convolution (a1, a3, a4, a5 along x)
-        SpanGuard g(h, st, 0);
+    SpanGuard g(h, st, 0);   // K1: phasor + x-convolution (a1, a3, a4, a5 along x)
+    const int row_ctas = (t.NP + L.RPC - 1) / L.RPC;
+    int jsplit = 1;
+    if ((long long)row_ctas * Fc >= 2LL * h->x_resident_ctas || t.KX < 6) {
         // split the x-tilt loop only as far as needed to fill the machine (>= 8 waves of 2 CTAs/SM),
         // keeping >= 3 tilts per CTA so the one-off phasor stays amortised
-        const int row_ctas = (t.NP + L.RPC - 1) / L.RPC;
-        int jsplit = 1;
-        if ((long long)row_ctas * Fc >= 2LL * h->x_resident_ctas || t.KX < 6) {
-            // split the x-tilt loop only as far as needed to fill the machine (>= 8 waves of 2 CTAs/SM)
-            while ((long long)row_ctas * Fc * jsplit < 16LL * h->num_sms && t.KX / (jsplit + 1) >= 3) ++jsplit;
-        } else {   // small batch: (waves of resident CTAs) x (x-tilts per CTA + 1 for the phasor), >= 3 tilts per CTA
-            double best = 1e300;
-            for (int c = 1; c <= t.KX / 3; ++c) {
-                const long long ctas = (long long)row_ctas * Fc * c;
-                const double waves = (double)((ctas + h->x_resident_ctas - 1) / h->x_resident_ctas);
-                const double cost = waves * ((t.KX + c - 1) / c + 1.0);
-                if (cost < best * (1.0 - 1e-9)) { best = cost; jsplit = c; }
-            }
+        while ((long long)row_ctas * Fc * jsplit < 16LL * h->num_sms && t.KX / (jsplit + 1) >= 3) ++jsplit;
+    } else {   // small batch: (waves of resident CTAs) x (x-tilts per CTA + 1 for the phasor), >= 3 tilts per CTA
+        double best = 1e300;
+        for (int c = 1; c <= t.KX / 3; ++c) {
+            const long long ctas = (long long)row_ctas * Fc * c;
+            const double waves = (double)((ctas + h->x_resident_ctas - 1) / h->x_resident_ctas);
+            const double cost = waves * ((t.KX + c - 1) / c + 1.0);
+            if (cost < best * (1.0 - 1e-9)) { best = cost; jsplit = c; }
         }
-        L.launch_x(dim3(row_ctas, jsplit, Fc), st, t, d_phase, h->T, jsplit);
     }
-    {   // K2: y-convolution + |E|^2 over k + y-rebin (a3, a4, a5 along y, a6, a7)
-        SpanGuard g(h, st, 1);
-        const int per_cta = L.NB * L.WPB_Y;
-        L.launch_y(dim3((t.ncols + per_cta - 1) / per_cta, ks, Fc), st, t, h->T, h->colbin, ks);
-    }
+    L.launch_x(dim3(row_ctas, jsplit, Fc), st, t, d_phase, h->T, jsplit);
+    return PWFS_OK;
+}
+
+static int launch_k2(pwfs_t *h, int Fc, int ks, cudaStream_t st) {
+    const DevTables &t = h->tab;
+    const Launcher &L = h->L;
+    SpanGuard g(h, st, 1);   // K2: y-convolution + |E|^2 over k + y-rebin (a3, a4, a5 along y, a6, a7)
+    const int per_cta = L.NB * L.WPB_Y;
+    L.launch_y(dim3((t.ncols + per_cta - 1) / per_cta, ks, Fc), st, t, h->T, h->colbin, ks);
+    return PWFS_OK;
+}
+
+static int launch_tail(pwfs_t *h, int Fc, float *d_frames, float *d_slopes, int ks, cudaStream_t st) {
+    const DevTables &t = h->tab;
     {   // K3a: x-rebin (a7)
         SpanGuard g(h, st, 2);
         const int threads = std::min(256, (t.D + 31) / 32 * 32);
@@ -566,6 +573,20 @@ static int run_chunk(pwfs_t *h, const float *d_phase, int Fc, float *d_frames, f
     return PWFS_OK;
 }
 
+// per-chunk events of the two-stream schedule below
+static int ensure_chunk_events(pwfs_t *h, size_t n_chunks) {
+    while (h->in_ev.size() < n_chunks) {
+        cudaEvent_t a, b, c;
+        PWFS_CUDA(h, cudaEventCreateWithFlags(&a, cudaEventDisableTiming));
+        h->in_ev.push_back(a);
+        PWFS_CUDA(h, cudaEventCreateWithFlags(&b, cudaEventDisableTiming));
+        h->done_ev.push_back(b);
+        PWFS_CUDA(h, cudaEventCreateWithFlags(&c, cudaEventDisableTiming));
+        h->tail_ev.push_back(c);
+    }
+    return PWFS_OK;
+}
+
 int pwfs_run(pwfs_t *h, const float *d_phase, int32_t B, float *d_frames, float *d_slopes, void *cuda_stream) {
     if (!h || B < 0) return PWFS_EINVAL;
     if (B == 0) return PWFS_OK;
@@ -577,12 +598,30 @@ int pwfs_run(pwfs_t *h, const float *d_phase, int32_t B, float *d_frames, float 
     schedule(h, B, &F, &ks);
     int rc = ensure_scratch(h, F, ks);
     if (rc) return rc;
-    const size_t NN = (size_t)t.N * t.N, DD = (size_t)t.D * t.D;
-    for (int f0 = 0; f0 < B; f0 += F) {
-        rc = run_chunk(h, d_phase + (size_t)f0 * NN, std::min(F, B - f0), d_frames + (size_t)f0 * DD,
-                       d_slopes ? d_slopes + (size_t)f0 * 2 * t.n_valid : nullptr, ks, st);
-        if (rc) return rc;
+    const size_t NN = (size_t)t.N * t.N, DD = (size_t)t.D * t.D, SS = (size_t)2 * t.n_valid;
+    const size_t n_chunks = ((size_t)B + F - 1) / F;
+    if (n_chunks == 1) {                       // a single chunk (closed loop): everything in order on the caller's stream
+        if ((rc = launch_k1(h, d_phase, B, st))) return rc;
+        if ((rc = launch_k2(h, B, ks, st))) return rc;
+        return launch_tail(h, B, d_frames, d_slopes, ks, st);
     }
+    // several chunks: the small, latency-bound tail kernels of chunk c run on a side stream under the row pass of
+    // chunk c+1; the column pass of chunk c+1 waits for them (they read colbin), the caller's stream joins at the end
+    if (!h->out_stream) PWFS_CUDA(h, cudaStreamCreateWithFlags(&h->out_stream, cudaStreamNonBlocking));
+    if ((rc = ensure_chunk_events(h, n_chunks))) return rc;
+    size_t c = 0;
+    for (int f0 = 0; f0 < B; f0 += F, ++c) {
+        const int Fc = std::min(F, B - f0);
+        if ((rc = launch_k1(h, d_phase + (size_t)f0 * NN, Fc, st))) return rc;
+        if (c > 0) PWFS_CUDA(h, cudaStreamWaitEvent(st, h->tail_ev[c - 1], 0));
+        if ((rc = launch_k2(h, Fc, ks, st))) return rc;
+        PWFS_CUDA(h, cudaEventRecord(h->done_ev[c], st));
+        PWFS_CUDA(h, cudaStreamWaitEvent(h->out_stream, h->done_ev[c], 0));
+        if ((rc = launch_tail(h, Fc, d_frames + (size_t)f0 * DD, d_slopes ? d_slopes + (size_t)f0 * SS : nullptr, ks, h->out_stream)))
+            return rc;
+        PWFS_CUDA(h, cudaEventRecord(h->tail_ev[c], h->out_stream));
+    }
+    PWFS_CUDA(h, cudaStreamWaitEvent(st, h->tail_ev[n_chunks - 1], 0));
     return PWFS_OK;
 }
 
@@ -612,15 +651,9 @@ int pwfs_run_host(pwfs_t *h, const float *h_phase, int32_t B, float *h_frames, f
     int rc = ensure_scratch(h, F, ks);
     if (rc) return rc;
     const size_t n_chunks = ((size_t)B + F - 1) / F;
-    while (h->in_ev.size() < n_chunks) {
-        cudaEvent_t a, b;
-        PWFS_CUDA(h, cudaEventCreateWithFlags(&a, cudaEventDisableTiming));
-        h->in_ev.push_back(a);
-        PWFS_CUDA(h, cudaEventCreateWithFlags(&b, cudaEventDisableTiming));
-        h->done_ev.push_back(b);
-    }
-    // three streams, chunk by chunk: the copy-in of chunk c+1 and the copy-out of chunk c-1 run under
-    // the kernels of chunk c (pinned host memory; pageable memory degrades to staged copies)
+    if ((rc = ensure_chunk_events(h, n_chunks))) return rc;
+    // three streams, chunk by chunk: the copy-in of chunk c+1, and the tail kernels and the copy-out of chunk c-1,
+    // run under the FFT kernels of chunk c (pinned host memory; pageable memory degrades to staged copies)
     size_t c = 0;
     for (int f0 = 0; f0 < B; f0 += F, ++c) {
         const int Fc = std::min(F, B - f0);
@@ -628,10 +661,13 @@ int pwfs_run_host(pwfs_t *h, const float *h_phase, int32_t B, float *h_frames, f
         PWFS_CUDA(h, cudaMemcpyAsync(dp, h_phase + (size_t)f0 * NN, (size_t)Fc * NN * sizeof(float), cudaMemcpyHostToDevice, h->in_stream));
         PWFS_CUDA(h, cudaEventRecord(h->in_ev[c], h->in_stream));
         PWFS_CUDA(h, cudaStreamWaitEvent(h->hstream, h->in_ev[c], 0));
-        rc = run_chunk(h, dp, Fc, df, h_slopes ? ds : nullptr, ks, h->hstream);
-        if (rc) return rc;
+        if ((rc = launch_k1(h, dp, Fc, h->hstream))) return rc;
+        if (c > 0) PWFS_CUDA(h, cudaStreamWaitEvent(h->hstream, h->tail_ev[c - 1], 0));   // colbin is free again
+        if ((rc = launch_k2(h, Fc, ks, h->hstream))) return rc;
         PWFS_CUDA(h, cudaEventRecord(h->done_ev[c], h->hstream));
         PWFS_CUDA(h, cudaStreamWaitEvent(h->out_stream, h->done_ev[c], 0));
+        if ((rc = launch_tail(h, Fc, df, h_slopes ? ds : nullptr, ks, h->out_stream))) return rc;
+        PWFS_CUDA(h, cudaEventRecord(h->tail_ev[c], h->out_stream));
         PWFS_CUDA(h, cudaMemcpyAsync(h_frames + (size_t)f0 * DD, df, (size_t)Fc * DD * sizeof(float), cudaMemcpyDeviceToHost, h->out_stream));
         if (h_slopes)
             PWFS_CUDA(h, cudaMemcpyAsync(h_slopes + (size_t)f0 * SS, ds, (size_t)Fc * SS * sizeof(float), cudaMemcpyDeviceToHost, h->out_stream));
