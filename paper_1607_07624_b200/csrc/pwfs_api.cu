@@ -62,7 +62,7 @@ struct pwfs {
     int user_fpc = 0, user_ksplit = 0;
     int num_sms = 148;
     int x_resident_ctas = 296, y_resident_warps = 1184;   // what the device holds at once (occupancy query at create)
-    size_t scratch_budget = (size_t)4 << 30;
+    size_t scratch_budget = (size_t)16 << 30;   // of the 180 GB; PWFS_SCRATCH_MB overrides
     // instrumentation
     int timing = 0;
     std::vector<TimedSpan> spans;
@@ -268,15 +268,24 @@ int build_tables(pwfs *h) {
 }
 
 // frames per chunk and k-split for a batch of B frames
-void schedule(const pwfs *h, int B, int *fpc, int *ksplit) {
+// Frames per chunk and split of the modulation loop.  Chunks are as large as the scratch budget allows: every launch
+// ends with a partly filled wave of CTAs, so fewer, larger launches waste less of the machine (cfg 4: 13.9 ms per 100
+// frames in chunks of 15, 13.4 ms in one chunk).  `min_chunks` > 1 (host-buffer path) keeps at least that many chunks so
+// that copies still overlap the kernels.
+void schedule(const pwfs *h, int B, int *fpc, int *ksplit, int min_chunks = 1) {
     const DevTables &t = h->tab;
     const size_t T_frame = (size_t)t.KX * t.M * t.NP * sizeof(float2);   // T[f][j][x][y], x over the whole grid
     const int col_warps = (t.ncols + h->L.NB - 1) / h->L.NB;           // column-pass warps per frame
     const int slots = h->num_sms * 12;                                  // resident warps we aim to fill
-    int F = h->user_fpc > 0 ? h->user_fpc : (8 * slots + col_warps - 1) / col_warps;
-    const size_t maxF = std::max<size_t>(1, h->scratch_budget / std::max<size_t>(T_frame, 1));
+    const size_t maxF = std::min<size_t>(65535 /* grid.z */, std::max<size_t>(1, h->scratch_budget / std::max<size_t>(T_frame, 1)));
+    int F = h->user_fpc > 0 ? h->user_fpc : (int)std::min<size_t>(maxF, (size_t)std::max(B, 1));
+    if (h->user_fpc <= 0 && min_chunks > 1 && B >= 2 * min_chunks) F = std::min(F, (B + min_chunks - 1) / min_chunks);
     F = (int)std::min<size_t>((size_t)F, maxF);
     F = std::max(1, std::min(F, std::max(B, 1)));
+    if (h->user_fpc <= 0 && F < B) {          // equal chunks: ceil(B / n) frames for the smallest n that fits
+        const int n = (B + F - 1) / F;
+        F = (B + n - 1) / n;
+    }
     int ks = h->user_ksplit > 0 ? h->user_ksplit : 1;
     if (h->user_ksplit <= 0 && (long long)F * col_warps < 2LL * slots) {
         // too few warps for the machine (small batches, B = 1 in a closed loop): split the modulation loop, >= 4
@@ -647,7 +656,7 @@ int pwfs_run_host(pwfs_t *h, const float *h_phase, int32_t B, float *h_frames, f
     if (!h->in_stream) PWFS_CUDA(h, cudaStreamCreateWithFlags(&h->in_stream, cudaStreamNonBlocking));
     if (!h->out_stream) PWFS_CUDA(h, cudaStreamCreateWithFlags(&h->out_stream, cudaStreamNonBlocking));
     int F, ks;
-    schedule(h, B, &F, &ks);
+    schedule(h, B, &F, &ks, 6);
     int rc = ensure_scratch(h, F, ks);
     if (rc) return rc;
     const size_t n_chunks = ((size_t)B + F - 1) / F;
