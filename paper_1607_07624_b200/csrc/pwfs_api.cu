@@ -656,16 +656,18 @@ int pwfs_run_host(pwfs_t *h, const float *h_phase, int32_t B, float *h_frames, f
     if (!h->in_stream) PWFS_CUDA(h, cudaStreamCreateWithFlags(&h->in_stream, cudaStreamNonBlocking));
     if (!h->out_stream) PWFS_CUDA(h, cudaStreamCreateWithFlags(&h->out_stream, cudaStreamNonBlocking));
     int F, ks;
-    schedule(h, B, &F, &ks, 6);
+    // a short first chunk (the only copy-in nothing can hide), then three large ones (few partly filled last waves)
+    const int first = (h->user_fpc <= 0 && B >= 16) ? std::max(1, B / 16) : 0;
+    schedule(h, B - first, &F, &ks, 3);
     int rc = ensure_scratch(h, F, ks);
     if (rc) return rc;
-    const size_t n_chunks = ((size_t)B + F - 1) / F;
+    const size_t n_chunks = (first ? 1 : 0) + ((size_t)(B - first) + F - 1) / F;
     if ((rc = ensure_chunk_events(h, n_chunks))) return rc;
     // three streams, chunk by chunk: the copy-in of chunk c+1, and the tail kernels and the copy-out of chunk c-1,
     // run under the FFT kernels of chunk c (pinned host memory; pageable memory degrades to staged copies)
     size_t c = 0;
-    for (int f0 = 0; f0 < B; f0 += F, ++c) {
-        const int Fc = std::min(F, B - f0);
+    for (int f0 = 0, Fc = 0; f0 < B; f0 += Fc, ++c) {
+        Fc = (c == 0 && first) ? first : std::min(F, B - f0);
         float *dp = h->d_phase + (size_t)f0 * NN, *df = h->d_frames + (size_t)f0 * DD, *ds = h->d_slopes + (size_t)f0 * SS;
         PWFS_CUDA(h, cudaMemcpyAsync(dp, h_phase + (size_t)f0 * NN, (size_t)Fc * NN * sizeof(float), cudaMemcpyHostToDevice, h->in_stream));
         PWFS_CUDA(h, cudaEventRecord(h->in_ev[c], h->in_stream));
