@@ -9,7 +9,8 @@
 namespace pwk {
 namespace {
 
-using C = CfgFor<PWFS_INST_R1>::type;
+using C = CfgFor<PWFS_INST_R1>::type;     // row pass
+using CY = CfgForY<PWFS_INST_R1>::type;   // column pass
 
 template <bool QM>
 void launch_x_t(dim3 grid, cudaStream_t st, const DevTables &t, const float *phase, float2 *T, int jsplit) {
@@ -17,15 +18,15 @@ void launch_x_t(dim3 grid, cudaStream_t st, const DevTables &t, const float *pha
 }
 template <bool QM>
 void launch_y_t(dim3 grid, cudaStream_t st, const DevTables &t, const float2 *T, float *colbin, int ksplit) {
-    ypass_kernel<C, QM><<<grid, 32 * C::WPB_Y, C::smem_y, st>>>(t, T, colbin, ksplit);
+    ypass_kernel<CY, QM><<<grid, 32 * CY::WPB_Y, CY::smem_y, st>>>(t, T, colbin, ksplit);
 }
 template <bool QM>
 Launcher make() {
     Launcher l;
-    l.R1 = C::R1; l.NB = C::NB; l.WPB_X = C::WPB_X; l.WPB_Y = C::WPB_Y; l.RPC = C::RPC;
-    l.smem_x = QM ? C::smem_x_q : C::smem_x_t; l.smem_y = C::smem_y;
+    l.R1 = C::R1; l.NB = CY::NB; l.WPB_X = C::WPB_X; l.WPB_Y = CY::WPB_Y; l.RPC = C::RPC;
+    l.smem_x = QM ? C::smem_x_q : C::smem_x_t; l.smem_y = CY::smem_y;
     l.xfn = (const void *)xpass_kernel<C, QM>;
-    l.yfn = (const void *)ypass_kernel<C, QM>;
+    l.yfn = (const void *)ypass_kernel<CY, QM>;
     l.launch_x = launch_x_t<QM>;
     l.launch_y = launch_y_t<QM>;
     return l;

@@ -41,8 +41,15 @@ template <> struct CfgFor<54> { using type = PassCfg<54, 1, 8, 4, 1, 1>; };   //
 template <> struct CfgFor<60> { using type = PassCfg<60, 1, 8, 4, 1, 1>; };   // M = 1920
 template <> struct CfgFor<64> { using type = PassCfg<64, 1, 8, 4, 1, 1>; };   // M = 2048
 
+// The column pass may batch more transforms per warp than the row pass (whose shared memory also parks the base
+// phasor): more of the 32 lanes busy in the size-32 stage.  Default: the same configuration.  (R1 = 25 with NB = 5,
+// 125 items, was tried: the exchange buffers then allow only 6 warps per SM and the column pass ran 1.6x slower.)
+template <int R1> struct CfgForY { using type = typename CfgFor<R1>::type; };
+template <> struct CfgForY<15> { using type = PassCfg<15, 4, 8, 4, 2, 1>; };   // 60 items: two full rounds (was 30 of 32)
+template <> struct CfgForY<20> { using type = PassCfg<20, 3, 8, 4, 2, 1>; };   // 60 items (was 20 of 32)
+
 struct Launcher {
-    int R1, NB, WPB_X, WPB_Y, RPC;
+    int R1, NB, WPB_X, WPB_Y, RPC;   // NB, WPB_Y: column pass; WPB_X, RPC: row pass
     size_t smem_x, smem_y;
     const void *xfn, *yfn;
     void (*launch_x)(dim3, cudaStream_t, const DevTables &, const float *, float2 *, int);
