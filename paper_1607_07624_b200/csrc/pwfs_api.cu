@@ -658,7 +658,7 @@ int pwfs_run_host(pwfs_t *h, const float *h_phase, int32_t B, float *h_frames, f
     int F, ks;
     // a short first chunk (the only copy-in nothing can hide), then three large ones (few partly filled last waves)
     const int first = (h->user_fpc <= 0 && B >= 16) ? std::max(1, B / 16) : 0;
-    schedule(h, B - first, &F, &ks, 3);
+    schedule(h, B - first, &F, &ks, first ? 3 : 1);              // small batches: one chunk, copies are short anyway
     int rc = ensure_scratch(h, F, ks);
     if (rc) return rc;
     const size_t n_chunks = (first ? 1 : 0) + ((size_t)(B - first) + F - 1) / F;
