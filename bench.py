@@ -429,6 +429,9 @@ def run_ours(args, cfg):
                          "launch_ms": avg_launch_s * 1e3, "launches": n_launch,
                          "nominal_flops_per_launch": flops_per_launch,
                          "path_achieved": path_tflops, "path_frac": path_tflops / FP32_PEAK_TFLOPS,
+                         # 1-D transform pairs executed / the 2 K M pairs the nominal count assumes (shared x-pass,
+                         # pupil rows and window columns only): path_frac above this ratio x pipe utilisation is saving
+                         "executed_pair_ratio": (geo["k_unique"] * cfg.n_pupil + K * geo["n_cols"]) / (2.0 * K * M),
                          "kernel_ms_per_step": {k: v / args.steps for k, v in kernel_ms.items()},
                          "kernel_ms_note": "CUDA events around every launch; xrebin and slopes of chunk c run on a side stream "
                                            "under the row pass of chunk c+1, so their bracketed times include waiting for SM "
