@@ -218,6 +218,7 @@ struct PsfLauncher {
     void (*row)(dim3, cudaStream_t, const PsfDev &, const float *, float2 *);
     void (*col)(dim3, cudaStream_t, const PsfDev &, const float2 *, int, int, float *, float *);
     cudaError_t (*prepare)();
+    int (*col_ctas_per_sm)();       // occupancy of the column-pass kernel
 };
 
 template <class C>
@@ -235,7 +236,13 @@ cudaError_t prepare_t() {
     return e;
 }
 template <class C>
-PsfLauncher make() { return PsfLauncher{C::NB, C::WPB, C::RPC, C::smem, row_t<C>, col_t<C>, prepare_t<C>}; }
+int col_occ_t() {
+    int n = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, psf_col_kernel<C>, 32 * C::WPB, C::smem) != cudaSuccess || n < 1) n = 1;
+    return n;
+}
+template <class C>
+PsfLauncher make() { return PsfLauncher{C::NB, C::WPB, C::RPC, C::smem, row_t<C>, col_t<C>, prepare_t<C>, col_occ_t<C>}; }
 
 bool find_psf_launcher(int M, PsfLauncher *out) {
     if (M % 32) return false;
@@ -284,6 +291,7 @@ struct pwfs_psf {
     float *partial = nullptr; int partial_split = 0;
     long long count = 0;
     int num_sms = 148;
+    int col_resident = 148;          // column-pass CTAs the device holds at once
     size_t scratch_budget = (size_t)2 << 30;
 };
 
@@ -325,6 +333,7 @@ int pwfs_psf_create(const pwfs_psf_params *p, pwfs_psf_t **out) {
     if (e == cudaSuccess) {
         int sms = 0;
         if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, p->device) == cudaSuccess && sms > 0) h->num_sms = sms;
+        h->col_resident = h->num_sms * L.col_ctas_per_sm();
     }
     if (e != cudaSuccess) { int rc = cuda_rc(e); pwfs_psf_destroy(h); return rc; }
     PsfDev &d = h->dev;
@@ -348,8 +357,18 @@ int pwfs_psf_accumulate(pwfs_psf_t *h, const float *d_phase, int32_t B, float *d
     const int F = (int)std::min<size_t>((size_t)B, std::max<size_t>(1, h->scratch_budget / per_frame));
     // column pass: ~32 warps per SM in flight; the frame loop is split only as far as that needs
     const int col_ctas = (d.M + L.NB * L.WPB - 1) / (L.NB * L.WPB);
-    int fsplit = (32 * h->num_sms + col_ctas * L.WPB - 1) / (col_ctas * L.WPB);
-    fsplit = std::max(1, std::min(fsplit, F));
+    // split of the frame loop: minimise (waves of resident CTAs) x (frames per CTA + 2 for its prologue and the
+    // write of its partial PSF), at most 32 partials
+    int fsplit = 1;
+    {
+        double best = 1e300;
+        for (int c = 1; c <= std::min(F, 32); ++c) {
+            const long long ctas = (long long)col_ctas * c;
+            const double waves = (double)((ctas + h->col_resident - 1) / h->col_resident);
+            const double cost = waves * ((F + c - 1) / c + 2.0);
+            if (cost < best * (1.0 - 1e-9)) { best = cost; fsplit = c; }
+        }
+    }
     if ((size_t)F > h->T_frames) {
         if (h->T) cudaFree(h->T);
         h->T = nullptr; h->T_frames = 0;
