@@ -183,6 +183,25 @@ def test_schedule_knobs_do_not_change_results(torch_cuda):
         sensor.close()
 
 
+def test_host_buffer_pipeline_with_several_chunks(torch_cuda):
+    """B >= 16: pwfs_run_host works in a short first chunk and three large ones on three streams (copy-in, kernels,
+    tail + copy-out); every frame must come out as on the device path (FP32 summation order aside)."""
+    from paper_1607_07624_b200.pwfs import from_config
+    torch = torch_cuda
+    cfg = wl.CONFIGS["cfg1_tiny"]
+    phase = np.concatenate([wl.phase_batch(cfg, steps=10)] * 5)[:47]                # ragged: 2 + 15 + 15 + 15
+    phase = np.ascontiguousarray(phase + np.arange(47, dtype=np.float32)[:, None, None] * 0.01)   # all frames differ
+    with from_config(cfg) as sensor:
+        fd, sd = sensor.run(torch.from_numpy(phase).cuda())
+        fh = torch.empty((47, cfg.det_size, cfg.det_size), dtype=torch.float32).pin_memory()
+        sh = torch.empty((47, 2 * sensor.n_valid), dtype=torch.float32).pin_memory()
+        for _ in range(2):                                                          # second call re-uses events and scratch
+            fh.zero_(); sh.zero_()
+            sensor.run_host(torch.from_numpy(phase).pin_memory(), fh, sh)
+            assert ((fd.cpu() - fh).abs().amax(dim=(1, 2)) <= 2e-6 * fd.cpu().abs().amax(dim=(1, 2))).all()
+            assert (sd.cpu() - sh).abs().max() <= 1e-5
+
+
 def test_host_buffer_entry_point_matches_device_entry_point(torch_cuda):
     from paper_1607_07624_b200.pwfs import from_config
     torch = torch_cuda
