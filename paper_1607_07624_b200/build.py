@@ -62,9 +62,13 @@ def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJDIR, exist_ok=True)
     with ThreadPoolExecutor(max_workers=min(len(UNITS), os.cpu_count() or 4)) as pool:
         objs = list(pool.map(lambda u: _compile(u, force, verbose), UNITS))
-    tmp = LIB + f".tmp{os.getpid()}"
-    subprocess.run([nvcc_path(), "--shared", "-o", tmp] + objs, check=True)
-    os.replace(tmp, LIB)
+    tmp = os.path.join(OBJDIR, f"libpwfs.so.{os.getpid()}")     # link inside the ignored build/ directory
+    try:
+        subprocess.run([nvcc_path(), "--shared", "-o", tmp] + objs, check=True)
+        os.replace(tmp, LIB)
+    finally:
+        if os.path.exists(tmp):
+            os.remove(tmp)
     return LIB
 
 
