@@ -2,7 +2,10 @@
 """bench.py -- pyramid-WFS frames/s and fraction of roofline on B200.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
-                    [--config cfg4_elt] [--no-cpu-baseline]
+                    [--config cfg4_elt] [--no-cpu-baseline] [--no-stages] [--no-configs]
+
+--gpus N > 1 without a launcher starts N ranks itself (torch.distributed.run on
+127.0.0.1, one per GPU); under a launcher (WORLD_SIZE set) it must equal WORLD_SIZE.
 
 One "step" = one pass of the whole hot path (phasor+tilt -> pad -> FFT2 -> mask
 -> IFFT2 -> sum_k |E|^2 -> rebin -> slopes) over the full batch of the named
@@ -282,69 +285,235 @@ def run_reference(args, cfg):
     print(json.dumps(line), flush=True)
 
 
+class DryRunSensor:
+    """--dry-run only: a CPU stand-in with the sensor's interface, so that the launch / sharding / timing /
+    reporting plumbing of this file can be driven by a world-size-2 gloo test on a box without GPUs.  It
+    computes nothing of the method (its "frames" are per-frame means of the phase) and its line says so."""
+
+    def __init__(self, cfg):
+        self.det_size, self.n_valid, self.cfg = cfg.det_size, 4, cfg
+
+    def geometry(self, batch):
+        return dict(n_cols=2 * self.cfg.n_pupil, k_unique=self.cfg.mod_points // 2 + 1, frames_per_chunk=batch, k_split=1)
+
+    def run(self, phase, frames, slopes):
+        frames[:] = phase.mean(dim=(1, 2))[:, None, None]
+        slopes.zero_()
+        return frames, slopes
+
+    def set_timing(self, on):
+        pass
+
+    def get_timing(self):
+        return {k: 0.0 for k in ("xpass", "ypass", "xrebin", "slopes")}, {k: 0 for k in ("xpass", "ypass", "xrebin", "slopes")}
+
+    def close(self):
+        pass
+
+
+def time_hot_path(sensor, phase, frames, slopes, steps, warmup, flush, stream, barrier, sampler=None):
+    """W untimed calls, then K timed calls of sensor.run over the whole batch, each bracketed by CUDA events on the
+    launching stream with the L2 flushed (untimed) before it; barrier + synchronize on both sides.  Returns
+    (summed ms over the K steps on this rank, per-kernel ms, per-kernel launch counts, clock record)."""
+    import torch
+    for _ in range(warmup):
+        sensor.run(phase, frames, slopes)
+    barrier()
+    sensor.get_timing()                                  # reset counters
+    sensor.set_timing(True)
+    if sampler is not None:
+        sampler.start()
+    barrier()
+    if stream is None:                                   # --dry-run: no device, wall clock
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            sensor.run(phase, frames, slopes)
+        ms_total = (time.perf_counter() - t0) * 1e3
+        barrier()
+    else:
+        ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(steps)]
+        ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(steps)]
+        for i in range(steps):
+            flush.zero_()                                # evict L2 between timed steps (not timed)
+            ev0[i].record(stream)
+            sensor.run(phase, frames, slopes)
+            ev1[i].record(stream)
+        barrier()
+        ms_total = sum(a.elapsed_time(b) for a, b in zip(ev0, ev1))
+    clocks = sampler.stop() if sampler is not None else None
+    kernel_ms, launches = sensor.get_timing()
+    sensor.set_timing(False)
+    return ms_total, kernel_ms, launches, clocks
+
+
+def roofline_numbers(cfg, geo, B, steps, ms_per_step, kernel_ms, launches, peak_tflops):
+    """Fractions of the FP32 roofline from one timed run: the whole path against the nominal 2 x 5 M^2 log2 M^2
+    flop per modulation point, and the dominant kernel against its half of that."""
+    M, K = cfg.m_grid, cfg.mod_points
+    dom = max(kernel_ms, key=kernel_ms.get)
+    n_launch = max(1, launches[dom])
+    units_per_launch = B * K * steps / n_launch                          # modulation points per launch
+    share = {"xpass": 0.5, "ypass": 0.5}.get(dom, 0.0)
+    flops_per_launch = share * nominal_flops_per_modpoint(M) * units_per_launch
+    avg_launch_s = kernel_ms[dom] * 1e-3 / n_launch
+    achieved = flops_per_launch / avg_launch_s / 1e12 if avg_launch_s > 0 else 0.0
+    path_tflops = nominal_flops_per_modpoint(M) * B * K / (ms_per_step * 1e-3) / 1e12
+    return {"kernel": dom, "achieved": achieved, "frac": achieved / peak_tflops, "launch_ms": avg_launch_s * 1e3,
+            "launches": n_launch, "nominal_flops_per_launch": flops_per_launch, "path_achieved": path_tflops,
+            "path_frac": path_tflops / peak_tflops,
+            # 1-D transform pairs executed / the 2 K M pairs the nominal count assumes (shared x-pass, pupil rows
+            # and window columns only): path_frac above this ratio x pipe utilisation is algorithmic saving
+            "executed_pair_ratio": (geo["k_unique"] * cfg.n_pupil + K * geo["n_cols"]) / (2.0 * K * M),
+            "kernel_ms_per_step": {k: v / steps for k, v in kernel_ms.items()}}
+
+
+def bench_other_configs(main_name, dev, flush, steps, warmup) -> dict:
+    """Every BASELINE.json config timed like the headline one (full batch per step, warm-up, L2 flushed before each
+    timed step, CUDA events, per-kernel brackets): frames/s, ms per step, fraction of the FP32 roofline for the path
+    and for the dominant kernel.  Frozen-flow inputs come from the f1 device kernel on the same seeded screens."""
+    import torch
+    from paper_1607_07624_b200.atmo import Atmosphere
+    from paper_1607_07624_b200.pwfs import from_config
+    stream = torch.cuda.current_stream(dev)
+    out = {}
+    for name in wl.CONFIG_ORDER:
+        if name == main_name:
+            continue
+        cfg = wl.CONFIGS[name]
+        if cfg.independent_screens:
+            phase = torch.from_numpy(wl.phase_batch(cfg)).to(dev)
+            src = "numpy generator (independent screens)"
+        else:
+            atm = wl.atmosphere(cfg)
+            with Atmosphere(**{k: v for k, v in atm.items() if k != "dt"}, device=dev.index) as a:
+                phase = a.propagate(0, cfg.steps, atm["dt"])
+                torch.cuda.synchronize(dev)
+            src = "f1 device propagation of the seeded screens"
+        B = phase.shape[0]
+        with from_config(cfg, device=dev.index) as sensor:
+            geo = sensor.geometry(B)
+            D, nv = sensor.det_size, sensor.n_valid
+            frames = torch.empty((B, D, D), dtype=torch.float32, device=dev)
+            slopes = torch.empty((B, 2 * nv), dtype=torch.float32, device=dev)
+            sync = lambda: torch.cuda.synchronize(dev)
+            ms_total, kernel_ms, launches, _ = time_hot_path(sensor, phase, frames, slopes, steps, warmup, flush, stream, sync)
+        ms = ms_total / steps
+        r = roofline_numbers(cfg, geo, B, steps, ms, kernel_ms, launches, FP32_PEAK_TFLOPS)
+        out[name] = {"frames_per_step": B, "frames_per_s": B / (ms * 1e-3), "ms_per_step": ms,
+                     "modpoint_ffts_per_s": B * cfg.mod_points / (ms * 1e-3), "m_grid": cfg.m_grid, "n_pupil": cfg.n_pupil,
+                     "mod_points": cfg.mod_points, "frames_per_chunk": geo["frames_per_chunk"], "k_split": geo["k_split"],
+                     "path_frac": r["path_frac"], "dominant_kernel": r["kernel"], "dominant_frac": r["frac"],
+                     "executed_pair_ratio": r["executed_pair_ratio"], "kernel_ms_per_step": r["kernel_ms_per_step"],
+                     "steps": steps, "warmup": warmup, "input": src}
+        del phase, frames, slopes
+    return out
+
+
+def measure_fp32_peak(local: int) -> dict:
+    """pwfs_peak_fp32 (FFMA and FFMA2 streams on every SM) with the SM clock sampled while it runs."""
+    from paper_1607_07624_b200.pwfs import peak_fp32
+    sampler = ClockSampler(local)
+    sampler.start()
+    res = {}
+    for _ in range(3):                                   # ~50 ms each: long enough for a few clock samples
+        for nm, packed in (("ffma", False), ("ffma2", True)):
+            tf, ms = peak_fp32(local, packed)
+            res[nm] = max(res.get(nm, 0.0), tf)
+    clk = sampler.stop()
+    best = max(res.values())
+    return {"tflops": best, "ffma_tflops": res["ffma"], "ffma2_tflops": res["ffma2"], "sm_mhz": clk["sm_mhz"],
+            "how": "pwfs_peak_fp32: independent FFMA / FFMA2 chains, 64 warps per SM, best of 3 x 5 launches, CUDA events"}
+
+
 def run_ours(args, cfg):
     import torch
     import torch.distributed as dist
     from paper_1607_07624_b200 import sharding
-    from paper_1607_07624_b200.pwfs import from_config
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}: launch one rank per GPU "
+                         f"(python bench.py --gpus N starts them itself)")
+    dry = args.dry_run
+    if dry:
+        dev = torch.device("cpu")
+    else:
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+        if torch.cuda.device_count() < world:
+            raise SystemExit(f"bench.py: --gpus {world} needs {world} CUDA devices, this node has {torch.cuda.device_count()}")
+        torch.cuda.set_device(local)
+        dev = torch.device("cuda", local)
     if world > 1:
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=dev)
+        if dry:
+            dist.init_process_group("gloo")
+        else:
+            dist.init_process_group("nccl", device_id=dev)
 
-    # weak scaling: every rank runs the full batch of the config on its own seeded slice of time
-    steps_cfg = cfg.steps
-    phase_np = wl.phase_batch(cfg, steps=steps_cfg, first_step=rank * steps_cfg)
+    # weak scaling: the job is world x (the config's batch); rank r owns the contiguous block of frames
+    # sharding.my_frames gives it (whole simulation steps), i.e. its own seeded slice of time.  No data-path
+    # collective: outputs stay on the GPU that holds their inputs.
+    B_cfg = cfg.batch
+    lo, hi = sharding.my_frames(world * B_cfg)
+    assert lo % cfg.instances == 0 and hi - lo == B_cfg
+    phase_np = wl.phase_batch(cfg, steps=(hi - lo) // cfg.instances, first_step=lo // cfg.instances)
     B = phase_np.shape[0]
-    sensor = from_config(cfg, device=local)
+    if dry:
+        sensor = DryRunSensor(cfg)
+    else:
+        from paper_1607_07624_b200.pwfs import from_config
+        sensor = from_config(cfg, device=local)
     geo = sensor.geometry(B)
     phase = torch.from_numpy(phase_np).to(dev)
     D, nv = sensor.det_size, sensor.n_valid
     frames = torch.empty((B, D, D), dtype=torch.float32, device=dev)
     slopes = torch.empty((B, 2 * nv), dtype=torch.float32, device=dev)
-    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
-    stream = torch.cuda.current_stream(dev)
+    flush = None if dry else torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+    stream = None if dry else torch.cuda.current_stream(dev)
 
     def barrier():
-        torch.cuda.synchronize(dev)
+        if not dry:
+            torch.cuda.synchronize(dev)
         if world > 1:
             dist.barrier()
-            torch.cuda.synchronize(dev)
+            if not dry:
+                torch.cuda.synchronize(dev)
 
     def max_over_ranks(x: float) -> float:
         return sharding.max_over_ranks(x, dev)
 
     # ---- device-resident timing (value) -------------------------------------
-    for _ in range(args.warmup):
-        sensor.run(phase, frames, slopes)
-    barrier()
-    sensor.get_timing()                                  # reset counters
-    sensor.set_timing(True)
-    sampler = ClockSampler(local)
-    ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
-    ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
-    sampler.start()
-    barrier()
-    for i in range(args.steps):
-        flush.zero_()                                    # evict L2 between timed steps (not timed)
-        ev0[i].record(stream)
-        sensor.run(phase, frames, slopes)
-        ev1[i].record(stream)
-    barrier()
-    clocks = sampler.stop()
-    ms_total = sum(a.elapsed_time(b) for a, b in zip(ev0, ev1))
-    kernel_ms, launches = sensor.get_timing()
-    sensor.set_timing(False)
-    ms_total = max_over_ranks(ms_total)
+    sampler = None if dry else ClockSampler(local)
+    ms_rank, kernel_ms, launches, clocks = time_hot_path(sensor, phase, frames, slopes, args.steps, args.warmup, flush,
+                                                         stream, barrier, sampler)
+    ms_total = max_over_ranks(ms_rank)
     ms_per_step = ms_total / args.steps
     value = world * B * args.steps / (ms_total * 1e-3)
+    per_rank = None
+    if world > 1:                                        # every rank's own frames/s, gathered for the report
+        t = torch.tensor([B * args.steps / (ms_rank * 1e-3)], dtype=torch.float64, device=dev)
+        allv = [torch.zeros_like(t) for _ in range(world)]
+        dist.all_gather(allv, t)
+        per_rank = [float(v.item()) for v in allv]
+
+    if dry:
+        if rank == 0:
+            print(json.dumps({"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                              "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
+                              "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                              "dry_run": True, "per_rank_frames_per_s": per_rank,
+                              "config": {"workload": cfg.name, "frames_per_step": world * B, "frames_per_rank": B,
+                                         "first_frame_of_rank0": lo,
+                                         "parallelism": f"frames sharded over {world} rank(s), no collective"},
+                              "note": "--dry-run: CPU stand-in sensor, plumbing test only, NOT a measurement",
+                              "gpu_launches": 0}), flush=True)
+        if world > 1:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
 
     # ---- closed-loop latency: one frame per call (B = 1), eager and replayed from a CUDA graph
     latency = None
@@ -392,16 +561,8 @@ def run_ours(args, cfg):
 
     if rank == 0:
         M, K = cfg.m_grid, cfg.mod_points
-        # dominant kernel = column pass; its share of the nominal work is the y-direction
-        # transforms, i.e. half of 2 x 5 M^2 log2(M^2) per modulation point
-        dom = max(kernel_ms, key=kernel_ms.get)
-        n_launch = max(1, launches[dom])
-        units_per_launch = B * K * args.steps / n_launch                 # modulation points per launch
-        share = {"xpass": 0.5, "ypass": 0.5}.get(dom, 0.0)
-        flops_per_launch = share * nominal_flops_per_modpoint(M) * units_per_launch
-        avg_launch_s = kernel_ms[dom] * 1e-3 / n_launch
-        achieved = flops_per_launch / avg_launch_s / 1e12 if avg_launch_s > 0 else 0.0
-        path_tflops = nominal_flops_per_modpoint(M) * B * K / (ms_per_step * 1e-3) / 1e12
+        r = roofline_numbers(cfg, geo, B, args.steps, ms_per_step, kernel_ms, launches, FP32_PEAK_TFLOPS)
+        dom, n_launch = r["kernel"], r["launches"]
         traffic = None                                                   # dram bytes per launch, from the committed ncu capture
         tpath = os.path.join(ROOT, "profiles", "traffic.csv")
         if os.path.exists(tpath):
@@ -411,38 +572,48 @@ def run_ours(args, cfg):
                     if row["config"] == cfg.name and row["kernel"] == dom:
                         per_frame = float(row["dram_bytes_per_launch"]) / float(row["frames_per_launch"])
                         traffic = per_frame * B * args.steps / n_launch
+        peak_m = measure_fp32_peak(local)
+        roof = {"bound": "alu", "kernel": dom, "achieved": r["achieved"], "peak": FP32_PEAK_TFLOPS,
+                "unit": "TFLOP/s", "frac": r["frac"], "traffic": traffic,
+                "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (guide unit counts/clocks)",
+                "peak_measured": peak_m["tflops"], "peak_measured_detail": peak_m,
+                "frac_vs_measured": r["achieved"] / peak_m["tflops"],
+                "path_frac_vs_measured": r["path_achieved"] / peak_m["tflops"]}
+        roof.update({k: r[k] for k in ("launch_ms", "launches", "nominal_flops_per_launch", "path_achieved", "path_frac",
+                                       "executed_pair_ratio", "kernel_ms_per_step")})
+        roof["kernel_ms_note"] = ("CUDA events around every launch; xrebin and slopes of chunk c run on a side stream "
+                                  "under the row pass of chunk c+1, so their bracketed times include waiting for SM "
+                                  "slots and overlap xpass")
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": cfg.name, "n_pupil": cfg.n_pupil, "m_grid": M, "mod_points": K,
-                       "mod_radius": cfg.mod_radius, "n_subap": cfg.n_subap, "frames_per_step": B,
+                       "mod_radius": cfg.mod_radius, "n_subap": cfg.n_subap, "frames_per_step": world * B,
+                       "frames_per_rank": B,
                        "frames_per_chunk": geo["frames_per_chunk"], "k_split": geo["k_split"],
                        "k_unique_xtilts": geo["k_unique"], "columns_computed": geo["n_cols"],
                        "l2": f"flushed between timed steps ({L2_FLUSH_BYTES >> 20} MiB memset, untimed)",
                        "parallelism": f"frames sharded over {world} GPU(s), no collective"},
             "modpoint_ffts_per_s": value * K,
             "transforms_2d_per_s": 2 * value * K,
-            "roofline": {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": FP32_PEAK_TFLOPS,
-                         "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS, "traffic": traffic,
-                         "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (guide unit counts/clocks)",
-                         "launch_ms": avg_launch_s * 1e3, "launches": n_launch,
-                         "nominal_flops_per_launch": flops_per_launch,
-                         "path_achieved": path_tflops, "path_frac": path_tflops / FP32_PEAK_TFLOPS,
-                         # 1-D transform pairs executed / the 2 K M pairs the nominal count assumes (shared x-pass,
-                         # pupil rows and window columns only): path_frac above this ratio x pipe utilisation is saving
-                         "executed_pair_ratio": (geo["k_unique"] * cfg.n_pupil + K * geo["n_cols"]) / (2.0 * K * M),
-                         "kernel_ms_per_step": {k: v / args.steps for k, v in kernel_ms.items()},
-                         "kernel_ms_note": "CUDA events around every launch; xrebin and slopes of chunk c run on a side stream "
-                                           "under the row pass of chunk c+1, so their bracketed times include waiting for SM "
-                                           "slots and overlap xpass (alone they take ~0.13 and ~0.06 ms per step)"},
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h_phase.numel() * 4),
-                    "d2h_bytes_per_step": int(h_frames.numel() * 4 + h_slopes.numel() * 4),
+            "per_rank_frames_per_s": per_rank,
+            "roofline": roof,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h_phase.numel() * 4) * world,
+                    "d2h_bytes_per_step": int(h_frames.numel() * 4 + h_slopes.numel() * 4) * world,
                     "matches_device_path": same},
             "gpu_launches": int(sum(launches.values())),
             "latency_b1": latency,
             "clocks": clocks,
         }
+        if not args.no_configs and world == 1:
+            line["configs"] = bench_other_configs(cfg.name, dev, flush, steps=max(3, min(args.steps, 5)), warmup=3)
+            line["configs"][cfg.name] = {
+                "frames_per_step": B, "frames_per_s": value, "ms_per_step": ms_per_step, "modpoint_ffts_per_s": value * K,
+                "m_grid": M, "n_pupil": cfg.n_pupil, "mod_points": K, "frames_per_chunk": geo["frames_per_chunk"],
+                "k_split": geo["k_split"], "path_frac": r["path_frac"], "dominant_kernel": dom, "dominant_frac": r["frac"],
+                "executed_pair_ratio": r["executed_pair_ratio"], "kernel_ms_per_step": r["kernel_ms_per_step"],
+                "steps": args.steps, "warmup": args.warmup, "input": "numpy generator (the headline run above)"}
         if not args.no_stages:
             line["stages"] = bench_stages(cfg, dev, phase, frames, flush)
         if not args.no_cpu_baseline:
@@ -457,6 +628,24 @@ def run_ours(args, cfg):
         dist.destroy_process_group()
 
 
+def spawn_ranks(args) -> None:
+    """`python bench.py --gpus N` without a launcher: start N ranks of this file on this node (one per GPU) the way
+    the driver does -- torch.distributed.run, rendezvous on 127.0.0.1 -- and replace this process by the launcher."""
+    import socket
+    if not args.dry_run:
+        import torch
+        n_dev = torch.cuda.device_count() if torch.cuda.is_available() else 0
+        if n_dev < args.gpus:
+            raise SystemExit(f"bench.py: --gpus {args.gpus} needs {args.gpus} CUDA devices, this node has {n_dev}")
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    sys.stdout.flush()
+    os.execv(sys.executable, cmd)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -466,12 +655,19 @@ def main():
     ap.add_argument("--config", default="cfg4_elt", choices=wl.CONFIG_ORDER)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-stages", action="store_true", help="skip the per-stage timings of the 8(f) rows")
+    ap.add_argument("--no-configs", action="store_true", help="skip the timings of the other four configs")
+    ap.add_argument("--dry-run", action="store_true",
+                    help="CPU stand-in sensor on gloo: exercises launch/sharding/timing/report plumbing only")
     args = ap.parse_args()
     if args.steps < 1 or args.warmup < 0:
         raise SystemExit("bench.py: need --steps >= 1 and --warmup >= 0")
     cfg = wl.CONFIGS[args.config]
+    if args.gpus < 1:
+        raise SystemExit("bench.py: need --gpus >= 1")
     if args.impl == "reference":
         run_reference(args, cfg)
+    elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        spawn_ranks(args)
     else:
         run_ours(args, cfg)
 

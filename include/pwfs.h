@@ -62,7 +62,11 @@ typedef struct {
     const float *pupil_amp; /* HOST ptr, N*N floats row-major [y][x]; amplitude A >= 0; copied */
     int32_t mask_shift_px;  /* s : pupil-image offset in px (mask phase 2 pi s (|u~|+|v~|)/M).
                                <= 0 selects the default M/4 (needs M % 4 == 0).
-                               Needs N <= 2 s and s <= M/2 - N/2 (windows disjoint, in grid)  */
+                               Needs N <= 2 s and s <= M/2 - N/2 (windows disjoint, in grid).
+                               An INTEGER by design: the pupil images are read back through
+                               windows of whole grid pixels (O7's origin M/2 +- s - N/2), and
+                               DESIGN.md reading A8 fixes s to whole pixels; a half-pixel shift
+                               would need an interpolating window and is not part of the model */
     float mod_radius;       /* r >= 0 in lambda/D                                             */
     int32_t mod_points;     /* K >= 1 points equally spaced on the circle (K=1, r=0: none)    */
     float mod_angle0;       /* theta_0 [rad] of point 0, counter-clockwise from +x            */
@@ -125,10 +129,22 @@ int pwfs_valid_mask(const pwfs_t *h, uint8_t *host_mask);
  * (1,1); may be NULL.  cuda_stream: a cudaStream_t (NULL = default stream).
  * Asynchronous: work is enqueued on the stream and the call returns; buffers
  * must stay alive until the stream reaches that point.  B = 0 is a no-op.
- * Does not allocate once scratch has been sized for a batch this large.
+ * Does not allocate once scratch has been sized for a batch this large
+ * (pwfs_reserve, or an earlier call); when a larger batch arrives it frees and
+ * re-allocates its scratch -- except while `cuda_stream` is being captured into a
+ * CUDA graph, where it returns PWFS_EINVAL and enqueues nothing.  The CUDA device
+ * that was current on entry is current again on return.
  * Defined by: north_star "pwfs_run(phase batch -> frames, slopes)". */
 int pwfs_run(pwfs_t *h, const float *d_phase, int32_t B, float *d_frames, float *d_slopes,
              void *cuda_stream);
+
+/* Size the handle's scratch memory (and, for batches that run in several chunks,
+ * its internal side stream and events) for pwfs_run calls of up to B frames, so
+ * that those calls neither allocate nor create anything.  Required before a
+ * pwfs_run of a batch size the handle has not seen is captured into a CUDA graph:
+ * cudaMalloc is not allowed during stream capture, and pwfs_run then returns
+ * PWFS_EINVAL instead of allocating.  Synchronous; may free and re-allocate. */
+int pwfs_reserve(pwfs_t *h, int32_t B);
 
 /* Same computation with HOST buffers (h_slopes may be NULL): copies the phase
  * batch host->device, runs, copies frames and slopes device->host and returns
@@ -146,6 +162,10 @@ const char *pwfs_strerror(int code);
 
 /* cudaError_t (as int) of the last failing CUDA call on this handle, 0 if none. */
 int pwfs_last_cuda_error(const pwfs_t *h);
+
+/* Kernel class (see pwfs_get_timing) of the last launch the CUDA runtime refused on
+ * this handle, -1 if none: pwfs_run checks cudaGetLastError after every launch. */
+int pwfs_last_failed_kernel(const pwfs_t *h);
 
 /* 1 if this build has kernels for an M-point grid, else 0. */
 int pwfs_supported_grid(int32_t m_grid);
@@ -174,6 +194,15 @@ int pwfs_get_timing(pwfs_t *h, float ms[PWFS_NUM_KERNEL_CLASSES],
  * and k_split as they would be used for a batch of B frames. */
 int pwfs_geometry(const pwfs_t *h, int32_t B, int32_t *n_cols, int32_t *k_unique,
                   int32_t *frames_per_chunk, int32_t *k_split);
+
+/* Measurement aid, not part of the hot path: the FP32 arithmetic peak of `device`
+ * as a stream of independent FFMA (packed = 0) or packed FFMA2 (packed = 1)
+ * instructions on every SM (64 resident warps each, 8 independent accumulator
+ * pairs per thread), best of five launches of ~10^12 flop, timed with CUDA events.
+ * *tflops counts an FMA as 2 flop.  This is the measured counterpart of the
+ * derived "148 SMs x 128 lanes x 2 x f_SM" roofline denominator that SURVEY.md
+ * 8(d) asks for.  Synchronous; uses the legacy default stream. */
+int pwfs_peak_fp32(int32_t device, int32_t packed, double *tflops, double *elapsed_ms);
 
 #ifdef __cplusplus
 }

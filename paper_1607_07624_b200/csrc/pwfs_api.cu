@@ -36,6 +36,17 @@ bool find_launcher(int M, bool quarter, Launcher *out) {
 
 struct TimedSpan { cudaEvent_t a, b; int cls; };
 
+// Makes `dev` current for the duration of a call and restores the caller's device afterwards.
+struct DeviceGuard {
+    int prev = -1, dev;
+    cudaError_t err;
+    explicit DeviceGuard(int d) : dev(d) {
+        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+        err = (prev == dev) ? cudaSuccess : cudaSetDevice(dev);
+    }
+    ~DeviceGuard() { if (prev >= 0 && prev != dev) cudaSetDevice(prev); }
+};
+
 }  // namespace
 
 struct pwfs {
@@ -70,6 +81,7 @@ struct pwfs {
     float ms_acc[PWFS_NUM_KERNEL_CLASSES] = {0, 0, 0, 0};
     int64_t launches[PWFS_NUM_KERNEL_CLASSES] = {0, 0, 0, 0};
     int last_cuda = 0;
+    int last_kernel = -1;                    // kernel class of the last launch that failed, -1 none
 };
 
 namespace {
@@ -303,10 +315,17 @@ void schedule(const pwfs *h, int B, int *fpc, int *ksplit, int min_chunks = 1) {
     *fpc = F; *ksplit = ks;
 }
 
-int ensure_scratch(pwfs *h, int F, int ksplit) {
+// `st`: the stream the caller is about to enqueue on.  cudaMalloc/cudaFree are not allowed while it is being
+// captured into a CUDA graph: a batch that needs more scratch than the handle holds is refused with PWFS_EINVAL
+// (pwfs_reserve, or one eager pwfs_run of that size, before the capture avoids it).
+int ensure_scratch(pwfs *h, int F, int ksplit, cudaStream_t st = nullptr, bool check_capture = false) {
     const DevTables &t = h->tab;
     const size_t needT = (size_t)F * t.KX * t.M * t.NP;
     const size_t needC = (size_t)F * ksplit * t.ncols * t.D;
+    if (check_capture && (needT > h->T_elems || needC > h->colbin_elems || (size_t)F * t.D > h->nsum_elems)) {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(st, &cs) == cudaSuccess && cs != cudaStreamCaptureStatusNone) return PWFS_EINVAL;
+    }
     if (needT > h->T_elems) {
         if (h->T) cudaFree(h->T);
         h->T = nullptr; h->T_elems = 0;
@@ -419,7 +438,8 @@ int pwfs_create_ex(const pwfs_params *p, const pwfs_ext *x, pwfs_t **out) {
             h->list_w.push_back(x->tilt_w ? (double)x->tilt_w[k] : 1.0);
         }
     int rc = PWFS_OK;
-    cudaError_t e = cudaSetDevice(p->device);
+    DeviceGuard dg(p->device);
+    cudaError_t e = dg.err;
     if (e != cudaSuccess) { h->last_cuda = (int)e; rc = PWFS_ECUDA; }
     if (!rc) {
         cudaDeviceProp prop;
@@ -453,7 +473,7 @@ int pwfs_create_ex(const pwfs_params *p, const pwfs_ext *x, pwfs_t **out) {
 
 void pwfs_destroy(pwfs_t *h) {
     if (!h) return;
-    cudaSetDevice(h->device);
+    DeviceGuard dg(h->device);
     for (void *d : h->dev_allocs) cudaFree(d);
     if (h->T) cudaFree(h->T);
     if (h->colbin) cudaFree(h->colbin);
@@ -486,6 +506,8 @@ int pwfs_valid_mask(const pwfs_t *h, uint8_t *host_mask) {
 }
 
 int pwfs_last_cuda_error(const pwfs_t *h) { return h ? h->last_cuda : 0; }
+
+int pwfs_last_failed_kernel(const pwfs_t *h) { return h ? h->last_kernel : -1; }
 
 int pwfs_set_schedule(pwfs_t *h, int32_t frames_per_chunk, int32_t k_split) {
     if (!h || frames_per_chunk < 0 || k_split < 0 || k_split > h->tab.K) return PWFS_EINVAL;
@@ -532,6 +554,15 @@ int pwfs_get_timing(pwfs_t *h, float ms[PWFS_NUM_KERNEL_CLASSES], int64_t launch
     return PWFS_OK;
 }
 
+// A launch that the runtime refuses (bad configuration, sticky fault) is reported at once, with its kernel class.
+static int check_launch(pwfs_t *h, int cls) {
+    const cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) return PWFS_OK;
+    h->last_cuda = (int)e;
+    h->last_kernel = cls;
+    return PWFS_ECUDA;
+}
+
 // One chunk of Fc <= F frames is three enqueue steps: K1 (row pass), K2 (column pass), tail (x-rebin + slopes).
 static int launch_k1(pwfs_t *h, const float *d_phase, int Fc, cudaStream_t st) {
     const DevTables &t = h->tab;
@@ -553,7 +584,7 @@ static int launch_k1(pwfs_t *h, const float *d_phase, int Fc, cudaStream_t st) {
         }
     }
     L.launch_x(dim3(row_ctas, jsplit, Fc), st, t, d_phase, h->T, jsplit);
-    return PWFS_OK;
+    return check_launch(h, 0);
 }
 
 static int launch_k2(pwfs_t *h, int Fc, int ks, cudaStream_t st) {
@@ -562,7 +593,7 @@ static int launch_k2(pwfs_t *h, int Fc, int ks, cudaStream_t st) {
     SpanGuard g(h, st, 1);   // K2: y-convolution + |E|^2 over k + y-rebin (a3, a4, a5 along y, a6, a7)
     const int per_cta = L.NB * L.WPB_Y;
     L.launch_y(dim3((t.ncols + per_cta - 1) / per_cta, ks, Fc), st, t, h->T, h->colbin, ks);
-    return PWFS_OK;
+    return check_launch(h, 1);
 }
 
 static int launch_tail(pwfs_t *h, int Fc, float *d_frames, float *d_slopes, int ks, cudaStream_t st) {
@@ -573,12 +604,13 @@ static int launch_tail(pwfs_t *h, int Fc, float *d_frames, float *d_slopes, int 
         // 1/K of O6; the quarter-mask kernels leave O5's 1/M per axis (1/M^4 on |E|^2) to this scale
         const double m4 = h->quarter ? std::pow((double)t.M, 4.0) : 1.0;
         xrebin_kernel<<<dim3(t.D, Fc), threads, 0, st>>>(t, h->colbin, d_frames, h->nsum, ks, (float)(1.0 / ((double)t.K * m4)));
+        if (int rc = check_launch(h, 2)) return rc;
     }
     if (d_slopes) {   // K3b: slopes (a8)
         SpanGuard g(h, st, 3);
         slopes_kernel<<<dim3((t.n_valid + 255) / 256, Fc), 256, 0, st>>>(t, d_frames, h->nsum, d_slopes);
+        if (int rc = check_launch(h, 3)) return rc;
     }
-    PWFS_CUDA(h, cudaGetLastError());
     return PWFS_OK;
 }
 
@@ -596,16 +628,33 @@ static int ensure_chunk_events(pwfs_t *h, size_t n_chunks) {
     return PWFS_OK;
 }
 
+int pwfs_reserve(pwfs_t *h, int32_t B) {
+    if (!h || B < 1) return PWFS_EINVAL;
+    DeviceGuard dg(h->device);
+    PWFS_CUDA(h, dg.err);
+    int F, ks;
+    schedule(h, B, &F, &ks);
+    int rc = ensure_scratch(h, F, ks);
+    if (rc) return rc;
+    const size_t n_chunks = ((size_t)B + F - 1) / F;
+    if (n_chunks > 1) {
+        if (!h->out_stream) PWFS_CUDA(h, cudaStreamCreateWithFlags(&h->out_stream, cudaStreamNonBlocking));
+        if ((rc = ensure_chunk_events(h, n_chunks))) return rc;
+    }
+    return PWFS_OK;
+}
+
 int pwfs_run(pwfs_t *h, const float *d_phase, int32_t B, float *d_frames, float *d_slopes, void *cuda_stream) {
     if (!h || B < 0) return PWFS_EINVAL;
     if (B == 0) return PWFS_OK;
     if (!d_phase || !d_frames) return PWFS_EINVAL;
-    PWFS_CUDA(h, cudaSetDevice(h->device));
+    DeviceGuard dg(h->device);
+    PWFS_CUDA(h, dg.err);
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const DevTables &t = h->tab;
     int F, ks;
     schedule(h, B, &F, &ks);
-    int rc = ensure_scratch(h, F, ks);
+    int rc = ensure_scratch(h, F, ks, st, true);
     if (rc) return rc;
     const size_t NN = (size_t)t.N * t.N, DD = (size_t)t.D * t.D, SS = (size_t)2 * t.n_valid;
     const size_t n_chunks = ((size_t)B + F - 1) / F;
@@ -638,7 +687,8 @@ int pwfs_run_host(pwfs_t *h, const float *h_phase, int32_t B, float *h_frames, f
     if (!h || B < 0) return PWFS_EINVAL;
     if (B == 0) return PWFS_OK;
     if (!h_phase || !h_frames) return PWFS_EINVAL;
-    PWFS_CUDA(h, cudaSetDevice(h->device));
+    DeviceGuard dg(h->device);
+    PWFS_CUDA(h, dg.err);
     const DevTables &t = h->tab;
     const size_t NN = (size_t)t.N * t.N, DD = (size_t)t.D * t.D, SS = (size_t)2 * t.n_valid;
     if (!h->hstream) PWFS_CUDA(h, cudaStreamCreateWithFlags(&h->hstream, cudaStreamNonBlocking));
@@ -657,8 +707,9 @@ int pwfs_run_host(pwfs_t *h, const float *h_phase, int32_t B, float *h_frames, f
     if (!h->out_stream) PWFS_CUDA(h, cudaStreamCreateWithFlags(&h->out_stream, cudaStreamNonBlocking));
     int F, ks;
     // a short first chunk (the only copy-in nothing can hide), then three large ones (few partly filled last waves)
-    const int first = (h->user_fpc <= 0 && B >= 16) ? std::max(1, B / 16) : 0;
+    int first = (h->user_fpc <= 0 && B >= 16) ? std::max(1, B / 16) : 0;
     schedule(h, B - first, &F, &ks, first ? 3 : 1);              // small batches: one chunk, copies are short anyway
+    first = std::min(first, F);                                  // scratch (and grid.z) hold F frames, the short chunk too
     int rc = ensure_scratch(h, F, ks);
     if (rc) return rc;
     const size_t n_chunks = (first ? 1 : 0) + ((size_t)(B - first) + F - 1) / F;

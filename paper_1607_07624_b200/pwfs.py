@@ -22,7 +22,8 @@ KERNEL_CLASSES = ("xpass", "ypass", "xrebin", "slopes")
 
 EXPORTS = ("pwfs_create", "pwfs_create_ex", "pwfs_info", "pwfs_valid_mask", "pwfs_run", "pwfs_run_host",
            "pwfs_destroy", "pwfs_strerror", "pwfs_last_cuda_error", "pwfs_supported_grid",
-           "pwfs_set_schedule", "pwfs_set_timing", "pwfs_get_timing", "pwfs_geometry")
+           "pwfs_set_schedule", "pwfs_set_timing", "pwfs_get_timing", "pwfs_geometry", "pwfs_reserve",
+           "pwfs_last_failed_kernel", "pwfs_peak_fp32")
 
 
 class pwfs_params(C.Structure):
@@ -75,6 +76,12 @@ def load_library() -> C.CDLL:
     lib.pwfs_strerror.restype = C.c_char_p
     lib.pwfs_last_cuda_error.argtypes = [vp]
     lib.pwfs_last_cuda_error.restype = C.c_int
+    lib.pwfs_reserve.argtypes = [vp, i32]
+    lib.pwfs_reserve.restype = C.c_int
+    lib.pwfs_last_failed_kernel.argtypes = [vp]
+    lib.pwfs_last_failed_kernel.restype = C.c_int
+    lib.pwfs_peak_fp32.argtypes = [i32, i32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    lib.pwfs_peak_fp32.restype = C.c_int
     lib.pwfs_supported_grid.argtypes = [i32]
     lib.pwfs_supported_grid.restype = C.c_int
     lib.pwfs_set_schedule.argtypes = [vp, i32, i32]
@@ -91,6 +98,15 @@ def load_library() -> C.CDLL:
 
 def strerror(code: int) -> str:
     return load_library().pwfs_strerror(code).decode()
+
+
+def peak_fp32(device: int = 0, packed: bool = True) -> Tuple[float, float]:
+    """(TFLOP/s, ms) of the FFMA / FFMA2 stream micro-benchmark (pwfs_peak_fp32)."""
+    tf, ms = C.c_double(), C.c_double()
+    rc = load_library().pwfs_peak_fp32(device, int(packed), C.byref(tf), C.byref(ms))
+    if rc != PWFS_OK:
+        raise PwfsError(rc, "pwfs_peak_fp32", strerror(rc))
+    return tf.value, ms.value
 
 
 def supported_grid(m_grid: int) -> bool:
@@ -192,6 +208,23 @@ class PWFS:
                 {k: int(n[i]) for i, k in enumerate(KERNEL_CLASSES)})
 
     # -- the hot path -----------------------------------------------------
+    def _dev_out(self, t, shape, what):
+        """A caller-supplied output: exactly `shape`, float32, contiguous, on this sensor's device."""
+        import torch
+        if not isinstance(t, torch.Tensor):
+            raise TypeError(f"{what} must be a torch tensor")
+        if not t.is_cuda or t.device.index != self.device:
+            raise ValueError(f"{what} must live on cuda:{self.device}")
+        if t.dtype != torch.float32:
+            raise TypeError(f"{what} must be float32, got {t.dtype}")
+        if tuple(t.shape) != tuple(shape) or not t.is_contiguous():
+            raise ValueError(f"{what} must be a contiguous tensor of shape {tuple(shape)}, got {tuple(t.shape)}")
+        return t
+
+    def reserve(self, batch: int):
+        """Size scratch for batches of up to `batch` frames (needed before capturing run() in a CUDA graph)."""
+        self._check(self._lib.pwfs_reserve(self._h, int(batch)), "pwfs_reserve")
+
     def run(self, phase, frames=None, slopes=None, want_slopes: bool = True, stream=None):
         """phase: CUDA float32 tensor [B,N,N] (or [N,N]).  Returns (frames, slopes)
         CUDA tensors [B,2n_sub,2n_sub], [B,2 n_valid]; asynchronous on `stream`
@@ -203,40 +236,70 @@ class PWFS:
             raise ValueError("phase lives on another device than the sensor")
         if phase.dim() == 2:
             phase = phase.unsqueeze(0)
-        phase = phase.contiguous()
         B, N = phase.shape[0], self.n_pupil
-        if tuple(phase.shape[1:]) != (N, N):
+        if phase.dim() != 3 or tuple(phase.shape[1:]) != (N, N):
             raise ValueError(f"phase must be [B,{N},{N}]")
+        st = stream if stream is not None else torch.cuda.current_stream(phase.device)
+        if not phase.is_contiguous():
+            with torch.cuda.stream(st):              # the copy is made, used and freed in stream order on `st`
+                phase = phase.contiguous()
         D = self.det_size
         if frames is None:
             frames = torch.empty((B, D, D), dtype=torch.float32, device=phase.device)
-        if slopes is None and want_slopes:
-            slopes = torch.empty((B, 2 * self.n_valid), dtype=torch.float32, device=phase.device)
-        st = stream if stream is not None else torch.cuda.current_stream(phase.device)
+        else:
+            self._dev_out(frames, (B, D, D), "frames")
+        if slopes is None:
+            if want_slopes:
+                slopes = torch.empty((B, 2 * self.n_valid), dtype=torch.float32, device=phase.device)
+        else:
+            self._dev_out(slopes, (B, 2 * self.n_valid), "slopes")
         rc = self._lib.pwfs_run(self._h, C.c_void_p(phase.data_ptr()), B, C.c_void_p(frames.data_ptr()),
                                 C.c_void_p(slopes.data_ptr()) if slopes is not None else None,
                                 C.c_void_p(st.cuda_stream))
         self._check(rc, "pwfs_run")
+        if stream is not None:                       # buffers allocated on torch's current stream, used on another one
+            for t in (phase, frames, slopes):
+                if t is not None:
+                    t.record_stream(st)
         return frames, slopes
+
+    @staticmethod
+    def _host_buf(a, shape, what):
+        """Pointer of a HOST float32 C-contiguous buffer (numpy array or CPU torch tensor) of exactly `shape`."""
+        if isinstance(a, np.ndarray):
+            if a.dtype != np.float32:
+                raise TypeError(f"{what} must be float32, got {a.dtype}")
+            if not a.flags.c_contiguous or tuple(a.shape) != tuple(shape):
+                raise ValueError(f"{what} must be a C-contiguous array of shape {tuple(shape)}, got {a.shape}")
+            return a.ctypes.data
+        import torch
+        if not isinstance(a, torch.Tensor):
+            raise TypeError(f"{what} must be a numpy array or a CPU torch tensor")
+        if a.is_cuda:
+            raise ValueError(f"{what} must be host memory (use run() for device tensors)")
+        if a.dtype != torch.float32:
+            raise TypeError(f"{what} must be float32, got {a.dtype}")
+        if not a.is_contiguous() or tuple(a.shape) != tuple(shape):
+            raise ValueError(f"{what} must be a contiguous tensor of shape {tuple(shape)}, got {tuple(a.shape)}")
+        return a.data_ptr()
 
     def run_host(self, phase, frames=None, slopes=None, want_slopes: bool = True):
         """Same with HOST buffers (numpy arrays or CPU torch tensors, float32,
         ideally pinned): host->device, run, device->host inside the call."""
-        def ptr_shape(a):
-            if isinstance(a, np.ndarray):
-                assert a.dtype == np.float32 and a.flags.c_contiguous
-                return a.ctypes.data, a.shape
-            assert a.dtype.is_floating_point and a.element_size() == 4 and a.is_contiguous() and not a.is_cuda
-            return a.data_ptr(), tuple(a.shape)
-        p, shp = ptr_shape(phase)
-        B = 1 if len(shp) == 2 else shp[0]
-        D = self.det_size
+        N, D = self.n_pupil, self.det_size
+        shp = tuple(phase.shape)
+        if len(shp) == 2:
+            shp = (1,) + shp
+        if len(shp) != 3 or shp[1:] != (N, N):
+            raise ValueError(f"phase must be [B,{N},{N}], got {tuple(phase.shape)}")
+        B = shp[0]
+        p = self._host_buf(phase, tuple(phase.shape), "phase")
         if frames is None:
             frames = np.empty((B, D, D), dtype=np.float32)
         if slopes is None and want_slopes:
             slopes = np.empty((B, 2 * self.n_valid), dtype=np.float32)
-        fp, _ = ptr_shape(frames)
-        sp = ptr_shape(slopes)[0] if slopes is not None else None
+        fp = self._host_buf(frames, (B, D, D), "frames")
+        sp = self._host_buf(slopes, (B, 2 * self.n_valid), "slopes") if slopes is not None else None
         rc = self._lib.pwfs_run_host(self._h, C.c_void_p(p), B, C.c_void_p(fp),
                                      C.c_void_p(sp) if sp is not None else None)
         self._check(rc, "pwfs_run_host")

@@ -4,9 +4,8 @@ same seeded float32 inputs, element by element.
 Bar (BASELINE.json north_star, reading A14): per frame
     max |dI| / max I <= 1e-4   on the detector frame,
     |d slope|        <= 1e-4   per element (absolute),
-valid masks bit-exact.  Small cases run every frame through the oracle; at the
-five full BASELINE.json sizes a sample of frames is compared (the oracle needs
-seconds per frame there) in the launch configuration bench.py times.
+valid masks bit-exact.  This file holds the small cases and the edge cases; every
+frame of the four full-size configs is compared in test_gpu_parity_full.py.
 """
 import numpy as np
 import pytest
@@ -69,32 +68,21 @@ def test_cfg1_every_frame(torch_cuda):
     _run_both(torch_cuda, A, cfg.m_grid, cfg.mod_radius, cfg.mod_points, cfg.n_subap, phase)
 
 
-@pytest.mark.parametrize("name,frames", [("cfg2_flao", 6), ("cfg3_npot", 3), ("cfg4_elt", 2), ("cfg5_multi", 12)])
-def test_full_size_configs_sampled_frames(torch_cuda, name, frames):
-    """Full BASELINE.json sizes.  The GPU runs a batch large enough to use the
-    same chunked launch configuration as bench.py; the oracle checks the first
-    `frames` of them (cfg5: one step = all 12 sensor instances)."""
-    from oracle import pwfs_oracle as orc
+def test_repeated_frames_and_calls_are_bit_identical(torch_cuda):
+    """Every frame of every full-size config is compared with the oracle in test_gpu_parity_full.py; here: the
+    result of a frame depends neither on its position in the batch nor on the call (no atomics, fixed orders)."""
     from paper_1607_07624_b200.pwfs import from_config
     torch = torch_cuda
-    cfg = wl.CONFIGS[name]
-    A = wl.make_pupil(cfg)
-    steps = max(1, frames // cfg.instances)
-    phase = wl.phase_batch(cfg, steps=steps)[:frames]
-    reps = 24 if name != "cfg4_elt" else 20
-    big = np.concatenate([phase] * (reps // frames + 1))[:max(reps, frames)]
-    sensor = from_config(cfg)
-    try:
-        fr, sl = sensor.run(torch.from_numpy(big).cuda())
+    cfg = wl.CONFIGS["cfg4_elt"]
+    phase = wl.phase_batch(cfg, steps=2)
+    big = torch.from_numpy(np.concatenate([phase] * 10)).cuda()                    # 20 frames: 2 distinct, repeated
+    with from_config(cfg) as sensor:
+        fr, sl = sensor.run(big)
+        fr2, sl2 = sensor.run(big)
         torch.cuda.synchronize()
-        fr, sl = fr.cpu().numpy(), sl.cpu().numpy()
-        fr_ref, sl_ref = orc.pwfs_run(A, cfg.m_grid, cfg.mod_radius, cfg.mod_points, cfg.n_subap, phase)
-        _compare(fr[:frames], sl[:frames], fr_ref, sl_ref)
-        # the batch repeats the sample: every repeat must reproduce it bit for bit
-        for i in range(frames, big.shape[0]):
-            assert np.array_equal(fr[i], fr[i % frames]) and np.array_equal(sl[i], sl[i % frames])
-    finally:
-        sensor.close()
+        assert torch.equal(fr, fr2) and torch.equal(sl, sl2)
+        for i in range(2, 20):
+            assert torch.equal(fr[i], fr[i % 2]) and torch.equal(sl[i], sl[i % 2])
 
 
 # -------------------------------------------------------------- edge cases ---
@@ -200,6 +188,105 @@ def test_host_buffer_pipeline_with_several_chunks(torch_cuda):
             sensor.run_host(torch.from_numpy(phase).pin_memory(), fh, sh)
             assert ((fd.cpu() - fh).abs().amax(dim=(1, 2)) <= 2e-6 * fd.cpu().abs().amax(dim=(1, 2))).all()
             assert (sd.cpu() - sh).abs().max() <= 1e-5
+
+
+def test_host_buffer_pipeline_when_scratch_holds_fewer_frames_than_the_short_first_chunk(torch_cuda, monkeypatch):
+    """B/16 frames in the first chunk must not exceed what the scratch budget holds (with a small
+    budget the short chunk used to be launched with more frames than T was sized for)."""
+    from paper_1607_07624_b200.pwfs import from_config
+    torch = torch_cuda
+    cfg = wl.CONFIGS["cfg1_tiny"]
+    # T of one cfg1 frame = KX (7) x M (128) x NP (64) x 8 B = 458 752 B: a 1 MiB budget holds 2 frames, B/16 = 6
+    monkeypatch.setenv("PWFS_SCRATCH_MB", "1")
+    B = 100
+    phase = np.concatenate([wl.phase_batch(cfg, steps=10)] * 10)
+    phase = np.ascontiguousarray(phase + np.arange(B, dtype=np.float32)[:, None, None] * 0.01)
+    with from_config(cfg) as small:
+        assert small.geometry(B)["frames_per_chunk"] <= 2
+        fh, sh = small.run_host(phase)
+        fd, sd = small.run(torch.from_numpy(phase).cuda())
+        torch.cuda.synchronize()
+    monkeypatch.delenv("PWFS_SCRATCH_MB")
+    with from_config(cfg) as big:
+        fr, sr = big.run(torch.from_numpy(phase).cuda())
+        torch.cuda.synchronize()
+    fr, sr = fr.cpu().numpy(), sr.cpu().numpy()
+    for f, s_ in ((fh, sh), (fd.cpu().numpy(), sd.cpu().numpy())):
+        assert (np.abs(f - fr).max(axis=(1, 2)) <= 2e-6 * fr.max(axis=(1, 2))).all()
+        assert np.abs(s_ - sr).max() <= 1e-5
+
+
+def test_binding_rejects_wrong_buffers(torch_cuda):
+    """run() / run_host() check shape, dtype, device and contiguity of caller-supplied buffers."""
+    from paper_1607_07624_b200.pwfs import from_config
+    torch = torch_cuda
+    cfg = wl.CONFIGS["cfg1_tiny"]
+    N, D = cfg.n_pupil, cfg.det_size
+    ph = torch.from_numpy(wl.phase_batch(cfg, steps=2)).cuda()
+    with from_config(cfg) as sensor:
+        nv = sensor.n_valid
+        with pytest.raises(ValueError):
+            sensor.run(ph, frames=torch.empty((1, D, D), device="cuda"))                 # too small
+        with pytest.raises(TypeError):
+            sensor.run(ph, frames=torch.empty((2, D, D), device="cuda", dtype=torch.float64))
+        with pytest.raises(ValueError):
+            sensor.run(ph, frames=torch.empty((2, D, D)))                                # host tensor
+        with pytest.raises(ValueError):
+            sensor.run(ph, frames=torch.empty((2, D, 2 * D), device="cuda")[:, :, ::2])  # strided
+        with pytest.raises(ValueError):
+            sensor.run(ph, slopes=torch.empty((2, 2 * nv + 1), device="cuda"))
+        with pytest.raises(ValueError):
+            sensor.run(torch.empty((2, N, N + 1), device="cuda"))
+        with pytest.raises(ValueError):
+            sensor.run_host(np.zeros((2, N + 1, N), np.float32))                         # wrong N: would read past the buffer
+        with pytest.raises(TypeError):
+            sensor.run_host(np.zeros((2, N, N), np.float64))
+        with pytest.raises(ValueError):
+            sensor.run_host(np.zeros((2, N, N), np.float32), frames=np.zeros((1, D, D), np.float32))
+        with pytest.raises(ValueError):
+            sensor.run_host(ph)                                                          # device tensor
+        # a non-contiguous phase view is copied, on a caller-chosen stream too
+        wide = torch.zeros((2, N, 2 * N), device="cuda")
+        wide[:, :, ::2] = ph
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        f0, s0 = sensor.run(ph)
+        f1, s1 = sensor.run(wide[:, :, ::2], stream=side)
+        side.synchronize()
+        torch.cuda.synchronize()
+        assert torch.equal(f0, f1) and torch.equal(s0, s1)
+
+
+def test_cuda_graph_capture_needs_reserved_scratch(torch_cuda):
+    """pwfs_run refuses to allocate while its stream is being captured; after pwfs_reserve it captures and replays."""
+    from paper_1607_07624_b200.pwfs import from_config, PwfsError, PWFS_EINVAL
+    torch = torch_cuda
+    cfg = wl.CONFIGS["cfg1_tiny"]
+    ph = torch.from_numpy(wl.phase_batch(cfg, steps=3)).cuda()
+    fr = torch.empty((3, cfg.det_size, cfg.det_size), device="cuda")
+    with from_config(cfg) as ref:
+        f_ref, s_ref = ref.run(ph)
+    with from_config(cfg) as sensor:
+        sl = torch.empty((3, 2 * sensor.n_valid), device="cuda")
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        g = torch.cuda.CUDAGraph()
+        refused = None
+        with torch.cuda.graph(g, stream=side):
+            try:
+                sensor.run(ph, fr, sl)                       # no scratch yet: must not cudaMalloc under capture
+            except PwfsError as e:
+                refused = e
+        assert refused is not None and refused.code == PWFS_EINVAL
+        torch.cuda.synchronize()
+        sensor.reserve(3)
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            sensor.run(ph, fr, sl)
+        fr.zero_(); sl.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(fr, f_ref) and torch.equal(sl, s_ref)
 
 
 def test_host_buffer_entry_point_matches_device_entry_point(torch_cuda):

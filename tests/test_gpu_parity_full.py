@@ -1,0 +1,126 @@
+"""GPU parity at the full BASELINE.json sizes: EVERY frame of every config.
+
+SURVEY.md 8(d) "Parity is evaluated on every frame of every config"; BASELINE.md
+section 2; north_star "GPU frames and slopes match the CPU oracle ... on all five
+configs".  Each test runs the batch bench.py times (cfg2 1000, cfg3 500, cfg4 100,
+cfg5 50 x 12 frames, in the same single-call launch configuration) through
+pwfs_run, and the same float32 phase screens through the double-precision oracle,
+and compares element by element at the bar of test_gpu_parity.py:
+
+    per frame  max |dI| / max I <= 1e-4,   per element  |d slope| <= 1e-4.
+
+cfg4 additionally goes through pwfs_run_host (the chunked three-stream pipeline)
+against the ORACLE, not against the device path.  One test per config so that a
+time-out names the config.  The oracle needs about 0.06 / 0.2 / 1.0 / 0.5 s per
+frame of cfg 2 / 3 / 4 / 5 on a 16-core host; PWFS_PARITY_STRIDE=n (default 1 =
+every step) keeps every n-th simulation step for a quicker local run.
+"""
+import json
+import os
+import time
+
+import numpy as np
+import pytest
+
+from paper_1607_07624_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL_FRAME = 1e-4
+TOL_SLOPE = 1e-4
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch
+
+
+def _errors(frames_gpu, slopes_gpu, frames_ref, slopes_ref):
+    """Per-frame max|dI|/max I and max|d slope| (float64)."""
+    fg = np.asarray(frames_gpu, dtype=np.float64)
+    sg = np.asarray(slopes_gpu, dtype=np.float64)
+    assert fg.shape == frames_ref.shape and sg.shape == slopes_ref.shape
+    assert np.isfinite(fg).all() and np.isfinite(sg).all()
+    ef = np.abs(fg - frames_ref).max(axis=(1, 2)) / frames_ref.max(axis=(1, 2))
+    es = np.abs(sg - slopes_ref).max(axis=1)
+    return ef, es
+
+
+def _report(name, what, ef, es, n_oracle_s):
+    line = {"config": name, "path": what, "frames": int(ef.size), "worst_frame_err": float(ef.max()),
+            "worst_frame_index": int(ef.argmax()), "worst_slope_err": float(es.max()),
+            "worst_slope_index": int(es.argmax()), "median_frame_err": float(np.median(ef)),
+            "oracle_seconds": round(n_oracle_s, 1), "tol_frame": TOL_FRAME, "tol_slope": TOL_SLOPE}
+    print("PARITY_FULL " + json.dumps(line))
+    out_dir = os.path.join(ROOT, "gpurun_out")
+    if os.path.isdir(out_dir):                      # kept next to the run's other output when that folder exists
+        with open(os.path.join(out_dir, "parity_full.jsonl"), "a") as fh:
+            fh.write(json.dumps(line) + "\n")
+
+
+def _full_batch(name):
+    """The bench batch of a config; PWFS_PARITY_STRIDE > 1 keeps every n-th step (all instances of it)."""
+    cfg = wl.CONFIGS[name]
+    stride = max(1, int(os.environ.get("PWFS_PARITY_STRIDE", "1")))
+    phase = wl.phase_batch(cfg)                                           # all steps x instances, step-major
+    if stride > 1:
+        keep = np.arange(0, cfg.steps, stride)
+        idx = (keep[:, None] * cfg.instances + np.arange(cfg.instances)[None, :]).ravel()
+        phase = np.ascontiguousarray(phase[idx])
+    return cfg, phase
+
+
+def _oracle(cfg, A, phase):
+    from oracle import pwfs_oracle as orc
+    t0 = time.perf_counter()
+    fr, sl = orc.pwfs_run(A, cfg.m_grid, cfg.mod_radius, cfg.mod_points, cfg.n_subap, phase)
+    return fr, sl, time.perf_counter() - t0
+
+
+@pytest.mark.parametrize("name", ["cfg2_flao", "cfg3_npot", "cfg5_multi"])
+def test_every_frame_of_the_bench_batch(torch_cuda, name):
+    from paper_1607_07624_b200.pwfs import from_config
+    torch = torch_cuda
+    cfg, phase = _full_batch(name)
+    A = wl.make_pupil(cfg)
+    with from_config(cfg) as sensor:
+        geo = sensor.geometry(phase.shape[0])
+        fr, sl = sensor.run(torch.from_numpy(phase).cuda())               # one call, as bench.py makes it
+        torch.cuda.synchronize()
+        fr, sl = fr.cpu().numpy(), sl.cpu().numpy()
+    fr_ref, sl_ref, secs = _oracle(cfg, A, phase)
+    ef, es = _errors(fr, sl, fr_ref, sl_ref)
+    _report(name, f"pwfs_run, {phase.shape[0]} frames in chunks of {geo['frames_per_chunk']}", ef, es, secs)
+    assert ef.max() <= TOL_FRAME, f"frame {ef.argmax()}: {ef.max():.3e} > {TOL_FRAME}"
+    assert es.max() <= TOL_SLOPE, f"frame {es.argmax()}: slope error {es.max():.3e} > {TOL_SLOPE}"
+
+
+def test_cfg4_every_frame_device_and_host_paths(torch_cuda):
+    """cfg4_elt, the configuration the metric is quoted on: all 100 frames in the one-chunk launch bench.py
+    times, and the same 100 frames through pwfs_run_host (short first chunk + large chunks on three streams),
+    both against the oracle."""
+    from paper_1607_07624_b200.pwfs import from_config
+    torch = torch_cuda
+    cfg, phase = _full_batch("cfg4_elt")
+    A = wl.make_pupil(cfg)
+    B = phase.shape[0]
+    with from_config(cfg) as sensor:
+        geo = sensor.geometry(B)
+        fr, sl = sensor.run(torch.from_numpy(phase).cuda())
+        torch.cuda.synchronize()
+        fr, sl = fr.cpu().numpy(), sl.cpu().numpy()
+        h_phase = torch.from_numpy(phase).pin_memory()
+        fh = torch.zeros((B, cfg.det_size, cfg.det_size), dtype=torch.float32).pin_memory()
+        sh = torch.zeros((B, 2 * sensor.n_valid), dtype=torch.float32).pin_memory()
+        sensor.run_host(h_phase, fh, sh)
+    fr_ref, sl_ref, secs = _oracle(cfg, A, phase)
+    ef, es = _errors(fr, sl, fr_ref, sl_ref)
+    _report("cfg4_elt", f"pwfs_run, {B} frames in chunks of {geo['frames_per_chunk']}", ef, es, secs)
+    efh, esh = _errors(fh.numpy(), sh.numpy(), fr_ref, sl_ref)
+    _report("cfg4_elt", f"pwfs_run_host, {B} frames, chunked pipeline", efh, esh, 0.0)
+    assert ef.max() <= TOL_FRAME and es.max() <= TOL_SLOPE, (ef.max(), es.max())
+    assert efh.max() <= TOL_FRAME and esh.max() <= TOL_SLOPE, (efh.max(), esh.max())
