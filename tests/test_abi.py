@@ -21,7 +21,7 @@ def lib():
 def _declared_functions(header):
     src = open(os.path.join(ROOT, "include", header)).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(pwfs_[a-z_]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(pwfs_[a-z0-9_]+)\s*\(", src)))
 
 
 def test_header_symbols_are_exported(lib):
