@@ -179,6 +179,10 @@ int build_tables(pwfs *h) {
     DevTables &t = h->tab;
     t.N = N; t.M = M; t.NP = (N + 31) / 32 * 32; t.K = K;
     t.D = 2 * n_sub; t.n_sub = n_sub; t.slope_norm = p.slope_norm;
+    // PWFS_DEBUG_T_ALIAS=1 (measurement only, results are wrong): every frame of a chunk uses the T slabs of frame 0,
+    // so the row<->column intermediate stays L2-resident -- what the step would cost if T never reached HBM
+    const char *alias = std::getenv("PWFS_DEBUG_T_ALIAS");
+    t.t_frames = (alias && alias[0] == '1') ? 1 : 0;
 
     // O0: modulation points; distinct x-tilts (the row pass depends on k only through dx_k)
     // f3: an explicit list (dx, dy, w) replaces the circle; I = sum_k w_k |E_k|^2 / sum_k w_k.  The weight

@@ -32,8 +32,13 @@ namespace pwk {
 
 constexpr float kInv2PiHi = 0.15915493667125702f;   // fl32(1/(2 pi))
 constexpr float kInv2PiLo = 6.4206382e-09f;          // 1/(2 pi) - kInv2PiHi
-constexpr int kPitch = 33;  // float2 row pitch of the exchange buffer: conflict-free LDS.64/STS.64
-constexpr int kTB = 8;      // the row pass writes T[f][j][x][y] in runs of kTB consecutive y (64 bytes) per column
+// float2 row pitch of the exchange buffer.  34 = 272 bytes: rows are 16-byte aligned, so the size-32 stage moves its
+// rows with LDS.128 / STS.128 (lane w starts at 16-byte unit 17 w: the 8 lanes of a quarter warp hit 8 different units),
+// and the column-wise 64-bit accesses of the register stages (lane = column) stay conflict-free.
+constexpr int kPitch = 34;
+// T is stored in blocks of kTB consecutive rows y: T[f][j][y / kTB][x][y % kTB].  A row-pass CTA that owns kTB rows
+// writes, per x-tilt, one contiguous block of M * kTB float2; the column pass reads 64-byte runs.
+constexpr int kTB = 8;
 
 template <int R1_, int NB_, int WPB_X_, int WPB_Y_, int MINB_X_ = 1, int MINB_Y_ = 1>
 struct PassCfg {
@@ -43,9 +48,10 @@ struct PassCfg {
     static constexpr int NZ = (R1_ + 1) / 2; // M >= 2N  =>  at most ceil(R1/2) non-zero inputs per lane
     static constexpr int ITEMS = NB_ * R1_;  // size-32 DFTs per warp batch
     static constexpr int ROUNDS = (ITEMS + 31) / 32;
-    // float2 per warp.  The row pass's write-out reads TB rows (= TB/NB warps' buffers) x a few adjacent
-    // columns per instruction: a warp stride of 2 (mod 16) 64-bit banks keeps those reads conflict-free.
-    static constexpr int WARP_BUF = (ITEMS * kPitch + 15) / 16 * 16 + 2;
+    // float2 per transform / per warp.  The row pass's write-out reads kTB rows (= kTB transforms' buffers) x 4 adjacent
+    // columns per instruction: a transform stride of 2 (mod 16) 64-bit banks keeps those reads conflict-free.
+    static constexpr int TBUF = (R1_ * kPitch + 13) / 16 * 16 + 2;
+    static constexpr int WARP_BUF = NB_ * TBUF;
     static constexpr int TAB = R1_ * kPitch;              // float2 per table (twiddle, mask)
     // M = 2048: the row pass's shared memory is full, the general-mask table a(u)/M is read through L1 instead
     static constexpr bool AM_GLOBAL = R1_ > 32;
@@ -70,6 +76,7 @@ struct DevTables {
     int ncols;                // pupil-plane columns computed
     int D, n_sub, cmax;       // detector size 2 n_sub, rebin support
     int n_valid, slope_norm;
+    int t_frames;             // frames T holds (normally the chunk; 1 = every frame aliases slab set 0: a timing experiment)
     const float *amp;         // [N][N]
     const float2 *txc;        // [KX][NXP] exp(i tilt_x,j(x)), zero for x >= N
     const float2 *tyt;        // [K][NP]  exp(i tilt_y,k(y)), zero for y >= N
@@ -132,12 +139,16 @@ __device__ __forceinline__ void stage32(float2 *buf, const float2 *s_tw, const f
     for (int rd = 0; rd < C::ROUNDS; ++rd) {
         int w = rd * 32 + lane;
         if (w < C::ITEMS) {
-            int k1 = w % C::R1;
-            float2 *row = buf + w * kPitch;
-            const float2 *twr = s_tw + k1 * kPitch;
+            const int b = w / C::R1, k1 = w - b * C::R1;
+            float4 *row = reinterpret_cast<float4 *>(buf + b * C::TBUF + k1 * kPitch);         // 16-byte aligned rows
+            const float4 *twr = reinterpret_cast<const float4 *>(s_tw + k1 * kPitch);
             float2 u[32];
 #pragma unroll
-            for (int n2 = 0; n2 < 32; ++n2) u[n2] = cmul(row[n2], twr[n2]);
+            for (int q = 0; q < 16; ++q) {
+                const float4 x = row[q], tw = twr[q];
+                u[2 * q] = cmul(make_float2(x.x, x.y), make_float2(tw.x, tw.y));
+                u[2 * q + 1] = cmul(make_float2(x.z, x.w), make_float2(tw.z, tw.w));
+            }
             Dft<32, -1>::run(u);
             if constexpr (QM) {
                 sfor<32>([&](auto kc) {
@@ -154,7 +165,11 @@ __device__ __forceinline__ void stage32(float2 *buf, const float2 *s_tw, const f
                 Dft<32, +1>::run(u);
             }
 #pragma unroll
-            for (int n2 = 0; n2 < 32; ++n2) row[n2] = cmulc(u[n2], twr[n2]);
+            for (int q = 0; q < 16; ++q) {
+                const float4 tw = twr[q];
+                const float2 a = cmulc(u[2 * q], make_float2(tw.x, tw.y)), c = cmulc(u[2 * q + 1], make_float2(tw.z, tw.w));
+                row[q] = make_float4(a.x, a.y, c.x, c.y);
+            }
         }
     }
 }
@@ -181,8 +196,12 @@ __device__ __forceinline__ void apply_ipow_k1(float2 (&v)[R1]) {
 //
 // The last register stage is done "transposed": thread (r, n2) takes row r of the CTA
 // (another warp's exchange buffer) and column residue n2, so that adjacent lanes hold
-// adjacent rows y of the same column x = 32 n1 + n2 and the results go straight from
-// registers to T[f][j][x][y] as runs of >= 64 bytes -- no staging pass for the transposition.
+// adjacent rows y of the same column x = 32 n1 + n2.  T is blocked by kTB rows,
+// T[f][j][y / 8][x][y % 8]: the 8 lanes (r % 8) x 4 adjacent n2 of a warp write 256 contiguous
+// bytes per store, every store of a thread is a compile-time offset (n1 * 256 float2) from one
+// base address, and a CTA's output per x-tilt is RPC/8 contiguous blocks of M * 64 bytes -- no
+// staging pass for the transposition, no address arithmetic, no partial lines.  All M columns
+// are written (T spans the whole grid); the column pass reads the window columns only.
 template <class C, bool QM>
 __global__ void __launch_bounds__(32 * C::WPB_X, C::MINB_X)
 xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ T, int jsplit) {
@@ -226,27 +245,20 @@ xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ 
         }
     }
 
-    // transposed last stage: this thread's items (r, n2), it < NB, and which of their outputs
-    // x = 32 n1 + n2 lie inside a pupil-image window (bit n1 of wmask[it])
-    int item_src[C::NB];          // exchange-buffer offset of (row r, k1 = 0, n2)
-    int item_dst[C::NB];          // T offset of (x = n2, y = y0 + r) within the (f, j) slab
-    using wmask_t = std::conditional_t<(C::R1 > 32), unsigned long long, unsigned>;
-    wmask_t wmask[C::NB];
+    // transposed last stage: this thread's items it < NB are (row r = 8 r_hi + r_lo, column residue n2) with
+    // r_lo = i % 8, n2 = (i / 8) % 32, r_hi = i / 256 for i = threadIdx.x + it * blockDim.x
+    int item_src[C::NB];          // exchange-buffer offset of (row r, k1 = 0, n2): transform r of the CTA
+    int item_dst[C::NB];          // T offset of (x = n2, y = y0 + r) within the (f, j) slab; < 0: row beyond NP
 #pragma unroll
     for (int it = 0; it < C::NB; ++it) {
         const int i = threadIdx.x + it * 32 * C::WPB_X;
-        const int r = i % C::RPC, n2 = i / C::RPC;
-        item_src[it] = (r / C::NB) * C::WARP_BUF + (r % C::NB) * C::R1 * kPitch + n2;
-        item_dst[it] = n2 * t.NP + y0 + r;
-        wmask_t m = 0;
-        if (y0 + r < t.NP)
-            for (int n1 = 0; n1 < C::R1; ++n1) m |= (wmask_t)(__ldg(t.xc_of_x + 32 * n1 + n2) >= 0 ? 1u : 0u) << n1;
-        wmask[it] = m;
+        const int r = (i >> 8) * kTB + (i & 7), n2 = (i >> 3) & 31;
+        item_src[it] = r * C::TBUF + n2;
+        item_dst[it] = (y0 + r < t.NP) ? ((y0 + r) / kTB) * (C::M * kTB) + n2 * kTB + (i & 7) : -1;
     }
 
     const int j_lo = (int)(((long long)js * t.KX) / jsplit), j_hi = (int)(((long long)(js + 1) * t.KX) / jsplit);
-    const size_t slab = (size_t)t.M * t.NP;
-    const int n1_stride = 32 * t.NP;
+    const size_t slab = (size_t)C::M * t.NP;
     __syncthreads();   // tables loaded (s_p is private to the warp that wrote it)
     for (int j = j_lo; j < j_hi; ++j) {
         // step A: x-tilt, zero-padded DFT of size R1 over n1
@@ -263,7 +275,7 @@ xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ 
             for (int n1 = 0; n1 < C::NZ; ++n1) v[n1] = cmul(pw[(b * C::NZ + n1) * 32], tx[n1]);
             DftP<C::R1, -1, C::NZ>::run(v);
 #pragma unroll
-            for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitch + lane] = v[k1];
+            for (int k1 = 0; k1 < C::R1; ++k1) buf[b * C::TBUF + k1 * kPitch + lane] = v[k1];
         }
         __syncwarp();
         stage32<C, QM>(buf, s_tw, s_am, lane);
@@ -271,8 +283,8 @@ xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ 
         if (j + 1 < j_hi && threadIdx.x < 2 * C::NZ)
             asm volatile("prefetch.global.L1 [%0];" ::"l"(t.txc + (size_t)(j + 1) * t.NXP + 16 * threadIdx.x));
         __syncthreads();
-        // step A'': inverse DFT of size R1 over k1 for item (r, n2) -> T[f][j][32 n1 + n2][y0 + r]
-        float2 *Tj = T + ((size_t)f * t.KX + j) * slab;
+        // step A'': inverse DFT of size R1 over k1 for item (r, n2) -> T[f][j][(y0 + r) / 8][32 n1 + n2][r % 8]
+        float2 *Tj = T + ((size_t)(t.t_frames == 1 ? 0 : f) * t.KX + j) * slab;
 #pragma unroll
         for (int it = 0; it < C::NB; ++it) {
             float2 v[C::R1];
@@ -281,11 +293,11 @@ xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ 
             for (int k1 = 0; k1 < C::R1; ++k1) v[k1] = src[k1 * kPitch];
             apply_ipow_k1<C::R1, QM>(v);
             Dft<C::R1, +1>::run(v);
-            float2 *dst = Tj + item_dst[it];
-            const wmask_t m = wmask[it];
+            if (item_dst[it] >= 0) {
+                float2 *dst = Tj + item_dst[it];
 #pragma unroll
-            for (int n1 = 0; n1 < C::R1; ++n1)
-                if ((m >> n1) & 1u) dst[n1 * n1_stride] = v[n1];
+                for (int n1 = 0; n1 < C::R1; ++n1) dst[n1 * (32 * kTB)] = v[n1];
+            }
         }
         __syncthreads();   // the next x-tilt overwrites the buffers
     }
@@ -320,12 +332,13 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
         for (int n1 = 0; n1 < C::R1; ++n1) acc[b][n1] = 0.f;
 
     const int k_lo = (int)(((long long)ks * t.K) / ksplit), k_hi = (int)(((long long)(ks + 1) * t.K) / ksplit);
-    // T[f][j][x][y]: grid column x of compact column xc from the colx table (windows may leave gaps)
-    const size_t frame_stride = (size_t)t.M * NP;
-    const float2 *Tf = T + (size_t)f * t.KX * frame_stride + lane;
+    // T[f][j][y / 8][x][y % 8]: grid column x of compact column xc from the colx table (windows may leave gaps);
+    // lane reads y = 32 n1 + lane, i.e. block 4 n1 + lane / 8, row lane % 8 of it: 64-byte runs
+    const size_t frame_stride = (size_t)C::M * NP;
+    const float2 *Tf = T + (size_t)(t.t_frames == 1 ? 0 : f) * t.KX * frame_stride + (lane >> 3) * (C::M * kTB) + (lane & 7);
     int colofs[C::NB];
 #pragma unroll
-    for (int b = 0; b < C::NB; ++b) colofs[b] = (xc0 + b < t.ncols) ? __ldg(t.colx + xc0 + b) * NP : 0;
+    for (int b = 0; b < C::NB; ++b) colofs[b] = (xc0 + b < t.ncols) ? __ldg(t.colx + xc0 + b) * kTB : 0;
 
     // The warp walks its share of the modulation points in x-tilt order (korder): points that share a slab
     // T[f][j] come one after the other and the column is fetched once for them.
@@ -336,7 +349,7 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
         for (int b = 0; b < C::NB; ++b)
 #pragma unroll
             for (int n1 = 0; n1 < C::NZ; ++n1)
-                pre[b][n1] = (32 * n1 < NP && xc0 + b < t.ncols) ? __ldg(src + colofs[b] + 32 * n1)
+                pre[b][n1] = (32 * n1 < NP && xc0 + b < t.ncols) ? __ldg(src + colofs[b] + n1 * (32 * C::M))
                                                                  : make_float2(0.f, 0.f);
     };
     int k = 0, j = -1, k_next = 0, j_next = -1;
@@ -363,7 +376,7 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
             if (b == C::NB - 1 && idx + 1 < k_hi && j_next != j) fetch(j_next);
             DftP<C::R1, -1, C::NZ>::run(v);
 #pragma unroll
-            for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitch + lane] = v[k1];
+            for (int k1 = 0; k1 < C::R1; ++k1) buf[b * C::TBUF + k1 * kPitch + lane] = v[k1];
         }
         __syncwarp();
         stage32<C, QM>(buf, s_tw, s_am, lane);
@@ -372,7 +385,7 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
         for (int b = 0; b < C::NB; ++b) {
             float2 v[C::R1];
 #pragma unroll
-            for (int k1 = 0; k1 < C::R1; ++k1) v[k1] = buf[(b * C::R1 + k1) * kPitch + lane];
+            for (int k1 = 0; k1 < C::R1; ++k1) v[k1] = buf[b * C::TBUF + k1 * kPitch + lane];
             apply_ipow_k1<C::R1, QM>(v);
             Dft<C::R1, +1>::run(v);
 #pragma unroll
@@ -381,7 +394,7 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
         // next iteration's step-A stores touch only this lane's column, which only this lane read
     }
     // y-rebin: column of summed intensity -> 2 n_sub detector rows
-    float *colI = reinterpret_cast<float *>(buf);          // NB*M floats <= buffer
+    float *colI = reinterpret_cast<float *>(buf);          // NB*M floats <= the warp's buffer (NB * TBUF float2)
     __syncwarp();
 #pragma unroll
     for (int b = 0; b < C::NB; ++b)
