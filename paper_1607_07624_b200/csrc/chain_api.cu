@@ -17,6 +17,7 @@
 #include <cooperative_groups.h>
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -219,6 +220,60 @@ rec_kernel(const float *__restrict__ R, int n_modes, int ldk, const float *__res
         }
 }
 
+// ---- single frame (closed loop): a pure stream of recmat, 4 bytes per element, HBM-bound -------------------------
+// One CTA = one row of recmat at a time, its 8 warps each a contiguous eighth of the row; every thread keeps ITS
+// slope values in registers for the whole launch (thread t always meets slope indices 4 (t + 256 i) .. + 3), so per
+// row a thread issues NK independent 128-bit loads (all in flight together: NK * 4 KB per CTA) and 4 NK FMAs.  Rows
+// go round-robin over a grid of a few CTAs per SM: thousands of rows over ~600 CTAs leave no ragged last wave (the
+// row-per-warp kernel above runs 512 CTAs of 8 rows on 148 SMs: 3 or 4 CTAs per SM, 13 % idle).  Warp partials
+// meet in shared memory and are added in warp order: deterministic.
+template <int NK>
+__global__ void __launch_bounds__(256, 3)
+rec_gemv_kernel(const float *__restrict__ R, int n_modes, int ldk, const float *__restrict__ S, int ns,
+                float *__restrict__ out) {
+    __shared__ float red[2][8];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int n4 = ldk >> 2;
+    float4 sv[NK];
+#pragma unroll
+    for (int i = 0; i < NK; ++i) {
+        const int k = 4 * (tid + 256 * i);
+        sv[i].x = k + 0 < ns ? __ldg(S + k + 0) : 0.f;
+        sv[i].y = k + 1 < ns ? __ldg(S + k + 1) : 0.f;
+        sv[i].z = k + 2 < ns ? __ldg(S + k + 2) : 0.f;
+        sv[i].w = k + 3 < ns ? __ldg(S + k + 3) : 0.f;
+    }
+    int par = 0;
+    for (int m = blockIdx.x; m < n_modes; m += gridDim.x, par ^= 1) {
+        const float4 *row = reinterpret_cast<const float4 *>(R + (size_t)m * ldk);
+        float4 rv[NK];
+#pragma unroll
+        for (int i = 0; i < NK; ++i) {
+            const int k4 = tid + 256 * i;
+            rv[i] = k4 < n4 ? __ldcs(row + k4) : make_float4(0.f, 0.f, 0.f, 0.f);      // streamed once: evict first
+        }
+        float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+#pragma unroll
+        for (int i = 0; i < NK; ++i) {
+            a0 = fmaf(rv[i].x, sv[i].x, a0);
+            a1 = fmaf(rv[i].y, sv[i].y, a1);
+            a2 = fmaf(rv[i].z, sv[i].z, a2);
+            a3 = fmaf(rv[i].w, sv[i].w, a3);
+        }
+        float v = (a0 + a1) + (a2 + a3);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) red[par][warp] = v;
+        __syncthreads();                         // red[par] complete; red[par ^ 1] is free again after the next barrier
+        if (tid == 0) {
+            float t = 0.f;
+#pragma unroll
+            for (int w = 0; w < 8; ++w) t += red[par][w];
+            out[m] = t;
+        }
+    }
+}
+
 constexpr int kRecTcMinBatch = 24;              // below this the FP32 kernel's register tiles win
 constexpr long long kRecTcMinElems = 1 << 16;   // recmat elements
 
@@ -410,6 +465,15 @@ int pwfs_rec_run(pwfs_rec_t *h, const float *d_slopes, int32_t B, float *d_modes
         }
         if (h->tc) return rec_tc_run(h->tc, d_slopes, B, d_modes, (cudaStream_t)cuda_stream);
     }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (B == 1 && h->ldk <= 4 * 256 * 12 && h->n_modes >= 64) {      // closed loop: one frame, recmat streamed once
+        const int nk = (h->ldk / 4 + 255) / 256;
+        const int grid = std::min(h->n_modes, 4 * h->num_sms);
+        if (nk <= 4)      rec_gemv_kernel<4><<<grid, 256, 0, st>>>(h->d_R, h->n_modes, h->ldk, d_slopes, h->n_slopes, d_modes);
+        else if (nk <= 8) rec_gemv_kernel<8><<<grid, 256, 0, st>>>(h->d_R, h->n_modes, h->ldk, d_slopes, h->n_slopes, d_modes);
+        else              rec_gemv_kernel<12><<<grid, 256, 0, st>>>(h->d_R, h->n_modes, h->ldk, d_slopes, h->n_slopes, d_modes);
+        return cudaGetLastError() == cudaSuccess ? PWFS_OK : PWFS_ECUDA;
+    }
     // frames per warp tile: the whole batch when it is small, else 16 or 8, whichever pads less
     int FB = 1;
     while (FB < B && FB < 16) FB *= 2;
@@ -417,7 +481,6 @@ int pwfs_rec_run(pwfs_rec_t *h, const float *d_slopes, int32_t B, float *d_modes
     const bool vec = (h->n_slopes % 4 == 0) && ((uintptr_t)d_slopes % 16 == 0);
     // four rows per warp once that still leaves >= 2 CTAs per SM
     const long long ctas4 = (long long)((h->n_modes + kRecWarps * 4 - 1) / (kRecWarps * 4)) * ((B + FB - 1) / FB);
-    cudaStream_t st = (cudaStream_t)cuda_stream;
     if (ctas4 >= 2LL * h->num_sms) launch_rec_fb<4>(FB, vec, st, h->d_R, h->n_modes, h->ldk, d_slopes, h->n_slopes, B, d_modes);
     else                           launch_rec_fb<1>(FB, vec, st, h->d_R, h->n_modes, h->ldk, d_slopes, h->n_slopes, B, d_modes);
     return cudaGetLastError() == cudaSuccess ? PWFS_OK : PWFS_ECUDA;

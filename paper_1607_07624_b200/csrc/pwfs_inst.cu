@@ -9,8 +9,31 @@
 namespace pwk {
 namespace {
 
-using C = CfgFor<PWFS_INST_R1>::type;     // row pass
-using CY = CfgForY<PWFS_INST_R1>::type;   // column pass
+// Tuning hook: -DPWFS_TX_NB / _TX_WPB / _TX_MINB (row pass) and -DPWFS_TY_NB / _TY_WPB / _TY_MINB (column pass)
+// replace the configuration of this translation unit's grid size; used to build experimental variants of the
+// library, the shipped build sets none of them.
+using C0 = CfgFor<PWFS_INST_R1>::type;
+using CY0 = CfgForY<PWFS_INST_R1>::type;
+#ifndef PWFS_TX_NB
+#define PWFS_TX_NB C0::NB
+#endif
+#ifndef PWFS_TX_WPB
+#define PWFS_TX_WPB C0::WPB_X
+#endif
+#ifndef PWFS_TX_MINB
+#define PWFS_TX_MINB C0::MINB_X
+#endif
+#ifndef PWFS_TY_NB
+#define PWFS_TY_NB CY0::NB
+#endif
+#ifndef PWFS_TY_WPB
+#define PWFS_TY_WPB CY0::WPB_Y
+#endif
+#ifndef PWFS_TY_MINB
+#define PWFS_TY_MINB CY0::MINB_Y
+#endif
+using C = PassCfg<PWFS_INST_R1, PWFS_TX_NB, PWFS_TX_WPB, C0::WPB_Y, PWFS_TX_MINB, C0::MINB_Y>;      // row pass
+using CY = PassCfg<PWFS_INST_R1, PWFS_TY_NB, CY0::WPB_X, PWFS_TY_WPB, CY0::MINB_X, PWFS_TY_MINB>;   // column pass
 
 template <bool QM>
 void launch_x_t(dim3 grid, cudaStream_t st, const DevTables &t, const float *phase, float2 *T, int jsplit) {

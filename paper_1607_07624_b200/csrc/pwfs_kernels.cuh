@@ -32,13 +32,38 @@ namespace pwk {
 
 constexpr float kInv2PiHi = 0.15915493667125702f;   // fl32(1/(2 pi))
 constexpr float kInv2PiLo = 6.4206382e-09f;          // 1/(2 pi) - kInv2PiHi
-// float2 row pitch of the exchange buffer.  34 = 272 bytes: rows are 16-byte aligned, so the size-32 stage moves its
-// rows with LDS.128 / STS.128 (lane w starts at 16-byte unit 17 w: the 8 lanes of a quarter warp hit 8 different units),
-// and the column-wise 64-bit accesses of the register stages (lane = column) stay conflict-free.
-constexpr int kPitch = 34;
+constexpr int kPitch = 33;  // float2 row pitch of the exchange buffer: conflict-free LDS.64/STS.64 along rows and columns
 // T is stored in blocks of kTB consecutive rows y: T[f][j][y / kTB][x][y % kTB].  A row-pass CTA that owns kTB rows
 // writes, per x-tilt, one contiguous block of M * kTB float2; the column pass reads 64-byte runs.
 constexpr int kTB = 8;
+
+// Padding (float2) between the exchange buffers of consecutive warps.  Inside a warp's buffer the NB * R1 rows are
+// contiguous (the size-32 stage reads row w at w * kPitch: 16 consecutive lanes hit 16 different 64-bit banks).  The row
+// pass's transposed last stage reads, per instruction, 8 rows r = 8 r_hi + r_lo of the CTA (= 8 transforms, spread over
+// 8 / NB warps) x 2 adjacent columns per half warp; the pad is chosen so that those 16 accesses fall in as many different
+// banks as possible (all 16 for NB = 1 and for R1 = 6, 10, 18).
+constexpr int pick_warp_pad(int R1, int NB, int RPC) {
+    int best_pad = 0, best = 1 << 30;
+    for (int pad = 0; pad < 16; ++pad) {
+        const int wb = NB * R1 * kPitch + pad;
+        int tot = 0;
+        for (int rhi = 0; rhi < RPC / kTB; ++rhi) {
+            int cnt[16] = {};
+            int worst = 0;
+            for (int rlo = 0; rlo < kTB; ++rlo) {
+                const int r = kTB * rhi + rlo;
+                const int off = (r / NB) * wb + (r % NB) * R1 * kPitch;
+                for (int n2 = 0; n2 < 2; ++n2) {
+                    const int c = ++cnt[(off + n2) % 16];
+                    worst = c > worst ? c : worst;
+                }
+            }
+            tot += worst;
+        }
+        if (tot < best) { best = tot; best_pad = pad; }
+    }
+    return best_pad;
+}
 
 template <int R1_, int NB_, int WPB_X_, int WPB_Y_, int MINB_X_ = 1, int MINB_Y_ = 1>
 struct PassCfg {
@@ -48,10 +73,7 @@ struct PassCfg {
     static constexpr int NZ = (R1_ + 1) / 2; // M >= 2N  =>  at most ceil(R1/2) non-zero inputs per lane
     static constexpr int ITEMS = NB_ * R1_;  // size-32 DFTs per warp batch
     static constexpr int ROUNDS = (ITEMS + 31) / 32;
-    // float2 per transform / per warp.  The row pass's write-out reads kTB rows (= kTB transforms' buffers) x 4 adjacent
-    // columns per instruction: a transform stride of 2 (mod 16) 64-bit banks keeps those reads conflict-free.
-    static constexpr int TBUF = (R1_ * kPitch + 13) / 16 * 16 + 2;
-    static constexpr int WARP_BUF = NB_ * TBUF;
+    static constexpr int WARP_BUF = ITEMS * kPitch + pick_warp_pad(R1_, NB_, NB_ * WPB_X_);   // float2 per warp
     static constexpr int TAB = R1_ * kPitch;              // float2 per table (twiddle, mask)
     // M = 2048: the row pass's shared memory is full, the general-mask table a(u)/M is read through L1 instead
     static constexpr bool AM_GLOBAL = R1_ > 32;
@@ -139,16 +161,12 @@ __device__ __forceinline__ void stage32(float2 *buf, const float2 *s_tw, const f
     for (int rd = 0; rd < C::ROUNDS; ++rd) {
         int w = rd * 32 + lane;
         if (w < C::ITEMS) {
-            const int b = w / C::R1, k1 = w - b * C::R1;
-            float4 *row = reinterpret_cast<float4 *>(buf + b * C::TBUF + k1 * kPitch);         // 16-byte aligned rows
-            const float4 *twr = reinterpret_cast<const float4 *>(s_tw + k1 * kPitch);
+            const int k1 = w % C::R1;
+            float2 *row = buf + w * kPitch;
+            const float2 *twr = s_tw + k1 * kPitch;
             float2 u[32];
 #pragma unroll
-            for (int q = 0; q < 16; ++q) {
-                const float4 x = row[q], tw = twr[q];
-                u[2 * q] = cmul(make_float2(x.x, x.y), make_float2(tw.x, tw.y));
-                u[2 * q + 1] = cmul(make_float2(x.z, x.w), make_float2(tw.z, tw.w));
-            }
+            for (int n2 = 0; n2 < 32; ++n2) u[n2] = cmul(row[n2], twr[n2]);
             Dft<32, -1>::run(u);
             if constexpr (QM) {
                 sfor<32>([&](auto kc) {
@@ -165,11 +183,7 @@ __device__ __forceinline__ void stage32(float2 *buf, const float2 *s_tw, const f
                 Dft<32, +1>::run(u);
             }
 #pragma unroll
-            for (int q = 0; q < 16; ++q) {
-                const float4 tw = twr[q];
-                const float2 a = cmulc(u[2 * q], make_float2(tw.x, tw.y)), c = cmulc(u[2 * q + 1], make_float2(tw.z, tw.w));
-                row[q] = make_float4(a.x, a.y, c.x, c.y);
-            }
+            for (int n2 = 0; n2 < 32; ++n2) row[n2] = cmulc(u[n2], twr[n2]);
         }
     }
 }
@@ -253,7 +267,7 @@ xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ 
     for (int it = 0; it < C::NB; ++it) {
         const int i = threadIdx.x + it * 32 * C::WPB_X;
         const int r = (i >> 8) * kTB + (i & 7), n2 = (i >> 3) & 31;
-        item_src[it] = r * C::TBUF + n2;
+        item_src[it] = (r / C::NB) * C::WARP_BUF + (r % C::NB) * C::R1 * kPitch + n2;
         item_dst[it] = (y0 + r < t.NP) ? ((y0 + r) / kTB) * (C::M * kTB) + n2 * kTB + (i & 7) : -1;
     }
 
@@ -275,7 +289,7 @@ xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ 
             for (int n1 = 0; n1 < C::NZ; ++n1) v[n1] = cmul(pw[(b * C::NZ + n1) * 32], tx[n1]);
             DftP<C::R1, -1, C::NZ>::run(v);
 #pragma unroll
-            for (int k1 = 0; k1 < C::R1; ++k1) buf[b * C::TBUF + k1 * kPitch + lane] = v[k1];
+            for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitch + lane] = v[k1];
         }
         __syncwarp();
         stage32<C, QM>(buf, s_tw, s_am, lane);
@@ -336,9 +350,10 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
     // lane reads y = 32 n1 + lane, i.e. block 4 n1 + lane / 8, row lane % 8 of it: 64-byte runs
     const size_t frame_stride = (size_t)C::M * NP;
     const float2 *Tf = T + (size_t)(t.t_frames == 1 ? 0 : f) * t.KX * frame_stride + (lane >> 3) * (C::M * kTB) + (lane & 7);
+    constexpr int colmul = kTB, n1_stride = 32 * C::M;
     int colofs[C::NB];
 #pragma unroll
-    for (int b = 0; b < C::NB; ++b) colofs[b] = (xc0 + b < t.ncols) ? __ldg(t.colx + xc0 + b) * kTB : 0;
+    for (int b = 0; b < C::NB; ++b) colofs[b] = (xc0 + b < t.ncols) ? __ldg(t.colx + xc0 + b) * colmul : 0;
 
     // The warp walks its share of the modulation points in x-tilt order (korder): points that share a slab
     // T[f][j] come one after the other and the column is fetched once for them.
@@ -349,7 +364,7 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
         for (int b = 0; b < C::NB; ++b)
 #pragma unroll
             for (int n1 = 0; n1 < C::NZ; ++n1)
-                pre[b][n1] = (32 * n1 < NP && xc0 + b < t.ncols) ? __ldg(src + colofs[b] + n1 * (32 * C::M))
+                pre[b][n1] = (32 * n1 < NP && xc0 + b < t.ncols) ? __ldg(src + colofs[b] + n1 * n1_stride)
                                                                  : make_float2(0.f, 0.f);
     };
     int k = 0, j = -1, k_next = 0, j_next = -1;
@@ -376,7 +391,7 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
             if (b == C::NB - 1 && idx + 1 < k_hi && j_next != j) fetch(j_next);
             DftP<C::R1, -1, C::NZ>::run(v);
 #pragma unroll
-            for (int k1 = 0; k1 < C::R1; ++k1) buf[b * C::TBUF + k1 * kPitch + lane] = v[k1];
+            for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitch + lane] = v[k1];
         }
         __syncwarp();
         stage32<C, QM>(buf, s_tw, s_am, lane);
@@ -385,7 +400,7 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
         for (int b = 0; b < C::NB; ++b) {
             float2 v[C::R1];
 #pragma unroll
-            for (int k1 = 0; k1 < C::R1; ++k1) v[k1] = buf[b * C::TBUF + k1 * kPitch + lane];
+            for (int k1 = 0; k1 < C::R1; ++k1) v[k1] = buf[(b * C::R1 + k1) * kPitch + lane];
             apply_ipow_k1<C::R1, QM>(v);
             Dft<C::R1, +1>::run(v);
 #pragma unroll
@@ -394,7 +409,7 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
         // next iteration's step-A stores touch only this lane's column, which only this lane read
     }
     // y-rebin: column of summed intensity -> 2 n_sub detector rows
-    float *colI = reinterpret_cast<float *>(buf);          // NB*M floats <= the warp's buffer (NB * TBUF float2)
+    float *colI = reinterpret_cast<float *>(buf);          // NB*M floats <= the warp's buffer
     __syncwarp();
 #pragma unroll
     for (int b = 0; b < C::NB; ++b)

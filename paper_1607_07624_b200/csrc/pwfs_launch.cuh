@@ -11,26 +11,30 @@ namespace pwk {
 #define PWFS_FOR_EACH_R1(X) X(4) X(5) X(6) X(8) X(9) X(10) X(12) X(15) X(16) X(18) X(20) X(24) X(25) X(27) X(30) X(32) \
     X(36) X(40) X(45) X(48) X(50) X(54) X(60) X(64)
 
-// PassCfg<R1, NB, warps/CTA row pass, warps/CTA column pass, min CTAs/SM row pass, column pass>:
-// NB transforms per warp so that NB * R1 fills whole rounds of 32 lanes in the size-32 stage as far as
-// the register file allows (accumulators NB * R1, prefetch NB * ceil(R1/2) complex).
+// PassCfg<R1, NB, warps/CTA row pass, warps/CTA column pass, min CTAs/SM row pass, column pass>.  CfgFor is the row
+// pass; the column pass takes its NB from CfgForY below.  Row pass (measured on B200, profiles/r2_tuning.md): small
+// CTAs -- 4 warps x NB rows = 8 (or 16, 24) rows -- with a register budget that leaves no spills beat 8-warp CTAs
+// capped at 128 registers (M = 1024: 3.65 -> 3.20 ms per 100 frames; M = 320: 1.96 -> 1.81; M = 480: 3.53 -> 3.14;
+// M = 800: 11.8 -> 11.5): fewer warps wait at each of the two CTA barriers per x-tilt, and the 14-17 spilled registers
+// of the 128-register build went through the same LSU queue that limits the kernel.  NB * R1 fills whole rounds of 32
+// lanes in the size-32 stage as far as shared memory allows (NB * R1 * 264 bytes per warp + the parked phasor).
 template <int R1> struct CfgFor;
 template <> struct CfgFor<4>  { using type = PassCfg<4, 8, 4, 4>; };          // M = 128
 template <> struct CfgFor<5>  { using type = PassCfg<5, 6, 4, 4>; };          // M = 160
 template <> struct CfgFor<6>  { using type = PassCfg<6, 5, 8, 4>; };          // M = 192
 template <> struct CfgFor<8>  { using type = PassCfg<8, 4, 4, 4>; };          // M = 256
 template <> struct CfgFor<9>  { using type = PassCfg<9, 3, 8, 4>; };          // M = 288
-template <> struct CfgFor<10> { using type = PassCfg<10, 3, 8, 4, 2, 1>; };   // M = 320
+template <> struct CfgFor<10> { using type = PassCfg<10, 6, 4, 4, 2, 1>; };   // M = 320
 template <> struct CfgFor<12> { using type = PassCfg<12, 5, 8, 4>; };         // M = 384
-template <> struct CfgFor<15> { using type = PassCfg<15, 2, 8, 4, 2, 1>; };   // M = 480
-template <> struct CfgFor<16> { using type = PassCfg<16, 2, 8, 4, 2, 1>; };   // M = 512
+template <> struct CfgFor<15> { using type = PassCfg<15, 2, 4, 4, 4, 1>; };   // M = 480
+template <> struct CfgFor<16> { using type = PassCfg<16, 2, 4, 4, 4, 1>; };   // M = 512
 template <> struct CfgFor<18> { using type = PassCfg<18, 3, 8, 4, 2, 1>; };   // M = 576
-template <> struct CfgFor<20> { using type = PassCfg<20, 1, 8, 4, 2, 1>; };   // M = 640
-template <> struct CfgFor<24> { using type = PassCfg<24, 1, 8, 4, 2, 1>; };   // M = 768
-template <> struct CfgFor<25> { using type = PassCfg<25, 1, 8, 4, 2, 1>; };   // M = 800
-template <> struct CfgFor<27> { using type = PassCfg<27, 1, 8, 4, 2, 1>; };   // M = 864
-template <> struct CfgFor<30> { using type = PassCfg<30, 1, 8, 4, 2, 1>; };   // M = 960
-template <> struct CfgFor<32> { using type = PassCfg<32, 1, 8, 4, 2, 2>; };   // M = 1024
+template <> struct CfgFor<20> { using type = PassCfg<20, 2, 4, 4, 2, 1>; };   // M = 640
+template <> struct CfgFor<24> { using type = PassCfg<24, 2, 4, 4, 2, 1>; };   // M = 768
+template <> struct CfgFor<25> { using type = PassCfg<25, 2, 4, 4, 2, 1>; };   // M = 800
+template <> struct CfgFor<27> { using type = PassCfg<27, 2, 4, 4, 2, 1>; };   // M = 864
+template <> struct CfgFor<30> { using type = PassCfg<30, 2, 4, 4, 2, 1>; };   // M = 960
+template <> struct CfgFor<32> { using type = PassCfg<32, 2, 4, 4, 3, 2>; };   // M = 1024
 // R1 > 32: the size-32 stage runs in two rounds (the second with R1 - 32 lanes), one CTA per SM in both passes
 template <> struct CfgFor<36> { using type = PassCfg<36, 1, 8, 4, 1, 1>; };   // M = 1152
 template <> struct CfgFor<40> { using type = PassCfg<40, 1, 8, 4, 1, 1>; };   // M = 1280
@@ -45,8 +49,15 @@ template <> struct CfgFor<64> { using type = PassCfg<64, 1, 8, 4, 1, 1>; };   //
 // phasor): more of the 32 lanes busy in the size-32 stage.  Default: the same configuration.  (R1 = 25 with NB = 5,
 // 125 items, was tried: the exchange buffers then allow only 6 warps per SM and the column pass ran 1.6x slower.)
 template <int R1> struct CfgForY { using type = typename CfgFor<R1>::type; };
+template <> struct CfgForY<10> { using type = PassCfg<10, 3, 8, 4, 2, 1>; };   // 30 items
 template <> struct CfgForY<15> { using type = PassCfg<15, 4, 8, 4, 2, 1>; };   // 60 items: two full rounds (was 30 of 32)
+template <> struct CfgForY<16> { using type = PassCfg<16, 2, 8, 4, 2, 1>; };
 template <> struct CfgForY<20> { using type = PassCfg<20, 3, 8, 4, 2, 1>; };   // 60 items (was 20 of 32)
+template <> struct CfgForY<24> { using type = PassCfg<24, 1, 8, 4, 2, 1>; };
+template <> struct CfgForY<25> { using type = PassCfg<25, 1, 8, 4, 2, 1>; };
+template <> struct CfgForY<27> { using type = PassCfg<27, 1, 8, 4, 2, 1>; };
+template <> struct CfgForY<30> { using type = PassCfg<30, 1, 8, 4, 2, 1>; };
+template <> struct CfgForY<32> { using type = PassCfg<32, 1, 8, 4, 2, 2>; };
 
 struct Launcher {
     int R1, NB, WPB_X, WPB_Y, RPC;   // NB, WPB_Y: column pass; WPB_X, RPC: row pass

@@ -157,6 +157,9 @@ def test_slopec_agrees_with_the_hot_path_slopes(torch_cuda):
 # ------------------------------------------------------------ reconstructor ---
 @pytest.mark.parametrize("n_modes,ns,B", [(54, 2512, 1), (5, 416, 3), (37, 1030, 17), (1, 1, 1), (33, 7, 2),
                                           (300, 2528, 40), (1200, 416, 9), (4096, 11712, 1),
+                                          # single frames: the streaming GEMV kernel (4, 8, 12 slope registers per thread,
+                                          # ragged rows, more rows than CTAs), and one row longer than it takes
+                                          (700, 1030, 1), (100, 6001, 1), (64, 12288, 1), (65, 12290, 1), (2500, 2049, 1),
                                           # batches >= 24 frames run on the tensor cores (rec_tc.cu): ragged tiles in
                                           # every dimension, K not a multiple of 32, two frame tiles, one K block
                                           (130, 1000, 24), (257, 515, 130), (128, 2048, 128), (2100, 31, 33),
