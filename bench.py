@@ -239,6 +239,33 @@ def bench_stages(cfg, dev, phase, frames, flush, reps: int = 5) -> dict:
                                       "note": "closed-loop order, one step per iteration, all on the device: propagate -> "
                                               "pyramid (4 kernels) -> CCD -> slopes - reference -> modes (GEMV); eager "
                                               "launches, device time per step over 50 consecutive steps"}
+            # the same 8 launches per step replayed from one CUDA graph of 10 consecutive steps (their own step indices
+            # and noise frames): what a loop that submits whole blocks of steps pays per step
+            n_cap = 10
+            step[0] = 0
+            sensor.reserve(n_inst)
+            g = torch.cuda.CUDAGraph()
+            side = torch.cuda.Stream(dev)
+            side.wait_stream(stream)
+            with torch.cuda.graph(g, stream=side):
+                for _ in range(n_cap):
+                    a.propagate(step[0], 1, atm["dt"], out=ph, stream=side)
+                    sensor.run(ph, fr, want_slopes=False, stream=side)
+                    ccd.run(fr, first_out_frame=step[0] * n_inst, out=px, stream=side)
+                    sc.run(px, out=s1, stream=side)
+                    rec.run(s1, out=md, stream=side)
+                    step[0] += 1
+            torch.cuda.synchronize(dev)
+
+            def replay():
+                for _ in range(n_loop // n_cap):
+                    g.replay()
+            ms_g = timed(replay) / n_loop
+            out["chain_loop_step_graph"] = {"ms": ms_g, "steps_per_s": 1e3 / ms_g, "frames_per_step": n_inst,
+                                            "steps_per_graph": n_cap,
+                                            "note": "the same step captured 10 times (consecutive step indices) in one CUDA "
+                                                    "graph; device time per step over 50 steps = 5 replays"}
+            del g
     del R
     # f4: PSF camera on the same grid, Shack-Hartmann on the same pupil
     with PsfCamera(wl.make_pupil(cfg), M, phase_scale=0.45, device=dev.index) as cam:

@@ -195,6 +195,23 @@ int pwfs_get_timing(pwfs_t *h, float ms[PWFS_NUM_KERNEL_CLASSES],
 int pwfs_geometry(const pwfs_t *h, int32_t B, int32_t *n_cols, int32_t *k_unique,
                   int32_t *frames_per_chunk, int32_t *k_split);
 
+/* TEST-ONLY exports (SURVEY.md 8(b) "optional test-only export", pins P2 / P7 of 8(c)).
+ * pwfs_debug_intensity runs the row pass and the column pass of the hot path -- the
+ * same kernels pwfs_run launches -- one frame at a time and returns the FULL-resolution
+ * intensity I = (1/K) sum_k |E_k|^2 before rebinning: DEVICE float [B][M][M], row-major
+ * [y][x] in the placement of definition O2 (pupil at offset M/2 - N/2 on both axes,
+ * i.e. directly comparable with the definition).  Only the columns that hold a pupil
+ * image are computed (all of them when M = 2N); the others are returned as zero.
+ * Synchronous; allocates and frees a temporary buffer; not for production use.
+ * pwfs_debug_create is pwfs_create_ex with the mask shift given explicitly
+ * (mask_shift_px >= 0; 0 is the identity mask) and WITHOUT the window constraints
+ * N <= 2 s <= M - N, so that the identity case s = 0 (I = A^2 embedded at the pupil's
+ * place) can be checked on the CUDA path; such a handle serves pwfs_debug_intensity
+ * only (pwfs_run returns PWFS_EINVAL). */
+int pwfs_debug_create(const pwfs_params *p, const pwfs_ext *x, int32_t mask_shift_px, pwfs_t **out);
+int pwfs_debug_intensity(pwfs_t *h, const float *d_phase, int32_t B, float *d_intensity,
+                         void *cuda_stream);
+
 /* Measurement aid, not part of the hot path: the FP32 arithmetic peak of `device`
  * as a stream of independent FFMA (packed = 0) or packed FFMA2 (packed = 1)
  * instructions on every SM (64 resident warps each, 8 independent accumulator

@@ -6,6 +6,8 @@
 
 #include <cuda_runtime.h>
 
+#include "device_guard.cuh"
+
 #include <cmath>
 #include <new>
 #include <vector>
@@ -152,7 +154,8 @@ int pwfs_atmo_create(const pwfs_atmo_params *p, pwfs_atmo_t **out) {
     if (!h) return PWFS_ENOMEM;
     h->device = p->device;
     int rc = PWFS_OK;
-    cudaError_t e = cudaSetDevice(p->device);
+    pwk::DeviceGuard dg(p->device);
+    cudaError_t e = dg.err;
     if (e != cudaSuccess) { h->last_cuda = (int)e; rc = PWFS_ECUDA; }
     AtmoDev &a = h->dev;
     a.L = p->n_layers; a.G = p->screen_px; a.S = p->n_dirs; a.W = p->n_wl; a.N = p->n_pupil;
@@ -177,7 +180,8 @@ int pwfs_atmo_propagate(pwfs_atmo_t *h, int64_t first_step, int32_t n_steps, dou
     if (!h || n_steps < 0 || !std::isfinite(dt)) return PWFS_EINVAL;
     if (n_steps == 0) return PWFS_OK;
     if (!d_phase) return PWFS_EINVAL;
-    cudaError_t e = cudaSetDevice(h->device);
+    pwk::DeviceGuard dg(h->device);
+    cudaError_t e = dg.err;
     if (e != cudaSuccess) { h->last_cuda = (int)e; return PWFS_ECUDA; }
     const AtmoDev &a = h->dev;
     const int per_launch = 65535 / a.S;                  // grid.z limit
@@ -196,7 +200,7 @@ int pwfs_atmo_propagate(pwfs_atmo_t *h, int64_t first_step, int32_t n_steps, dou
 
 void pwfs_atmo_destroy(pwfs_atmo_t *h) {
     if (!h) return;
-    cudaSetDevice(h->device);
+    pwk::DeviceGuard dg(h->device);
     for (void *d : h->allocs) cudaFree(d);
     delete h;
 }

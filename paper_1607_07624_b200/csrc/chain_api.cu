@@ -17,6 +17,8 @@
 #include <cooperative_groups.h>
 #include <cuda_runtime.h>
 
+#include "device_guard.cuh"
+
 #include <algorithm>
 #include <cmath>
 #include <cstdlib>
@@ -352,7 +354,8 @@ int pwfs_ccd_run(pwfs_ccd_t *h, const float *d_frames, int32_t n_steps, int64_t 
     if (!h || n_steps < 0 || n_steps % h->dev.n_int != 0) return PWFS_EINVAL;
     if (n_steps == 0) return PWFS_OK;
     if (!d_frames || !d_pixels) return PWFS_EINVAL;
-    if (cudaSetDevice(h->device) != cudaSuccess) return PWFS_ECUDA;
+    pwk::DeviceGuard dg(h->device);
+    if (dg.err != cudaSuccess) return PWFS_ECUDA;
     const long long n_out = (long long)(n_steps / h->dev.n_int) * h->dev.n_inst;
     const long long total = n_out * h->dev.D * h->dev.D;
     const long long blocks = (total + 255) / 256;
@@ -376,7 +379,8 @@ int pwfs_slopec_create(int32_t n_sub, const uint8_t *h_valid, int32_t slope_norm
     pwfs_slopec *h = new (std::nothrow) pwfs_slopec();
     if (!h) return PWFS_ENOMEM;
     h->device = device;
-    cudaError_t e = cudaSetDevice(device);
+    pwk::DeviceGuard dg(device);
+    cudaError_t e = dg.err;
     if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_vidx, vidx.size() * sizeof(int));
     if (e == cudaSuccess) e = cudaMemcpy(h->d_vidx, vidx.data(), vidx.size() * sizeof(int), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_sn, 2 * vidx.size() * sizeof(float));
@@ -392,7 +396,8 @@ int pwfs_slopec_create(int32_t n_sub, const uint8_t *h_valid, int32_t slope_norm
 int pwfs_slopec_set_reference(pwfs_slopec_t *h, const float *h_sn) {
     if (!h) return PWFS_EINVAL;
     if (!h_sn) { h->dev.sn = nullptr; return PWFS_OK; }
-    if (cudaSetDevice(h->device) != cudaSuccess) return PWFS_ECUDA;
+    pwk::DeviceGuard dg(h->device);
+    if (dg.err != cudaSuccess) return PWFS_ECUDA;
     if (cudaMemcpy(h->d_sn, h_sn, (size_t)2 * h->dev.n_valid * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess)
         return PWFS_ECUDA;
     h->dev.sn = h->d_sn;
@@ -409,7 +414,8 @@ int pwfs_slopec_run(pwfs_slopec_t *h, const float *d_pixels, int32_t B, float *d
     if (!h || B < 0) return PWFS_EINVAL;
     if (B == 0) return PWFS_OK;
     if (!d_pixels || !d_slopes) return PWFS_EINVAL;
-    if (cudaSetDevice(h->device) != cudaSuccess) return PWFS_ECUDA;
+    pwk::DeviceGuard dg(h->device);
+    if (dg.err != cudaSuccess) return PWFS_ECUDA;
     for (int b0 = 0; b0 < B; b0 += 65535) {                      // grid.y limit
         const int Bc = B - b0 < 65535 ? B - b0 : 65535;
         slopec_kernel<<<dim3(kSlopecCluster, Bc), 256, 0, (cudaStream_t)cuda_stream>>>(
@@ -420,7 +426,7 @@ int pwfs_slopec_run(pwfs_slopec_t *h, const float *d_pixels, int32_t B, float *d
 
 void pwfs_slopec_destroy(pwfs_slopec_t *h) {
     if (!h) return;
-    cudaSetDevice(h->device);
+    pwk::DeviceGuard dg(h->device);
     if (h->d_vidx) cudaFree(h->d_vidx);
     if (h->d_sn) cudaFree(h->d_sn);
     delete h;
@@ -434,7 +440,8 @@ int pwfs_rec_create(int32_t n_modes, int32_t n_slopes, const float *h_recmat, in
     if (!h) return PWFS_ENOMEM;
     h->device = device; h->n_modes = n_modes; h->n_slopes = n_slopes; h->ldk = (n_slopes + 3) / 4 * 4;
     const size_t bytes = (size_t)n_modes * h->ldk * sizeof(float);
-    cudaError_t e = cudaSetDevice(device);
+    pwk::DeviceGuard dg(device);
+    cudaError_t e = dg.err;
     if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_R, bytes);
     if (e == cudaSuccess && h->ldk != n_slopes) e = cudaMemset(h->d_R, 0, bytes);
     if (e == cudaSuccess)
@@ -455,7 +462,8 @@ int pwfs_rec_run(pwfs_rec_t *h, const float *d_slopes, int32_t B, float *d_modes
     if (!h || B < 0) return PWFS_EINVAL;
     if (B == 0) return PWFS_OK;
     if (!d_slopes || !d_modes) return PWFS_EINVAL;
-    if (cudaSetDevice(h->device) != cudaSuccess) return PWFS_ECUDA;
+    pwk::DeviceGuard dg(h->device);
+    if (dg.err != cudaSuccess) return PWFS_ECUDA;
     // batches: TF32x3 on the tensor cores (rec_tc.cu); single frames and small problems: FP32 FMA below
     if (!h->tc_off && B >= kRecTcMinBatch && (long long)h->n_modes * h->n_slopes >= kRecTcMinElems) {
         if (!h->tc) {
@@ -488,7 +496,7 @@ int pwfs_rec_run(pwfs_rec_t *h, const float *d_slopes, int32_t B, float *d_modes
 
 void pwfs_rec_destroy(pwfs_rec_t *h) {
     if (!h) return;
-    cudaSetDevice(h->device);
+    pwk::DeviceGuard dg(h->device);
     if (h->d_R) cudaFree(h->d_R);
     rec_tc_destroy(h->tc);
     delete h;

@@ -18,6 +18,8 @@
 
 #include <cuda_runtime.h>
 
+#include "device_guard.cuh"
+
 #include <algorithm>
 #include <cmath>
 #include <new>
@@ -322,7 +324,8 @@ int pwfs_psf_create(const pwfs_psf_params *p, pwfs_psf_t **out) {
     if (!h) return PWFS_ENOMEM;
     h->device = p->device; h->L = L; h->sumA2 = sumA2;
     const size_t MM = (size_t)M * M;
-    cudaError_t e = cudaSetDevice(p->device);
+    pwk::DeviceGuard dg(p->device);
+    cudaError_t e = dg.err;
     if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_amp, (size_t)N * N * sizeof(float));
     if (e == cudaSuccess) e = cudaMemcpy(h->d_amp, p->pupil_amp, (size_t)N * N * sizeof(float), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_tw, tw.size() * sizeof(float2));
@@ -349,7 +352,8 @@ int pwfs_psf_accumulate(pwfs_psf_t *h, const float *d_phase, int32_t B, float *d
     if (!h || B < 0) return PWFS_EINVAL;
     if (B == 0) return PWFS_OK;
     if (!d_phase) return PWFS_EINVAL;
-    if (cudaSetDevice(h->device) != cudaSuccess) return PWFS_ECUDA;
+    pwk::DeviceGuard dg(h->device);
+    if (dg.err != cudaSuccess) return PWFS_ECUDA;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const PsfDev &d = h->dev;
     const PsfLauncher &L = h->L;
@@ -397,7 +401,8 @@ int pwfs_psf_accumulate(pwfs_psf_t *h, const float *d_phase, int32_t B, float *d
 
 int pwfs_psf_read(pwfs_psf_t *h, float *d_psf, int64_t *frames_out, void *cuda_stream) {
     if (!h || !d_psf) return PWFS_EINVAL;
-    if (cudaSetDevice(h->device) != cudaSuccess) return PWFS_ECUDA;
+    pwk::DeviceGuard dg(h->device);
+    if (dg.err != cudaSuccess) return PWFS_ECUDA;
     const size_t MM = (size_t)h->dev.M * h->dev.M;
     const double scale = h->count > 0 ? 1.0 / ((double)h->count * (double)MM * h->sumA2) : 0.0;
     psf_read_kernel<<<(unsigned)((MM + 255) / 256), 256, 0, (cudaStream_t)cuda_stream>>>(h->d_acc, d_psf, (float)scale, MM);
@@ -407,7 +412,8 @@ int pwfs_psf_read(pwfs_psf_t *h, float *d_psf, int64_t *frames_out, void *cuda_s
 
 int pwfs_psf_reset(pwfs_psf_t *h, void *cuda_stream) {
     if (!h) return PWFS_EINVAL;
-    if (cudaSetDevice(h->device) != cudaSuccess) return PWFS_ECUDA;
+    pwk::DeviceGuard dg(h->device);
+    if (dg.err != cudaSuccess) return PWFS_ECUDA;
     const size_t MM = (size_t)h->dev.M * h->dev.M;
     if (cudaMemsetAsync(h->d_acc, 0, MM * sizeof(float), (cudaStream_t)cuda_stream) != cudaSuccess) return PWFS_ECUDA;
     h->count = 0;
@@ -416,7 +422,7 @@ int pwfs_psf_reset(pwfs_psf_t *h, void *cuda_stream) {
 
 void pwfs_psf_destroy(pwfs_psf_t *h) {
     if (!h) return;
-    cudaSetDevice(h->device);
+    pwk::DeviceGuard dg(h->device);
     if (h->d_amp) cudaFree(h->d_amp);
     if (h->d_tw) cudaFree(h->d_tw);
     if (h->d_acc) cudaFree(h->d_acc);

@@ -14,6 +14,7 @@
 #include <new>
 #include <vector>
 
+#include "device_guard.cuh"
 #include "pwfs_launch.cuh"
 
 using namespace pwk;
@@ -35,17 +36,6 @@ bool find_launcher(int M, bool quarter, Launcher *out) {
 }
 
 struct TimedSpan { cudaEvent_t a, b; int cls; };
-
-// Makes `dev` current for the duration of a call and restores the caller's device afterwards.
-struct DeviceGuard {
-    int prev = -1, dev;
-    cudaError_t err;
-    explicit DeviceGuard(int d) : dev(d) {
-        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
-        err = (prev == dev) ? cudaSuccess : cudaSetDevice(dev);
-    }
-    ~DeviceGuard() { if (prev >= 0 && prev != dev) cudaSetDevice(prev); }
-};
 
 }  // namespace
 
@@ -73,7 +63,7 @@ struct pwfs {
     int user_fpc = 0, user_ksplit = 0;
     int num_sms = 148;
     int x_resident_ctas = 296, y_resident_warps = 1184;   // what the device holds at once (occupancy query at create)
-    size_t scratch_budget = (size_t)16 << 30;   // of the 180 GB; PWFS_SCRATCH_MB overrides
+    size_t scratch_budget = (size_t)32 << 30;   // of the 180 GB; PWFS_SCRATCH_MB overrides
     // instrumentation
     int timing = 0;
     std::vector<TimedSpan> spans;
@@ -82,6 +72,7 @@ struct pwfs {
     int64_t launches[PWFS_NUM_KERNEL_CLASSES] = {0, 0, 0, 0};
     int last_cuda = 0;
     int last_kernel = -1;                    // kernel class of the last launch that failed, -1 none
+    bool debug_only = false;                 // pwfs_debug_create with relaxed window checks: pwfs_debug_intensity only
 };
 
 namespace {
@@ -398,7 +389,18 @@ int pwfs_supported_grid(int32_t m_grid) {
 
 int pwfs_create(const pwfs_params *p, pwfs_t **out) { return pwfs_create_ex(p, nullptr, out); }
 
-int pwfs_create_ex(const pwfs_params *p, const pwfs_ext *x, pwfs_t **out) {
+static int create_impl(const pwfs_params *p, const pwfs_ext *x, int s_debug, pwfs_t **out);
+
+int pwfs_create_ex(const pwfs_params *p, const pwfs_ext *x, pwfs_t **out) { return create_impl(p, x, -1, out); }
+
+int pwfs_debug_create(const pwfs_params *p, const pwfs_ext *x, int32_t mask_shift_px, pwfs_t **out) {
+    if (mask_shift_px < 0) { if (out) *out = nullptr; return PWFS_EINVAL; }
+    return create_impl(p, x, mask_shift_px, out);
+}
+
+// s_debug >= 0: the mask shift is taken as given (0 = identity mask) and the window constraints are not checked;
+// the handle then serves pwfs_debug_intensity only.
+static int create_impl(const pwfs_params *p, const pwfs_ext *x, int s_debug, pwfs_t **out) {
     if (out) *out = nullptr;
     if (!p || !out || !p->pupil_amp) return PWFS_EINVAL;
     const int N = p->n_pupil, M = p->m_grid;
@@ -423,8 +425,13 @@ int pwfs_create_ex(const pwfs_params *p, const pwfs_ext *x, pwfs_t **out) {
     if (p->slope_norm != 0 && p->slope_norm != 1) return PWFS_EINVAL;
     if (p->illum_thresh > 1.f || !std::isfinite(p->illum_thresh)) return PWFS_EINVAL;
     int s = p->mask_shift_px;
-    if (s <= 0) { if (M % 4) return PWFS_EINVAL; s = M / 4; }
-    if (2 * s < N || s > M / 2 - N / 2) return PWFS_EINVAL;
+    if (s_debug >= 0) {
+        s = s_debug;
+        if (s > M / 2) return PWFS_EINVAL;
+    } else {
+        if (s <= 0) { if (M % 4) return PWFS_EINVAL; s = M / 4; }
+        if (2 * s < N || s > M / 2 - N / 2) return PWFS_EINVAL;
+    }
     for (size_t i = 0; i < (size_t)N * N; ++i)
         if (!(p->pupil_amp[i] >= 0.f) || !std::isfinite(p->pupil_amp[i])) return PWFS_EINVAL;
     Launcher L;
@@ -434,6 +441,7 @@ int pwfs_create_ex(const pwfs_params *p, const pwfs_ext *x, pwfs_t **out) {
     pwfs *h = new (std::nothrow) pwfs();
     if (!h) return PWFS_ENOMEM;
     h->prm = *p; h->s = s; h->quarter = quarter; h->L = L; h->device = p->device;
+    h->debug_only = s_debug >= 0;
     h->stop_h = stop_h;
     if (listed)
         for (int k = 0; k < x->n_tilts; ++k) {
@@ -651,7 +659,7 @@ int pwfs_reserve(pwfs_t *h, int32_t B) {
 int pwfs_run(pwfs_t *h, const float *d_phase, int32_t B, float *d_frames, float *d_slopes, void *cuda_stream) {
     if (!h || B < 0) return PWFS_EINVAL;
     if (B == 0) return PWFS_OK;
-    if (!d_phase || !d_frames) return PWFS_EINVAL;
+    if (!d_phase || !d_frames || h->debug_only) return PWFS_EINVAL;
     DeviceGuard dg(h->device);
     PWFS_CUDA(h, dg.err);
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -687,10 +695,44 @@ int pwfs_run(pwfs_t *h, const float *d_phase, int32_t B, float *d_frames, float 
     return PWFS_OK;
 }
 
+int pwfs_debug_intensity(pwfs_t *h, const float *d_phase, int32_t B, float *d_intensity, void *cuda_stream) {
+    if (!h || B < 0) return PWFS_EINVAL;
+    if (B == 0) return PWFS_OK;
+    if (!d_phase || !d_intensity) return PWFS_EINVAL;
+    DeviceGuard dg(h->device);
+    PWFS_CUDA(h, dg.err);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    DevTables &t = h->tab;
+    const size_t NN = (size_t)t.N * t.N, MM = (size_t)t.M * t.M;
+    // one frame at a time, the whole modulation loop in one warp (k_split 1) so that dbg holds the complete sum
+    int rc = ensure_scratch(h, 1, 1, st, true);
+    if (rc) return rc;
+    float *dbg = nullptr;
+    PWFS_CUDA(h, cudaMalloc((void **)&dbg, (size_t)t.ncols * t.M * sizeof(float)));
+    const double m4 = h->quarter ? std::pow((double)t.M, 4.0) : 1.0;
+    const int o = t.M / 2 - t.N / 2;                                  // O2: the oracle's pupil sits at [o, o + N)
+    cudaError_t e = cudaMemsetAsync(d_intensity, 0, (size_t)B * MM * sizeof(float), st);
+    for (int b = 0; b < B && e == cudaSuccess && !rc; ++b) {
+        t.dbg_I = dbg;
+        rc = launch_k1(h, d_phase + (size_t)b * NN, 1, st);
+        if (!rc) rc = launch_k2(h, 1, 1, st);
+        t.dbg_I = nullptr;
+        if (!rc) {
+            debug_scatter_kernel<<<dim3(t.ncols, 1), 256, 0, st>>>(t, dbg, d_intensity + (size_t)b * MM, o,
+                                                                   (float)(1.0 / ((double)t.K * m4)));
+            rc = check_launch(h, 2);
+        }
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);               // test-only: synchronous, then free the buffer
+    cudaFree(dbg);
+    if (e != cudaSuccess) { h->last_cuda = (int)e; return PWFS_ECUDA; }
+    return rc;
+}
+
 int pwfs_run_host(pwfs_t *h, const float *h_phase, int32_t B, float *h_frames, float *h_slopes) {
     if (!h || B < 0) return PWFS_EINVAL;
     if (B == 0) return PWFS_OK;
-    if (!h_phase || !h_frames) return PWFS_EINVAL;
+    if (!h_phase || !h_frames || h->debug_only) return PWFS_EINVAL;
     DeviceGuard dg(h->device);
     PWFS_CUDA(h, dg.err);
     const DevTables &t = h->tab;

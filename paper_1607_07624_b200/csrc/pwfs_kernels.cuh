@@ -99,6 +99,7 @@ struct DevTables {
     int D, n_sub, cmax;       // detector size 2 n_sub, rebin support
     int n_valid, slope_norm;
     int t_frames;             // frames T holds (normally the chunk; 1 = every frame aliases slab set 0: a timing experiment)
+    float *dbg_I;             // test-only (pwfs_debug_intensity): [F][ncols][M] full-resolution sum_k |E|^2, else nullptr
     const float *amp;         // [N][N]
     const float2 *txc;        // [KX][NXP] exp(i tilt_x,j(x)), zero for x >= N
     const float2 *tyt;        // [K][NP]  exp(i tilt_y,k(y)), zero for y >= N
@@ -416,6 +417,10 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
 #pragma unroll
         for (int n1 = 0; n1 < C::R1; ++n1) colI[b * C::M + 32 * n1 + lane] = acc[b][n1];
     __syncwarp();
+    if (t.dbg_I != nullptr) {   // test-only export of the un-rebinned column (pins P2 / P7 of SURVEY.md 8(c))
+        for (int b = 0; b < C::NB && xc0 + b < t.ncols; ++b)
+            for (int y = lane; y < C::M; y += 32) t.dbg_I[((size_t)f * t.ncols + xc0 + b) * C::M + y] = colI[b * C::M + y];
+    }
     const int D = t.D, cmax = t.cmax;
     for (int b = 0; b < C::NB; ++b) {
         const int xc = xc0 + b;
@@ -486,6 +491,16 @@ static __global__ void xrebin_kernel(DevTables t, const float *__restrict__ colb
         for (int i = 0; i < (int)((blockDim.x + 31) >> 5); ++i) v += red[i];
         nsum[(size_t)f * D + jx] = v;
     }
+}
+
+// test-only: dbg[f][xc][y] (corner-placed grid, unscaled) -> I[f][(y + o) % M][(x + o) % M] * scale, the oracle's
+// centred coordinates; columns that were not computed stay zero (I is cleared by the caller).  grid (ncols, F).
+static __global__ void debug_scatter_kernel(DevTables t, const float *__restrict__ dbg, float *__restrict__ I, int o,
+                                            float scale) {
+    const int xc = blockIdx.x, f = blockIdx.y, M = t.M;
+    const int x = (__ldg(t.colx + xc) + o) % M;
+    const float *src = dbg + ((size_t)f * t.ncols + xc) * M;
+    for (int y = threadIdx.x; y < M; y += blockDim.x) I[((size_t)f * M + (y + o) % M) * M + x] = src[y] * scale;
 }
 
 // ------------------------------------------------------------------ K3b -----

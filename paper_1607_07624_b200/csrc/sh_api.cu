@@ -23,6 +23,8 @@
 
 #include <cuda_runtime.h>
 
+#include "device_guard.cuh"
+
 #include <algorithm>
 #include <cmath>
 #include <cstring>
@@ -340,7 +342,8 @@ int pwfs_sh_create(const pwfs_sh_params *p, pwfs_sh_t **out) {
     h->nc = nc;
     h->kernel = sh_pick(b, nc);
     h->smem = smem_of(lg);
-    cudaError_t e = cudaSetDevice(p->device);
+    pwk::DeviceGuard dg(p->device);
+    cudaError_t e = dg.err;
     if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_amp, (size_t)N * N * sizeof(float));
     if (e == cudaSuccess) e = cudaMemcpy(h->d_amp, p->pupil_amp, (size_t)N * N * sizeof(float), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_wtab, wtab.size() * sizeof(float4));
@@ -386,7 +389,8 @@ int pwfs_sh_run(pwfs_sh_t *h, const float *d_phase, int32_t B, float *d_frames, 
     if (!h || B < 0) return PWFS_EINVAL;
     if (B == 0) return PWFS_OK;
     if (!d_phase || !d_frames) return PWFS_EINVAL;
-    if (cudaSetDevice(h->device) != cudaSuccess) return PWFS_ECUDA;
+    pwk::DeviceGuard dg(h->device);
+    if (dg.err != cudaSuccess) return PWFS_ECUDA;
     ShDev d = h->dev;
     const int tasks = d.n_sub * d.gpr, D = d.n_sub * d.n_px;
     const size_t NN = (size_t)d.N * d.N, DD = (size_t)D * D;
@@ -402,7 +406,7 @@ int pwfs_sh_run(pwfs_sh_t *h, const float *d_phase, int32_t B, float *d_frames, 
 
 void pwfs_sh_destroy(pwfs_sh_t *h) {
     if (!h) return;
-    cudaSetDevice(h->device);
+    pwk::DeviceGuard dg(h->device);
     if (h->d_amp) cudaFree(h->d_amp);
     if (h->d_wtab) cudaFree(h->d_wtab);
     if (h->d_pix) cudaFree(h->d_pix);

@@ -23,7 +23,7 @@ KERNEL_CLASSES = ("xpass", "ypass", "xrebin", "slopes")
 EXPORTS = ("pwfs_create", "pwfs_create_ex", "pwfs_info", "pwfs_valid_mask", "pwfs_run", "pwfs_run_host",
            "pwfs_destroy", "pwfs_strerror", "pwfs_last_cuda_error", "pwfs_supported_grid",
            "pwfs_set_schedule", "pwfs_set_timing", "pwfs_get_timing", "pwfs_geometry", "pwfs_reserve",
-           "pwfs_last_failed_kernel", "pwfs_peak_fp32")
+           "pwfs_last_failed_kernel", "pwfs_peak_fp32", "pwfs_debug_create", "pwfs_debug_intensity")
 
 
 class pwfs_params(C.Structure):
@@ -80,6 +80,10 @@ def load_library() -> C.CDLL:
     lib.pwfs_reserve.restype = C.c_int
     lib.pwfs_last_failed_kernel.argtypes = [vp]
     lib.pwfs_last_failed_kernel.restype = C.c_int
+    lib.pwfs_debug_create.argtypes = [C.POINTER(pwfs_params), C.POINTER(pwfs_ext), i32, C.POINTER(vp)]
+    lib.pwfs_debug_create.restype = C.c_int
+    lib.pwfs_debug_intensity.argtypes = [vp, vp, i32, vp, vp]
+    lib.pwfs_debug_intensity.restype = C.c_int
     lib.pwfs_peak_fp32.argtypes = [i32, i32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     lib.pwfs_peak_fp32.restype = C.c_int
     lib.pwfs_supported_grid.argtypes = [i32]
@@ -119,9 +123,10 @@ class PWFS:
     def __init__(self, pupil_amp: np.ndarray, m_grid: int, mod_radius: float, mod_points: int,
                  n_subap: int, mask_shift_px: int = 0, mod_angle0: float = 0.0,
                  illum_thresh: float = 0.5, slope_norm: int = 0, device: int = 0,
-                 tilt_list=None, field_stop_px: float = -1.0):
+                 tilt_list=None, field_stop_px: float = -1.0, debug_shift_px: Optional[int] = None):
         """tilt_list = (x, y[, w]) arrays in lambda/D replaces the modulation circle;
-        field_stop_px >= 0 adds the square focal-plane stop (include/pwfs.h, pwfs_ext)."""
+        field_stop_px >= 0 adds the square focal-plane stop (include/pwfs.h, pwfs_ext).
+        debug_shift_px (tests only): pwfs_debug_create with this mask shift, window checks off."""
         self._h = None
         self._lib = load_library()
         amp = np.ascontiguousarray(pupil_amp, dtype=np.float32)
@@ -131,7 +136,10 @@ class PWFS:
                           mask_shift_px, mod_radius, mod_points, mod_angle0, n_subap, illum_thresh,
                           slope_norm, device)
         h = C.c_void_p()
-        if tilt_list is None and field_stop_px < 0:
+        if debug_shift_px is not None and tilt_list is None:
+            ext = pwfs_ext(0, None, None, None, field_stop_px)
+            rc = self._lib.pwfs_debug_create(C.byref(prm), C.byref(ext), int(debug_shift_px), C.byref(h))
+        elif tilt_list is None and field_stop_px < 0:
             rc = self._lib.pwfs_create(C.byref(prm), C.byref(h))
         else:
             fp = C.POINTER(C.c_float)
@@ -220,6 +228,22 @@ class PWFS:
         if tuple(t.shape) != tuple(shape) or not t.is_contiguous():
             raise ValueError(f"{what} must be a contiguous tensor of shape {tuple(shape)}, got {tuple(t.shape)}")
         return t
+
+    def debug_intensity(self, phase):
+        """Tests only: full-resolution I[B,M,M] = mean_k |E_k|^2 from the hot path's own row and column kernels
+        (pwfs_debug_intensity), in the placement of the definition."""
+        import torch
+        if phase.dim() == 2:
+            phase = phase.unsqueeze(0)
+        phase = phase.contiguous()
+        B, N, M = phase.shape[0], self.n_pupil, self.m_grid
+        if not (phase.is_cuda and phase.dtype == torch.float32 and tuple(phase.shape[1:]) == (N, N)):
+            raise ValueError(f"phase must be a CUDA float32 tensor [B,{N},{N}]")
+        out = torch.empty((B, M, M), dtype=torch.float32, device=phase.device)
+        st = torch.cuda.current_stream(phase.device)
+        self._check(self._lib.pwfs_debug_intensity(self._h, C.c_void_p(phase.data_ptr()), B, C.c_void_p(out.data_ptr()),
+                                                   C.c_void_p(st.cuda_stream)), "pwfs_debug_intensity")
+        return out
 
     def reserve(self, batch: int):
         """Size scratch for batches of up to `batch` frames (needed before capturing run() in a CUDA graph)."""

@@ -85,6 +85,39 @@ def test_repeated_frames_and_calls_are_bit_identical(torch_cuda):
             assert torch.equal(fr[i], fr[i % 2]) and torch.equal(sl[i], sl[i % 2])
 
 
+def test_full_resolution_intensity_before_rebinning(torch_cuda):
+    """The un-rebinned I = mean_k |E_k|^2 of the hot path's own kernels (test-only export pwfs_debug_intensity)
+    against the oracle's orc_intensity on the whole M x M grid, M = 2N so that every column is computed."""
+    from oracle import pwfs_oracle as orc
+    from paper_1607_07624_b200.pwfs import PWFS, from_config
+    torch = torch_cuda
+    cfg = wl.CONFIGS["cfg1_tiny"]
+    A = wl.make_pupil(cfg)
+    phase = wl.phase_batch(cfg, steps=2)
+    with from_config(cfg) as sensor:
+        I = sensor.debug_intensity(torch.from_numpy(phase).cuda()).cpu().numpy().astype(np.float64)
+    for b in range(2):
+        ref = orc.intensity(A, phase[b], cfg.m_grid, cfg.mod_points, cfg.mod_radius)
+        assert np.abs(I[b] - ref).max() <= TOL_FRAME * ref.max()
+    # a radix-5 grid with a general mask shift (table-mask kernels)
+    N, M, s = 80, 160, 44
+    rng = np.random.default_rng(3)
+    c = np.arange(N) - (N - 1) / 2.0
+    X, Y = np.meshgrid(c, c)
+    A2 = (np.hypot(X, Y) <= N / 2.0).astype(np.float32)
+    ph = (rng.standard_normal((1, N, N)) * 2.0).astype(np.float32)
+    with PWFS(A2, M, 1.5, 6, 20, debug_shift_px=s) as sensor:
+        I2 = sensor.debug_intensity(torch.from_numpy(ph).cuda()).cpu().numpy().astype(np.float64)[0]
+    ref = orc.intensity(A2, ph[0], M, 6, 1.5, s=s)
+    # columns outside the two pupil-image windows are not computed (returned as zero): compare the computed ones
+    o = M // 2 - N // 2
+    cols = np.zeros(M, bool)
+    for g in ((M - s) % M, s % M):
+        cols[(g + np.arange(N) + o) % M] = True
+    assert np.abs(I2[:, cols] - ref[:, cols]).max() <= TOL_FRAME * ref.max()
+    assert np.abs(I2[:, ~cols]).max() == 0.0
+
+
 # -------------------------------------------------------------- edge cases ---
 @pytest.mark.parametrize("N,M,ns,K,r", [
     (64, 128, 16, 12, 3.0),      # cfg1 geometry

@@ -123,3 +123,43 @@ def test_non_finite_phase_propagates_to_its_own_frame_only(torch_cuda):
     assert not np.isfinite(fr[1]).all() and not np.isfinite(sl[1]).all()
     assert np.isfinite(fr[0]).all() and np.isfinite(fr[2]).all()
     assert np.isfinite(sl[0]).all() and np.isfinite(sl[2]).all()
+
+
+# ---- full-resolution intensity through the test-only export (pins P2, P3, P7 on the CUDA path) -------
+def test_identity_mask_returns_the_embedded_pupil(torch_cuda):
+    """P7: s = 0 (mask == 1), r = 0, K = 1: IDFT2(DFT2(G)) = G, so I is A^2 at offset o = M/2 - N/2 whatever the phase.
+    Checks padding offset, both transform scalings and the window/column bookkeeping of the kernels."""
+    from paper_1607_07624_b200.pwfs import PWFS
+    torch = torch_cuda
+    for N, M in [(64, 128), (60, 128), (160, 320), (100, 256)]:
+        rng = np.random.default_rng(N + M)
+        A = (rng.random((N, N)) > 0.2).astype(np.float32) * (0.5 + rng.random((N, N))).astype(np.float32)
+        phase = (rng.standard_normal((2, N, N)) * 5.0).astype(np.float32)
+        with PWFS(A, M, 0.0, 1, N // 4, debug_shift_px=0) as sensor:
+            I = sensor.debug_intensity(torch.from_numpy(phase).cuda()).cpu().numpy().astype(np.float64)
+            with pytest.raises(Exception):
+                sensor.run(torch.from_numpy(phase).cuda())                   # a debug handle does not serve the hot path
+        o = M // 2 - N // 2
+        want = np.zeros((M, M))
+        want[o:o + N, o:o + N] = A.astype(np.float64) ** 2
+        for b in range(2):
+            assert np.abs(I[b] - want).max() < 2e-6 * want.max(), (N, M, b, np.abs(I[b] - want).max())
+
+
+def test_full_resolution_flux_and_flat_wavefront_symmetry(torch_cuda, golden):
+    """P2: sum I = sum A^2 over the whole grid (Parseval through both transforms, unit-modulus mask, mean over k);
+    P3: flat wavefront -> I mirror-symmetric in x and y and under transposition (cfg1: symmetric pupil, K % 4 == 0)."""
+    from paper_1607_07624_b200.pwfs import from_config
+    torch = torch_cuda
+    cfg = wl.CONFIGS["cfg1_tiny"]
+    N, M = cfg.n_pupil, cfg.m_grid
+    phase = np.concatenate([np.zeros((1, N, N), np.float32), wl.phase_batch(cfg, steps=1)])
+    with from_config(cfg) as sensor:
+        I = sensor.debug_intensity(torch.from_numpy(phase).cuda()).cpu().numpy().astype(np.float64)
+    lit = golden["P2_cfg1_total_flux"]
+    for b in range(2):
+        assert abs(I[b].sum() / lit - 1.0) < 1e-5
+    flat = I[0]
+    assert np.abs(flat - flat[:, ::-1]).max() < 1e-5 * flat.max()
+    assert np.abs(flat - flat[::-1, :]).max() < 1e-5 * flat.max()
+    assert np.abs(flat - flat.T).max() < 1e-5 * flat.max()
