@@ -216,6 +216,36 @@ def atmosphere(cfg: WfsConfig) -> dict:
                 dt=cfg.dt, n_pupil=cfg.n_pupil)
 
 
+def zernike_ifs(A: np.ndarray, n_modes: int) -> Tuple[np.ndarray, np.ndarray]:
+    """Test / bench input for the DM (Table 1 `dm`: type 'zernike', nmodes 54): the first n_modes
+    Zernike polynomials after piston (Noll order j = 2 ..), sampled at the centres of the lit pixels of the
+    pupil A[N][N] (unit disc = the N-px pupil, same coordinates as make_pupil), each scaled to unit rms over
+    those pixels.  Returns (ifs float32 [n_modes][n_pix], pix int32 [n_pix] = flat indices y*N + x).
+    An input generator only: how the DM uses it is the method (csrc/dm_api.cu, oracle/dm_oracle.py)."""
+    N = A.shape[0]
+    c = (np.arange(N) - (N - 1) / 2.0) / (N / 2.0)
+    X, Y = np.meshgrid(c, c)
+    lit = np.flatnonzero(A.ravel() > 0)
+    rho, th = np.hypot(X, Y).ravel()[lit], np.arctan2(Y, X).ravel()[lit]
+    out = np.empty((n_modes, lit.size), dtype=np.float64)
+    j, n = 1, 0
+    rows = 0
+    while rows < n_modes:
+        n += 1
+        for m in range(n % 2, n + 1, 2):                     # |m| = n, n-2, ... (ascending |m|: Noll-like order)
+            rad = np.zeros_like(rho)
+            for k in range((n - m) // 2 + 1):
+                rad += ((-1) ** k * math.factorial(n - k)
+                        / (math.factorial(k) * math.factorial((n + m) // 2 - k) * math.factorial((n - m) // 2 - k))) * rho ** (n - 2 * k)
+            for trig in ((None,) if m == 0 else (np.cos, np.sin)):
+                if rows >= n_modes:
+                    break
+                z = rad if trig is None else rad * trig(m * th)
+                out[rows] = z / np.sqrt(np.mean(z * z))
+                rows += 1
+    return out.astype(np.float32), lit.astype(np.int32)
+
+
 def tilt_phase(N: int, alpha_x: float, alpha_y: float = 0.0) -> np.ndarray:
     """Test input: a pure tilt of (alpha_x, alpha_y) lambda/D across the N-px
     pupil, phi = 2 pi (alpha_x (x-c) + alpha_y (y-c)) / N, float32."""
