@@ -18,11 +18,11 @@ LIB = os.path.join(HERE, "libpwfs.so")
 GRID_R1 = (4, 5, 6, 8, 9, 10, 12, 15, 16, 18, 20, 24, 25, 27, 30, 32, 36, 40, 45, 48, 50, 54, 60, 64)   # PWFS_FOR_EACH_R1 of csrc/pwfs_launch.cuh
 # (source, extra flags, object name): the FFT kernels of each grid size M = 32 R1 are their own translation unit
 UNITS = [(os.path.join(CSRC, n), [], n[:-3] + ".o")
-         for n in ("pwfs_api.cu", "atmo_api.cu", "chain_api.cu", "rec_tc.cu", "psf_api.cu", "sh_api.cu", "peak_fp32.cu")] + \
+         for n in ("pwfs_api.cu", "atmo_api.cu", "chain_api.cu", "rec_tc.cu", "psf_api.cu", "sh_api.cu", "peak_fp32.cu", "dm_api.cu")] + \
         [(os.path.join(CSRC, "pwfs_inst.cu"), [f"-DPWFS_INST_R1={r}"], f"pwfs_inst_r{r}.o") for r in GRID_R1]
 SOURCES = sorted({u[0] for u in UNITS})
 HEADERS = [os.path.join(CSRC, n) for n in ("pwfs_kernels.cuh", "pwfs_dft.cuh", "pwfs_launch.cuh", "rec_tc.cuh", "device_guard.cuh")] + \
-          [os.path.join(ROOT, "include", n) for n in ("pwfs.h", "pwfs_atmo.h", "pwfs_chain.h", "pwfs_psf.h", "pwfs_sh.h")]
+          [os.path.join(ROOT, "include", n) for n in ("pwfs.h", "pwfs_atmo.h", "pwfs_chain.h", "pwfs_psf.h", "pwfs_sh.h", "pwfs_dm.h")]
 OBJDIR = os.path.join(HERE, "build")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]

@@ -221,7 +221,7 @@ def zernike_ifs(A: np.ndarray, n_modes: int) -> Tuple[np.ndarray, np.ndarray]:
     Zernike polynomials after piston (Noll order j = 2 ..), sampled at the centres of the lit pixels of the
     pupil A[N][N] (unit disc = the N-px pupil, same coordinates as make_pupil), each scaled to unit rms over
     those pixels.  Returns (ifs float32 [n_modes][n_pix], pix int32 [n_pix] = flat indices y*N + x).
-    An input generator only: how the DM uses it is the method (csrc/dm_api.cu, oracle/dm_oracle.py)."""
+    An input generator only: how the DM uses it is the method, which lives elsewhere."""
     N = A.shape[0]
     c = (np.arange(N) - (N - 1) / 2.0) / (N / 2.0)
     X, Y = np.meshgrid(c, c)

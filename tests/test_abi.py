@@ -25,9 +25,9 @@ def _declared_functions(header):
 
 
 def test_header_symbols_are_exported(lib):
-    from paper_1607_07624_b200 import atmo, chain, psf, pwfs, sh
+    from paper_1607_07624_b200 import atmo, chain, dm, psf, pwfs, sh
     bindings = {"pwfs.h": pwfs.EXPORTS, "pwfs_atmo.h": atmo.EXPORTS, "pwfs_chain.h": chain.EXPORTS,
-                "pwfs_psf.h": psf.EXPORTS, "pwfs_sh.h": sh.EXPORTS}
+                "pwfs_psf.h": psf.EXPORTS, "pwfs_sh.h": sh.EXPORTS, "pwfs_dm.h": dm.EXPORTS}
     assert sorted(os.listdir(os.path.join(ROOT, "include"))) == sorted(bindings)
     for header, exports in bindings.items():
         names = _declared_functions(header)
