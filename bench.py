@@ -129,6 +129,7 @@ def bench_stages(cfg, dev, phase, frames, flush, reps: int = 5) -> dict:
     import torch
     from paper_1607_07624_b200.atmo import Atmosphere
     from paper_1607_07624_b200.chain import CCD, Reconstructor, SlopeComputer
+    from paper_1607_07624_b200.dm import DeformableMirror, Integrator
     from paper_1607_07624_b200.psf import PsfCamera
     from paper_1607_07624_b200.sh import ShackHartmann
     from paper_1607_07624_b200.pwfs import from_config
@@ -209,6 +210,19 @@ def bench_stages(cfg, dev, phase, frames, flush, reps: int = 5) -> dict:
         m1 = torch.empty((1, n_modes), dtype=torch.float32, device=dev)
         ms = timed(lambda: rec.run(sl[:1], out=m1))
         out["f2_rec_gemv"] = hbm_row(ms, n_modes * 2 * nv * 4, 1, "one frame: recmat streamed once")
+    # DM: influence-function multiply, one frame of commands -> phase layer added to the phase.
+    # Random influence functions on the lit pixels (synthetic; 1024 actuators keep the matrix at ~0.6 GB here)
+    Apup = wl.make_pupil(cfg)
+    pix = np.flatnonzero(Apup.ravel() > 0).astype(np.int32)
+    n_act = min(1024, n_modes)
+    ifs = rng.standard_normal((n_act, pix.size), dtype=np.float32)
+    with DeformableMirror(ifs, pix, N, device=dev.index) as dm:
+        cmd1 = torch.zeros((1, n_act), dtype=torch.float32, device=dev)
+        ph1 = phase[:1].clone()
+        ms = timed(lambda: dm.apply(cmd1, ph1, alpha=1.0, beta=1.0))
+        out["dm_apply"] = hbm_row(ms, n_act * pix.size * 4 + 2 * pix.size * 4, 1,
+                                  f"{n_act} actuators x {pix.size} pupil pixels, one frame: the influence matrix streamed once")
+    del ifs
     # the whole device chain as a loop runs it: one simulation step per iteration (f1 -> a1-a8 -> f2), n_inst frames
     if not cfg.independent_screens:
         atm = wl.atmosphere(cfg)

@@ -223,37 +223,44 @@ rec_kernel(const float *__restrict__ R, int n_modes, int ldk, const float *__res
 }
 
 // ---- single frame (closed loop): a pure stream of recmat, 4 bytes per element, HBM-bound -------------------------
-// One CTA = one row of recmat at a time, its 8 warps each a contiguous eighth of the row; every thread keeps ITS
-// slope values in registers for the whole launch (thread t always meets slope indices 4 (t + 256 i) .. + 3), so per
-// row a thread issues NK independent 128-bit loads (all in flight together: NK * 4 KB per CTA) and 4 NK FMAs.  Rows
-// go round-robin over a grid of a few CTAs per SM: thousands of rows over ~600 CTAs leave no ragged last wave (the
-// row-per-warp kernel above runs 512 CTAs of 8 rows on 148 SMs: 3 or 4 CTAs per SM, 13 % idle).  Warp partials
-// meet in shared memory and are added in warp order: deterministic.
+// One CTA of 16 warps = one row of recmat at a time, each warp a contiguous sixteenth of the row; every thread keeps
+// ITS slope values in registers for the whole launch (thread t always meets slope indices 4 (t + 512 i) .. + 3), so per
+// row a thread issues NK independent 128-bit loads and 4 NK FMAs.  The loads of the CTA's NEXT row are issued before the
+// current row is reduced, so the memory system always has one to two rows (up to 96 KB) per SM in flight and the
+// per-row barrier costs nothing.  One CTA per SM, rows round-robin: thousands of rows leave no ragged last wave.
+// Warp partials meet in shared memory and are added in warp order: deterministic.
+constexpr int kGemvThreads = 512;
+
 template <int NK>
-__global__ void __launch_bounds__(256, 3)
+__global__ void __launch_bounds__(kGemvThreads, 1)
 rec_gemv_kernel(const float *__restrict__ R, int n_modes, int ldk, const float *__restrict__ S, int ns,
                 float *__restrict__ out) {
-    __shared__ float red[2][8];
+    __shared__ float red[2][kGemvThreads / 32];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int n4 = ldk >> 2;
     float4 sv[NK];
 #pragma unroll
     for (int i = 0; i < NK; ++i) {
-        const int k = 4 * (tid + 256 * i);
+        const int k = 4 * (tid + kGemvThreads * i);
         sv[i].x = k + 0 < ns ? __ldg(S + k + 0) : 0.f;
         sv[i].y = k + 1 < ns ? __ldg(S + k + 1) : 0.f;
         sv[i].z = k + 2 < ns ? __ldg(S + k + 2) : 0.f;
         sv[i].w = k + 3 < ns ? __ldg(S + k + 3) : 0.f;
     }
-    int par = 0;
-    for (int m = blockIdx.x; m < n_modes; m += gridDim.x, par ^= 1) {
+    float4 rv[NK], rn[NK];
+    auto fetch = [&](float4 (&dst)[NK], int m) {
         const float4 *row = reinterpret_cast<const float4 *>(R + (size_t)m * ldk);
-        float4 rv[NK];
 #pragma unroll
         for (int i = 0; i < NK; ++i) {
-            const int k4 = tid + 256 * i;
-            rv[i] = k4 < n4 ? __ldcs(row + k4) : make_float4(0.f, 0.f, 0.f, 0.f);      // streamed once: evict first
+            const int k4 = tid + kGemvThreads * i;
+            dst[i] = k4 < n4 ? __ldcs(row + k4) : make_float4(0.f, 0.f, 0.f, 0.f);      // streamed once: evict first
         }
+    };
+    int par = 0;
+    if ((int)blockIdx.x < n_modes) fetch(rv, blockIdx.x);
+    for (int m = blockIdx.x; m < n_modes; m += gridDim.x, par ^= 1) {
+        const int m_next = m + gridDim.x;
+        if (m_next < n_modes) fetch(rn, m_next);
         float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
 #pragma unroll
         for (int i = 0; i < NK; ++i) {
@@ -270,9 +277,11 @@ rec_gemv_kernel(const float *__restrict__ R, int n_modes, int ldk, const float *
         if (tid == 0) {
             float t = 0.f;
 #pragma unroll
-            for (int w = 0; w < 8; ++w) t += red[par][w];
+            for (int w = 0; w < kGemvThreads / 32; ++w) t += red[par][w];
             out[m] = t;
         }
+#pragma unroll
+        for (int i = 0; i < NK; ++i) rv[i] = rn[i];
     }
 }
 
@@ -474,12 +483,12 @@ int pwfs_rec_run(pwfs_rec_t *h, const float *d_slopes, int32_t B, float *d_modes
         if (h->tc) return rec_tc_run(h->tc, d_slopes, B, d_modes, (cudaStream_t)cuda_stream);
     }
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    if (B == 1 && h->ldk <= 4 * 256 * 12 && h->n_modes >= 64) {      // closed loop: one frame, recmat streamed once
-        const int nk = (h->ldk / 4 + 255) / 256;
-        const int grid = std::min(h->n_modes, 4 * h->num_sms);
-        if (nk <= 4)      rec_gemv_kernel<4><<<grid, 256, 0, st>>>(h->d_R, h->n_modes, h->ldk, d_slopes, h->n_slopes, d_modes);
-        else if (nk <= 8) rec_gemv_kernel<8><<<grid, 256, 0, st>>>(h->d_R, h->n_modes, h->ldk, d_slopes, h->n_slopes, d_modes);
-        else              rec_gemv_kernel<12><<<grid, 256, 0, st>>>(h->d_R, h->n_modes, h->ldk, d_slopes, h->n_slopes, d_modes);
+    if (B == 1 && h->ldk <= 4 * kGemvThreads * 6 && h->n_modes >= 64) {   // closed loop: one frame, recmat streamed once
+        const int nk = (h->ldk / 4 + kGemvThreads - 1) / kGemvThreads;
+        const int grid = std::min(h->n_modes, h->num_sms);
+        if (nk <= 2)      rec_gemv_kernel<2><<<grid, kGemvThreads, 0, st>>>(h->d_R, h->n_modes, h->ldk, d_slopes, h->n_slopes, d_modes);
+        else if (nk <= 4) rec_gemv_kernel<4><<<grid, kGemvThreads, 0, st>>>(h->d_R, h->n_modes, h->ldk, d_slopes, h->n_slopes, d_modes);
+        else              rec_gemv_kernel<6><<<grid, kGemvThreads, 0, st>>>(h->d_R, h->n_modes, h->ldk, d_slopes, h->n_slopes, d_modes);
         return cudaGetLastError() == cudaSuccess ? PWFS_OK : PWFS_ECUDA;
     }
     // frames per warp tile: the whole batch when it is small, else 16 or 8, whichever pads less

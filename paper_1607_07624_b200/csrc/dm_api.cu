@@ -7,7 +7,9 @@
 //                   frames, the commands of a block of actuators sit in shared memory (broadcast reads).
 //                   Loads are issued 8 actuators ahead of their FMAs.  HBM-bound: 4 bytes per matrix
 //                   element per group of FB <= 8 frames; a closed loop (B = sensor instances per step)
-//                   streams the matrix once per step.
+//                   streams the matrix once per step.  The actuator range is split over gridDim.z so that
+//                   a few thousand pixel columns still fill the machine; the partial sums meet in
+//   dm_fold_kernel  phase = beta phase + alpha (part[0] + part[1] + ...), fixed order: deterministic.
 //   int_kernel      one CTA: c += gain * delta; ring[t % (d+1)] = c; out = ring[(t - d) % (d+1)] or 0.
 #include "../../include/pwfs_dm.h"
 
@@ -26,11 +28,13 @@ constexpr int kDmThreads = 128;
 constexpr int kDmChunk = 256;     // actuators whose commands are staged in shared memory at a time
 constexpr int kDmAhead = 8;       // independent 128-bit loads in flight per thread
 
-// grid (ceil(ldp / 4 / kDmThreads), ceil(B / FB))
+// grid (ceil(ldp / 4 / kDmThreads), ceil(B / FB), msplit).  msplit == 1: writes the phase itself; else the partial
+// sums part[z][b][p] of actuators [z n_act / msplit, (z + 1) n_act / msplit), folded by dm_fold_kernel.
 template <int FB>
 __global__ void __launch_bounds__(kDmThreads)
 dm_kernel(const float *__restrict__ ifs, int n_act, int ldp, const int *__restrict__ pix, int n_pix, int npx2,
-          const float *__restrict__ cmd, int B, float *__restrict__ phase, float alpha, int accumulate) {
+          const float *__restrict__ cmd, int B, float *__restrict__ phase, float alpha, int accumulate,
+          float *__restrict__ part) {
     __shared__ float s_cmd[FB][kDmChunk];
     const int p4 = (blockIdx.x * kDmThreads + threadIdx.x) * 4;
     const int b0 = blockIdx.y * FB;
@@ -42,8 +46,9 @@ dm_kernel(const float *__restrict__ ifs, int n_act, int ldp, const int *__restri
     for (int f = 0; f < FB; ++f)
 #pragma unroll
         for (int q = 0; q < 4; ++q) acc[f][q] = 0.f;
-    for (int m0 = 0; m0 < n_act; m0 += kDmChunk) {
-        const int mc = min(kDmChunk, n_act - m0);
+    const int m_lo = (int)(((long long)blockIdx.z * n_act) / gridDim.z), m_hi = (int)(((long long)(blockIdx.z + 1) * n_act) / gridDim.z);
+    for (int m0 = m_lo; m0 < m_hi; m0 += kDmChunk) {
+        const int mc = min(kDmChunk, m_hi - m0);
         __syncthreads();                                   // the previous chunk's commands are no longer read
         for (int i = threadIdx.x; i < FB * kDmChunk; i += kDmThreads) {
             const int f = i / kDmChunk, mm = i - f * kDmChunk;
@@ -70,6 +75,14 @@ dm_kernel(const float *__restrict__ ifs, int n_act, int ldp, const int *__restri
         }
     }
     if (!live) return;
+    if (gridDim.z > 1) {                                   // partial sums, folded in a fixed order afterwards
+#pragma unroll
+        for (int f = 0; f < FB; ++f)
+            if (b0 + f < B)
+                *reinterpret_cast<float4 *>(part + ((size_t)blockIdx.z * B + b0 + f) * ldp + p4) =
+                    make_float4(acc[f][0], acc[f][1], acc[f][2], acc[f][3]);
+        return;
+    }
     int idx[4];
 #pragma unroll
     for (int q = 0; q < 4; ++q) idx[q] = p4 + q < n_pix ? __ldg(pix + p4 + q) : -1;
@@ -81,6 +94,18 @@ dm_kernel(const float *__restrict__ ifs, int n_act, int ldp, const int *__restri
         for (int q = 0; q < 4; ++q)
             if (idx[q] >= 0) out[idx[q]] = accumulate ? fmaf(alpha, acc[f][q], out[idx[q]]) : alpha * acc[f][q];
     }
+}
+
+// grid (ceil(n_pix / 256), B)
+__global__ void __launch_bounds__(256)
+dm_fold_kernel(const float *__restrict__ part, int msplit, int ldp, const int *__restrict__ pix, int n_pix, int npx2, int B,
+               float *__restrict__ phase, float alpha, int accumulate) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
+    if (p >= n_pix) return;
+    float s = 0.f;
+    for (int z = 0; z < msplit; ++z) s += __ldg(part + ((size_t)z * B + b) * ldp + p);
+    float *out = phase + (size_t)b * npx2 + __ldg(pix + p);
+    *out = accumulate ? fmaf(alpha, s, *out) : alpha * s;
 }
 
 // one CTA of 256 threads; t lives on the device (graph replays advance it)
@@ -105,10 +130,14 @@ int cuda_rc(cudaError_t e) { return e == cudaErrorMemoryAllocation ? PWFS_ENOMEM
 
 }  // namespace
 
+constexpr int kDmMaxFrames = 8;   // frames per register tile (and per partial-sum buffer)
+
 struct pwfs_dm {
     int device = 0, n_act = 0, n_pupil = 0, n_pix = 0, ldp = 0;
+    int msplit = 1;                 // actuator-range split (fixed at create: results do not depend on the batch)
     float *d_ifs = nullptr;
     int *d_pix = nullptr;
+    float *d_part = nullptr;        // [msplit][kDmMaxFrames][ldp]
 };
 
 struct pwfs_int {
@@ -145,6 +174,15 @@ int pwfs_dm_create(int32_t n_act, int32_t n_pupil, int32_t n_pix, const int32_t 
                          (size_t)n_pix * sizeof(float), (size_t)n_act, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_pix, (size_t)n_pix * sizeof(int));
     if (e == cudaSuccess) e = cudaMemcpy(h->d_pix, h_pix, (size_t)n_pix * sizeof(int), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        // enough CTAs for ~12 per SM (128 threads, 32 registers: the loads in flight are what hides HBM latency), at
+        // least 32 actuators per part
+        int sms = 148;
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
+        const int gx = (h->ldp / 4 + kDmThreads - 1) / kDmThreads;
+        h->msplit = std::max(1, std::min(std::min(n_act / 32, 64), (12 * sms + gx - 1) / gx));
+        if (h->msplit > 1) e = cudaMalloc((void **)&h->d_part, (size_t)h->msplit * kDmMaxFrames * h->ldp * sizeof(float));
+    }
     if (e != cudaSuccess) { const int rc = cuda_rc(e); pwfs_dm_destroy(h); return rc; }
     *out = h;
     return PWFS_OK;
@@ -163,18 +201,23 @@ int pwfs_dm_apply(pwfs_dm_t *h, const float *d_cmd, int32_t B, float *d_phase, f
     const unsigned gx = (unsigned)((h->ldp / 4 + kDmThreads - 1) / kDmThreads);
     // frames per register tile: the whole batch when it is small (the matrix is then streamed once)
     int FB = 1;
-    while (FB < B && FB < 8) FB *= 2;
-    for (int b0 = 0; b0 < B; b0 += 65535 * FB) {                       // grid.y limit
-        const int Bc = std::min(B - b0, 65535 * FB);
-        const dim3 grid(gx, (unsigned)((Bc + FB - 1) / FB));
+    while (FB < B && FB < kDmMaxFrames) FB *= 2;
+    const int ms = h->msplit;
+    const int step = ms > 1 ? kDmMaxFrames : 65535 * FB;               // partial buffer holds 8 frames; grid.y limit
+    for (int b0 = 0; b0 < B; b0 += step) {
+        const int Bc = std::min(B - b0, step);
+        const dim3 grid(gx, (unsigned)((Bc + FB - 1) / FB), (unsigned)ms);
         const float *c = d_cmd + (size_t)b0 * h->n_act;
         float *ph = d_phase + (size_t)b0 * npx2;
         switch (FB) {
-            case 1: dm_kernel<1><<<grid, kDmThreads, 0, st>>>(h->d_ifs, h->n_act, h->ldp, h->d_pix, h->n_pix, npx2, c, Bc, ph, alpha, acc); break;
-            case 2: dm_kernel<2><<<grid, kDmThreads, 0, st>>>(h->d_ifs, h->n_act, h->ldp, h->d_pix, h->n_pix, npx2, c, Bc, ph, alpha, acc); break;
-            case 4: dm_kernel<4><<<grid, kDmThreads, 0, st>>>(h->d_ifs, h->n_act, h->ldp, h->d_pix, h->n_pix, npx2, c, Bc, ph, alpha, acc); break;
-            default: dm_kernel<8><<<grid, kDmThreads, 0, st>>>(h->d_ifs, h->n_act, h->ldp, h->d_pix, h->n_pix, npx2, c, Bc, ph, alpha, acc); break;
+            case 1: dm_kernel<1><<<grid, kDmThreads, 0, st>>>(h->d_ifs, h->n_act, h->ldp, h->d_pix, h->n_pix, npx2, c, Bc, ph, alpha, acc, h->d_part); break;
+            case 2: dm_kernel<2><<<grid, kDmThreads, 0, st>>>(h->d_ifs, h->n_act, h->ldp, h->d_pix, h->n_pix, npx2, c, Bc, ph, alpha, acc, h->d_part); break;
+            case 4: dm_kernel<4><<<grid, kDmThreads, 0, st>>>(h->d_ifs, h->n_act, h->ldp, h->d_pix, h->n_pix, npx2, c, Bc, ph, alpha, acc, h->d_part); break;
+            default: dm_kernel<8><<<grid, kDmThreads, 0, st>>>(h->d_ifs, h->n_act, h->ldp, h->d_pix, h->n_pix, npx2, c, Bc, ph, alpha, acc, h->d_part); break;
         }
+        if (ms > 1)
+            dm_fold_kernel<<<dim3((unsigned)((h->n_pix + 255) / 256), (unsigned)Bc), 256, 0, st>>>(
+                h->d_part, ms, h->ldp, h->d_pix, h->n_pix, npx2, Bc, ph, alpha, acc);
     }
     return cudaGetLastError() == cudaSuccess ? PWFS_OK : PWFS_ECUDA;
 }
@@ -184,6 +227,7 @@ void pwfs_dm_destroy(pwfs_dm_t *h) {
     pwk::DeviceGuard dg(h->device);
     if (h->d_ifs) cudaFree(h->d_ifs);
     if (h->d_pix) cudaFree(h->d_pix);
+    if (h->d_part) cudaFree(h->d_part);
     delete h;
 }
 

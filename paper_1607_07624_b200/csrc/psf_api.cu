@@ -6,12 +6,17 @@
 // forward only, so the result stays in the "k1 + R1 k2" register order and is consumed there.
 //
 //   psf_row_kernel   N pupil rows per frame: phasor (phase rescaled to the imaging wavelength)
-//                    -> DFT over x -> T[f][u][y], transposed through shared memory so that the
-//                    column pass reads 128-byte lines.
-//   psf_col_kernel   one warp per NB columns u, looping over its share of the frames: DFT over
-//                    y (only the N non-zero inputs are read), |.|^2 accumulated over the frames in
-//                    registers; Strehl ratio from the (0,0) bin; one partial PSF per frame split.
-//   psf_fold_kernel  accumulator += sum of the partial PSFs (fixed order: deterministic).
+//                    -> DFT over x -> T[f][y / 8][c][y % 8], c = 32 k1 + k2 the position of frequency
+//                    u = k1 + R1 k2 in the exchange buffer: the CTA's 8 (16, ..) rows leave as ONE
+//                    contiguous block of M * 64 bytes per 8 rows, a straight copy out of shared memory
+//                    (same blocked layout as the pyramid path's T).  A CTA keeps its rows for several
+//                    frames, so the twiddle table is loaded once.
+//   psf_col_kernel   one warp per NB columns c, looping over its share of the frames: DFT over
+//                    y (only the N non-zero inputs are read, 64-byte runs), |.|^2 accumulated over the
+//                    frames in registers; Strehl ratio from the (0,0) bin; one partial PSF per frame
+//                    split, written column-major [u][v] so that a warp's stores are contiguous.
+//   psf_fold_kernel  accumulator[v][u] += sum of the partial PSFs [u][v] (fixed order: deterministic),
+//                    transposing 32 x 32 tiles through shared memory.
 //   psf_read_kernel  long exposure = accumulator / (frames M^2 sum A^2).
 // Work per frame: (N + M) transforms of length M; HBM: phase in, T out and back, nothing else.
 #include "../../include/pwfs_psf.h"
@@ -44,9 +49,11 @@ struct PsfCfg {
     static constexpr int ROUNDS = (ITEMS + 31) / 32; // lanes take them in rounds (R1 > 32: two)
     static constexpr bool PREFETCH = R1_ <= 32;      // column pass: next frame's inputs in registers while this one runs
     static_assert(ITEMS <= 32 || NB_ == 1, "more than one round only for a single transform per warp");
-    static constexpr int WARP_BUF = ITEMS * kPitchP + 1;
+    // pad so that the row pass's copy-out (8 rows x 4 adjacent k2 per warp instruction) is conflict-free for NB = 1
+    static constexpr int WARP_BUF = ITEMS * kPitchP + ((2 - (ITEMS * kPitchP) % 16) + 16) % 16;
     static constexpr int TAB = R1_ * kPitchP;
     static constexpr int RPC = NB_ * WPB_;           // rows per CTA, row pass
+
     static constexpr size_t smem = (size_t)(TAB + WPB_ * WARP_BUF) * sizeof(float2);
 };
 
@@ -63,63 +70,87 @@ __device__ __forceinline__ void load_tw(float2 *s_tw, const PsfDev &t) {
     for (int i = threadIdx.x; i < C::R1 * 32; i += blockDim.x) s_tw[(i >> 5) * kPitchP + (i & 31)] = __ldg(t.tw + i);
 }
 
-// grid (ceil(NP / RPC), F); block 32 * WPB.
+constexpr int kRowFrames = 4;    // frames a row-pass CTA works through (amortises the twiddle-table load)
+
+// grid (ceil(NP / RPC), ceil(F / kRowFrames)); block 32 * WPB.
 template <class C>
 __global__ void __launch_bounds__(32 * C::WPB)
-psf_row_kernel(PsfDev t, const float *__restrict__ phase, float2 *__restrict__ T) {
+psf_row_kernel(PsfDev t, const float *__restrict__ phase, float2 *__restrict__ T, int F) {
+    static_assert(C::RPC % 8 == 0, "row pass: rows per CTA must be whole 8-row blocks of T");
     extern __shared__ float2 smem[];
     float2 *s_tw = smem, *s_buf = smem + C::TAB;
     const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
-    const int N = t.N, f = blockIdx.y, y0 = blockIdx.x * C::RPC;
+    const int N = t.N, y0 = blockIdx.x * C::RPC;
     float2 *buf = s_buf + wl * C::WARP_BUF;
     load_tw<C>(s_tw, t);
+    float am[C::NB][C::NZ];
 #pragma unroll
-    for (int b = 0; b < C::NB; ++b) {
-        const int y = y0 + wl * C::NB + b;
-        float2 v[C::R1];
+    for (int b = 0; b < C::NB; ++b)
 #pragma unroll
         for (int n1 = 0; n1 < C::NZ; ++n1) {
-            const int x = 32 * n1 + lane;
-            const bool ok = (y < N) && (x < N);
-            const float ph = ok ? __ldg(phase + ((size_t)f * N + y) * N + x) * t.scale : 0.f;
-            const float am = ok ? __ldg(t.amp + (size_t)y * N + x) : 0.f;
-            // phase in turns, reduced with a two-term 1/(2 pi) (exact integer part, FMA keeps the low bits)
-            const float q = rintf(ph * kInv2PiHiP);
-            float tr = fmaf(ph, kInv2PiHiP, -q);
-            tr = fmaf(ph, kInv2PiLoP, tr);
-            float sn, cs;
-            __sincosf(tr * 6.283185307179586f, &sn, &cs);
-            v[n1] = make_float2(am * cs, am * sn);
+            const int y = y0 + wl * C::NB + b, x = 32 * n1 + lane;
+            am[b][n1] = (y < N && x < N) ? __ldg(t.amp + (size_t)y * N + x) : 0.f;
         }
-        DftP<C::R1, -1, C::NZ>::run(v);
+    const int f_end = min(F, (int)(blockIdx.y + 1) * kRowFrames);
+    // the next frame's phase is fetched while this frame is transformed
+    float ph[C::NB][C::NZ];
+    auto fetch = [&](int f) {
 #pragma unroll
-        for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitchP + lane] = v[k1];
-    }
-    __syncthreads();
+        for (int b = 0; b < C::NB; ++b)
 #pragma unroll
-    for (int rd = 0; rd < C::ROUNDS; ++rd) {
-        const int w = rd * 32 + lane;
-        if (w < C::ITEMS) {
-            const int k1 = w % C::R1;
-            float2 *row = buf + w * kPitchP;
-            const float2 *twr = s_tw + k1 * kPitchP;
-            float2 u[32];
+            for (int n1 = 0; n1 < C::NZ; ++n1) {
+                const int y = y0 + wl * C::NB + b, x = 32 * n1 + lane;
+                ph[b][n1] = (y < N && x < N) ? __ldg(phase + ((size_t)f * N + y) * N + x) : 0.f;
+            }
+    };
+    if ((int)blockIdx.y * kRowFrames < f_end) fetch(blockIdx.y * kRowFrames);
+    for (int f = blockIdx.y * kRowFrames; f < f_end; ++f) {
 #pragma unroll
-            for (int n2 = 0; n2 < 32; ++n2) u[n2] = cmul(row[n2], twr[n2]);
-            Dft<32, -1>::run(u);
+        for (int b = 0; b < C::NB; ++b) {
+            float2 v[C::R1];
 #pragma unroll
-            for (int k2 = 0; k2 < 32; ++k2) row[k2] = u[k2];
+            for (int n1 = 0; n1 < C::NZ; ++n1) {
+                const float p = ph[b][n1] * t.scale;
+                // phase in turns, reduced with a two-term 1/(2 pi) (exact integer part, FMA keeps the low bits)
+                const float q = rintf(p * kInv2PiHiP);
+                float tr = fmaf(p, kInv2PiHiP, -q);
+                tr = fmaf(p, kInv2PiLoP, tr);
+                float sn, cs;
+                __sincosf(tr * 6.283185307179586f, &sn, &cs);
+                v[n1] = make_float2(am[b][n1] * cs, am[b][n1] * sn);
+            }
+            if (b == C::NB - 1 && f + 1 < f_end) fetch(f + 1);
+            DftP<C::R1, -1, C::NZ>::run(v);
+#pragma unroll
+            for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitchP + lane] = v[k1];
         }
-    }
-    __syncthreads();
-    // X[u = k1 + R1 k2] of CTA row r sits at s_buf[(r/NB) WARP_BUF + ((r%NB) R1 + k1) pitch + k2];
-    // adjacent threads take adjacent rows y of one u: runs of RPC * 8 bytes in T[f][u][y]
-    float2 *Tf = T + (size_t)f * C::M * t.NP;
-    for (int i = threadIdx.x; i < C::RPC * C::M; i += 32 * C::WPB) {
-        const int r = i % C::RPC, uu = i / C::RPC;
-        const int k1 = uu % C::R1, k2 = uu / C::R1;
-        if (y0 + r < t.NP)
-            Tf[(size_t)uu * t.NP + y0 + r] = s_buf[(r / C::NB) * C::WARP_BUF + ((r % C::NB) * C::R1 + k1) * kPitchP + k2];
+        __syncthreads();     // also: the twiddle table is complete (first pass)
+#pragma unroll
+        for (int rd = 0; rd < C::ROUNDS; ++rd) {
+            const int w = rd * 32 + lane;
+            if (w < C::ITEMS) {
+                const int k1 = w % C::R1;
+                float2 *row = buf + w * kPitchP;
+                const float2 *twr = s_tw + k1 * kPitchP;
+                float2 u[32];
+#pragma unroll
+                for (int n2 = 0; n2 < 32; ++n2) u[n2] = cmul(row[n2], twr[n2]);
+                Dft<32, -1>::run(u);
+#pragma unroll
+                for (int k2 = 0; k2 < 32; ++k2) row[k2] = u[k2];
+            }
+        }
+        __syncthreads();
+        // X[u = k1 + R1 k2] of CTA row r sits at s_buf[(r/NB) WARP_BUF + ((r%NB) R1 + k1) pitch + k2].  Element
+        // i = r_lo + 8 (c + M r_hi), c = 32 k1 + k2, r = 8 r_hi + r_lo, goes to T[f][y0/8 + r_hi][c][r_lo]: for this CTA
+        // one contiguous run of RPC * M float2, written in order.
+        float2 *dst = T + (size_t)f * C::M * t.NP + (size_t)(y0 / 8) * (C::M * 8);
+        const int n_out = min(C::RPC, t.NP - y0) * C::M;              // whole 8-row blocks (NP % 32 == 0)
+        for (int i = threadIdx.x; i < n_out; i += 32 * C::WPB) {
+            const int r_hi = i / (8 * C::M), c = (i >> 3) - r_hi * C::M, r = 8 * r_hi + (i & 7);
+            dst[i] = s_buf[(r / C::NB) * C::WARP_BUF + ((r % C::NB) * C::R1 + (c >> 5)) * kPitchP + (c & 31)];
+        }
+        __syncthreads();     // the next frame overwrites the buffers
     }
 }
 
@@ -144,13 +175,14 @@ psf_col_kernel(PsfDev t, const float2 *__restrict__ T, int F, int fsplit, float 
 #pragma unroll
         for (int k2 = 0; k2 < 32; ++k2) acc[rd][k2] = 0.f;
     float2 pre[C::NB][C::NZ];
+    // T[f][y / 8][c][y % 8]: lane reads y = 32 n1 + lane, i.e. block 4 n1 + lane / 8, row lane % 8 of column c = u0 + b
     auto fetch = [&](int f) {
-        const float2 *src = T + ((size_t)f * C::M + u0) * NP + lane;
+        const float2 *src = T + (size_t)f * C::M * NP + (size_t)(lane >> 3) * (C::M * 8) + (size_t)u0 * 8 + (lane & 7);
 #pragma unroll
         for (int b = 0; b < C::NB; ++b)
 #pragma unroll
             for (int n1 = 0; n1 < C::NZ; ++n1)
-                pre[b][n1] = (32 * n1 < NP && u0 + b < C::M) ? __ldg(src + (size_t)b * NP + 32 * n1) : make_float2(0.f, 0.f);
+                pre[b][n1] = (32 * n1 < NP && u0 + b < C::M) ? __ldg(src + b * 8 + (size_t)n1 * (32 * C::M)) : make_float2(0.f, 0.f);
     };
     if (C::PREFETCH && f_lo < f_hi) fetch(f_lo);
     for (int f = f_lo; f < f_hi; ++f) {
@@ -179,7 +211,7 @@ psf_col_kernel(PsfDev t, const float2 *__restrict__ T, int F, int fsplit, float 
                 Dft<32, -1>::run(u);
 #pragma unroll
                 for (int k2 = 0; k2 < 32; ++k2) acc[rd][k2] = fmaf(u[k2].x, u[k2].x, fmaf(u[k2].y, u[k2].y, acc[rd][k2]));
-                if (sr && my_k1 == 0 && u0 + my_b == 0)          // F4c: the (0, 0) bin
+                if (sr && my_k1 == 0 && u0 + my_b == 0)          // F4c: the (0, 0) bin (column c = 0 is u = 0)
                     sr[f] = fmaf(u[0].x, u[0].x, u[0].y * u[0].y) * t.inv_sumA_sq;
             }
         }
@@ -190,23 +222,34 @@ psf_col_kernel(PsfDev t, const float2 *__restrict__ T, int F, int fsplit, float 
         const int w = rd * 32 + lane;
         const int my_b = w / C::R1, my_k1 = w % C::R1;
         if (w < C::ITEMS && u0 + my_b < C::M) {
-            const int uo = (u0 + my_b + C::M / 2) % C::M;
-            float *dst = partial + (size_t)fs * C::M * C::M + uo;
+            const int c = u0 + my_b, uu = (c >> 5) + C::R1 * (c & 31);      // column c of T holds frequency u
+            const int uo = (uu + C::M / 2) % C::M;
+            float *dst = partial + ((size_t)fs * C::M + uo) * C::M;          // [fs][u][v]: the lanes' v are adjacent
 #pragma unroll
             for (int k2 = 0; k2 < 32; ++k2) {
                 const int vo = (my_k1 + C::R1 * k2 + C::M / 2) % C::M;
-                dst[(size_t)vo * C::M] = acc[rd][k2];
+                dst[vo] = acc[rd][k2];
             }
         }
     }
 }
 
-__global__ void psf_fold_kernel(float *__restrict__ accum, const float *__restrict__ partial, int fsplit, size_t MM) {
-    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= MM) return;
-    float s = accum[i];
-    for (int k = 0; k < fsplit; ++k) s += __ldg(partial + (size_t)k * MM + i);
-    accum[i] = s;
+// accum[v][u] += sum_k partial[k][u][v]; grid (M / 32, M / 32), block (32, 8)
+__global__ void psf_fold_kernel(float *__restrict__ accum, const float *__restrict__ partial, int fsplit, int M) {
+    __shared__ float tile[32][33];
+    const size_t MM = (size_t)M * M;
+    const int u0 = blockIdx.y * 32, v0 = blockIdx.x * 32;
+    for (int j = threadIdx.y; j < 32; j += 8) {                       // tile[u][v], coalesced along v
+        float s = 0.f;
+        const float *src = partial + (size_t)(u0 + j) * M + v0 + threadIdx.x;
+        for (int k = 0; k < fsplit; ++k) s += __ldg(src + (size_t)k * MM);
+        tile[j][threadIdx.x] = s;
+    }
+    __syncthreads();
+    for (int j = threadIdx.y; j < 32; j += 8) {                       // accum[v][u], coalesced along u
+        float *dst = accum + (size_t)(v0 + j) * M + u0 + threadIdx.x;
+        *dst += tile[threadIdx.x][j];
+    }
 }
 
 __global__ void psf_read_kernel(const float *__restrict__ accum, float *__restrict__ out, float scale, size_t MM) {
@@ -217,24 +260,24 @@ __global__ void psf_read_kernel(const float *__restrict__ accum, float *__restri
 struct PsfLauncher {
     int NB, WPB, RPC;
     size_t smem;
-    void (*row)(dim3, cudaStream_t, const PsfDev &, const float *, float2 *);
+    void (*row)(dim3, cudaStream_t, const PsfDev &, const float *, float2 *, int);
     void (*col)(dim3, cudaStream_t, const PsfDev &, const float2 *, int, int, float *, float *);
     cudaError_t (*prepare)();
     int (*col_ctas_per_sm)();       // occupancy of the column-pass kernel
 };
 
 template <class C>
-void row_t(dim3 g, cudaStream_t st, const PsfDev &t, const float *ph, float2 *T) {
-    psf_row_kernel<C><<<g, 32 * C::WPB, C::smem, st>>>(t, ph, T);
+void row_t(dim3 g, cudaStream_t st, const PsfDev &t, const float *ph, float2 *T, int F) {
+    psf_row_kernel<C><<<g, 32 * C::WPB, C::smem, st>>>(t, ph, T, F);
 }
 template <class C>
 void col_t(dim3 g, cudaStream_t st, const PsfDev &t, const float2 *T, int F, int fsplit, float *part, float *sr) {
     psf_col_kernel<C><<<g, 32 * C::WPB, C::smem, st>>>(t, T, F, fsplit, part, sr);
 }
-template <class C>
+template <class C, class CC>
 cudaError_t prepare_t() {
     cudaError_t e = cudaFuncSetAttribute(psf_row_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(psf_col_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(psf_col_kernel<CC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CC::smem);
     return e;
 }
 template <class C>
@@ -243,36 +286,38 @@ int col_occ_t() {
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, psf_col_kernel<C>, 32 * C::WPB, C::smem) != cudaSuccess || n < 1) n = 1;
     return n;
 }
-template <class C>
-PsfLauncher make() { return PsfLauncher{C::NB, C::WPB, C::RPC, C::smem, row_t<C>, col_t<C>, prepare_t<C>, col_occ_t<C>}; }
+// C: row pass; CC: column pass (same R1 and NB; 4-warp CTAs for the large grids: two CTAs per SM fill the machine better
+// than one of 8 warps when a launch has only M / 8 of them)
+template <class C, class CC = C>
+PsfLauncher make() { return PsfLauncher{CC::NB, CC::WPB, C::RPC, C::smem, row_t<C>, col_t<CC>, prepare_t<C, CC>, col_occ_t<CC>}; }
 
 bool find_psf_launcher(int M, PsfLauncher *out) {
     if (M % 32) return false;
     switch (M / 32) {
         case 4:  *out = make<PsfCfg<4, 8, 4>>(); return true;
         case 5:  *out = make<PsfCfg<5, 6, 4>>(); return true;
-        case 6:  *out = make<PsfCfg<6, 5, 4>>(); return true;
+        case 6:  *out = make<PsfCfg<6, 5, 8>>(); return true;
         case 8:  *out = make<PsfCfg<8, 4, 4>>(); return true;
-        case 9:  *out = make<PsfCfg<9, 3, 4>>(); return true;
-        case 10: *out = make<PsfCfg<10, 3, 4>>(); return true;
+        case 9:  *out = make<PsfCfg<9, 3, 8>>(); return true;
+        case 10: *out = make<PsfCfg<10, 3, 8>>(); return true;
         case 12: *out = make<PsfCfg<12, 2, 4>>(); return true;
         case 15: *out = make<PsfCfg<15, 2, 4>>(); return true;
         case 16: *out = make<PsfCfg<16, 2, 4>>(); return true;
-        case 18: *out = make<PsfCfg<18, 1, 8>>(); return true;
-        case 20: *out = make<PsfCfg<20, 1, 8>>(); return true;
-        case 24: *out = make<PsfCfg<24, 1, 8>>(); return true;
-        case 25: *out = make<PsfCfg<25, 1, 8>>(); return true;
-        case 27: *out = make<PsfCfg<27, 1, 8>>(); return true;
-        case 30: *out = make<PsfCfg<30, 1, 8>>(); return true;
-        case 32: *out = make<PsfCfg<32, 1, 8>>(); return true;
-        case 36: *out = make<PsfCfg<36, 1, 8>>(); return true;
-        case 40: *out = make<PsfCfg<40, 1, 8>>(); return true;
-        case 45: *out = make<PsfCfg<45, 1, 8>>(); return true;
-        case 48: *out = make<PsfCfg<48, 1, 8>>(); return true;
-        case 50: *out = make<PsfCfg<50, 1, 8>>(); return true;
-        case 54: *out = make<PsfCfg<54, 1, 8>>(); return true;
-        case 60: *out = make<PsfCfg<60, 1, 8>>(); return true;
-        case 64: *out = make<PsfCfg<64, 1, 8>>(); return true;
+        case 18: *out = make<PsfCfg<18, 1, 8>, PsfCfg<18, 1, 4>>(); return true;
+        case 20: *out = make<PsfCfg<20, 1, 8>, PsfCfg<20, 1, 4>>(); return true;
+        case 24: *out = make<PsfCfg<24, 1, 8>, PsfCfg<24, 1, 4>>(); return true;
+        case 25: *out = make<PsfCfg<25, 1, 8>, PsfCfg<25, 1, 4>>(); return true;
+        case 27: *out = make<PsfCfg<27, 1, 8>, PsfCfg<27, 1, 4>>(); return true;
+        case 30: *out = make<PsfCfg<30, 1, 8>, PsfCfg<30, 1, 4>>(); return true;
+        case 32: *out = make<PsfCfg<32, 1, 8>, PsfCfg<32, 1, 4>>(); return true;
+        case 36: *out = make<PsfCfg<36, 1, 8>, PsfCfg<36, 1, 4>>(); return true;
+        case 40: *out = make<PsfCfg<40, 1, 8>, PsfCfg<40, 1, 4>>(); return true;
+        case 45: *out = make<PsfCfg<45, 1, 8>, PsfCfg<45, 1, 4>>(); return true;
+        case 48: *out = make<PsfCfg<48, 1, 8>, PsfCfg<48, 1, 4>>(); return true;
+        case 50: *out = make<PsfCfg<50, 1, 8>, PsfCfg<50, 1, 4>>(); return true;
+        case 54: *out = make<PsfCfg<54, 1, 8>, PsfCfg<54, 1, 4>>(); return true;
+        case 60: *out = make<PsfCfg<60, 1, 8>, PsfCfg<60, 1, 4>>(); return true;
+        case 64: *out = make<PsfCfg<64, 1, 8>, PsfCfg<64, 1, 4>>(); return true;
         default: return false;
     }
 }
@@ -390,9 +435,9 @@ int pwfs_psf_accumulate(pwfs_psf_t *h, const float *d_phase, int32_t B, float *d
     for (int f0 = 0; f0 < B; f0 += F) {
         const int Fc = std::min(F, B - f0);
         const int fsp = std::min(fsplit, Fc);
-        L.row(dim3((d.NP + L.RPC - 1) / L.RPC, Fc), st, d, d_phase + (size_t)f0 * d.N * d.N, h->T);
+        L.row(dim3((d.NP + L.RPC - 1) / L.RPC, (Fc + kRowFrames - 1) / kRowFrames), st, d, d_phase + (size_t)f0 * d.N * d.N, h->T, Fc);
         L.col(dim3(col_ctas, fsp), st, d, h->T, Fc, fsp, h->partial, d_sr ? d_sr + f0 : nullptr);
-        psf_fold_kernel<<<(unsigned)((MM + 255) / 256), 256, 0, st>>>(h->d_acc, h->partial, fsp, MM);
+        psf_fold_kernel<<<dim3(d.M / 32, d.M / 32), dim3(32, 8), 0, st>>>(h->d_acc, h->partial, fsp, d.M);
     }
     if (cudaGetLastError() != cudaSuccess) return PWFS_ECUDA;
     h->count += B;

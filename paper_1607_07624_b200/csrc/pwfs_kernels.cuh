@@ -275,14 +275,16 @@ xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ 
     const int j_lo = (int)(((long long)js * t.KX) / jsplit), j_hi = (int)(((long long)(js + 1) * t.KX) / jsplit);
     const size_t slab = (size_t)C::M * t.NP;
     __syncthreads();   // tables loaded (s_p is private to the warp that wrote it)
+    // the x-tilt table row of the NEXT tilt is fetched into registers while this tilt's size-32 stage and write-out
+    // run: with the shared memory this kernel uses L1 keeps ~10 KB, so a load at the point of use waits for L2
+    float2 tx[C::NZ];
+    {
+        const float2 *txj = t.txc + (size_t)j_lo * t.NXP + lane;
+#pragma unroll
+        for (int n1 = 0; n1 < C::NZ; ++n1) tx[n1] = __ldg(txj + 32 * n1);
+    }
     for (int j = j_lo; j < j_hi; ++j) {
         // step A: x-tilt, zero-padded DFT of size R1 over n1
-        float2 tx[C::NZ];
-        {
-            const float2 *txj = t.txc + (size_t)j * t.NXP + lane;
-#pragma unroll
-            for (int n1 = 0; n1 < C::NZ; ++n1) tx[n1] = __ldg(txj + 32 * n1);
-        }
 #pragma unroll
         for (int b = 0; b < C::NB; ++b) {
             float2 v[C::R1];
@@ -292,11 +294,13 @@ xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ 
 #pragma unroll
             for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitch + lane] = v[k1];
         }
+        if (j + 1 < j_hi) {
+            const float2 *txj = t.txc + (size_t)(j + 1) * t.NXP + lane;
+#pragma unroll
+            for (int n1 = 0; n1 < C::NZ; ++n1) tx[n1] = __ldg(txj + 32 * n1);
+        }
         __syncwarp();
         stage32<C, QM>(buf, s_tw, s_am, lane);
-        // pull the next tilt's table row (NXP float2 = NZ * 2 cache lines) into L1 while the last stage runs
-        if (j + 1 < j_hi && threadIdx.x < 2 * C::NZ)
-            asm volatile("prefetch.global.L1 [%0];" ::"l"(t.txc + (size_t)(j + 1) * t.NXP + 16 * threadIdx.x));
         __syncthreads();
         // step A'': inverse DFT of size R1 over k1 for item (r, n2) -> T[f][j][(y0 + r) / 8][32 n1 + n2][r % 8]
         float2 *Tj = T + ((size_t)(t.t_frames == 1 ? 0 : f) * t.KX + j) * slab;

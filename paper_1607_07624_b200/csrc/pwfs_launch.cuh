@@ -34,7 +34,7 @@ template <> struct CfgFor<24> { using type = PassCfg<24, 2, 4, 4, 2, 1>; };   //
 template <> struct CfgFor<25> { using type = PassCfg<25, 2, 4, 4, 2, 1>; };   // M = 800
 template <> struct CfgFor<27> { using type = PassCfg<27, 2, 4, 4, 2, 1>; };   // M = 864
 template <> struct CfgFor<30> { using type = PassCfg<30, 2, 4, 4, 2, 1>; };   // M = 960
-template <> struct CfgFor<32> { using type = PassCfg<32, 2, 4, 4, 3, 2>; };   // M = 1024
+template <> struct CfgFor<32> { using type = PassCfg<32, 2, 4, 4, 2, 2>; };   // M = 1024
 // R1 > 32: the size-32 stage runs in two rounds (the second with R1 - 32 lanes), one CTA per SM in both passes
 template <> struct CfgFor<36> { using type = PassCfg<36, 1, 8, 4, 1, 1>; };   // M = 1152
 template <> struct CfgFor<40> { using type = PassCfg<40, 1, 8, 4, 1, 1>; };   // M = 1280

@@ -6,20 +6,23 @@
 // operand is split into two TF32-representable planes, x = hi + lo + O(2^-22 |x|), and the product is
 //   R S^T ~= Rhi Shi^T + Rhi Slo^T + Rlo Shi^T        (dropped terms <= 3 * 2^-22 |R||S| = 7e-7)
 // accumulated in FP32 in tensor memory: three tcgen05.mma.kind::tf32 per K step, same accumulator.
-// recmat's planes are built once at create (it is static calibration data); the slope planes are
-// written by a small split kernel per call.
+// recmat is streamed from HBM as it is (FP32, 4 bytes per element) and split INSIDE the pipeline; the
+// (small) slope planes are written by a split kernel per call.
 //
 // Kernel (one 128 x 128 output tile of one K split per CTA, 192 threads):
-//   warp 0 (one lane)  TMA producer: four 128 x 32 FP32 boxes (Rhi, Rlo, Shi, Slo; 128-byte swizzle)
-//                      per stage into a 3-stage ring, completion on the stage's "full" mbarrier;
-//   warp 1 (one lane)  MMA issuer: per stage 4 K steps x 3 UMMAs (M 128, N 128, K 8) from shared-memory
-//                      descriptors into 128 TMEM columns; tcgen05.commit releases the stage ("empty")
-//                      and, after the last one, signals the epilogue;
-//   warps 2-5          epilogue: tcgen05.ld 32 lanes x 32 columns at a time, rows = modes so that a
+//   warp 0 (one lane)  TMA producer: three 128 x 32 FP32 boxes per stage (recmat raw, Shi, Slo;
+//                      128-byte swizzle) into a 3-stage ring, completion on the stage's "full" mbarrier;
+//   warps 2-5          converters: read the raw recmat tile, write hi = tf32(x) back in place and
+//                      lo = tf32(x - hi) into the stage's fourth tile (element-wise, so the swizzle
+//                      does not matter), fence.proxy.async, arrive on the stage's "conv" mbarrier;
+//   warp 1 (one lane)  MMA issuer: waits for "conv", per stage 4 K steps x 3 UMMAs (M 128, N 128, K 8)
+//                      from shared-memory descriptors into 128 TMEM columns; tcgen05.commit releases
+//                      the stage ("empty") and, after the last one, signals the epilogue;
+//   warps 2-5 again    epilogue: tcgen05.ld 32 lanes x 32 columns at a time, rows = modes so that a
 //                      column store is one coalesced 128-byte line of modes[b][m0..m0+32).
 // Tiles x K splits ~ number of SMs; the split-K partial sums are added in a fixed order by a second
-// kernel (deterministic, no atomics).  HBM-bound by design: 8 bytes of recmat planes per matrix
-// element per call, against 3 x 2 M N K TF32 flop.
+// kernel (deterministic, no atomics).  Per stage the CTA needs 16 KB from HBM, 768 tensor-core cycles
+// (12 UMMAs of 64 cycles) and 48 KB of converter traffic through shared memory: balanced by design.
 #include "rec_tc.cuh"
 
 #include <cuda.h>
@@ -36,6 +39,8 @@ constexpr int kTileBytes = BM * BK * 4;               // 16 KB, one operand plan
 constexpr int kStageBytes = 4 * kTileBytes;           // Rhi, Rlo, Shi, Slo
 constexpr int kThreads = 192;
 constexpr uint32_t kTmemCols = 128;
+constexpr int kLoadBytes = 3 * kTileBytes;            // what TMA brings per stage: recmat raw, Shi, Slo
+constexpr int kConvThreads = 128;                     // warps 2..5
 constexpr size_t kSmemBytes = (size_t)STAGES * kStageBytes + 1024 /* alignment slack */ + 256 /* barriers */;
 static_assert(BK * 4 == 128, "one K block is one 128-byte swizzle row");
 
@@ -50,6 +55,14 @@ __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
 }
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ uint32_t to_tf32(float x) {
+    uint32_t r;
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
+    return r;
 }
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     uint32_t done;
@@ -101,21 +114,26 @@ __device__ __forceinline__ void tmem_ld_32x32(uint32_t taddr, uint32_t (&r)[32])
 // grid (m_tiles, ksplit, n_tiles); block 192; dynamic smem kSmemBytes.
 // dst: modes [B][n_modes] when ksplit == 1, else partials [ksplit][B][n_modes].
 __global__ void __launch_bounds__(kThreads, 1)
-rec_tc_kernel(const __grid_constant__ CUtensorMap mRhi, const __grid_constant__ CUtensorMap mRlo,
+rec_tc_kernel(const __grid_constant__ CUtensorMap mR,
               const __grid_constant__ CUtensorMap mShi, const __grid_constant__ CUtensorMap mSlo,
               float *__restrict__ dst, int n_modes, int B, int nkb, int ksplit) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;          // 128-byte swizzle needs 1024-byte tiles
     const uint32_t bars = base + STAGES * kStageBytes;
-    // barriers: full[s] at +8 s, empty[s] at +8 (STAGES + s), accumulator-ready at +8 (2 STAGES); then the TMEM address
-    const uint32_t bar_acc = bars + 8 * (2 * STAGES);
-    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem_raw + (bars - smem_u32(smem_raw)) + 8 * (2 * STAGES + 1));
+    // barriers: full[s] at +8 s, empty[s] at +8 (STAGES + s), conv[s] at +8 (2 STAGES + s), accumulator-ready at
+    // +8 (3 STAGES); then the TMEM address
+    const uint32_t bar_acc = bars + 8 * (3 * STAGES);
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem_raw + (bars - smem_u32(smem_raw)) + 8 * (3 * STAGES + 1));
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int m_tile = blockIdx.x, ks = blockIdx.y, n_tile = blockIdx.z;
     const int kb_lo = (int)(((long long)ks * nkb) / ksplit), kb_hi = (int)(((long long)(ks + 1) * nkb) / ksplit);
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < STAGES; ++s) { mbar_init(bars + 8 * s, 1); mbar_init(bars + 8 * (STAGES + s), 1); }
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(bars + 8 * s, 1);
+            mbar_init(bars + 8 * (STAGES + s), 1);
+            mbar_init(bars + 8 * (2 * STAGES + s), kConvThreads);
+        }
         mbar_init(bar_acc, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -135,9 +153,8 @@ rec_tc_kernel(const __grid_constant__ CUtensorMap mRhi, const __grid_constant__ 
                 const int s = it % STAGES;
                 const uint32_t full = bars + 8 * s, empty = bars + 8 * (STAGES + s), st = base + s * kStageBytes;
                 mbar_wait(empty, ((it / STAGES) & 1) ^ 1);
-                mbar_expect_tx(full, kStageBytes);
-                tma_load_2d(st + 0 * kTileBytes, &mRhi, full, kb * BK, m_tile * BM);
-                tma_load_2d(st + 1 * kTileBytes, &mRlo, full, kb * BK, m_tile * BM);
+                mbar_expect_tx(full, kLoadBytes);
+                tma_load_2d(st + 0 * kTileBytes, &mR, full, kb * BK, m_tile * BM);      // raw FP32; becomes the hi plane
                 tma_load_2d(st + 2 * kTileBytes, &mShi, full, kb * BK, n_tile * BN);
                 tma_load_2d(st + 3 * kTileBytes, &mSlo, full, kb * BK, n_tile * BN);
             }
@@ -147,8 +164,8 @@ rec_tc_kernel(const __grid_constant__ CUtensorMap mRhi, const __grid_constant__ 
             int it = 0;
             for (int kb = kb_lo; kb < kb_hi; ++kb, ++it) {
                 const int s = it % STAGES;
-                const uint32_t full = bars + 8 * s, empty = bars + 8 * (STAGES + s), st = base + s * kStageBytes;
-                mbar_wait(full, (it / STAGES) & 1);
+                const uint32_t conv = bars + 8 * (2 * STAGES + s), empty = bars + 8 * (STAGES + s), st = base + s * kStageBytes;
+                mbar_wait(conv, (it / STAGES) & 1);                       // TMA landed AND recmat has been split
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll
                 for (int k = 0; k < BK / UK; ++k) {
@@ -163,7 +180,32 @@ rec_tc_kernel(const __grid_constant__ CUtensorMap mRhi, const __grid_constant__ 
             }
             umma_commit(bar_acc);
         }
-    } else {                                                              // ---- epilogue, warps 2..5
+    } else {                                                              // ---- warps 2..5: converters, then epilogue
+        {
+            const int ct = threadIdx.x - 64;                              // 0..127
+            int it = 0;
+            for (int kb = kb_lo; kb < kb_hi; ++kb, ++it) {
+                const int s = it % STAGES;
+                const uint32_t full = bars + 8 * s, conv = bars + 8 * (2 * STAGES + s);
+                mbar_wait(full, (it / STAGES) & 1);
+                float4 *hi = reinterpret_cast<float4 *>(smem_raw + (base - smem_u32(smem_raw)) + s * kStageBytes);
+                float4 *lo = hi + kTileBytes / 16;
+#pragma unroll
+                for (int j = 0; j < kTileBytes / 16 / kConvThreads; ++j) {
+                    const float4 x = hi[j * kConvThreads + ct];
+                    const uint32_t hx = to_tf32(x.x), hy = to_tf32(x.y), hz = to_tf32(x.z), hw = to_tf32(x.w);
+                    float4 l;
+                    l.x = __uint_as_float(to_tf32(x.x - __uint_as_float(hx)));
+                    l.y = __uint_as_float(to_tf32(x.y - __uint_as_float(hy)));
+                    l.z = __uint_as_float(to_tf32(x.z - __uint_as_float(hz)));
+                    l.w = __uint_as_float(to_tf32(x.w - __uint_as_float(hw)));
+                    hi[j * kConvThreads + ct] = make_float4(__uint_as_float(hx), __uint_as_float(hy), __uint_as_float(hz), __uint_as_float(hw));
+                    lo[j * kConvThreads + ct] = l;
+                }
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to the UMMA's reads
+                mbar_arrive(conv);
+            }
+        }
         const int q = warp & 3;                                           // TMEM lane quarter this warp may read
         mbar_wait(bar_acc, 0);
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
@@ -242,11 +284,10 @@ int cuda_rc(cudaError_t e) { return e == cudaErrorMemoryAllocation ? PWFS_ENOMEM
 struct RecTc {
     int device = 0, n_modes = 0, n_slopes = 0, ldp = 0, num_sms = 148;
     EncodeTiledFn enc = nullptr;
-    float *d_Rhi = nullptr, *d_Rlo = nullptr;
     float *d_Shi = nullptr, *d_Slo = nullptr, *d_part = nullptr;
     int b_cap = 0;                  // frames the slope planes / partials are sized for
     size_t part_cap = 0;            // floats in d_part
-    CUtensorMap mRhi, mRlo, mShi, mSlo;
+    CUtensorMap mR, mShi, mSlo;
 };
 
 int rec_tc_create(RecTc **out, const float *d_R, int n_modes, int n_slopes, int ldk, int device, int num_sms) {
@@ -257,17 +298,11 @@ int rec_tc_create(RecTc **out, const float *d_R, int n_modes, int n_slopes, int 
     h->ldp = (n_slopes + BK - 1) / BK * BK;
     h->enc = encode_tiled_fn();
     if (!h->enc) { delete h; return PWFS_EUNSUPPORTED; }
-    const size_t bytes = (size_t)n_modes * h->ldp * sizeof(float);
-    cudaError_t e = cudaMalloc((void **)&h->d_Rhi, bytes);
-    if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_Rlo, bytes);
-    if (e == cudaSuccess) {
-        split_tf32_kernel<<<dim3((h->ldp + 255) / 256, n_modes), 256>>>(d_R, (size_t)ldk, n_slopes, h->ldp, h->d_Rhi, h->d_Rlo);
-        e = cudaGetLastError();
-    }
-    if (e == cudaSuccess) e = cudaDeviceSynchronize();
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(rec_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+    // recmat itself is the TMA source: [n_modes][ldk] FP32, ldk % 4 == 0 (16-byte row pitch), zero padded; K blocks
+    // beyond ldk are filled with zeros by TMA
+    cudaError_t e = cudaFuncSetAttribute(rec_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
     if (e != cudaSuccess) { int rc = cuda_rc(e); rec_tc_destroy(h); return rc; }
-    if (!make_map(h->enc, &h->mRhi, h->d_Rhi, n_modes, h->ldp) || !make_map(h->enc, &h->mRlo, h->d_Rlo, n_modes, h->ldp)) {
+    if (!make_map(h->enc, &h->mR, d_R, n_modes, ldk)) {
         rec_tc_destroy(h);
         return PWFS_ECUDA;
     }
@@ -308,7 +343,7 @@ int rec_tc_run(RecTc *h, const float *d_slopes, int B, float *d_modes, cudaStrea
     split_tf32_kernel<<<dim3((h->ldp + 255) / 256, B), 256, 0, st>>>(d_slopes, (size_t)h->n_slopes, h->n_slopes, h->ldp,
                                                                     h->d_Shi, h->d_Slo);
     rec_tc_kernel<<<dim3(m_tiles, ksplit, n_tiles), kThreads, kSmemBytes, st>>>(
-        h->mRhi, h->mRlo, h->mShi, h->mSlo, ksplit > 1 ? h->d_part : d_modes, h->n_modes, B, nkb, ksplit);
+        h->mR, h->mShi, h->mSlo, ksplit > 1 ? h->d_part : d_modes, h->n_modes, B, nkb, ksplit);
     if (ksplit > 1) {
         const size_t n = (size_t)B * h->n_modes;
         splitk_sum_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(h->d_part, n, ksplit, d_modes);
@@ -318,6 +353,6 @@ int rec_tc_run(RecTc *h, const float *d_slopes, int B, float *d_modes, cudaStrea
 
 void rec_tc_destroy(RecTc *h) {
     if (!h) return;
-    cudaFree(h->d_Rhi); cudaFree(h->d_Rlo); cudaFree(h->d_Shi); cudaFree(h->d_Slo); cudaFree(h->d_part);
+    cudaFree(h->d_Shi); cudaFree(h->d_Slo); cudaFree(h->d_part);
     delete h;
 }
