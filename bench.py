@@ -346,7 +346,8 @@ class DryRunSensor:
         pass
 
     def get_timing(self):
-        return {k: 0.0 for k in ("xpass", "ypass", "xrebin", "slopes")}, {k: 0 for k in ("xpass", "ypass", "xrebin", "slopes")}
+        ks = ("xpass", "ypass", "xrebin", "slopes", "fused")
+        return {k: 0.0 for k in ks}, {k: 0 for k in ks}
 
     def close(self):
         pass
@@ -394,7 +395,7 @@ def roofline_numbers(cfg, geo, B, steps, ms_per_step, kernel_ms, launches, peak_
     dom = max(kernel_ms, key=kernel_ms.get)
     n_launch = max(1, launches[dom])
     units_per_launch = B * K * steps / n_launch                          # modulation points per launch
-    share = {"xpass": 0.5, "ypass": 0.5}.get(dom, 0.0)
+    share = {"xpass": 0.5, "ypass": 0.5, "fused": 1.0}.get(dom, 0.0)
     flops_per_launch = share * nominal_flops_per_modpoint(M) * units_per_launch
     avg_launch_s = kernel_ms[dom] * 1e-3 / n_launch
     achieved = flops_per_launch / avg_launch_s / 1e12 if avg_launch_s > 0 else 0.0

@@ -173,17 +173,21 @@ int pwfs_supported_grid(int32_t m_grid);
 /* Scheduling knobs (0 keeps the built-in heuristic): frames processed per
  * kernel chunk, and the number of ways the K modulation points are split
  * across warps in the column pass.  Results do not depend on them beyond FP32
- * summation order. */
+ * summation order.  Non-zero knobs also select the two-kernel path where the
+ * fused small-grid kernel would otherwise run (M = 128, N <= 64, n_sub <= 32,
+ * batches of up to ~16 SMs' worth of x-tilts; environment PWFS_SMALL=0 / 1
+ * forces it off / on whenever the geometry allows). */
 int pwfs_set_schedule(pwfs_t *h, int32_t frames_per_chunk, int32_t k_split);
 
 /* Instrumentation.  Kernel classes: 0 = row pass (phasor + x-convolution),
  * 1 = column pass (y-convolution + |E|^2 accumulation + y-rebin),
- * 2 = x-rebin, 3 = slopes.  pwfs_set_timing(h, 1) makes pwfs_run bracket every
+ * 2 = x-rebin, 3 = slopes, 4 = the fused single-kernel path that serves small
+ * batches on the M = 128 grid (all of the above in one launch).  pwfs_set_timing(h, 1) makes pwfs_run bracket every
  * kernel with CUDA events on the caller's stream; pwfs_get_timing then
  * synchronises those events and returns, for everything run since timing was
  * enabled (or last read), the summed device time per class in milliseconds and
  * the launch count per class.  launches[] is counted even when timing is off. */
-#define PWFS_NUM_KERNEL_CLASSES 4
+#define PWFS_NUM_KERNEL_CLASSES 5
 int pwfs_set_timing(pwfs_t *h, int32_t enable);
 int pwfs_get_timing(pwfs_t *h, float ms[PWFS_NUM_KERNEL_CLASSES],
                     int64_t launches[PWFS_NUM_KERNEL_CLASSES]);

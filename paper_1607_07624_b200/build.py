@@ -21,7 +21,7 @@ UNITS = [(os.path.join(CSRC, n), [], n[:-3] + ".o")
          for n in ("pwfs_api.cu", "atmo_api.cu", "chain_api.cu", "rec_tc.cu", "psf_api.cu", "sh_api.cu", "peak_fp32.cu", "dm_api.cu")] + \
         [(os.path.join(CSRC, "pwfs_inst.cu"), [f"-DPWFS_INST_R1={r}"], f"pwfs_inst_r{r}.o") for r in GRID_R1]
 SOURCES = sorted({u[0] for u in UNITS})
-HEADERS = [os.path.join(CSRC, n) for n in ("pwfs_kernels.cuh", "pwfs_dft.cuh", "pwfs_launch.cuh", "rec_tc.cuh", "device_guard.cuh")] + \
+HEADERS = [os.path.join(CSRC, n) for n in ("pwfs_kernels.cuh", "pwfs_dft.cuh", "pwfs_launch.cuh", "pwfs_small.cuh", "rec_tc.cuh", "device_guard.cuh")] + \
           [os.path.join(ROOT, "include", n) for n in ("pwfs.h", "pwfs_atmo.h", "pwfs_chain.h", "pwfs_psf.h", "pwfs_sh.h", "pwfs_dm.h")]
 OBJDIR = os.path.join(HERE, "build")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

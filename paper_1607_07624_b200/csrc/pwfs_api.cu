@@ -54,6 +54,9 @@ struct pwfs {
     float2 *T = nullptr; size_t T_elems = 0;
     float *colbin = nullptr; size_t colbin_elems = 0;
     float *nsum = nullptr; size_t nsum_elems = 0;      // [F][D] per-column sums over valid detector pixels
+    // fused small-grid kernel (M = 128): partial frames, per-frame completion counters
+    float *spart = nullptr; unsigned *scount = nullptr; size_t small_frames = 0;
+    int small_mode = -1;                               // PWFS_SMALL: 0 never, 1 whenever possible, -1 by batch size
     // host-buffer path
     cudaStream_t hstream = nullptr, in_stream = nullptr, out_stream = nullptr;   // compute, H2D, D2H
     std::vector<cudaEvent_t> in_ev, done_ev, tail_ev;                            // per chunk
@@ -68,8 +71,8 @@ struct pwfs {
     int timing = 0;
     std::vector<TimedSpan> spans;
     std::vector<cudaEvent_t> event_pool;
-    float ms_acc[PWFS_NUM_KERNEL_CLASSES] = {0, 0, 0, 0};
-    int64_t launches[PWFS_NUM_KERNEL_CLASSES] = {0, 0, 0, 0};
+    float ms_acc[PWFS_NUM_KERNEL_CLASSES] = {0, 0, 0, 0, 0};
+    int64_t launches[PWFS_NUM_KERNEL_CLASSES] = {0, 0, 0, 0, 0};
     int last_cuda = 0;
     int last_kernel = -1;                    // kernel class of the last launch that failed, -1 none
     bool debug_only = false;                 // pwfs_debug_create with relaxed window checks: pwfs_debug_intensity only
@@ -472,6 +475,12 @@ static int create_impl(const pwfs_params *p, const pwfs_ext *x, int s_debug, pwf
         h->x_resident_ctas = h->num_sms * std::max(1, nx);
         h->y_resident_warps = h->num_sms * std::max(1, ny) * L.WPB_Y;
     }
+    if (!rc && L.sfn) {
+        e = cudaFuncSetAttribute(L.sfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem_s);
+        if (e != cudaSuccess) { h->last_cuda = (int)e; rc = PWFS_ECUDA; }
+        const char *sm = std::getenv("PWFS_SMALL");
+        if (sm && (sm[0] == '0' || sm[0] == '1')) h->small_mode = sm[0] - '0';
+    }
     if (!rc) {
         const char *env = std::getenv("PWFS_SCRATCH_MB");
         if (env && std::atol(env) > 0) h->scratch_budget = (size_t)std::atol(env) << 20;
@@ -490,6 +499,8 @@ void pwfs_destroy(pwfs_t *h) {
     if (h->T) cudaFree(h->T);
     if (h->colbin) cudaFree(h->colbin);
     if (h->nsum) cudaFree(h->nsum);
+    if (h->spart) cudaFree(h->spart);
+    if (h->scount) cudaFree(h->scount);
     if (h->d_phase) cudaFree(h->d_phase);
     if (h->d_frames) cudaFree(h->d_frames);
     if (h->d_slopes) cudaFree(h->d_slopes);
@@ -640,10 +651,54 @@ static int ensure_chunk_events(pwfs_t *h, size_t n_chunks) {
     return PWFS_OK;
 }
 
+// The fused kernel serves M = 128 sensors whose pupil, window columns and detector fit its shared-memory plan, when the
+// caller has not pinned the schedule; by default for batches that leave the two-kernel path launch-bound.
+static bool small_applies(const pwfs_t *h, int B) {
+    const DevTables &t = h->tab;
+    if (!h->L.launch_s || h->small_mode == 0 || h->user_fpc > 0 || h->user_ksplit > 0) return false;
+    if (t.N > 64 || t.ncols > 128 || t.D > 64) return false;
+    if (h->small_mode == 1) return true;
+    return (long long)B * t.K <= 16LL * h->num_sms;
+}
+
+static int ensure_small(pwfs_t *h, int B, cudaStream_t st, bool check_capture) {
+    if ((size_t)B <= h->small_frames) return PWFS_OK;
+    if (check_capture) {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(st, &cs) == cudaSuccess && cs != cudaStreamCaptureStatusNone) return PWFS_EINVAL;
+    }
+    const DevTables &t = h->tab;
+    if (h->spart) cudaFree(h->spart);
+    if (h->scount) cudaFree(h->scount);
+    h->spart = nullptr; h->scount = nullptr; h->small_frames = 0;
+    cudaError_t e = cudaMalloc((void **)&h->spart, (size_t)B * t.K * t.D * t.D * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&h->scount, (size_t)B * sizeof(unsigned));
+    if (e == cudaSuccess) e = cudaMemset(h->scount, 0, (size_t)B * sizeof(unsigned));
+    if (e != cudaSuccess) { h->last_cuda = (int)e; return e == cudaErrorMemoryAllocation ? PWFS_ENOMEM : PWFS_ECUDA; }
+    h->small_frames = (size_t)B;
+    return PWFS_OK;
+}
+
+static int run_small(pwfs_t *h, const float *d_phase, int B, float *d_frames, float *d_slopes, cudaStream_t st) {
+    const DevTables &t = h->tab;
+    const size_t NN = (size_t)t.N * t.N, DD = (size_t)t.D * t.D, SS = (size_t)2 * t.n_valid;
+    const double m4 = h->quarter ? std::pow((double)t.M, 4.0) : 1.0;
+    for (int f0 = 0; f0 < B; f0 += 65535) {                        // grid.y limit
+        const int Fc = std::min(65535, B - f0);
+        SpanGuard g(h, st, 4);
+        h->L.launch_s(dim3(t.K, Fc), st, t, d_phase + (size_t)f0 * NN, h->spart + (size_t)f0 * t.K * DD,
+                      h->scount + f0, d_frames + (size_t)f0 * DD, d_slopes ? d_slopes + (size_t)f0 * SS : nullptr,
+                      (float)(1.0 / ((double)t.K * m4)));
+        if (int rc = check_launch(h, 4)) return rc;
+    }
+    return PWFS_OK;
+}
+
 int pwfs_reserve(pwfs_t *h, int32_t B) {
     if (!h || B < 1) return PWFS_EINVAL;
     DeviceGuard dg(h->device);
     PWFS_CUDA(h, dg.err);
+    if (small_applies(h, B)) return ensure_small(h, B, nullptr, false);
     int F, ks;
     schedule(h, B, &F, &ks);
     int rc = ensure_scratch(h, F, ks);
@@ -664,6 +719,10 @@ int pwfs_run(pwfs_t *h, const float *d_phase, int32_t B, float *d_frames, float 
     PWFS_CUDA(h, dg.err);
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const DevTables &t = h->tab;
+    if (small_applies(h, B)) {                                     // M = 128, small batch: the whole path in one kernel
+        if (int rc = ensure_small(h, B, st, true)) return rc;
+        return run_small(h, d_phase, B, d_frames, d_slopes, st);
+    }
     int F, ks;
     schedule(h, B, &F, &ks);
     int rc = ensure_scratch(h, F, ks, st, true);
@@ -748,6 +807,17 @@ int pwfs_run_host(pwfs_t *h, const float *h_phase, int32_t B, float *h_frames, f
         if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_slopes, (size_t)B * SS * sizeof(float));
         if (e != cudaSuccess) { h->last_cuda = (int)e; return e == cudaErrorMemoryAllocation ? PWFS_ENOMEM : PWFS_ECUDA; }
         h->d_cap_frames = (size_t)B;
+    }
+    if (small_applies(h, B)) {                                     // one fused launch between the two copies
+        int rc = ensure_small(h, B, h->hstream, false);
+        if (rc) return rc;
+        PWFS_CUDA(h, cudaMemcpyAsync(h->d_phase, h_phase, (size_t)B * NN * sizeof(float), cudaMemcpyHostToDevice, h->hstream));
+        if ((rc = run_small(h, h->d_phase, B, h->d_frames, h_slopes ? h->d_slopes : nullptr, h->hstream))) return rc;
+        PWFS_CUDA(h, cudaMemcpyAsync(h_frames, h->d_frames, (size_t)B * DD * sizeof(float), cudaMemcpyDeviceToHost, h->hstream));
+        if (h_slopes)
+            PWFS_CUDA(h, cudaMemcpyAsync(h_slopes, h->d_slopes, (size_t)B * SS * sizeof(float), cudaMemcpyDeviceToHost, h->hstream));
+        PWFS_CUDA(h, cudaStreamSynchronize(h->hstream));
+        return PWFS_OK;
     }
     if (!h->in_stream) PWFS_CUDA(h, cudaStreamCreateWithFlags(&h->in_stream, cudaStreamNonBlocking));
     if (!h->out_stream) PWFS_CUDA(h, cudaStreamCreateWithFlags(&h->out_stream, cudaStreamNonBlocking));

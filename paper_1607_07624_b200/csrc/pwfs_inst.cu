@@ -1,6 +1,7 @@
 // pwfs_inst.cu -- the row-pass / column-pass kernels of ONE grid size, M = 32 * PWFS_INST_R1, both
 // mask variants.  build.py compiles this file once per R1 of PWFS_FOR_EACH_R1 (pwfs_launch.cuh).
 #include "pwfs_launch.cuh"
+#include "pwfs_small.cuh"
 
 #ifndef PWFS_INST_R1
 #define PWFS_INST_R1 4   // a bare `nvcc -c` of this file still gives a valid object
@@ -44,6 +45,11 @@ void launch_y_t(dim3 grid, cudaStream_t st, const DevTables &t, const float2 *T,
     ypass_kernel<CY, QM><<<grid, 32 * CY::WPB_Y, CY::smem_y, st>>>(t, T, colbin, ksplit);
 }
 template <bool QM>
+void launch_s_t(dim3 grid, cudaStream_t st, const DevTables &t, const float *phase, float *part, unsigned *counter,
+                float *frames, float *slopes, float scale) {
+    small_kernel<QM><<<grid, 256, QM ? SmallCfg::smem_q : SmallCfg::smem_t, st>>>(t, phase, part, counter, frames, slopes, scale);
+}
+template <bool QM>
 Launcher make() {
     Launcher l;
     l.R1 = C::R1; l.NB = CY::NB; l.WPB_X = C::WPB_X; l.WPB_Y = CY::WPB_Y; l.RPC = C::RPC;
@@ -52,6 +58,11 @@ Launcher make() {
     l.yfn = (const void *)ypass_kernel<CY, QM>;
     l.launch_x = launch_x_t<QM>;
     l.launch_y = launch_y_t<QM>;
+#if PWFS_INST_R1 == 4
+    l.sfn = (const void *)small_kernel<QM>;
+    l.smem_s = QM ? SmallCfg::smem_q : SmallCfg::smem_t;
+    l.launch_s = launch_s_t<QM>;
+#endif
     return l;
 }
 

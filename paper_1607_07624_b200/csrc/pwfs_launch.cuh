@@ -65,6 +65,10 @@ struct Launcher {
     const void *xfn, *yfn;
     void (*launch_x)(dim3, cudaStream_t, const DevTables &, const float *, float2 *, int);
     void (*launch_y)(dim3, cudaStream_t, const DevTables &, const float2 *, float *, int);
+    // M = 128 only (else nullptr): the whole path in one kernel, pwfs_small.cuh.  grid (K, F)
+    const void *sfn = nullptr;
+    size_t smem_s = 0;
+    void (*launch_s)(dim3, cudaStream_t, const DevTables &, const float *, float *, unsigned *, float *, float *, float) = nullptr;
 };
 
 // quarter = the mask shift is exactly M/4 and there is no field stop: kernels with the table-free

@@ -17,8 +17,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("PWFS_LIB_PATH") or os.path.join(_HERE, "libpwfs.so")
 
 PWFS_OK, PWFS_EINVAL, PWFS_ENOMEM, PWFS_ECUDA, PWFS_EUNSUPPORTED = 0, -1, -2, -3, -4
-NUM_KERNEL_CLASSES = 4
-KERNEL_CLASSES = ("xpass", "ypass", "xrebin", "slopes")
+NUM_KERNEL_CLASSES = 5
+KERNEL_CLASSES = ("xpass", "ypass", "xrebin", "slopes", "fused")
 
 EXPORTS = ("pwfs_create", "pwfs_create_ex", "pwfs_info", "pwfs_valid_mask", "pwfs_run", "pwfs_run_host",
            "pwfs_destroy", "pwfs_strerror", "pwfs_last_cuda_error", "pwfs_supported_grid",

@@ -85,6 +85,46 @@ def test_repeated_frames_and_calls_are_bit_identical(torch_cuda):
             assert torch.equal(fr[i], fr[i % 2]) and torch.equal(sl[i], sl[i % 2])
 
 
+@pytest.mark.parametrize("N,M,ns,K,r,kw", [
+    (64, 128, 16, 12, 3.0, {}),                                   # cfg1 geometry, quarter mask
+    (60, 128, 23, 5, 1.5, {}),                                    # margins, non-integer binning, odd K
+    (50, 128, 7, 1, 0.0, {}),                                     # unmodulated, ragged N
+    (48, 128, 12, 7, 2.0, dict(mask_shift_px=30, mod_angle0=0.4, illum_thresh=0.3, slope_norm=1)),   # table mask
+    (64, 128, 32, 9, 2.5, {}),                                    # largest detector the kernel takes (D = 64)
+])
+def test_fused_small_grid_kernel_against_oracle_and_two_kernel_path(torch_cuda, monkeypatch, N, M, ns, K, r, kw):
+    """M = 128: small batches run the whole path in ONE kernel (pwfs_small.cuh).  It must match the oracle at the
+    parity bar, and the two-kernel path (PWFS_SMALL=0) to FP32 summation order; launches are counted per class."""
+    from paper_1607_07624_b200.pwfs import PWFS
+    torch = torch_cuda
+    rng = np.random.default_rng(N * 3 + K)
+    c = (np.arange(N) - (N - 1) / 2.0)
+    X, Y = np.meshgrid(c, c)
+    A = ((np.hypot(X, Y) <= N / 2.0) & (np.hypot(X, Y) >= 0.1 * N)).astype(np.float32)
+    phase = (rng.standard_normal((5, N, N)) * 3.0).astype(np.float32)
+    phase[1] = wl.tilt_phase(N, 0.3, -0.2)
+    monkeypatch.setenv("PWFS_SMALL", "1")
+    _run_both(torch, A, M, r, K, ns, phase, **kw)                  # fused kernel vs oracle
+    with PWFS(A, M, r, K, ns, **kw) as fused:
+        fused.get_timing()
+        f1, s1 = fused.run(torch.from_numpy(phase).cuda())
+        f1b, s1b = fused.run(torch.from_numpy(phase).cuda())       # second call: completion counters were reset
+        fh, sh = fused.run_host(phase)
+        _, launches = fused.get_timing()
+        assert launches["fused"] == 3 and launches["xpass"] == 0 and launches["ypass"] == 0
+        assert torch.equal(f1, f1b) and torch.equal(s1, s1b)
+        assert np.array_equal(fh, f1.cpu().numpy()) and np.array_equal(sh, s1.cpu().numpy())
+        f1n, _ = fused.run(torch.from_numpy(phase).cuda(), want_slopes=False)
+        assert torch.equal(f1, f1n)
+    monkeypatch.setenv("PWFS_SMALL", "0")
+    with PWFS(A, M, r, K, ns, **kw) as two:
+        f2, s2 = two.run(torch.from_numpy(phase).cuda())
+        _, launches = two.get_timing()
+        assert launches["fused"] == 0 and launches["xpass"] >= 1
+    assert ((f1 - f2).abs().amax(dim=(1, 2)) <= 2e-6 * f2.abs().amax(dim=(1, 2))).all()
+    assert (s1 - s2).abs().max() <= 1e-5
+
+
 def test_full_resolution_intensity_before_rebinning(torch_cuda):
     """The un-rebinned I = mean_k |E_k|^2 of the hot path's own kernels (test-only export pwfs_debug_intensity)
     against the oracle's orc_intensity on the whole M x M grid, M = 2N so that every column is computed."""
@@ -204,11 +244,12 @@ def test_schedule_knobs_do_not_change_results(torch_cuda):
         sensor.close()
 
 
-def test_host_buffer_pipeline_with_several_chunks(torch_cuda):
+def test_host_buffer_pipeline_with_several_chunks(torch_cuda, monkeypatch):
     """B >= 16: pwfs_run_host works in a short first chunk and three large ones on three streams (copy-in, kernels,
     tail + copy-out); every frame must come out as on the device path (FP32 summation order aside)."""
     from paper_1607_07624_b200.pwfs import from_config
     torch = torch_cuda
+    monkeypatch.setenv("PWFS_SMALL", "0")                          # cfg1 would otherwise take the fused single-kernel path
     cfg = wl.CONFIGS["cfg1_tiny"]
     phase = np.concatenate([wl.phase_batch(cfg, steps=10)] * 5)[:47]                # ragged: 2 + 15 + 15 + 15
     phase = np.ascontiguousarray(phase + np.arange(47, dtype=np.float32)[:, None, None] * 0.01)   # all frames differ
@@ -231,6 +272,7 @@ def test_host_buffer_pipeline_when_scratch_holds_fewer_frames_than_the_short_fir
     cfg = wl.CONFIGS["cfg1_tiny"]
     # T of one cfg1 frame = KX (7) x M (128) x NP (64) x 8 B = 458 752 B: a 1 MiB budget holds 2 frames, B/16 = 6
     monkeypatch.setenv("PWFS_SCRATCH_MB", "1")
+    monkeypatch.setenv("PWFS_SMALL", "0")                          # the chunked two-kernel pipeline is what is under test
     B = 100
     phase = np.concatenate([wl.phase_batch(cfg, steps=10)] * 10)
     phase = np.ascontiguousarray(phase + np.arange(B, dtype=np.float32)[:, None, None] * 0.01)
@@ -240,7 +282,7 @@ def test_host_buffer_pipeline_when_scratch_holds_fewer_frames_than_the_short_fir
         fd, sd = small.run(torch.from_numpy(phase).cuda())
         torch.cuda.synchronize()
     monkeypatch.delenv("PWFS_SCRATCH_MB")
-    with from_config(cfg) as big:
+    with from_config(cfg) as big:                                  # reference: one chunk, two-kernel path
         fr, sr = big.run(torch.from_numpy(phase).cuda())
         torch.cuda.synchronize()
     fr, sr = fr.cpu().numpy(), sr.cpu().numpy()
