@@ -198,11 +198,8 @@ def bench_stages(cfg, dev, phase, frames, flush, reps: int = 5) -> dict:
         if B >= 24 and os.environ.get("PWFS_REC_TC", "1") != "0":   # chain_api.cu: batches run the tcgen05 TF32x3 kernel
             row = hbm_row(ms, n_modes * ns * 4 + B * ns * 4 + B * n_modes * 4, 3,
                           f"{n_modes} modes x {ns} slopes x {B} frames, tcgen05 TF32x3 (FP32 bar): algorithmic bytes = "
-                          "recmat once + slopes in + modes out; the kernel streams the two TF32 planes of recmat "
-                          "(8 B per element), see plane_frac")
-            ldp = -(-ns // 32) * 32
-            row["plane_bytes"] = int(2 * n_modes * ldp * 4)
-            row["plane_frac"] = row["plane_bytes"] / (ms * 1e-3) / 1e9 / hbm
+                          "recmat once + slopes in + modes out; the kernel streams recmat once as FP32 (TMA) and splits it "
+                          "into TF32 hi/lo planes in tensor memory (A operand from TMEM), slope planes from a split kernel")
             row["tf32_tflops"] = 3 * 2.0 * B * n_modes * ns / (ms * 1e-3) / 1e12
             out["f2_rec_batch"] = row
         else:
@@ -280,6 +277,54 @@ def bench_stages(cfg, dev, phase, frames, flush, reps: int = 5) -> dict:
                                             "note": "the same step captured 10 times (consecutive step indices) in one CUDA "
                                                     "graph; device time per step over 50 steps = 5 replays"}
             del g
+        # the CLOSED loop of PAPER.md Table 2 (rec -> INT -> DM -> prop.add_layer): the DM layer of the delayed integrator
+        # command is added to the propagated phase before the sensor; n_cl modes drive n_cl actuators
+        n_cl = min(1024, n_modes)
+        Rc = rng.standard_normal((n_cl, 2 * nv), dtype=np.float32) / nv
+        ifc = rng.standard_normal((n_cl, pix.size), dtype=np.float32) * 1e-3
+        with Atmosphere(**{k: v for k, v in atm.items() if k != "dt"}, device=dev.index) as a, \
+                from_config(cfg, device=dev.index) as sensor, \
+                CCD(D, n_inst=n_inst, gain=n_ph / float((Apup.astype(np.float64) ** 2).sum()), quantum_eff=0.32,
+                    photon_noise=True, readout_noise=True, readout_level=1.0, seed=1, device=dev.index) as ccd, \
+                SlopeComputer(valid, sn=np.zeros(2 * nv, np.float32), device=dev.index) as sc, \
+                Reconstructor(Rc, device=dev.index) as rec, \
+                Integrator(np.full(n_cl, -0.3, np.float32), delay=1, device=dev.index) as integ, \
+                DeformableMirror(ifc, pix, N, device=dev.index) as dm:
+            if n_inst == 1:                                    # single-conjugate loop: one sensor drives the mirror
+                ph = torch.empty((1, N, N), dtype=torch.float32, device=dev)
+                fr = torch.empty((1, D, D), dtype=torch.float32, device=dev)
+                px, s1 = torch.empty_like(fr), torch.empty((1, 2 * nv), dtype=torch.float32, device=dev)
+                md = torch.empty((1, n_cl), dtype=torch.float32, device=dev)
+                cmd = torch.zeros((1, n_cl), dtype=torch.float32, device=dev)
+                sensor.reserve(1)
+
+                def cl_step(i, st=None):
+                    a.propagate(i, 1, atm["dt"], out=ph, stream=st)
+                    dm.apply(cmd, ph, alpha=1.0, beta=1.0, stream=st)
+                    sensor.run(ph, fr, want_slopes=False, stream=st)
+                    ccd.run(fr, first_out_frame=i, out=px, stream=st)
+                    sc.run(px, out=s1, stream=st)
+                    rec.run(s1, out=md, stream=st)
+                    integ.step(md.reshape(-1), out=cmd, stream=st)
+                for i in range(3):
+                    cl_step(i)
+                side = torch.cuda.Stream(dev)
+                side.wait_stream(stream)
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=side):
+                    for i in range(10):
+                        cl_step(3 + i, side)
+                torch.cuda.synchronize(dev)
+                ms_e = timed(lambda: [cl_step(20 + i) for i in range(50)]) / 50
+                ms_g = timed(lambda: [g.replay() for _ in range(5)]) / 50
+                out["closed_loop_step"] = {"ms": ms_e, "ms_cuda_graph": ms_g, "steps_per_s": 1e3 / ms_g, "launches": 11,
+                                           "modes": n_cl,
+                                           "note": "PASSATA's SCAO loop, every object on the device: propagate -> + DM layer "
+                                                   "(influence-function multiply, 2 launches) -> pyramid (4) -> CCD -> "
+                                                   "slopes -> modes (GEMV) -> integrator (delay 1); eager / one CUDA graph of "
+                                                   "10 steps, device time per step over 50 steps"}
+                del g
+        del Rc, ifc
     del R
     # f4: PSF camera on the same grid, Shack-Hartmann on the same pupil
     with PsfCamera(wl.make_pupil(cfg), M, phase_scale=0.45, device=dev.index) as cam:

@@ -11,18 +11,21 @@
 //
 // Kernel (one 128 x 128 output tile of one K split per CTA, 192 threads):
 //   warp 0 (one lane)  TMA producer: three 128 x 32 FP32 boxes per stage (recmat raw, Shi, Slo;
-//                      128-byte swizzle) into a 3-stage ring, completion on the stage's "full" mbarrier;
-//   warps 2-5          converters: read the raw recmat tile, write hi = tf32(x) back in place and
-//                      lo = tf32(x - hi) into the stage's fourth tile (element-wise, so the swizzle
-//                      does not matter), fence.proxy.async, arrive on the stage's "conv" mbarrier;
-//   warp 1 (one lane)  MMA issuer: waits for "conv", per stage 4 K steps x 3 UMMAs (M 128, N 128, K 8)
-//                      from shared-memory descriptors into 128 TMEM columns; tcgen05.commit releases
-//                      the stage ("empty") and, after the last one, signals the epilogue;
+//                      128-byte swizzle) into a 4-stage ring, completion on the stage's "full" mbarrier;
+//   warps 2-5          converters: thread = row of the recmat tile; reads its 32 raw values (undoing the
+//                      swizzle in the address), hi = tf32(x), lo = tf32(x - hi), and writes both planes
+//                      into TENSOR MEMORY (tcgen05.st 32x32b.x32: lane = row, column = k), then arrives on
+//                      the stage's "conv" mbarrier;
+//   warp 1 (one lane)  MMA issuer: waits for "conv", per stage 4 K steps x 3 UMMAs (M 128, N 128, K 8),
+//                      A (recmat hi / lo) from tensor memory, B (slope planes) from shared-memory
+//                      descriptors, into 128 TMEM columns; tcgen05.commit releases the stage ("empty")
+//                      and, after the last one, signals the epilogue;
 //   warps 2-5 again    epilogue: tcgen05.ld 32 lanes x 32 columns at a time, rows = modes so that a
 //                      column store is one coalesced 128-byte line of modes[b][m0..m0+32).
 // Tiles x K splits ~ number of SMs; the split-K partial sums are added in a fixed order by a second
 // kernel (deterministic, no atomics).  Per stage the CTA needs 16 KB from HBM, 768 tensor-core cycles
-// (12 UMMAs of 64 cycles) and 48 KB of converter traffic through shared memory: balanced by design.
+// (12 UMMAs of 64 cycles) and 64 KB of shared-memory reads (16 KB by the converters, 48 KB of B operands):
+// with recmat's planes in tensor memory the shared-memory port is no longer the limiter.
 #include "rec_tc.cuh"
 
 #include <cuda.h>
@@ -34,12 +37,13 @@
 
 namespace {
 
-constexpr int BM = 128, BN = 128, BK = 32, UK = 8, STAGES = 3;
+constexpr int BM = 128, BN = 128, BK = 32, UK = 8, STAGES = 4;
 constexpr int kTileBytes = BM * BK * 4;               // 16 KB, one operand plane of one stage
-constexpr int kStageBytes = 4 * kTileBytes;           // Rhi, Rlo, Shi, Slo
+constexpr int kStageBytes = 3 * kTileBytes;           // recmat raw, Shi, Slo
 constexpr int kThreads = 192;
-constexpr uint32_t kTmemCols = 128;
-constexpr int kLoadBytes = 3 * kTileBytes;            // what TMA brings per stage: recmat raw, Shi, Slo
+constexpr uint32_t kAccCols = 128;                    // accumulator: TMEM columns [0, 128)
+constexpr uint32_t kTmemCols = 512;                   // + per stage 32 columns of recmat hi and 32 of lo: 128 + 4 * 64 = 384 -> 512
+constexpr int kLoadBytes = 3 * kTileBytes;            // what TMA brings per stage
 constexpr int kConvThreads = 128;                     // warps 2..5
 constexpr size_t kSmemBytes = (size_t)STAGES * kStageBytes + 1024 /* alignment slack */ + 256 /* barriers */;
 static_assert(BK * 4 == 128, "one K block is one 128-byte swizzle row");
@@ -59,11 +63,11 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-__device__ __forceinline__ uint32_t to_tf32(float x) {
-    uint32_t r;
-    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
-    return r;
-}
+// Nearest TF32 value (10 mantissa bits, low 13 bits zero) by integer arithmetic: add half a TF32 ulp to the magnitude
+// and clear the low bits.  Two ALU instructions; cvt.rna.tf32.f32 is emulated on sm_100a with ~6 (ncu: the converter
+// warps were the pipeline's bottleneck with it).  Differs from cvt.rna only on exact ties (away from zero both) and
+// leaves Inf / NaN what they are.
+__device__ __forceinline__ uint32_t to_tf32(float x) { return (__float_as_uint(x) + 0x1000u) & 0xFFFFE000u; }
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     uint32_t done;
     do {
@@ -94,6 +98,26 @@ __device__ __forceinline__ void umma_tf32(uint32_t tmem_d, uint64_t adesc, uint6
         "setp.ne.b32 p, %4, 0;\n"
         "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n"
         "}\n" ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(kIdesc), "r"(accumulate) : "memory");
+}
+// A operand in tensor memory (lane = row of the 128 x 8 tile, one TF32 value per 32-bit column), B from shared memory
+__device__ __forceinline__ void umma_tf32_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t bdesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n"
+        "}\n" ::"r"(tmem_d), "r"(tmem_a), "l"(bdesc), "r"(kIdesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void tmem_st_32x32(uint32_t taddr, const uint32_t (&r)[32]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
+        "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};"
+        ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
+          "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]),
+          "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]),
+          "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
+        : "memory");
 }
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
@@ -154,9 +178,9 @@ rec_tc_kernel(const __grid_constant__ CUtensorMap mR,
                 const uint32_t full = bars + 8 * s, empty = bars + 8 * (STAGES + s), st = base + s * kStageBytes;
                 mbar_wait(empty, ((it / STAGES) & 1) ^ 1);
                 mbar_expect_tx(full, kLoadBytes);
-                tma_load_2d(st + 0 * kTileBytes, &mR, full, kb * BK, m_tile * BM);      // raw FP32; becomes the hi plane
-                tma_load_2d(st + 2 * kTileBytes, &mShi, full, kb * BK, n_tile * BN);
-                tma_load_2d(st + 3 * kTileBytes, &mSlo, full, kb * BK, n_tile * BN);
+                tma_load_2d(st + 0 * kTileBytes, &mR, full, kb * BK, m_tile * BM);      // raw FP32 recmat
+                tma_load_2d(st + 1 * kTileBytes, &mShi, full, kb * BK, n_tile * BN);
+                tma_load_2d(st + 2 * kTileBytes, &mSlo, full, kb * BK, n_tile * BN);
             }
         }
     } else if (warp == 1) {
@@ -167,14 +191,14 @@ rec_tc_kernel(const __grid_constant__ CUtensorMap mR,
                 const uint32_t conv = bars + 8 * (2 * STAGES + s), empty = bars + 8 * (STAGES + s), st = base + s * kStageBytes;
                 mbar_wait(conv, (it / STAGES) & 1);                       // TMA landed AND recmat has been split
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                const uint32_t a_hi = tmem + kAccCols + (uint32_t)s * 64u, a_lo = a_hi + 32u;
 #pragma unroll
                 for (int k = 0; k < BK / UK; ++k) {
                     const uint32_t ko = k * UK * 4;                      // 32 bytes along the swizzled row
-                    const uint64_t rhi = smem_desc(st + 0 * kTileBytes + ko), rlo = smem_desc(st + 1 * kTileBytes + ko);
-                    const uint64_t shi = smem_desc(st + 2 * kTileBytes + ko), slo = smem_desc(st + 3 * kTileBytes + ko);
-                    umma_tf32(tmem, rlo, shi, (it > 0 || k > 0) ? 1u : 0u);   // small terms first
-                    umma_tf32(tmem, rhi, slo, 1u);
-                    umma_tf32(tmem, rhi, shi, 1u);
+                    const uint64_t shi = smem_desc(st + 1 * kTileBytes + ko), slo = smem_desc(st + 2 * kTileBytes + ko);
+                    umma_tf32_ts(tmem, a_lo + k * UK, shi, (it > 0 || k > 0) ? 1u : 0u);   // small terms first
+                    umma_tf32_ts(tmem, a_hi + k * UK, slo, 1u);
+                    umma_tf32_ts(tmem, a_hi + k * UK, shi, 1u);
                 }
                 umma_commit(empty);                                       // frees the stage when these UMMAs retire
             }
@@ -182,27 +206,31 @@ rec_tc_kernel(const __grid_constant__ CUtensorMap mR,
         }
     } else {                                                              // ---- warps 2..5: converters, then epilogue
         {
-            const int ct = threadIdx.x - 64;                              // 0..127
             int it = 0;
             for (int kb = kb_lo; kb < kb_hi; ++kb, ++it) {
                 const int s = it % STAGES;
                 const uint32_t full = bars + 8 * s, conv = bars + 8 * (2 * STAGES + s);
                 mbar_wait(full, (it / STAGES) & 1);
-                float4 *hi = reinterpret_cast<float4 *>(smem_raw + (base - smem_u32(smem_raw)) + s * kStageBytes);
-                float4 *lo = hi + kTileBytes / 16;
+                // thread = row of the tile (TMEM lane 32 (warp % 4) + lane); its 32 K values are 8 chunks of 16 bytes that
+                // TMA's 128-byte swizzle has stored at chunk position c ^ (row % 8)
+                const int row = (warp & 3) * 32 + lane;
+                const uint8_t *tile = smem_raw + (base - smem_u32(smem_raw)) + s * kStageBytes + row * 128;
+                uint32_t hi[32], lo[32];
 #pragma unroll
-                for (int j = 0; j < kTileBytes / 16 / kConvThreads; ++j) {
-                    const float4 x = hi[j * kConvThreads + ct];
-                    const uint32_t hx = to_tf32(x.x), hy = to_tf32(x.y), hz = to_tf32(x.z), hw = to_tf32(x.w);
-                    float4 l;
-                    l.x = __uint_as_float(to_tf32(x.x - __uint_as_float(hx)));
-                    l.y = __uint_as_float(to_tf32(x.y - __uint_as_float(hy)));
-                    l.z = __uint_as_float(to_tf32(x.z - __uint_as_float(hz)));
-                    l.w = __uint_as_float(to_tf32(x.w - __uint_as_float(hw)));
-                    hi[j * kConvThreads + ct] = make_float4(__uint_as_float(hx), __uint_as_float(hy), __uint_as_float(hz), __uint_as_float(hw));
-                    lo[j * kConvThreads + ct] = l;
+                for (int c = 0; c < 8; ++c) {
+                    const float4 x = *reinterpret_cast<const float4 *>(tile + ((c ^ (row & 7)) << 4));
+                    const float xv[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        hi[4 * c + e] = to_tf32(xv[e]);
+                        lo[4 * c + e] = to_tf32(xv[e] - __uint_as_float(hi[4 * c + e]));
+                    }
                 }
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to the UMMA's reads
+                const uint32_t t_hi = tmem + ((uint32_t)((warp & 3) * 32) << 16) + kAccCols + (uint32_t)s * 64u;
+                tmem_st_32x32(t_hi, hi);
+                tmem_st_32x32(t_hi + 32u, lo);
+                asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+                asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
                 mbar_arrive(conv);
             }
         }
