@@ -115,16 +115,24 @@ int pwfs_rec_create(int32_t n_modes, int32_t n_slopes, const float *h_recmat, in
 /* d_slopes: DEVICE float [B][n_slopes]; d_modes: DEVICE float [B][n_modes],
  * modes[b][m] = sum_j recmat[m][j] * slopes[b][j] (F2g), FP32 accumulation in a
  * fixed order (deterministic).  B = 0 is a no-op.
- * Single frames and small problems run an FP32-FMA kernel.  Batches (B >= 24
- * and n_modes * n_slopes >= 65536) run on the tensor cores: recmat and the
- * slopes are each split into two TF32 planes and three tcgen05 products are
- * accumulated in FP32, which keeps the FP32 bar (error <= 7e-7 sum |R||s| from
- * the split, plus FP32 accumulation).  The first batched call builds the
- * planes of recmat (2 x the matrix in device memory) and sizes its scratch for
- * that B: it synchronises the stream and allocates; later calls with B no
- * larger do neither.  Environment PWFS_REC_TC=0 at create keeps every call on
- * the FP32 kernel. */
+ * WHICH ARITHMETIC RUNS DEPENDS ON THE BATCH SIZE: single frames and small
+ * problems run FP32-FMA kernels (B = 1: a streaming GEMV); batches (B >= 24 and
+ * n_modes * n_slopes >= 65536) run on the tensor cores: recmat (inside the
+ * kernel) and the slopes (by a small kernel) are each split into two TF32 planes
+ * and three tcgen05 products are accumulated in FP32, which keeps the FP32 bar
+ * (error <= 7e-7 sum |R||s| from the split, plus FP32 accumulation) -- so a frame's
+ * modes may differ in the last bits between a batched and a single-frame call.
+ * Environment PWFS_REC_TC=0 at create keeps every call on the FP32 kernels.
+ * The first batched call (or a larger batch later) sizes the slope planes and
+ * split-K scratch: it synchronises the stream and allocates; call
+ * pwfs_rec_reserve beforehand to keep pwfs_rec_run free of both.  While
+ * `cuda_stream` is being captured into a CUDA graph a call that would have to
+ * allocate returns PWFS_EINVAL instead. */
 int pwfs_rec_run(pwfs_rec_t *h, const float *d_slopes, int32_t B, float *d_modes, void *cuda_stream);
+
+/* Size the tensor-core path's scratch for batches of up to B frames (no-op for
+ * batch sizes the FP32 kernels serve).  Synchronous; allocates. */
+int pwfs_rec_reserve(pwfs_rec_t *h, int32_t B);
 
 void pwfs_rec_destroy(pwfs_rec_t *h); /* NULL-safe */
 

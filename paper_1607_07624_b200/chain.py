@@ -11,7 +11,7 @@ from .pwfs import PWFS_OK, PwfsError, load_library, strerror
 
 EXPORTS = ("pwfs_ccd_create", "pwfs_ccd_run", "pwfs_ccd_destroy",
            "pwfs_slopec_create", "pwfs_slopec_set_reference", "pwfs_slopec_n_slopes", "pwfs_slopec_run",
-           "pwfs_slopec_destroy", "pwfs_rec_create", "pwfs_rec_run", "pwfs_rec_destroy")
+           "pwfs_slopec_destroy", "pwfs_rec_create", "pwfs_rec_run", "pwfs_rec_reserve", "pwfs_rec_destroy")
 
 
 class pwfs_ccd_params(C.Structure):
@@ -36,8 +36,9 @@ def _lib():
         lib.pwfs_slopec_run.argtypes = [vp, vp, i32, vp, vp]
         lib.pwfs_rec_create.argtypes = [i32, i32, vp, i32, C.POINTER(vp)]
         lib.pwfs_rec_run.argtypes = [vp, vp, i32, vp, vp]
+        lib.pwfs_rec_reserve.argtypes = [vp, i32]
         for n in ("pwfs_ccd_create", "pwfs_ccd_run", "pwfs_slopec_create", "pwfs_slopec_set_reference",
-                  "pwfs_slopec_n_slopes", "pwfs_slopec_run", "pwfs_rec_create", "pwfs_rec_run"):
+                  "pwfs_slopec_n_slopes", "pwfs_slopec_run", "pwfs_rec_create", "pwfs_rec_run", "pwfs_rec_reserve"):
             getattr(lib, n).restype = C.c_int
         for n in ("pwfs_ccd_destroy", "pwfs_slopec_destroy", "pwfs_rec_destroy"):
             getattr(lib, n).argtypes = [vp]
@@ -171,6 +172,10 @@ class Reconstructor(_Handle):
         _check(self._lib.pwfs_rec_create(R.shape[0], R.shape[1], C.c_void_p(R.ctypes.data), device, C.byref(h)),
                "pwfs_rec_create")
         self._h = h
+
+    def reserve(self, batch: int):
+        """Size the batched (tensor-core) path's scratch so that run() neither allocates nor synchronises."""
+        _check(self._lib.pwfs_rec_reserve(self._h, int(batch)), "pwfs_rec_reserve")
 
     def run(self, slopes, out=None, stream=None):
         slopes = self._in(slopes, (self.n_slopes,), "slopes")

@@ -467,6 +467,26 @@ int pwfs_rec_create(int32_t n_modes, int32_t n_slopes, const float *h_recmat, in
     return PWFS_OK;
 }
 
+static int rec_uses_tc(pwfs_rec *h, int B) {
+    return !h->tc_off && B >= kRecTcMinBatch && (long long)h->n_modes * h->n_slopes >= kRecTcMinElems;
+}
+
+static int rec_ensure_tc(pwfs_rec *h) {
+    if (h->tc || h->tc_off) return PWFS_OK;
+    const int rc = rec_tc_create(&h->tc, h->d_R, h->n_modes, h->n_slopes, h->ldk, h->device, h->num_sms);
+    if (rc == PWFS_EUNSUPPORTED) { h->tc_off = true; return PWFS_OK; }
+    return rc;
+}
+
+int pwfs_rec_reserve(pwfs_rec_t *h, int32_t B) {
+    if (!h || B < 1) return PWFS_EINVAL;
+    pwk::DeviceGuard dg(h->device);
+    if (dg.err != cudaSuccess) return PWFS_ECUDA;
+    if (!rec_uses_tc(h, B)) return PWFS_OK;                    // the FP32 kernels need no scratch
+    if (int rc = rec_ensure_tc(h)) return rc;
+    return h->tc ? rec_tc_reserve(h->tc, B, nullptr) : PWFS_OK;
+}
+
 int pwfs_rec_run(pwfs_rec_t *h, const float *d_slopes, int32_t B, float *d_modes, void *cuda_stream) {
     if (!h || B < 0) return PWFS_EINVAL;
     if (B == 0) return PWFS_OK;
@@ -474,12 +494,8 @@ int pwfs_rec_run(pwfs_rec_t *h, const float *d_slopes, int32_t B, float *d_modes
     pwk::DeviceGuard dg(h->device);
     if (dg.err != cudaSuccess) return PWFS_ECUDA;
     // batches: TF32x3 on the tensor cores (rec_tc.cu); single frames and small problems: FP32 FMA below
-    if (!h->tc_off && B >= kRecTcMinBatch && (long long)h->n_modes * h->n_slopes >= kRecTcMinElems) {
-        if (!h->tc) {
-            const int rc = rec_tc_create(&h->tc, h->d_R, h->n_modes, h->n_slopes, h->ldk, h->device, h->num_sms);
-            if (rc == PWFS_EUNSUPPORTED) h->tc_off = true;
-            else if (rc != PWFS_OK) return rc;
-        }
+    if (rec_uses_tc(h, B)) {
+        if (int rc = rec_ensure_tc(h)) return rc;
         if (h->tc) return rec_tc_run(h->tc, d_slopes, B, d_modes, (cudaStream_t)cuda_stream);
     }
     cudaStream_t st = (cudaStream_t)cuda_stream;

@@ -338,36 +338,50 @@ int rec_tc_create(RecTc **out, const float *d_R, int n_modes, int n_slopes, int 
     return PWFS_OK;
 }
 
-int rec_tc_run(RecTc *h, const float *d_slopes, int B, float *d_modes, cudaStream_t st) {
+static int rec_tc_ksplit(const RecTc *h, int B) {
     const int m_tiles = (h->n_modes + BM - 1) / BM, n_tiles = (B + BN - 1) / BN, nkb = h->ldp / BK;
     int ksplit = h->num_sms / (m_tiles * n_tiles);
     if (ksplit > nkb / 4) ksplit = nkb / 4;                               // at least 4 K blocks per split
-    if (ksplit < 1) ksplit = 1;
-    const size_t part_need = ksplit > 1 ? (size_t)ksplit * B * h->n_modes : 0;
-    if (B > h->b_cap || part_need > h->part_cap) {                        // first call at this batch size: grow
-        if (cudaStreamSynchronize(st) != cudaSuccess) return PWFS_ECUDA;
-        if (B > h->b_cap) {
-            const int cap = (B + BN - 1) / BN * BN;
-            cudaFree(h->d_Shi); cudaFree(h->d_Slo);
-            h->d_Shi = h->d_Slo = nullptr; h->b_cap = 0;
-            const size_t bytes = (size_t)cap * h->ldp * sizeof(float);
-            cudaError_t e = cudaMalloc((void **)&h->d_Shi, bytes);
-            if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_Slo, bytes);
-            if (e == cudaSuccess) e = cudaMemset(h->d_Shi, 0, bytes);
-            if (e == cudaSuccess) e = cudaMemset(h->d_Slo, 0, bytes);
-            if (e != cudaSuccess) return cuda_rc(e);
-            if (!make_map(h->enc, &h->mShi, h->d_Shi, cap, h->ldp) || !make_map(h->enc, &h->mSlo, h->d_Slo, cap, h->ldp))
-                return PWFS_ECUDA;
-            h->b_cap = cap;
-        }
-        if (part_need > h->part_cap) {
-            cudaFree(h->d_part);
-            h->d_part = nullptr; h->part_cap = 0;
-            cudaError_t e = cudaMalloc((void **)&h->d_part, part_need * sizeof(float));
-            if (e != cudaSuccess) return cuda_rc(e);
-            h->part_cap = part_need;
-        }
+    return ksplit < 1 ? 1 : ksplit;
+}
+
+// Sizes the slope planes and the split-K partials for batches of up to B frames (allocates; synchronises `st` first
+// when it has to replace buffers that may be in use).  Returns 1 if nothing had to be done.
+int rec_tc_reserve(RecTc *h, int B, cudaStream_t st) {
+    const int ksplit = rec_tc_ksplit(h, B);
+    const size_t part_need = ksplit > 1 ? (size_t)ksplit * ((size_t)(B + BN - 1) / BN * BN) * h->n_modes : 0;
+    if (B <= h->b_cap && part_need <= h->part_cap) return PWFS_OK;
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cs) == cudaSuccess && cs != cudaStreamCaptureStatusNone) return PWFS_EINVAL;
+    if (cudaStreamSynchronize(st) != cudaSuccess) return PWFS_ECUDA;
+    if (B > h->b_cap) {
+        const int cap = (B + BN - 1) / BN * BN;
+        cudaFree(h->d_Shi); cudaFree(h->d_Slo);
+        h->d_Shi = h->d_Slo = nullptr; h->b_cap = 0;
+        const size_t bytes = (size_t)cap * h->ldp * sizeof(float);
+        cudaError_t e = cudaMalloc((void **)&h->d_Shi, bytes);
+        if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_Slo, bytes);
+        if (e == cudaSuccess) e = cudaMemset(h->d_Shi, 0, bytes);
+        if (e == cudaSuccess) e = cudaMemset(h->d_Slo, 0, bytes);
+        if (e != cudaSuccess) return cuda_rc(e);
+        if (!make_map(h->enc, &h->mShi, h->d_Shi, cap, h->ldp) || !make_map(h->enc, &h->mSlo, h->d_Slo, cap, h->ldp))
+            return PWFS_ECUDA;
+        h->b_cap = cap;
     }
+    if (part_need > h->part_cap) {
+        cudaFree(h->d_part);
+        h->d_part = nullptr; h->part_cap = 0;
+        cudaError_t e = cudaMalloc((void **)&h->d_part, part_need * sizeof(float));
+        if (e != cudaSuccess) return cuda_rc(e);
+        h->part_cap = part_need;
+    }
+    return PWFS_OK;
+}
+
+int rec_tc_run(RecTc *h, const float *d_slopes, int B, float *d_modes, cudaStream_t st) {
+    const int m_tiles = (h->n_modes + BM - 1) / BM, n_tiles = (B + BN - 1) / BN, nkb = h->ldp / BK;
+    const int ksplit = rec_tc_ksplit(h, B);
+    if (int rc = rec_tc_reserve(h, B, st)) return rc;                     // no-op once sized (pwfs_rec_reserve)
     split_tf32_kernel<<<dim3((h->ldp + 255) / 256, B), 256, 0, st>>>(d_slopes, (size_t)h->n_slopes, h->n_slopes, h->ldp,
                                                                     h->d_Shi, h->d_Slo);
     rec_tc_kernel<<<dim3(m_tiles, ksplit, n_tiles), kThreads, kSmemBytes, st>>>(

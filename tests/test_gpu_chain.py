@@ -249,3 +249,36 @@ def test_device_chain_f1_to_modes_matches_oracle_chain(torch_cuda):
             assert (np.abs(g_pix - pix) <= 1e-4 * pix.max()).all()
             tol = 1e-4 * np.abs(R.astype(np.float64)).sum(axis=1).max() * 2
             assert np.abs(g_modes - modes).max() <= tol
+
+
+def test_batched_reconstructor_is_capturable_after_reserve(torch_cuda):
+    """pwfs_rec_reserve sizes the tensor-core path's scratch, so a batched pwfs_rec_run neither allocates nor
+    synchronises and can be captured into a CUDA graph; without it the capture is refused (PWFS_EINVAL), not broken."""
+    from paper_1607_07624_b200.chain import Reconstructor
+    from paper_1607_07624_b200.pwfs import PwfsError, PWFS_EINVAL
+    torch = torch_cuda
+    rng = np.random.default_rng(9)
+    R = rng.standard_normal((200, 700)).astype(np.float32)
+    S = _dev(torch, 0.1 * rng.standard_normal((40, 700)))
+    out = torch.zeros((40, 200), device="cuda")
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with Reconstructor(R) as rec:
+        refused = None
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            try:
+                rec.run(S, out=out, stream=side)
+            except PwfsError as e:
+                refused = e
+        assert refused is not None and refused.code == PWFS_EINVAL
+        torch.cuda.synchronize()
+        rec.reserve(40)
+        want = rec.run(S).clone()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            rec.run(S, out=out, stream=side)
+        out.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(out, want)
