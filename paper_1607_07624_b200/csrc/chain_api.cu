@@ -55,12 +55,36 @@ __device__ __forceinline__ double box_muller(double ua, double ub) {
     return __dmul_rn(rad, cos(ang));
 }
 
+// The read-noise deviate only has to reach the pixel within a float ulp (it is added to the count and rounded to
+// float): cos(2 pi ub) is taken as cospi(2 ub) -- no multiply by a rounded 2 pi, no Payne-Hanek range reduction.
+__device__ __forceinline__ double box_muller_readout(double ua, double ub) {
+    const double rad = sqrt(__dmul_rn(-2.0, log(ua)));
+    return __dmul_rn(rad, cospi(__dadd_rn(ub, ub)));
+}
+
 struct CcdDev {
     int D, n_inst, n_int;
     double qe_gain, ron;
     int photon, readout;
     unsigned k0, k1;
+    const double *rcp;     // [kPoissonMaxN + 1] rcp[n] = RN(1 / n), correctly rounded on the host (rcp[0] unused)
 };
+
+constexpr int kPoissonMaxN = 4096;
+
+// RN(a / n) for 0 < a < 2^10 and an integer 1 <= n <= 4096 held as the double nd, with y = RN(1 / n) from the table:
+// two Newton steps on the quotient and Markstein's final correction -- q1 is within one ulp of a / n (its error before
+// rounding is O(2^-104)), the residual r1 = a - n q1 is exact in one FMA, and RN(q1 + r1 y) is then the correctly
+// rounded quotient (Markstein 1990).  Five FP64 pipe operations instead of the ~25 of the generic __ddiv_rn (which
+// also handles subnormals, infinities and exponent extremes that cannot occur here); the photon counts stay
+// bit-identical to the oracle's IEEE division (tests/test_gpu_chain.py compares millions of pixels exactly).
+__device__ __forceinline__ double div_small_int(double a, double nd, double y) {
+    const double q0 = __dmul_rn(a, y);
+    const double r0 = __fma_rn(-nd, q0, a);
+    const double q1 = __fma_rn(r0, y, q0);
+    const double r1 = __fma_rn(-nd, q1, a);
+    return __fma_rn(r1, y, q1);
+}
 
 constexpr double kPoissonSwitch = 128.0;   // F2c
 
@@ -88,20 +112,21 @@ ccd_kernel(CcdDev c, const float *__restrict__ frames, long long n_out, long lon
                 k = 0.0;
             } else if (lam < kPoissonSwitch) {
                 const double u = u01(r.x);
-                double pr = exp(-lam), s = pr;
+                double pr = exp(-lam), s = pr, nd = 0.0;
                 int n = 0;
-                while (u > s && n < 4096) {
+                while (u > s && n < kPoissonMaxN) {
                     ++n;
-                    pr = __dmul_rn(pr, __ddiv_rn(lam, (double)n));
+                    nd = __dadd_rn(nd, 1.0);
+                    pr = __dmul_rn(pr, div_small_int(lam, nd, __ldg(c.rcp + n)));
                     s = __dadd_rn(s, pr);
                 }
-                k = (double)n;
+                k = nd;
             } else {
                 const double z = box_muller(u01(r.x), u01(r.y));
                 k = fmax(0.0, floor(__dadd_rn(__dadd_rn(lam, __dmul_rn(sqrt(lam), z)), 0.5)));
             }
         }
-        if (c.readout) k = __dadd_rn(k, __dmul_rn(c.ron, box_muller(u01(r.z), u01(r.w))));   // F2d
+        if (c.readout) k = __dadd_rn(k, __dmul_rn(c.ron, box_muller_readout(u01(r.z), u01(r.w))));   // F2d
     }
     pix[idx] = (float)k;
 }
@@ -315,6 +340,7 @@ int cuda_rc(cudaError_t e) { return e == cudaErrorMemoryAllocation ? PWFS_ENOMEM
 struct pwfs_ccd {
     int device = 0;
     CcdDev dev{};
+    double *d_rcp = nullptr;
 };
 
 struct pwfs_slopec {
@@ -354,6 +380,16 @@ int pwfs_ccd_create(const pwfs_ccd_params *p, pwfs_ccd_t **out) {
     c.ron = p->readout_level;
     c.photon = p->photon_noise != 0; c.readout = p->readout_noise != 0;
     c.k0 = (unsigned)(p->seed & 0xFFFFFFFFull); c.k1 = (unsigned)(p->seed >> 32);
+    {
+        std::vector<double> rcp(kPoissonMaxN + 1, 0.0);
+        for (int n = 1; n <= kPoissonMaxN; ++n) rcp[n] = 1.0 / (double)n;       // IEEE division: correctly rounded
+        pwk::DeviceGuard dg(p->device);
+        cudaError_t e = dg.err;
+        if (e == cudaSuccess) e = cudaMalloc((void **)&h->d_rcp, rcp.size() * sizeof(double));
+        if (e == cudaSuccess) e = cudaMemcpy(h->d_rcp, rcp.data(), rcp.size() * sizeof(double), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) { const int rc = cuda_rc(e); pwfs_ccd_destroy(h); return rc; }
+        c.rcp = h->d_rcp;
+    }
     *out = h;
     return PWFS_OK;
 }
@@ -374,7 +410,14 @@ int pwfs_ccd_run(pwfs_ccd_t *h, const float *d_frames, int32_t n_steps, int64_t 
     return cudaGetLastError() == cudaSuccess ? PWFS_OK : PWFS_ECUDA;
 }
 
-void pwfs_ccd_destroy(pwfs_ccd_t *h) { delete h; }
+void pwfs_ccd_destroy(pwfs_ccd_t *h) {
+    if (!h) return;
+    if (h->d_rcp) {
+        pwk::DeviceGuard dg(h->device);
+        cudaFree(h->d_rcp);
+    }
+    delete h;
+}
 
 // ------------------------------------------------------- slope computer ---
 int pwfs_slopec_create(int32_t n_sub, const uint8_t *h_valid, int32_t slope_norm, const float *h_sn, int32_t device,
