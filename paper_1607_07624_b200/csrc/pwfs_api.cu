@@ -265,6 +265,9 @@ int build_tables(pwfs *h) {
     for (int k = 0; k < K; ++k) korder[k] = k;
     std::stable_sort(korder.begin(), korder.end(), [&](int a, int b) { return jx[a] < jx[b]; });
     if ((rc = upload(h, korder, &t.korder))) return rc;
+    std::vector<int2> kj(K);   // (k, x-tilt index of k) in that order: one load per modulation point in the column pass
+    for (int i = 0; i < K; ++i) kj[i] = make_int2(korder[i], jx[korder[i]]);
+    if ((rc = upload(h, kj, &t.kj))) return rc;
     if ((rc = upload(h, tw, &t.tw))) return rc;
     if ((rc = upload(h, am, &t.am))) return rc;
     if ((rc = upload(h, colx, &t.colx))) return rc;

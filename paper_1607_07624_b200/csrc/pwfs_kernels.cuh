@@ -37,35 +37,41 @@ constexpr int kPitch = 33;  // float2 row pitch of the exchange buffer: conflict
 // writes, per x-tilt, one contiguous block of M * kTB float2; the column pass reads 64-byte runs.
 constexpr int kTB = 8;
 
-// Padding (float2) between the exchange buffers of consecutive warps.  Inside a warp's buffer the NB * R1 rows are
-// contiguous (the size-32 stage reads row w at w * kPitch: 16 consecutive lanes hit 16 different 64-bit banks).  The row
-// pass's transposed last stage reads, per instruction, 8 rows r = 8 r_hi + r_lo of the CTA (= 8 transforms, spread over
-// 8 / NB warps) x 2 adjacent columns per half warp; the pad is chosen so that those 16 accesses fall in as many different
-// banks as possible (all 16 for NB = 1 and for R1 = 6, 10, 18).
-constexpr int pick_warp_pad(int R1, int NB, int RPC) {
-    int best_pad = 0, best = 1 << 30;
-    for (int pad = 0; pad < 16; ++pad) {
-        const int wb = NB * R1 * kPitch + pad;
-        int tot = 0;
-        for (int rhi = 0; rhi < RPC / kTB; ++rhi) {
-            int cnt[16] = {};
-            int worst = 0;
-            for (int rlo = 0; rlo < kTB; ++rlo) {
-                const int r = kTB * rhi + rlo;
-                const int off = (r / NB) * wb + (r % NB) * R1 * kPitch;
-                for (int n2 = 0; n2 < 2; ++n2) {
-                    const int c = ++cnt[(off + n2) % 16];
-                    worst = c > worst ? c : worst;
+// Padding (float2) of the exchange buffers.  Inside a warp's buffer the NB * R1 rows are contiguous (the size-32 stage
+// reads row w at w * kPitch: 16 consecutive lanes hit 16 different 64-bit banks), except that a pad TPAD may separate
+// the NB transforms when R1 is a multiple of 16 (a half warp of the size-32 stage then never straddles two transforms).
+// The row pass's transposed last stage reads, per instruction, 8 rows r = 8 r_hi + r_lo of the CTA (= 8 transforms,
+// spread over 8 / NB warps) x 2 adjacent columns per half warp; the pad between warps (low byte of the result) and
+// TPAD (next byte) are chosen so that those 16 accesses fall in as many different banks as possible: all 16 for
+// NB = 1, for R1 = 6, 10, 18 and, with TPAD, for R1 = 16, 32, 48, 64.
+constexpr int pick_pads(int R1, int NB, int RPC) {
+    int best_code = 0, best = 1 << 30;
+    const int tmax = (R1 % 16 == 0 && NB > 1) ? 16 : 1;
+    for (int tpad = 0; tpad < tmax; ++tpad)
+        for (int pad = 0; pad < 16; ++pad) {
+            const int wb = NB * R1 * kPitch + (NB - 1) * tpad + pad;
+            int tot = 0;
+            for (int rhi = 0; rhi < RPC / kTB; ++rhi) {
+                int cnt[16] = {};
+                int worst = 0;
+                for (int rlo = 0; rlo < kTB; ++rlo) {
+                    const int r = kTB * rhi + rlo;
+                    const int off = (r / NB) * wb + (r % NB) * (R1 * kPitch + tpad);
+                    for (int n2 = 0; n2 < 2; ++n2) {
+                        const int c = ++cnt[(off + n2) % 16];
+                        worst = c > worst ? c : worst;
+                    }
                 }
+                tot += worst;
             }
-            tot += worst;
+            if (tot < best) { best = tot; best_code = tpad * 256 + pad; }
         }
-        if (tot < best) { best = tot; best_pad = pad; }
-    }
-    return best_pad;
+    return best_code;
 }
 
-template <int R1_, int NB_, int WPB_X_, int WPB_Y_, int MINB_X_ = 1, int MINB_Y_ = 1>
+// YMODE_ (column pass): bit 0 = the T column is staged in shared memory by cp.async instead of waiting in registers,
+// bit 1 = the size-32 stage keeps its 32 twiddles in registers for both multiplies.
+template <int R1_, int NB_, int WPB_X_, int WPB_Y_, int MINB_X_ = 1, int MINB_Y_ = 1, int YMODE_ = 0>
 struct PassCfg {
     static constexpr int R1 = R1_;           // M / 32
     static constexpr int NB = NB_;           // transforms a warp works on at once
@@ -73,7 +79,11 @@ struct PassCfg {
     static constexpr int NZ = (R1_ + 1) / 2; // M >= 2N  =>  at most ceil(R1/2) non-zero inputs per lane
     static constexpr int ITEMS = NB_ * R1_;  // size-32 DFTs per warp batch
     static constexpr int ROUNDS = (ITEMS + 31) / 32;
-    static constexpr int WARP_BUF = ITEMS * kPitch + pick_warp_pad(R1_, NB_, NB_ * WPB_X_);   // float2 per warp
+    static constexpr int TPAD = pick_pads(R1_, NB_, NB_ * WPB_X_) / 256;            // float2 between the NB transforms
+    static constexpr int TR_BUF = R1_ * kPitch + TPAD;                               // float2 per transform
+    static constexpr int WARP_BUF = ITEMS * kPitch + (NB_ - 1) * TPAD + pick_pads(R1_, NB_, NB_ * WPB_X_) % 256;   // float2 per warp
+    // offset of exchange row (transform b, k1) in the warp's buffer; w = b * R1 + k1
+    __host__ __device__ static constexpr int row_off(int w) { return w * kPitch + (TPAD ? (w / R1_) * TPAD : 0); }
     static constexpr int TAB = R1_ * kPitch;              // float2 per table (twiddle, mask)
     // M = 2048: the row pass's shared memory is full, the general-mask table a(u)/M is read through L1 instead
     static constexpr bool AM_GLOBAL = R1_ > 32;
@@ -87,7 +97,13 @@ struct PassCfg {
     // row pass: tables (no mask table for the quarter mask) + exchange buffers + base phasor [RPC][NZ][32]
     static constexpr size_t smem_x_q = (size_t)(WPB_X_ * WARP_BUF + 1 * TAB + RPC * NZ * 32) * sizeof(float2);
     static constexpr size_t smem_x_t = (size_t)(WPB_X_ * WARP_BUF + (AM_GLOBAL ? 1 : 2) * TAB + RPC * NZ * 32) * sizeof(float2);
-    static constexpr size_t smem_y = (size_t)(WPB_Y_ * WARP_BUF + 2 * TAB) * sizeof(float2);
+    // column pass: tables + exchange buffers (+ the staged T column [NB][NZ][32] per warp when Y_ASYNC)
+    static constexpr int YMODE = YMODE_;
+    static constexpr bool Y_ASYNC = (YMODE_ & 1) != 0;
+    static constexpr bool Y_TWKEEP = (YMODE_ & 2) != 0;
+    static constexpr int PRE_BUF = Y_ASYNC ? NB_ * NZ * 32 : 0;
+    static constexpr size_t smem_y_q = (size_t)(WPB_Y_ * (WARP_BUF + PRE_BUF) + 1 * TAB) * sizeof(float2);
+    static constexpr size_t smem_y_t = (size_t)(WPB_Y_ * (WARP_BUF + PRE_BUF) + (AM_GLOBAL ? 1 : 2) * TAB) * sizeof(float2);
 };
 
 // Device-side view of a sensor's tables (all pointers are device memory).
@@ -105,6 +121,7 @@ struct DevTables {
     const float2 *tyt;        // [K][NP]  exp(i tilt_y,k(y)), zero for y >= N
     const int *jx;            // [K]      x-tilt index of modulation point k
     const int *korder;        // [K]      the modulation points sorted by x-tilt index
+    const int2 *kj;           // [K]      (korder[i], jx[korder[i]])
     const float2 *tw;         // [R1][32] exp(-2 pi i k1 n2 / M)
     const float2 *am;         // [R1][32] a(k1 + R1 k2) / M
     const int *colx;          // [ncols]  grid x of compact column xc
@@ -156,18 +173,24 @@ __device__ __forceinline__ void idft32_signed_upper(float2 (&x)[32], float2 sg2)
 // per-lane sign absorbed by idft32_signed_upper, and i^k1 is applied where k1 is a compile-time
 // register index (step A' of the callers, apply_ipow_k1).  The mask and its table cost nothing;
 // the 1/M per axis moves into the final frame scale.
-template <class C, bool QM>
+// KEEP: the 32 twiddles of the lane are read once into registers and serve both multiplies (64 registers for a third
+// less shared-memory traffic in this stage); otherwise the compiler decides whether the second multiply re-reads them.
+template <class C, bool QM, bool KEEP = false>
 __device__ __forceinline__ void stage32(float2 *buf, const float2 *s_tw, const float2 *s_am, int lane) {
 #pragma unroll
     for (int rd = 0; rd < C::ROUNDS; ++rd) {
         int w = rd * 32 + lane;
         if (w < C::ITEMS) {
             const int k1 = w % C::R1;
-            float2 *row = buf + w * kPitch;
+            float2 *row = buf + C::row_off(w);
             const float2 *twr = s_tw + k1 * kPitch;
             float2 u[32];
+            [[maybe_unused]] float2 twv[KEEP ? 32 : 1];
 #pragma unroll
-            for (int n2 = 0; n2 < 32; ++n2) u[n2] = cmul(row[n2], twr[n2]);
+            for (int n2 = 0; n2 < 32; ++n2) {
+                if constexpr (KEEP) { twv[n2] = twr[n2]; u[n2] = cmul(row[n2], twv[n2]); }
+                else u[n2] = cmul(row[n2], twr[n2]);
+            }
             Dft<32, -1>::run(u);
             if constexpr (QM) {
                 sfor<32>([&](auto kc) {
@@ -184,7 +207,7 @@ __device__ __forceinline__ void stage32(float2 *buf, const float2 *s_tw, const f
                 Dft<32, +1>::run(u);
             }
 #pragma unroll
-            for (int n2 = 0; n2 < 32; ++n2) row[n2] = cmulc(u[n2], twr[n2]);
+            for (int n2 = 0; n2 < 32; ++n2) row[n2] = cmulc(u[n2], KEEP ? twv[n2] : twr[n2]);
         }
     }
 }
@@ -268,7 +291,7 @@ xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ 
     for (int it = 0; it < C::NB; ++it) {
         const int i = threadIdx.x + it * 32 * C::WPB_X;
         const int r = (i >> 8) * kTB + (i & 7), n2 = (i >> 3) & 31;
-        item_src[it] = (r / C::NB) * C::WARP_BUF + (r % C::NB) * C::R1 * kPitch + n2;
+        item_src[it] = (r / C::NB) * C::WARP_BUF + (r % C::NB) * C::TR_BUF + n2;
         item_dst[it] = (y0 + r < t.NP) ? ((y0 + r) / kTB) * (C::M * kTB) + n2 * kTB + (i & 7) : -1;
     }
 
@@ -292,7 +315,7 @@ xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ 
             for (int n1 = 0; n1 < C::NZ; ++n1) v[n1] = cmul(pw[(b * C::NZ + n1) * 32], tx[n1]);
             DftP<C::R1, -1, C::NZ>::run(v);
 #pragma unroll
-            for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitch + lane] = v[k1];
+            for (int k1 = 0; k1 < C::R1; ++k1) buf[C::row_off(b * C::R1 + k1) + lane] = v[k1];
         }
         if (j + 1 < j_hi) {
             const float2 *txj = t.txc + (size_t)(j + 1) * t.NXP + lane;
@@ -312,6 +335,11 @@ xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ 
             for (int k1 = 0; k1 < C::R1; ++k1) v[k1] = src[k1 * kPitch];
             apply_ipow_k1<C::R1, QM>(v);
             Dft<C::R1, +1>::run(v);
+            // Under this guard ptxas moves each value to one register pair before its store, so a store is issued only
+            // when the LSU has taken the previous one (ncu: those moves wait on the long scoreboard).  That pacing is
+            // measured to HELP: with unguarded stores interleaved among the butterflies the same instruction mix runs
+            // 5 % slower (M = 1024: 3.19 vs 3.03 ms per 100 frames; profiles/r2_tuning.md) -- bursts of stores delay
+            // the shared-memory traffic of the warps that are in their size-32 stage.
             if (item_dst[it] >= 0) {
                 float2 *dst = Tj + item_dst[it];
 #pragma unroll
@@ -333,12 +361,13 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
     extern __shared__ float2 smem[];
     float2 *s_tw = smem;
     const float2 *s_am = C::AM_GLOBAL ? t.am : smem + C::TAB;
-    float2 *s_buf = smem + 2 * C::TAB;
+    float2 *s_buf = smem + ((QM || C::AM_GLOBAL) ? 1 : 2) * C::TAB;
     const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
     const int NP = t.NP;
     const int ks = blockIdx.y, f = blockIdx.z;
     const int xc0 = (blockIdx.x * C::WPB_Y + wl) * C::NB;
     float2 *buf = s_buf + wl * C::WARP_BUF;
+    [[maybe_unused]] float2 *spre = s_buf + C::WPB_Y * C::WARP_BUF + wl * C::PRE_BUF + lane;   // Y_ASYNC: [NB][NZ][32]
 
     load_tables<QM, C::AM_GLOBAL>(s_tw, smem + C::TAB, t, C::R1);
     __syncthreads();
@@ -360,52 +389,70 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
 #pragma unroll
     for (int b = 0; b < C::NB; ++b) colofs[b] = (xc0 + b < t.ncols) ? __ldg(t.colx + xc0 + b) * colmul : 0;
 
-    // The warp walks its share of the modulation points in x-tilt order (korder): points that share a slab
-    // T[f][j] come one after the other and the column is fetched once for them.
-    float2 pre[C::NB][C::NZ];
+    // The warp walks its share of the modulation points in x-tilt order (kj): points that share a slab T[f][j] come
+    // one after the other and the column is fetched once for them.  The column of the NEXT slab is fetched while the
+    // current point is transformed: into registers, or (Y_ASYNC) staged in shared memory by cp.async -- no registers
+    // held across the size-32 stage, 12 warps per SM instead of 8; every lane writes and reads only its own slots, so
+    // the only ordering needed is cp.async.wait_all in the lane.  (Staging the y-tilt row the same way was measured
+    // slower: M = 1024 9.72 vs 9.54 ms per 100 frames.)
+    [[maybe_unused]] float2 pre[C::Y_ASYNC ? 1 : C::NB][C::Y_ASYNC ? 1 : C::NZ];
+    if constexpr (C::Y_ASYNC) {
+#pragma unroll
+        for (int i = 0; i < C::NB * C::NZ; ++i) spre[i * 32] = make_float2(0.f, 0.f);
+    }
     auto fetch = [&](int j) {
         const float2 *src = Tf + (size_t)j * frame_stride;
 #pragma unroll
         for (int b = 0; b < C::NB; ++b)
 #pragma unroll
-            for (int n1 = 0; n1 < C::NZ; ++n1)
-                pre[b][n1] = (32 * n1 < NP && xc0 + b < t.ncols) ? __ldg(src + colofs[b] + n1 * n1_stride)
-                                                                 : make_float2(0.f, 0.f);
+            for (int n1 = 0; n1 < C::NZ; ++n1) {
+                if constexpr (C::Y_ASYNC) {
+                    if (32 * n1 < NP && xc0 + b < t.ncols) {
+                        const unsigned dst = (unsigned)__cvta_generic_to_shared(spre + (b * C::NZ + n1) * 32);
+                        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src + colofs[b] + n1 * n1_stride) : "memory");
+                    }
+                } else {
+                    pre[b][n1] = (32 * n1 < NP && xc0 + b < t.ncols) ? __ldg(src + colofs[b] + n1 * n1_stride)
+                                                                     : make_float2(0.f, 0.f);
+                }
+            }
     };
-    int k = 0, j = -1, k_next = 0, j_next = -1;
+    int2 kj = make_int2(0, -1), kj_next = make_int2(0, -1), kj_next2 = make_int2(0, -1);
     if (k_lo < k_hi) {
-        k_next = __ldg(t.korder + k_lo);
-        j_next = __ldg(t.jx + k_next);
-        fetch(j_next);
+        kj_next = __ldg(t.kj + k_lo);
+        if (k_lo + 1 < k_hi) kj_next2 = __ldg(t.kj + k_lo + 1);
+        fetch(kj_next.y);
     }
     for (int idx = k_lo; idx < k_hi; ++idx) {
-        k = k_next; j = j_next;
-        if (idx + 1 < k_hi) {
-            k_next = __ldg(t.korder + idx + 1);
-            j_next = __ldg(t.jx + k_next);
-        }
+        kj = kj_next; kj_next = kj_next2;
+        if (idx + 2 < k_hi) kj_next2 = __ldg(t.kj + idx + 2);
+        const int k = kj.x, j = kj.y, j_next = kj_next.y;
         const float2 *ty = t.tyt + (size_t)k * NP + lane;
         float2 tyv[C::NZ];
 #pragma unroll
         for (int n1 = 0; n1 < C::NZ; ++n1) tyv[n1] = (32 * n1 < NP) ? __ldg(ty + 32 * n1) : make_float2(0.f, 0.f);
+        if constexpr (C::Y_ASYNC) asm volatile("cp.async.wait_all;" ::: "memory");
 #pragma unroll
         for (int b = 0; b < C::NB; ++b) {
             float2 v[C::R1];
 #pragma unroll
-            for (int n1 = 0; n1 < C::NZ; ++n1) v[n1] = cmul(pre[b][n1], tyv[n1]);
+            for (int n1 = 0; n1 < C::NZ; ++n1) {
+                if constexpr (C::Y_ASYNC) v[n1] = cmul(spre[(b * C::NZ + n1) * 32], tyv[n1]);
+                else v[n1] = cmul(pre[b][n1], tyv[n1]);
+            }
             if (b == C::NB - 1 && idx + 1 < k_hi && j_next != j) fetch(j_next);
             DftP<C::R1, -1, C::NZ>::run(v);
 #pragma unroll
-            for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitch + lane] = v[k1];
+            for (int k1 = 0; k1 < C::R1; ++k1) buf[C::row_off(b * C::R1 + k1) + lane] = v[k1];
         }
         __syncwarp();
-        stage32<C, QM>(buf, s_tw, s_am, lane);
+        stage32<C, QM, C::Y_TWKEEP>(buf, s_tw, s_am, lane);
         __syncwarp();
 #pragma unroll
         for (int b = 0; b < C::NB; ++b) {
             float2 v[C::R1];
 #pragma unroll
-            for (int k1 = 0; k1 < C::R1; ++k1) v[k1] = buf[(b * C::R1 + k1) * kPitch + lane];
+            for (int k1 = 0; k1 < C::R1; ++k1) v[k1] = buf[C::row_off(b * C::R1 + k1) + lane];
             apply_ipow_k1<C::R1, QM>(v);
             Dft<C::R1, +1>::run(v);
 #pragma unroll

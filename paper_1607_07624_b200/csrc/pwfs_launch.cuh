@@ -48,16 +48,23 @@ template <> struct CfgFor<64> { using type = PassCfg<64, 1, 8, 4, 1, 1>; };   //
 // The column pass may batch more transforms per warp than the row pass (whose shared memory also parks the base
 // phasor): more of the 32 lanes busy in the size-32 stage.  Default: the same configuration.  (R1 = 25 with NB = 5,
 // 125 items, was tried: the exchange buffers then allow only 6 warps per SM and the column pass ran 1.6x slower.)
-template <int R1> struct CfgForY { using type = typename CfgFor<R1>::type; };
-template <> struct CfgForY<10> { using type = PassCfg<10, 3, 8, 4, 2, 1>; };   // 30 items
-template <> struct CfgForY<15> { using type = PassCfg<15, 4, 8, 4, 2, 1>; };   // 60 items: two full rounds (was 30 of 32)
-template <> struct CfgForY<16> { using type = PassCfg<16, 2, 8, 4, 2, 1>; };
-template <> struct CfgForY<20> { using type = PassCfg<20, 3, 8, 4, 2, 1>; };   // 60 items (was 20 of 32)
-template <> struct CfgForY<24> { using type = PassCfg<24, 1, 8, 4, 2, 1>; };
-template <> struct CfgForY<25> { using type = PassCfg<25, 1, 8, 4, 2, 1>; };
-template <> struct CfgForY<27> { using type = PassCfg<27, 1, 8, 4, 2, 1>; };
-template <> struct CfgForY<30> { using type = PassCfg<30, 1, 8, 4, 2, 1>; };
-template <> struct CfgForY<32> { using type = PassCfg<32, 1, 8, 4, 2, 2>; };
+// YMODE (last argument; measured on B200, profiles/r2_tuning.md): 2 = twiddles kept in registers through the size-32
+// stage (left to the compiler, an unrelated source change moved M = 800 between 33.3 and 40.3 ms per 600 frames);
+// 1 = T column staged by cp.async, 168 registers, 3 CTAs per SM (M = 1024: 9.74 -> 9.5x ms per 100 frames; M = 320:
+// 5.09 -> 5.0x; slower on M = 480 and 800).  R1 > 32 keeps the compiler's choice (64 register points per lane already).
+template <int R1> struct CfgForY {
+    using B = typename CfgFor<R1>::type;
+    using type = PassCfg<R1, B::NB, B::WPB_X, B::WPB_Y, B::MINB_X, B::MINB_Y, R1 <= 32 ? 2 : 0>;
+};
+template <> struct CfgForY<10> { using type = PassCfg<10, 3, 8, 4, 2, 3, 1>; };   // 30 items
+template <> struct CfgForY<15> { using type = PassCfg<15, 4, 8, 4, 2, 1, 2>; };   // 60 items: two full rounds (was 30 of 32)
+template <> struct CfgForY<16> { using type = PassCfg<16, 2, 8, 4, 2, 1, 2>; };
+template <> struct CfgForY<20> { using type = PassCfg<20, 3, 8, 4, 2, 1, 2>; };   // 60 items (was 20 of 32)
+template <> struct CfgForY<24> { using type = PassCfg<24, 1, 8, 4, 2, 1, 2>; };
+template <> struct CfgForY<25> { using type = PassCfg<25, 1, 8, 4, 2, 1, 2>; };
+template <> struct CfgForY<27> { using type = PassCfg<27, 1, 8, 4, 2, 1, 2>; };
+template <> struct CfgForY<30> { using type = PassCfg<30, 1, 8, 4, 2, 1, 2>; };
+template <> struct CfgForY<32> { using type = PassCfg<32, 1, 8, 4, 2, 3, 1>; };
 
 struct Launcher {
     int R1, NB, WPB_X, WPB_Y, RPC;   // NB, WPB_Y: column pass; WPB_X, RPC: row pass

@@ -77,7 +77,7 @@ small_kernel(DevTables t, const float *__restrict__ phase, float *__restrict__ p
             }
             DftP<C::R1, -1, C::NZ>::run(v);
 #pragma unroll
-            for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitch + lane] = v[k1];
+            for (int k1 = 0; k1 < C::R1; ++k1) buf[C::row_off(b * C::R1 + k1) + lane] = v[k1];
         }
         __syncwarp();
         stage32<C, QM>(buf, s_tw, s_am, lane);
@@ -87,7 +87,7 @@ small_kernel(DevTables t, const float *__restrict__ phase, float *__restrict__ p
             const int y = (rg * C::WARPS + wl) * C::NB + b;
             float2 v[C::R1];
 #pragma unroll
-            for (int k1 = 0; k1 < C::R1; ++k1) v[k1] = buf[(b * C::R1 + k1) * kPitch + lane];
+            for (int k1 = 0; k1 < C::R1; ++k1) v[k1] = buf[C::row_off(b * C::R1 + k1) + lane];
             apply_ipow_k1<C::R1, QM>(v);
             Dft<C::R1, +1>::run(v);
             if (y < NP) {
@@ -123,7 +123,7 @@ small_kernel(DevTables t, const float *__restrict__ phase, float *__restrict__ p
                                                                           : make_float2(0.f, 0.f);
                     DftP<C::R1, -1, C::NZ>::run(v);
 #pragma unroll
-                    for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitch + lane] = v[k1];
+                    for (int k1 = 0; k1 < C::R1; ++k1) buf[C::row_off(b * C::R1 + k1) + lane] = v[k1];
                 }
                 __syncwarp();
                 stage32<C, QM>(buf, s_tw, s_am, lane);
@@ -132,7 +132,7 @@ small_kernel(DevTables t, const float *__restrict__ phase, float *__restrict__ p
                 for (int b = 0; b < C::NB; ++b) {
                     float2 v[C::R1];
 #pragma unroll
-                    for (int k1 = 0; k1 < C::R1; ++k1) v[k1] = buf[(b * C::R1 + k1) * kPitch + lane];
+                    for (int k1 = 0; k1 < C::R1; ++k1) v[k1] = buf[C::row_off(b * C::R1 + k1) + lane];
                     apply_ipow_k1<C::R1, QM>(v);
                     Dft<C::R1, +1>::run(v);
 #pragma unroll
