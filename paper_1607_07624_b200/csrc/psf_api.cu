@@ -6,12 +6,13 @@
 // forward only, so the result stays in the "k1 + R1 k2" register order and is consumed there.
 //
 //   psf_row_kernel   N pupil rows per frame: phasor (phase rescaled to the imaging wavelength)
-//                    -> DFT over x -> T[f][y / 8][c][y % 8], c = 32 k1 + k2 the position of frequency
-//                    u = k1 + R1 k2 in the exchange buffer: the CTA's 8 (16, ..) rows leave as ONE
-//                    contiguous block of M * 64 bytes per 8 rows, a straight copy out of shared memory
-//                    (same blocked layout as the pyramid path's T).  A CTA keeps its rows for several
+//                    -> DFT over x -> T[f][y / 8][u][y % 8] in natural frequency order (same blocked layout
+//                    as the pyramid path's T).  The size-32 stage is done "transposed": a thread takes
+//                    exchange row k1 of another warp's pupil row, so adjacent lanes hold adjacent rows y and
+//                    the results go from registers straight to global memory (256 contiguous bytes per warp
+//                    store, compile-time offsets) -- no staging copy.  A CTA keeps its rows for several
 //                    frames, so the twiddle table is loaded once.
-//   psf_col_kernel   one warp per NB columns c, looping over its share of the frames: DFT over
+//   psf_col_kernel   one warp per NB columns u, looping over its share of the frames: DFT over
 //                    y (only the N non-zero inputs are read, 64-byte runs), |.|^2 accumulated over the
 //                    frames in registers; Strehl ratio from the (0,0) bin; one partial PSF per frame
 //                    split, written column-major [u][v] so that a warp's stores are contiguous.
@@ -125,30 +126,27 @@ psf_row_kernel(PsfDev t, const float *__restrict__ phase, float2 *__restrict__ T
             for (int k1 = 0; k1 < C::R1; ++k1) buf[(b * C::R1 + k1) * kPitchP + lane] = v[k1];
         }
         __syncthreads();     // also: the twiddle table is complete (first pass)
+        // Size-32 stage, done "transposed" like the last stage of the pyramid's row pass: thread item
+        // i = r_lo + 8 (k1 + R1 r_hi) takes exchange row k1 of CTA row r = 8 r_hi + r_lo (another warp's buffer), so that
+        // adjacent lanes hold adjacent rows y of one frequency.  X[u = k1 + R1 k2] goes from registers straight to
+        // T[f][(y0 + r) / 8][u][r_lo]: 8 lanes x 4 adjacent k1 write 256 contiguous bytes, every store of a thread is a
+        // compile-time offset (k2 * R1 * 8 float2) from one base.  No staging pass, no third barrier.
+        float2 *Tf = T + (size_t)f * C::M * t.NP + (size_t)(y0 / 8) * (C::M * 8);
 #pragma unroll
-        for (int rd = 0; rd < C::ROUNDS; ++rd) {
-            const int w = rd * 32 + lane;
-            if (w < C::ITEMS) {
-                const int k1 = w % C::R1;
-                float2 *row = buf + w * kPitchP;
+        for (int it = 0; it < C::ROUNDS; ++it) {
+            const int i = threadIdx.x + it * 32 * C::WPB;
+            const int q = i >> 3, r_hi = q / C::R1, k1 = q - r_hi * C::R1, r = 8 * r_hi + (i & 7);
+            if (i < C::RPC * C::R1 && y0 + r < t.NP) {
+                const float2 *row = s_buf + (r / C::NB) * C::WARP_BUF + ((r % C::NB) * C::R1 + k1) * kPitchP;
                 const float2 *twr = s_tw + k1 * kPitchP;
                 float2 u[32];
 #pragma unroll
                 for (int n2 = 0; n2 < 32; ++n2) u[n2] = cmul(row[n2], twr[n2]);
                 Dft<32, -1>::run(u);
+                float2 *dst = Tf + ((size_t)r_hi * C::M + k1) * 8 + (i & 7);
 #pragma unroll
-                for (int k2 = 0; k2 < 32; ++k2) row[k2] = u[k2];
+                for (int k2 = 0; k2 < 32; ++k2) dst[k2 * (C::R1 * 8)] = u[k2];
             }
-        }
-        __syncthreads();
-        // X[u = k1 + R1 k2] of CTA row r sits at s_buf[(r/NB) WARP_BUF + ((r%NB) R1 + k1) pitch + k2].  Element
-        // i = r_lo + 8 (c + M r_hi), c = 32 k1 + k2, r = 8 r_hi + r_lo, goes to T[f][y0/8 + r_hi][c][r_lo]: for this CTA
-        // one contiguous run of RPC * M float2, written in order.
-        float2 *dst = T + (size_t)f * C::M * t.NP + (size_t)(y0 / 8) * (C::M * 8);
-        const int n_out = min(C::RPC, t.NP - y0) * C::M;              // whole 8-row blocks (NP % 32 == 0)
-        for (int i = threadIdx.x; i < n_out; i += 32 * C::WPB) {
-            const int r_hi = i / (8 * C::M), c = (i >> 3) - r_hi * C::M, r = 8 * r_hi + (i & 7);
-            dst[i] = s_buf[(r / C::NB) * C::WARP_BUF + ((r % C::NB) * C::R1 + (c >> 5)) * kPitchP + (c & 31)];
         }
         __syncthreads();     // the next frame overwrites the buffers
     }
@@ -175,7 +173,7 @@ psf_col_kernel(PsfDev t, const float2 *__restrict__ T, int F, int fsplit, float 
 #pragma unroll
         for (int k2 = 0; k2 < 32; ++k2) acc[rd][k2] = 0.f;
     float2 pre[C::NB][C::NZ];
-    // T[f][y / 8][c][y % 8]: lane reads y = 32 n1 + lane, i.e. block 4 n1 + lane / 8, row lane % 8 of column c = u0 + b
+    // T[f][y / 8][u][y % 8]: lane reads y = 32 n1 + lane, i.e. block 4 n1 + lane / 8, row lane % 8 of column u = u0 + b
     auto fetch = [&](int f) {
         const float2 *src = T + (size_t)f * C::M * NP + (size_t)(lane >> 3) * (C::M * 8) + (size_t)u0 * 8 + (lane & 7);
 #pragma unroll
@@ -222,7 +220,7 @@ psf_col_kernel(PsfDev t, const float2 *__restrict__ T, int F, int fsplit, float 
         const int w = rd * 32 + lane;
         const int my_b = w / C::R1, my_k1 = w % C::R1;
         if (w < C::ITEMS && u0 + my_b < C::M) {
-            const int c = u0 + my_b, uu = (c >> 5) + C::R1 * (c & 31);      // column c of T holds frequency u
+            const int uu = u0 + my_b;                                        // column c of T holds frequency u = c
             const int uo = (uu + C::M / 2) % C::M;
             float *dst = partial + ((size_t)fs * C::M + uo) * C::M;          // [fs][u][v]: the lanes' v are adjacent
 #pragma unroll

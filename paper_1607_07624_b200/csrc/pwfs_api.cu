@@ -659,7 +659,7 @@ static int ensure_chunk_events(pwfs_t *h, size_t n_chunks) {
 static bool small_applies(const pwfs_t *h, int B) {
     const DevTables &t = h->tab;
     if (!h->L.launch_s || h->small_mode == 0 || h->user_fpc > 0 || h->user_ksplit > 0) return false;
-    if (t.N > 64 || t.ncols > 128 || t.D > 64) return false;
+    if (t.N > 64 || t.ncols > 128 || t.D > 64 || t.cmax > 8) return false;   // SmallCfg::MAXN, MAXCOLS, MAXD, MAXCMAX
     if (h->small_mode == 1) return true;
     return (long long)B * t.K <= 16LL * h->num_sms;
 }

@@ -19,7 +19,7 @@ namespace pwk {
 struct SmallCfg : PassCfg<4, 8, 8, 8> {
     static constexpr int WARPS = 8;
     static constexpr int PY = 65;                        // float2 pitch of a T column in shared memory (odd: conflict-free)
-    static constexpr int MAXN = 64, MAXCOLS = 128, MAXD = 64;
+    static constexpr int MAXN = 64, MAXCOLS = 128, MAXD = 64, MAXCMAX = 8;
     // tables + exchange buffers + T + y-rebinned columns
     static constexpr size_t smem_q = (size_t)(1 * TAB + WARPS * WARP_BUF + MAXCOLS * PY) * sizeof(float2) + (size_t)MAXCOLS * (MAXD + 1) * sizeof(float);
     static constexpr size_t smem_t = smem_q + (size_t)TAB * sizeof(float2);
@@ -40,6 +40,10 @@ small_kernel(DevTables t, const float *__restrict__ phase, float *__restrict__ p
     __shared__ float s_red[8];
     __shared__ float s_nbar;
     __shared__ int s_last;
+    // rebin tables in shared memory: the rebin loops chase start -> count -> weight, three dependent loads per
+    // detector bin that would each wait for L2 in a kernel every CTA runs through exactly once
+    __shared__ int s_rb_start[C::MAXD], s_rb_cnt[C::MAXD], s_xc_of_x[C::M];
+    __shared__ float s_rb_w[C::MAXD * C::MAXCMAX];
     const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
     const int N = t.N, NP = t.NP, D = t.D, ncols = t.ncols;
     const int k = blockIdx.x, f = blockIdx.y;
@@ -51,6 +55,10 @@ small_kernel(DevTables t, const float *__restrict__ phase, float *__restrict__ p
     for (int n1 = 0; n1 < C::NZ; ++n1) tyv[n1] = (32 * n1 < NP) ? __ldg(t.tyt + (size_t)k * NP + 32 * n1 + lane) : make_float2(0.f, 0.f);
 
     load_tables<QM, false>(s_tw, smem + C::TAB, t, C::R1);
+    const int cmax = t.cmax;
+    for (int i = threadIdx.x; i < D; i += blockDim.x) { s_rb_start[i] = __ldg(t.rb_start + i); s_rb_cnt[i] = __ldg(t.rb_cnt + i); }
+    for (int i = threadIdx.x; i < D * cmax; i += blockDim.x) s_rb_w[i] = __ldg(t.rb_w + i);
+    for (int i = threadIdx.x; i < C::M; i += blockDim.x) s_xc_of_x[i] = __ldg(t.xc_of_x + i);
     int xc_of[C::R1];                                      // compact column of this lane's x = 32 n1 + lane, -1 outside the windows
 #pragma unroll
     for (int n1 = 0; n1 < C::R1; ++n1) xc_of[n1] = __ldg(t.xc_of_x + 32 * n1 + lane);
@@ -100,75 +108,57 @@ small_kernel(DevTables t, const float *__restrict__ phase, float *__restrict__ p
     }
     __syncthreads();
 
-    // ---- column pass of this modulation point; |E|^2 in registers
+    // ---- column pass of this modulation point (|E|^2 in registers) and y-rebin of every column into s_cb[xc][jy];
+    // one loop over the groups of 64 columns (not unrolled: one copy of the size-32 stage in the instruction stream)
     constexpr int CPASS = C::MAXCOLS / (C::WARPS * C::NB);   // 2 groups of 64 columns
-    float acc[CPASS][C::NB][C::R1];
+    float *colI = reinterpret_cast<float *>(buf);          // NB * M floats <= the warp's buffer
+#pragma unroll 1
+    for (int cp = 0; cp < CPASS; ++cp) {
+        const int xc0 = (cp * C::WARPS + wl) * C::NB;
+        if (xc0 >= ncols) continue;                        // warp-uniform
+        float acc[C::NB][C::R1];
 #pragma unroll
-    for (int cp = 0; cp < CPASS; ++cp)
+        for (int b = 0; b < C::NB; ++b) {
+            float2 v[C::R1];
+#pragma unroll
+            for (int n1 = 0; n1 < C::NZ; ++n1)
+                v[n1] = (32 * n1 + lane < NP && xc0 + b < ncols) ? cmul(s_T[(xc0 + b) * C::PY + 32 * n1 + lane], tyv[n1])
+                                                                  : make_float2(0.f, 0.f);
+            DftP<C::R1, -1, C::NZ>::run(v);
+#pragma unroll
+            for (int k1 = 0; k1 < C::R1; ++k1) buf[C::row_off(b * C::R1 + k1) + lane] = v[k1];
+        }
+        __syncwarp();
+        stage32<C, QM>(buf, s_tw, s_am, lane);
+        __syncwarp();
+#pragma unroll
+        for (int b = 0; b < C::NB; ++b) {
+            float2 v[C::R1];
+#pragma unroll
+            for (int k1 = 0; k1 < C::R1; ++k1) v[k1] = buf[C::row_off(b * C::R1 + k1) + lane];
+            apply_ipow_k1<C::R1, QM>(v);
+            Dft<C::R1, +1>::run(v);
+#pragma unroll
+            for (int n1 = 0; n1 < C::R1; ++n1) acc[b][n1] = fmaf(v[n1].x, v[n1].x, v[n1].y * v[n1].y);
+        }
+        __syncwarp();
 #pragma unroll
         for (int b = 0; b < C::NB; ++b)
 #pragma unroll
-            for (int n1 = 0; n1 < C::R1; ++n1) acc[cp][b][n1] = 0.f;
-    {
-#pragma unroll
-        for (int cp = 0; cp < CPASS; ++cp) {
-            const int xc0 = (cp * C::WARPS + wl) * C::NB;
-            if (xc0 < ncols) {                             // warp-uniform
-#pragma unroll
-                for (int b = 0; b < C::NB; ++b) {
-                    float2 v[C::R1];
-#pragma unroll
-                    for (int n1 = 0; n1 < C::NZ; ++n1)
-                        v[n1] = (32 * n1 + lane < NP && xc0 + b < ncols) ? cmul(s_T[(xc0 + b) * C::PY + 32 * n1 + lane], tyv[n1])
-                                                                          : make_float2(0.f, 0.f);
-                    DftP<C::R1, -1, C::NZ>::run(v);
-#pragma unroll
-                    for (int k1 = 0; k1 < C::R1; ++k1) buf[C::row_off(b * C::R1 + k1) + lane] = v[k1];
+            for (int n1 = 0; n1 < C::R1; ++n1) colI[b * C::M + 32 * n1 + lane] = acc[b][n1];
+        __syncwarp();
+        for (int b = 0; b < C::NB && xc0 + b < ncols; ++b)
+            for (int jj = lane; jj < D; jj += 32) {
+                int y = s_rb_start[jj];
+                const int cnt = s_rb_cnt[jj];
+                float s = 0.f;
+                for (int c = 0; c < cnt; ++c) {
+                    s = fmaf(s_rb_w[jj * cmax + c], colI[b * C::M + y], s);
+                    if (++y == C::M) y = 0;
                 }
-                __syncwarp();
-                stage32<C, QM>(buf, s_tw, s_am, lane);
-                __syncwarp();
-#pragma unroll
-                for (int b = 0; b < C::NB; ++b) {
-                    float2 v[C::R1];
-#pragma unroll
-                    for (int k1 = 0; k1 < C::R1; ++k1) v[k1] = buf[C::row_off(b * C::R1 + k1) + lane];
-                    apply_ipow_k1<C::R1, QM>(v);
-                    Dft<C::R1, +1>::run(v);
-#pragma unroll
-                    for (int n1 = 0; n1 < C::R1; ++n1)
-                        acc[cp][b][n1] = fmaf(v[n1].x, v[n1].x, fmaf(v[n1].y, v[n1].y, acc[cp][b][n1]));
-                }
-                __syncwarp();
+                s_cb[(xc0 + b) * (D + 1) + jj] = s;
             }
-        }
-    }
-
-    // ---- y-rebin of every column into s_cb[xc][jy]
-    float *colI = reinterpret_cast<float *>(buf);          // NB * M floats <= the warp's buffer
-    const int cmax = t.cmax;
-#pragma unroll
-    for (int cp = 0; cp < CPASS; ++cp) {
-        const int xc0 = (cp * C::WARPS + wl) * C::NB;
-        if (xc0 < ncols) {
-#pragma unroll
-            for (int b = 0; b < C::NB; ++b)
-#pragma unroll
-                for (int n1 = 0; n1 < C::R1; ++n1) colI[b * C::M + 32 * n1 + lane] = acc[cp][b][n1];
-            __syncwarp();
-            for (int b = 0; b < C::NB && xc0 + b < ncols; ++b)
-                for (int jj = lane; jj < D; jj += 32) {
-                    int y = __ldg(t.rb_start + jj);
-                    const int cnt = __ldg(t.rb_cnt + jj);
-                    float s = 0.f;
-                    for (int c = 0; c < cnt; ++c) {
-                        s = fmaf(__ldg(t.rb_w + (size_t)jj * cmax + c), colI[b * C::M + y], s);
-                        if (++y == C::M) y = 0;
-                    }
-                    s_cb[(xc0 + b) * (D + 1) + jj] = s;
-                }
-            __syncwarp();
-        }
+        __syncwarp();
     }
     __syncthreads();
 
@@ -176,11 +166,11 @@ small_kernel(DevTables t, const float *__restrict__ phase, float *__restrict__ p
     float *my_part = part + ((size_t)f * gridDim.x + k) * D * D;
     for (int i = threadIdx.x; i < D * D; i += blockDim.x) {
         const int jy = i % D, jx = i / D;                  // jy fastest: conflict-free reads of s_cb
-        int x = __ldg(t.rb_start + jx);
-        const int cnt = __ldg(t.rb_cnt + jx);
+        int x = s_rb_start[jx];
+        const int cnt = s_rb_cnt[jx];
         float s = 0.f;
         for (int c = 0; c < cnt; ++c) {
-            s = fmaf(__ldg(t.rb_w + (size_t)jx * cmax + c), s_cb[__ldg(t.xc_of_x + x) * (D + 1) + jy], s);
+            s = fmaf(s_rb_w[jx * cmax + c], s_cb[s_xc_of_x[x] * (D + 1) + jy], s);
             if (++x == C::M) x = 0;
         }
         my_part[jy * D + jx] = s * scale;
