@@ -2,7 +2,7 @@
 """bench.py -- pyramid-WFS frames/s and fraction of roofline on B200.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
-                    [--config cfg4_elt] [--no-cpu-baseline] [--no-stages] [--no-configs]
+                    [--config cfg4_elt] [--no-cpu-baseline] [--no-stages] [--no-configs] [--no-loops]
 
 --gpus N > 1 without a launcher starts N ranks itself (torch.distributed.run on
 127.0.0.1, one per GPU); under a launcher (WORLD_SIZE set) it must equal WORLD_SIZE.
@@ -122,7 +122,7 @@ def measured_hbm_peak():
         return 6550.0, "fallback (B200_PROFILING.md)"
 
 
-def bench_stages(cfg, dev, phase, frames, flush, reps: int = 5) -> dict:
+def bench_stages(cfg, dev, phase, frames, flush, reps: int = 5, loops: bool = True) -> dict:
     """The rows of SURVEY.md 8(f) on this config's geometry, each timed alone with CUDA events on the
     launching stream (L2 flushed before every timed call) and set against the roofline that bounds it:
     algorithmic bytes / measured HBM copy bandwidth, or nominal flop / derived FP32 peak."""
@@ -221,7 +221,7 @@ def bench_stages(cfg, dev, phase, frames, flush, reps: int = 5) -> dict:
                                   f"{n_act} actuators x {pix.size} pupil pixels, one frame: the influence matrix streamed once")
     del ifs
     # the whole device chain as a loop runs it: one simulation step per iteration (f1 -> a1-a8 -> f2), n_inst frames
-    if not cfg.independent_screens:
+    if loops and not cfg.independent_screens:
         atm = wl.atmosphere(cfg)
         n_inst = len(atm["dirs_tan"]) * len(atm["wl_scale"])
         with Atmosphere(**{k: v for k, v in atm.items() if k != "dt"}, device=dev.index) as a, \
@@ -702,7 +702,7 @@ def run_ours(args, cfg):
                 "executed_pair_ratio": r["executed_pair_ratio"], "kernel_ms_per_step": r["kernel_ms_per_step"],
                 "steps": args.steps, "warmup": args.warmup, "input": "numpy generator (the headline run above)"}
         if not args.no_stages:
-            line["stages"] = bench_stages(cfg, dev, phase, frames, flush)
+            line["stages"] = bench_stages(cfg, dev, phase, frames, flush, loops=not args.no_loops)
         if not args.no_cpu_baseline:
             nfr = oracle_sample_frames(cfg)
             dt, cores = time_oracle(cfg, nfr)
@@ -743,6 +743,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-stages", action="store_true", help="skip the per-stage timings of the 8(f) rows")
     ap.add_argument("--no-configs", action="store_true", help="skip the timings of the other four configs")
+    ap.add_argument("--no-loops", action="store_true",
+                    help="stage timings without the chain / closed-loop rows (thousands of single-frame launches; for profiling runs)")
     ap.add_argument("--dry-run", action="store_true",
                     help="CPU stand-in sensor on gloo: exercises launch/sharding/timing/report plumbing only")
     args = ap.parse_args()

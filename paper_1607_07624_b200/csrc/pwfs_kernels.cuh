@@ -41,31 +41,34 @@ constexpr int kTB = 8;
 // reads row w at w * kPitch: 16 consecutive lanes hit 16 different 64-bit banks), except that a pad TPAD may separate
 // the NB transforms when R1 is a multiple of 16 (a half warp of the size-32 stage then never straddles two transforms).
 // The row pass's transposed last stage reads, per instruction, 8 rows r = 8 r_hi + r_lo of the CTA (= 8 transforms,
-// spread over 8 / NB warps) x 2 adjacent columns per half warp; the pad between warps (low byte of the result) and
-// TPAD (next byte) are chosen so that those 16 accesses fall in as many different banks as possible: all 16 for
-// NB = 1, for R1 = 6, 10, 18 and, with TPAD, for R1 = 16, 32, 48, 64.
+// spread over 8 / NB warps) x 2 columns per half warp -- adjacent columns n2, n2 + 1, or (SWAP) n2, n2 + 2 with the
+// other half warp taking n2 + 1, n2 + 3: the warp covers the same 8 rows x 4 columns either way.  The pad between
+// warps (bits 0-7 of the result), TPAD (bits 8-15) and SWAP (bit 16) are chosen so that those 16 accesses fall in as
+// many different banks as possible: all 16 for NB = 1, for R1 = 6, 10, 18, with TPAD for R1 = 16, 32, 48, 64, and with
+// SWAP for odd R1 and NB = 2 (R1 = 15, 25, 27: rows r, r + 1 are an odd number of banks apart).
 constexpr int pick_pads(int R1, int NB, int RPC) {
     int best_code = 0, best = 1 << 30;
     const int tmax = (R1 % 16 == 0 && NB > 1) ? 16 : 1;
-    for (int tpad = 0; tpad < tmax; ++tpad)
-        for (int pad = 0; pad < 16; ++pad) {
-            const int wb = NB * R1 * kPitch + (NB - 1) * tpad + pad;
-            int tot = 0;
-            for (int rhi = 0; rhi < RPC / kTB; ++rhi) {
-                int cnt[16] = {};
-                int worst = 0;
-                for (int rlo = 0; rlo < kTB; ++rlo) {
-                    const int r = kTB * rhi + rlo;
-                    const int off = (r / NB) * wb + (r % NB) * (R1 * kPitch + tpad);
-                    for (int n2 = 0; n2 < 2; ++n2) {
-                        const int c = ++cnt[(off + n2) % 16];
-                        worst = c > worst ? c : worst;
+    for (int swap = 0; swap < 2; ++swap)
+        for (int tpad = 0; tpad < tmax; ++tpad)
+            for (int pad = 0; pad < 16; ++pad) {
+                const int wb = NB * R1 * kPitch + (NB - 1) * tpad + pad;
+                int tot = 0;
+                for (int rhi = 0; rhi < RPC / kTB; ++rhi) {
+                    int cnt[16] = {};
+                    int worst = 0;
+                    for (int rlo = 0; rlo < kTB; ++rlo) {
+                        const int r = kTB * rhi + rlo;
+                        const int off = (r / NB) * wb + (r % NB) * (R1 * kPitch + tpad);
+                        for (int n2 = 0; n2 < 2; ++n2) {
+                            const int c = ++cnt[(off + (swap ? 2 * n2 : n2)) % 16];
+                            worst = c > worst ? c : worst;
+                        }
                     }
+                    tot += worst;
                 }
-                tot += worst;
+                if (tot < best) { best = tot; best_code = swap * 65536 + tpad * 256 + pad; }
             }
-            if (tot < best) { best = tot; best_code = tpad * 256 + pad; }
-        }
     return best_code;
 }
 
@@ -79,7 +82,8 @@ struct PassCfg {
     static constexpr int NZ = (R1_ + 1) / 2; // M >= 2N  =>  at most ceil(R1/2) non-zero inputs per lane
     static constexpr int ITEMS = NB_ * R1_;  // size-32 DFTs per warp batch
     static constexpr int ROUNDS = (ITEMS + 31) / 32;
-    static constexpr int TPAD = pick_pads(R1_, NB_, NB_ * WPB_X_) / 256;            // float2 between the NB transforms
+    static constexpr int TPAD = (pick_pads(R1_, NB_, NB_ * WPB_X_) >> 8) & 255;     // float2 between the NB transforms
+    static constexpr bool SWAP = (pick_pads(R1_, NB_, NB_ * WPB_X_) >> 16) != 0;     // column order of the transposed stage
     static constexpr int TR_BUF = R1_ * kPitch + TPAD;                               // float2 per transform
     static constexpr int WARP_BUF = ITEMS * kPitch + (NB_ - 1) * TPAD + pick_pads(R1_, NB_, NB_ * WPB_X_) % 256;   // float2 per warp
     // offset of exchange row (transform b, k1) in the warp's buffer; w = b * R1 + k1
@@ -284,13 +288,14 @@ xpass_kernel(DevTables t, const float *__restrict__ phase, float2 *__restrict__ 
     }
 
     // transposed last stage: this thread's items it < NB are (row r = 8 r_hi + r_lo, column residue n2) with
-    // r_lo = i % 8, n2 = (i / 8) % 32, r_hi = i / 256 for i = threadIdx.x + it * blockDim.x
+    // r_lo = i % 8, n2 = (i / 8) % 32 (its two low bits exchanged when C::SWAP), r_hi = i / 256 for i = threadIdx.x + it * blockDim.x
     int item_src[C::NB];          // exchange-buffer offset of (row r, k1 = 0, n2): transform r of the CTA
     int item_dst[C::NB];          // T offset of (x = n2, y = y0 + r) within the (f, j) slab; < 0: row beyond NP
 #pragma unroll
     for (int it = 0; it < C::NB; ++it) {
         const int i = threadIdx.x + it * 32 * C::WPB_X;
-        const int r = (i >> 8) * kTB + (i & 7), n2 = (i >> 3) & 31;
+        const int g = (i >> 3) & 31;
+        const int r = (i >> 8) * kTB + (i & 7), n2 = C::SWAP ? ((g & ~3) | ((g & 1) << 1) | ((g >> 1) & 1)) : g;
         item_src[it] = (r / C::NB) * C::WARP_BUF + (r % C::NB) * C::TR_BUF + n2;
         item_dst[it] = (y0 + r < t.NP) ? ((y0 + r) / kTB) * (C::M * kTB) + n2 * kTB + (i & 7) : -1;
     }

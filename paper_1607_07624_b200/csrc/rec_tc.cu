@@ -9,18 +9,20 @@
 // recmat is streamed from HBM as it is (FP32, 4 bytes per element) and split INSIDE the pipeline; the
 // (small) slope planes are written by a split kernel per call.
 //
-// Kernel (one 128 x 128 output tile of one K split per CTA, 192 threads):
+// Kernel (one 128 x 128 output tile of one K split per CTA, 320 threads):
 //   warp 0 (one lane)  TMA producer: three 128 x 32 FP32 boxes per stage (recmat raw, Shi, Slo;
 //                      128-byte swizzle) into a 4-stage ring, completion on the stage's "full" mbarrier;
-//   warps 2-5          converters: thread = row of the recmat tile; reads its 32 raw values (undoing the
-//                      swizzle in the address), hi = tf32(x), lo = tf32(x - hi), and writes both planes
-//                      into TENSOR MEMORY (tcgen05.st 32x32b.x32: lane = row, column = k), then arrives on
-//                      the stage's "conv" mbarrier;
-//   warp 1 (one lane)  MMA issuer: waits for "conv", per stage 4 K steps x 3 UMMAs (M 128, N 128, K 8),
+//   warps 2-9          converters: two warps per TMEM lane quarter, thread = (row of the recmat tile, half of
+//                      its 32 K values); reads its 16 raw values (undoing the swizzle in the address),
+//                      hi = tf32(x), lo = tf32(x - hi), and writes both planes into TENSOR MEMORY
+//                      (tcgen05.st 32x32b.x16: lane = row, column = k), then arrives on the stage's "conv"
+//                      mbarrier;
+//   warp 1 (one lane)  MMA issuer: waits for "conv", per stage 4 K steps x 3 UMMAs (M 128, N = frames rounded
+//                      up to 16, K 8),
 //                      A (recmat hi / lo) from tensor memory, B (slope planes) from shared-memory
 //                      descriptors, into 128 TMEM columns; tcgen05.commit releases the stage ("empty")
 //                      and, after the last one, signals the epilogue;
-//   warps 2-5 again    epilogue: tcgen05.ld 32 lanes x 32 columns at a time, rows = modes so that a
+//   warps 2-9 again    epilogue: tcgen05.ld 32 lanes x 32 columns at a time, rows = modes so that a
 //                      column store is one coalesced 128-byte line of modes[b][m0..m0+32).
 // Tiles x K splits ~ number of SMs; the split-K partial sums are added in a fixed order by a second
 // kernel (deterministic, no atomics).  Per stage the CTA needs 16 KB from HBM, 768 tensor-core cycles
@@ -31,6 +33,7 @@
 #include <cuda.h>
 
 #include <cstdint>
+#include <cstdlib>
 #include <new>
 
 #include "../../include/pwfs.h"
@@ -40,17 +43,20 @@ namespace {
 constexpr int BM = 128, BN = 128, BK = 32, UK = 8, STAGES = 4;
 constexpr int kTileBytes = BM * BK * 4;               // 16 KB, one operand plane of one stage
 constexpr int kStageBytes = 3 * kTileBytes;           // recmat raw, Shi, Slo
-constexpr int kThreads = 192;
+constexpr int kThreads = 320;                         // warp 0 TMA, warp 1 MMA, warps 2..9 converters / epilogue
 constexpr uint32_t kAccCols = 128;                    // accumulator: TMEM columns [0, 128)
 constexpr uint32_t kTmemCols = 512;                   // + per stage 32 columns of recmat hi and 32 of lo: 128 + 4 * 64 = 384 -> 512
 constexpr int kLoadBytes = 3 * kTileBytes;            // what TMA brings per stage
-constexpr int kConvThreads = 128;                     // warps 2..5
+constexpr int kConvThreads = 256;                     // warps 2..9: two per TMEM lane quarter, 16 K values each
 constexpr size_t kSmemBytes = (size_t)STAGES * kStageBytes + 1024 /* alignment slack */ + 256 /* barriers */;
 static_assert(BK * 4 == 128, "one K block is one 128-byte swizzle row");
 
 // tcgen05 instruction descriptor, kind::tf32: D = F32 (bits 4-5 = 1), A = B = TF32 (bits 7-9, 10-12 = 2),
 // both K-major (bits 15, 16 = 0), N >> 3 at bits 17-22, M >> 4 at bits 24-28.
-constexpr uint32_t kIdesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+// N is the frames of the tile rounded up to 16 (B = 100: N = 112, an eighth fewer tensor cycles than the full tile).
+__host__ __device__ constexpr uint32_t idesc_for(int n) {
+    return (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+}
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -91,22 +97,14 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map
 __device__ __forceinline__ uint64_t smem_desc(uint32_t saddr) {
     return (uint64_t)((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
 }
-__device__ __forceinline__ void umma_tf32(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t accumulate) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "setp.ne.b32 p, %4, 0;\n"
-        "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n"
-        "}\n" ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(kIdesc), "r"(accumulate) : "memory");
-}
 // A operand in tensor memory (lane = row of the 128 x 8 tile, one TF32 value per 32-bit column), B from shared memory
-__device__ __forceinline__ void umma_tf32_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t bdesc, uint32_t accumulate) {
+__device__ __forceinline__ void umma_tf32_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
         "setp.ne.b32 p, %4, 0;\n"
         "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n"
-        "}\n" ::"r"(tmem_d), "r"(tmem_a), "l"(bdesc), "r"(kIdesc), "r"(accumulate) : "memory");
+        "}\n" ::"r"(tmem_d), "r"(tmem_a), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
 }
 __device__ __forceinline__ void tmem_st_32x32(uint32_t taddr, const uint32_t (&r)[32]) {
     asm volatile(
@@ -117,6 +115,14 @@ __device__ __forceinline__ void tmem_st_32x32(uint32_t taddr, const uint32_t (&r
           "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]),
           "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]),
           "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
+        : "memory");
+}
+__device__ __forceinline__ void tmem_st_32x16(uint32_t taddr, const uint32_t (&r)[16]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
+        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
+        ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
+          "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
         : "memory");
 }
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
@@ -185,6 +191,8 @@ rec_tc_kernel(const __grid_constant__ CUtensorMap mR,
         }
     } else if (warp == 1) {
         if (lane == 0) {                                                  // ---- MMA issuer
+            const int n_here = min(BN, (B - n_tile * BN + 15) / 16 * 16);
+            const uint32_t idesc = idesc_for(n_here);
             int it = 0;
             for (int kb = kb_lo; kb < kb_hi; ++kb, ++it) {
                 const int s = it % STAGES;
@@ -196,29 +204,34 @@ rec_tc_kernel(const __grid_constant__ CUtensorMap mR,
                 for (int k = 0; k < BK / UK; ++k) {
                     const uint32_t ko = k * UK * 4;                      // 32 bytes along the swizzled row
                     const uint64_t shi = smem_desc(st + 1 * kTileBytes + ko), slo = smem_desc(st + 2 * kTileBytes + ko);
-                    umma_tf32_ts(tmem, a_lo + k * UK, shi, (it > 0 || k > 0) ? 1u : 0u);   // small terms first
-                    umma_tf32_ts(tmem, a_hi + k * UK, slo, 1u);
-                    umma_tf32_ts(tmem, a_hi + k * UK, shi, 1u);
+                    umma_tf32_ts(tmem, a_lo + k * UK, shi, idesc, (it > 0 || k > 0) ? 1u : 0u);   // small terms first
+                    umma_tf32_ts(tmem, a_hi + k * UK, slo, idesc, 1u);
+                    umma_tf32_ts(tmem, a_hi + k * UK, shi, idesc, 1u);
                 }
                 umma_commit(empty);                                       // frees the stage when these UMMAs retire
             }
             umma_commit(bar_acc);
         }
-    } else {                                                              // ---- warps 2..5: converters, then epilogue
+    } else {                                                              // ---- warps 2..9: converters, then epilogue
+        // A warp may touch the TMEM lanes 32 (warp % 4) .. + 32 only; the two warps of a lane quarter (warp, warp + 4)
+        // share its rows: `half` 0 takes the K values 0..15 of a row, `half` 1 the values 16..31.  (One warp per
+        // quarter converting all 32 values was the pipeline's bottleneck: ~300 dependent ALU instructions per stage
+        // on a scheduler that has nothing else to issue, against 768 tensor-core cycles.)
+        const int q = warp & 3, half = (warp - 2) >> 2;
         {
             int it = 0;
             for (int kb = kb_lo; kb < kb_hi; ++kb, ++it) {
                 const int s = it % STAGES;
                 const uint32_t full = bars + 8 * s, conv = bars + 8 * (2 * STAGES + s);
                 mbar_wait(full, (it / STAGES) & 1);
-                // thread = row of the tile (TMEM lane 32 (warp % 4) + lane); its 32 K values are 8 chunks of 16 bytes that
-                // TMA's 128-byte swizzle has stored at chunk position c ^ (row % 8)
-                const int row = (warp & 3) * 32 + lane;
+                // thread = (row of the tile = TMEM lane 32 q + lane, half); a row's 32 K values are 8 chunks of 16 bytes
+                // that TMA's 128-byte swizzle has stored at chunk position c ^ (row % 8)
+                const int row = q * 32 + lane;
                 const uint8_t *tile = smem_raw + (base - smem_u32(smem_raw)) + s * kStageBytes + row * 128;
-                uint32_t hi[32], lo[32];
+                uint32_t hi[16], lo[16];
 #pragma unroll
-                for (int c = 0; c < 8; ++c) {
-                    const float4 x = *reinterpret_cast<const float4 *>(tile + ((c ^ (row & 7)) << 4));
+                for (int c = 0; c < 4; ++c) {
+                    const float4 x = *reinterpret_cast<const float4 *>(tile + (((4 * half + c) ^ (row & 7)) << 4));
                     const float xv[4] = {x.x, x.y, x.z, x.w};
 #pragma unroll
                     for (int e = 0; e < 4; ++e) {
@@ -226,20 +239,19 @@ rec_tc_kernel(const __grid_constant__ CUtensorMap mR,
                         lo[4 * c + e] = to_tf32(xv[e] - __uint_as_float(hi[4 * c + e]));
                     }
                 }
-                const uint32_t t_hi = tmem + ((uint32_t)((warp & 3) * 32) << 16) + kAccCols + (uint32_t)s * 64u;
-                tmem_st_32x32(t_hi, hi);
-                tmem_st_32x32(t_hi + 32u, lo);
+                const uint32_t t_hi = tmem + ((uint32_t)(q * 32) << 16) + kAccCols + (uint32_t)s * 64u + (uint32_t)half * 16u;
+                tmem_st_32x16(t_hi, hi);
+                tmem_st_32x16(t_hi + 32u, lo);
                 asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
                 asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
                 mbar_arrive(conv);
             }
         }
-        const int q = warp & 3;                                           // TMEM lane quarter this warp may read
         mbar_wait(bar_acc, 0);
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         const int m = m_tile * BM + q * 32 + lane;
         float *out = dst + (size_t)ks * B * n_modes;
-        for (int c0 = 0; c0 < BN; c0 += 32) {
+        for (int c0 = 32 * half; c0 < BN; c0 += 64) {                    // the quarter's two warps alternate over the columns
             const int n0 = n_tile * BN + c0;
             if (n0 >= B) break;                                           // warp-uniform
             uint32_t r[32];
@@ -341,6 +353,7 @@ int rec_tc_create(RecTc **out, const float *d_R, int n_modes, int n_slopes, int 
 static int rec_tc_ksplit(const RecTc *h, int B) {
     const int m_tiles = (h->n_modes + BM - 1) / BM, n_tiles = (B + BN - 1) / BN, nkb = h->ldp / BK;
     int ksplit = h->num_sms / (m_tiles * n_tiles);
+    if (const char *e = std::getenv("PWFS_REC_KSPLIT")) { const int v = std::atoi(e); if (v > 0) ksplit = v; }   // tuning hook
     if (ksplit > nkb / 4) ksplit = nkb / 4;                               // at least 4 K blocks per split
     return ksplit < 1 ? 1 : ksplit;
 }
