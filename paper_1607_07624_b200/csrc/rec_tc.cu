@@ -90,6 +90,22 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map
         "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
         ::"r"(dst), "l"((uint64_t)map), "r"(bar), "r"(c0), "r"(c1) : "memory");
 }
+// The same load delivered to the CTAs of the cluster named in cta_mask (same shared-memory offset in each, completion
+// bytes on the mbarrier at the same offset in each)
+__device__ __forceinline__ void tma_load_2d_mc(uint32_t dst, const CUtensorMap *map, uint32_t bar, int c0, int c1, uint16_t cta_mask) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster [%0], [%1, {%3, %4}], [%2], %5;"
+        ::"r"(dst), "l"((uint64_t)map), "r"(bar), "r"(c0), "r"(c1), "h"(cta_mask) : "memory");
+}
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
 // Shared-memory matrix descriptor, K-major operand in the canonical 128-byte-swizzle layout (what TMA
 // SWIZZLE_128B writes for a box of 32 floats x rows): start >> 4 at bits 0-13, leading offset unused for
 // swizzled K-major (1), stride offset = 8 rows x 128 B = 1024 >> 4 at bits 32-45, descriptor version 1
@@ -106,17 +122,6 @@ __device__ __forceinline__ void umma_tf32_ts(uint32_t tmem_d, uint32_t tmem_a, u
         "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n"
         "}\n" ::"r"(tmem_d), "r"(tmem_a), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
 }
-__device__ __forceinline__ void tmem_st_32x32(uint32_t taddr, const uint32_t (&r)[32]) {
-    asm volatile(
-        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
-        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
-        "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};"
-        ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
-          "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]),
-          "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]),
-          "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
-        : "memory");
-}
 __device__ __forceinline__ void tmem_st_32x16(uint32_t taddr, const uint32_t (&r)[16]) {
     asm volatile(
         "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
@@ -127,6 +132,11 @@ __device__ __forceinline__ void tmem_st_32x16(uint32_t taddr, const uint32_t (&r
 }
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+// the same arrival on the mbarrier at this offset in every CTA of cta_mask
+__device__ __forceinline__ void umma_commit_mc(uint32_t bar, uint16_t cta_mask) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+                 ::"r"(bar), "h"(cta_mask) : "memory");
 }
 __device__ __forceinline__ void tmem_ld_32x32(uint32_t taddr, uint32_t (&r)[32]) {
     asm volatile(
@@ -141,12 +151,21 @@ __device__ __forceinline__ void tmem_ld_32x32(uint32_t taddr, uint32_t (&r)[32])
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
 
-// grid (m_tiles, ksplit, n_tiles); block 192; dynamic smem kSmemBytes.
+// grid (m_tiles rounded up to 2, ksplit, n_tiles) in clusters of two CTAs along x; block 320; dynamic smem kSmemBytes.
 // dst: modes [B][n_modes] when ksplit == 1, else partials [ksplit][B][n_modes].
-__global__ void __launch_bounds__(kThreads, 1)
+//
+// The two CTAs of a cluster work on neighbouring m tiles of the SAME K range and frame tile, so they need the same
+// slope planes: rank 0 loads Shi, rank 1 loads Slo, each as one TMA multicast to both CTAs.  Every recmat byte then
+// costs 2 instead of 3 bytes of L2 -> SM traffic (576 -> 384 MB per call on cfg 4).  A stage of either CTA may be
+// overwritten by the other's multicast, so a stage is free when BOTH MMA warps are done with it: tcgen05.commit
+// arrives on the "empty" barrier of both CTAs (count 2).  Measured: the call takes the same time with and without the
+// multicast (ncu: the converters wait for TMA, DRAM 40 %, tensor pipe 60 %) -- what limits the kernel is the HBM bytes
+// a CTA has in flight (four stages of 16 KB of recmat), not the traffic out of L2; kept because it takes a third of
+// that traffic away from whatever runs beside it.
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 rec_tc_kernel(const __grid_constant__ CUtensorMap mR,
               const __grid_constant__ CUtensorMap mShi, const __grid_constant__ CUtensorMap mSlo,
-              float *__restrict__ dst, int n_modes, int B, int nkb, int ksplit) {
+              float *__restrict__ dst, int n_modes, int B, int nkb, int ksplit, int m_tiles) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;          // 128-byte swizzle needs 1024-byte tiles
     const uint32_t bars = base + STAGES * kStageBytes;
@@ -161,7 +180,7 @@ rec_tc_kernel(const __grid_constant__ CUtensorMap mR,
     if (threadIdx.x == 0) {
         for (int s = 0; s < STAGES; ++s) {
             mbar_init(bars + 8 * s, 1);
-            mbar_init(bars + 8 * (STAGES + s), 1);
+            mbar_init(bars + 8 * (STAGES + s), 2);                        // both CTAs of the cluster release a stage
             mbar_init(bars + 8 * (2 * STAGES + s), kConvThreads);
         }
         mbar_init(bar_acc, 1);
@@ -173,8 +192,11 @@ rec_tc_kernel(const __grid_constant__ CUtensorMap mR,
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
+    cluster_sync_all();                                                   // the peer's barriers exist before anything is sent to them
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tmem = *tmem_slot;
+    const uint32_t crank = cluster_ctarank();
+    const int m_load = min(m_tile, m_tiles - 1);                          // padding CTA of an odd m_tiles: same protocol, nothing stored
 
     if (warp == 0) {
         if (lane == 0) {                                                  // ---- TMA producer
@@ -184,9 +206,9 @@ rec_tc_kernel(const __grid_constant__ CUtensorMap mR,
                 const uint32_t full = bars + 8 * s, empty = bars + 8 * (STAGES + s), st = base + s * kStageBytes;
                 mbar_wait(empty, ((it / STAGES) & 1) ^ 1);
                 mbar_expect_tx(full, kLoadBytes);
-                tma_load_2d(st + 0 * kTileBytes, &mR, full, kb * BK, m_tile * BM);      // raw FP32 recmat
-                tma_load_2d(st + 1 * kTileBytes, &mShi, full, kb * BK, n_tile * BN);
-                tma_load_2d(st + 2 * kTileBytes, &mSlo, full, kb * BK, n_tile * BN);
+                tma_load_2d(st + 0 * kTileBytes, &mR, full, kb * BK, m_load * BM);      // raw FP32 recmat
+                if (crank == 0) tma_load_2d_mc(st + 1 * kTileBytes, &mShi, full, kb * BK, n_tile * BN, (uint16_t)3);
+                else tma_load_2d_mc(st + 2 * kTileBytes, &mSlo, full, kb * BK, n_tile * BN, (uint16_t)3);
             }
         }
     } else if (warp == 1) {
@@ -208,7 +230,7 @@ rec_tc_kernel(const __grid_constant__ CUtensorMap mR,
                     umma_tf32_ts(tmem, a_hi + k * UK, slo, idesc, 1u);
                     umma_tf32_ts(tmem, a_hi + k * UK, shi, idesc, 1u);
                 }
-                umma_commit(empty);                                       // frees the stage when these UMMAs retire
+                umma_commit_mc(empty, (uint16_t)3);                       // frees the stage in BOTH CTAs when these UMMAs retire
             }
             umma_commit(bar_acc);
         }
@@ -265,6 +287,7 @@ rec_tc_kernel(const __grid_constant__ CUtensorMap mR,
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
+    cluster_sync_all();                                                   // no CTA leaves while the peer may still signal it
     if (warp == 2)
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(kTmemCols) : "memory");
 }
@@ -352,7 +375,7 @@ int rec_tc_create(RecTc **out, const float *d_R, int n_modes, int n_slopes, int 
 
 static int rec_tc_ksplit(const RecTc *h, int B) {
     const int m_tiles = (h->n_modes + BM - 1) / BM, n_tiles = (B + BN - 1) / BN, nkb = h->ldp / BK;
-    int ksplit = h->num_sms / (m_tiles * n_tiles);
+    int ksplit = h->num_sms / ((m_tiles + 1) / 2 * 2 * n_tiles);
     if (const char *e = std::getenv("PWFS_REC_KSPLIT")) { const int v = std::atoi(e); if (v > 0) ksplit = v; }   // tuning hook
     if (ksplit > nkb / 4) ksplit = nkb / 4;                               // at least 4 K blocks per split
     return ksplit < 1 ? 1 : ksplit;
@@ -397,8 +420,8 @@ int rec_tc_run(RecTc *h, const float *d_slopes, int B, float *d_modes, cudaStrea
     if (int rc = rec_tc_reserve(h, B, st)) return rc;                     // no-op once sized (pwfs_rec_reserve)
     split_tf32_kernel<<<dim3((h->ldp + 255) / 256, B), 256, 0, st>>>(d_slopes, (size_t)h->n_slopes, h->n_slopes, h->ldp,
                                                                     h->d_Shi, h->d_Slo);
-    rec_tc_kernel<<<dim3(m_tiles, ksplit, n_tiles), kThreads, kSmemBytes, st>>>(
-        h->mR, h->mShi, h->mSlo, ksplit > 1 ? h->d_part : d_modes, h->n_modes, B, nkb, ksplit);
+    rec_tc_kernel<<<dim3((m_tiles + 1) / 2 * 2, ksplit, n_tiles), kThreads, kSmemBytes, st>>>(
+        h->mR, h->mShi, h->mSlo, ksplit > 1 ? h->d_part : d_modes, h->n_modes, B, nkb, ksplit, m_tiles);
     if (ksplit > 1) {
         const size_t n = (size_t)B * h->n_modes;
         splitk_sum_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(h->d_part, n, ksplit, d_modes);
