@@ -73,7 +73,8 @@ constexpr int pick_pads(int R1, int NB, int RPC) {
 }
 
 // YMODE_ (column pass): bit 0 = the T column is staged in shared memory by cp.async instead of waiting in registers,
-// bit 1 = the size-32 stage keeps its 32 twiddles in registers for both multiplies.
+// bit 1 = the size-32 stage keeps its 32 twiddles in registers for both multiplies, bit 2 = they are read once per
+// kernel and stay in registers (single-round configurations: NB * R1 <= 32).
 template <int R1_, int NB_, int WPB_X_, int WPB_Y_, int MINB_X_ = 1, int MINB_Y_ = 1, int YMODE_ = 0>
 struct PassCfg {
     static constexpr int R1 = R1_;           // M / 32
@@ -105,6 +106,7 @@ struct PassCfg {
     static constexpr int YMODE = YMODE_;
     static constexpr bool Y_ASYNC = (YMODE_ & 1) != 0;
     static constexpr bool Y_TWKEEP = (YMODE_ & 2) != 0;
+    static constexpr bool Y_TWRES = (YMODE_ & 4) != 0;     // twiddles resident in registers for the whole kernel
     static constexpr int PRE_BUF = Y_ASYNC ? NB_ * NZ * 32 : 0;
     static constexpr size_t smem_y_q = (size_t)(WPB_Y_ * (WARP_BUF + PRE_BUF) + 1 * TAB) * sizeof(float2);
     static constexpr size_t smem_y_t = (size_t)(WPB_Y_ * (WARP_BUF + PRE_BUF) + (AM_GLOBAL ? 1 : 2) * TAB) * sizeof(float2);
@@ -177,10 +179,15 @@ __device__ __forceinline__ void idft32_signed_upper(float2 (&x)[32], float2 sg2)
 // per-lane sign absorbed by idft32_signed_upper, and i^k1 is applied where k1 is a compile-time
 // register index (step A' of the callers, apply_ipow_k1).  The mask and its table cost nothing;
 // the 1/M per axis moves into the final frame scale.
-// KEEP: the 32 twiddles of the lane are read once into registers and serve both multiplies (64 registers for a third
-// less shared-memory traffic in this stage); otherwise the compiler decides whether the second multiply re-reads them.
-template <class C, bool QM, bool KEEP = false>
-__device__ __forceinline__ void stage32(float2 *buf, const float2 *s_tw, const float2 *s_am, int lane) {
+// TW = 1 (keep): the 32 twiddles of the lane are read once into registers and serve both multiplies (64 registers for a
+// third less shared-memory traffic in this stage); TW = 0: the compiler decides whether the second multiply re-reads
+// them; TW = 2 (resident, single-round configurations only: the lane's k1 never changes): the caller read them once,
+// before its loop over the modulation points, and passes them in `twres`.
+template <class C, bool QM, int TW = 0>
+__device__ __forceinline__ void stage32(float2 *buf, const float2 *s_tw, const float2 *s_am, int lane,
+                                        const float2 *twres = nullptr) {
+    constexpr bool KEEP = TW == 1;
+    static_assert(TW != 2 || C::ROUNDS == 1, "resident twiddles need a single round of the size-32 stage");
 #pragma unroll
     for (int rd = 0; rd < C::ROUNDS; ++rd) {
         int w = rd * 32 + lane;
@@ -193,6 +200,7 @@ __device__ __forceinline__ void stage32(float2 *buf, const float2 *s_tw, const f
 #pragma unroll
             for (int n2 = 0; n2 < 32; ++n2) {
                 if constexpr (KEEP) { twv[n2] = twr[n2]; u[n2] = cmul(row[n2], twv[n2]); }
+                else if constexpr (TW == 2) u[n2] = cmul(row[n2], twres[n2]);
                 else u[n2] = cmul(row[n2], twr[n2]);
             }
             Dft<32, -1>::run(u);
@@ -211,7 +219,7 @@ __device__ __forceinline__ void stage32(float2 *buf, const float2 *s_tw, const f
                 Dft<32, +1>::run(u);
             }
 #pragma unroll
-            for (int n2 = 0; n2 < 32; ++n2) row[n2] = cmulc(u[n2], KEEP ? twv[n2] : twr[n2]);
+            for (int n2 = 0; n2 < 32; ++n2) row[n2] = cmulc(u[n2], KEEP ? twv[n2] : TW == 2 ? twres[n2] : twr[n2]);
         }
     }
 }
@@ -422,6 +430,12 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
                 }
             }
     };
+    [[maybe_unused]] float2 twres[C::Y_TWRES ? 32 : 1];
+    if constexpr (C::Y_TWRES) {
+        const float2 *twr = s_tw + (lane % C::R1) * kPitch;
+#pragma unroll
+        for (int n2 = 0; n2 < 32; ++n2) twres[n2] = twr[n2];
+    }
     int2 kj = make_int2(0, -1), kj_next = make_int2(0, -1), kj_next2 = make_int2(0, -1);
     if (k_lo < k_hi) {
         kj_next = __ldg(t.kj + k_lo);
@@ -451,7 +465,7 @@ ypass_kernel(DevTables t, const float2 *__restrict__ T, float *__restrict__ colb
             for (int k1 = 0; k1 < C::R1; ++k1) buf[C::row_off(b * C::R1 + k1) + lane] = v[k1];
         }
         __syncwarp();
-        stage32<C, QM, C::Y_TWKEEP>(buf, s_tw, s_am, lane);
+        stage32<C, QM, C::Y_TWRES ? 2 : C::Y_TWKEEP ? 1 : 0>(buf, s_tw, s_am, lane, twres);
         __syncwarp();
 #pragma unroll
         for (int b = 0; b < C::NB; ++b) {

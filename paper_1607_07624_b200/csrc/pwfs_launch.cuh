@@ -50,18 +50,20 @@ template <> struct CfgFor<64> { using type = PassCfg<64, 1, 8, 4, 1, 1>; };   //
 // 125 items, was tried: the exchange buffers then allow only 6 warps per SM and the column pass ran 1.6x slower.)
 // YMODE (last argument; measured on B200, profiles/r2_tuning.md): 2 = twiddles kept in registers through the size-32
 // stage (left to the compiler, an unrelated source change moved M = 800 between 33.3 and 40.3 ms per 600 frames);
-// 1 = T column staged by cp.async, 168 registers, 3 CTAs per SM (M = 1024: 9.74 -> 9.5x ms per 100 frames; M = 320:
-// 5.09 -> 5.0x; slower on M = 480 and 800).  R1 > 32 keeps the compiler's choice (64 register points per lane already).
+// 1 = T column staged by cp.async, 168 registers, 3 CTAs per SM (M = 1024: 9.74 -> 9.69 ms per 100 frames; M = 320:
+// 5.09 -> 5.04; slower on M = 480 and 800); 5 = staged T column AND the twiddles resident in registers for the whole
+// kernel, still 168 registers (M = 800: 33.05 -> 31.84; slower on M = 1024: 10.16, and M = 320: 5.16).  R1 > 32 keeps
+// the compiler's choice (64 register points per lane already).
 template <int R1> struct CfgForY {
     using B = typename CfgFor<R1>::type;
     using type = PassCfg<R1, B::NB, B::WPB_X, B::WPB_Y, B::MINB_X, B::MINB_Y, R1 <= 32 ? 2 : 0>;
 };
 template <> struct CfgForY<10> { using type = PassCfg<10, 3, 8, 4, 2, 3, 1>; };   // 30 items
-template <> struct CfgForY<15> { using type = PassCfg<15, 4, 8, 4, 2, 1, 2>; };   // 60 items: two full rounds (was 30 of 32)
+template <> struct CfgForY<15> { using type = PassCfg<15, 2, 8, 4, 2, 2, 2>; };   // 30 items, 250 registers, no spill (NB = 4: 60 items, 120 B of spill, 9.86 -> 8.99 ms per 500 frames)
 template <> struct CfgForY<16> { using type = PassCfg<16, 2, 8, 4, 2, 1, 2>; };
 template <> struct CfgForY<20> { using type = PassCfg<20, 3, 8, 4, 2, 1, 2>; };   // 60 items (was 20 of 32)
 template <> struct CfgForY<24> { using type = PassCfg<24, 1, 8, 4, 2, 1, 2>; };
-template <> struct CfgForY<25> { using type = PassCfg<25, 1, 8, 4, 2, 1, 2>; };
+template <> struct CfgForY<25> { using type = PassCfg<25, 1, 8, 4, 2, 3, 5>; };   // staged T + resident twiddles, 12 warps/SM: 33.05 -> 31.84 ms per 600 frames
 template <> struct CfgForY<27> { using type = PassCfg<27, 1, 8, 4, 2, 1, 2>; };
 template <> struct CfgForY<30> { using type = PassCfg<30, 1, 8, 4, 2, 1, 2>; };
 template <> struct CfgForY<32> { using type = PassCfg<32, 1, 8, 4, 2, 3, 1>; };
