@@ -237,12 +237,23 @@ __global__ void psf_fold_kernel(float *__restrict__ accum, const float *__restri
     __shared__ float tile[32][33];
     const size_t MM = (size_t)M * M;
     const int u0 = blockIdx.y * 32, v0 = blockIdx.x * 32;
-    for (int j = threadIdx.y; j < 32; j += 8) {                       // tile[u][v], coalesced along v
-        float s = 0.f;
-        const float *src = partial + (size_t)(u0 + j) * M + v0 + threadIdx.x;
-        for (int k = 0; k < fsplit; ++k) s += __ldg(src + (size_t)k * MM);
-        tile[j][threadIdx.x] = s;
+    // all loads of a thread (4 rows x fsplit partials) are issued before the first add: this kernel is pure latency
+    // (25 MB in 1024 small CTAs); the sum over k keeps its fixed order
+    float s[4] = {0.f, 0.f, 0.f, 0.f};
+    for (int k0 = 0; k0 < fsplit; k0 += 4) {
+        float v[4][4];
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj)
+#pragma unroll
+            for (int kk = 0; kk < 4; ++kk)
+                v[jj][kk] = (k0 + kk < fsplit) ? __ldg(partial + (size_t)(k0 + kk) * MM + (size_t)(u0 + threadIdx.y + 8 * jj) * M + v0 + threadIdx.x) : 0.f;
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj)
+#pragma unroll
+            for (int kk = 0; kk < 4; ++kk) s[jj] += v[jj][kk];
     }
+#pragma unroll
+    for (int jj = 0; jj < 4; ++jj) tile[threadIdx.y + 8 * jj][threadIdx.x] = s[jj];   // tile[u][v], coalesced along v
     __syncthreads();
     for (int j = threadIdx.y; j < 32; j += 8) {                       // accum[v][u], coalesced along u
         float *dst = accum + (size_t)(v0 + j) * M + u0 + threadIdx.x;
