@@ -538,13 +538,32 @@ static __global__ void xrebin_kernel(DevTables t, const float *__restrict__ colb
                 xc[u] = ok ? __ldg(t.xc_of_x + xx) : 0;
                 wc[u] = ok ? __ldg(w + c0 + u) : 0.f;
             }
-            for (int ks = 0; ks < ksplit; ++ks) {
-                const float *src = colbin + ((size_t)f * ksplit + ks) * t.ncols * D + jy;
-                float v[4];
+            if (ksplit < 3) {                                  // batches: one or two k-splits, four loads in flight
+                for (int ks = 0; ks < ksplit; ++ks) {
+                    const float *src = colbin + ((size_t)f * ksplit + ks) * t.ncols * D + jy;
+                    float v[4];
 #pragma unroll
-                for (int u = 0; u < 4; ++u) v[u] = c0 + u < cnt ? __ldg(src + (size_t)xc[u] * D) : 0.f;
+                    for (int u = 0; u < 4; ++u) v[u] = c0 + u < cnt ? __ldg(src + (size_t)xc[u] * D) : 0.f;
 #pragma unroll
-                for (int u = 0; u < 4; ++u) s = fmaf(wc[u], v[u], s);
+                    for (int u = 0; u < 4; ++u) s = fmaf(wc[u], v[u], s);
+                }
+                continue;
+            }
+            // four k-splits x four columns = up to 16 loads in flight (a single frame has 6-12 k-splits and this kernel
+            // is nothing but load latency); absent entries add an exact zero, the order of the sum stays ks-major
+            for (int ks0 = 0; ks0 < ksplit; ks0 += 4) {
+                float v[4][4];
+#pragma unroll
+                for (int kk = 0; kk < 4; ++kk) {
+                    const float *src = colbin + ((size_t)f * ksplit + min(ks0 + kk, ksplit - 1)) * t.ncols * D + jy;
+#pragma unroll
+                    for (int u = 0; u < 4; ++u)
+                        v[kk][u] = (ks0 + kk < ksplit && c0 + u < cnt) ? __ldg(src + (size_t)xc[u] * D) : 0.f;
+                }
+#pragma unroll
+                for (int kk = 0; kk < 4; ++kk)
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) s = fmaf(wc[u], v[kk][u], s);
             }
         }
         s *= scale;
