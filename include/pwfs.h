@@ -32,6 +32,13 @@
  *     slopes buffers.  A handle is not thread-safe; distinct handles are.
  *   - Non-finite phase values propagate to the outputs (no checking on the hot
  *     path).
+ *   - Environment, read once when a handle is created (tuning and measurement
+ *     hooks; none is needed for normal use): PWFS_SCRATCH_MB (scratch budget, default
+ *     32768), PWFS_SMALL=0/1 (never / always take the fused M = 128 kernel),
+ *     PWFS_DEBUG_T_ALIAS=1 (every frame aliases the intermediate of frame 0: timing
+ *     experiment, results are wrong), PWFS_REC_KSPLIT (K split of the tensor-core
+ *     reconstructor, pwfs_chain.h).  The Python binding loads the library named by
+ *     PWFS_LIB_PATH, else the in-tree libpwfs.so.
  */
 #ifndef PWFS_H
 #define PWFS_H

@@ -159,9 +159,9 @@ __device__ __forceinline__ void tmem_ld_32x32(uint32_t taddr, uint32_t (&r)[32])
 // costs 2 instead of 3 bytes of L2 -> SM traffic (576 -> 384 MB per call on cfg 4).  A stage of either CTA may be
 // overwritten by the other's multicast, so a stage is free when BOTH MMA warps are done with it: tcgen05.commit
 // arrives on the "empty" barrier of both CTAs (count 2).  Measured: the call takes the same time with and without the
-// multicast (ncu: the converters wait for TMA, DRAM 40 %, tensor pipe 60 %) -- what limits the kernel is the HBM bytes
-// a CTA has in flight (four stages of 16 KB of recmat), not the traffic out of L2; kept because it takes a third of
-// that traffic away from whatever runs beside it.
+// multicast (ncu: the converters wait for TMA, DRAM 40 %, tensor pipe 60 %) -- the traffic out of L2 is not what limits
+// the kernel (nor is the depth of the ring: three stages cost 5 %; profiles/r2_tuning.md section 11); kept because it
+// takes a third of that traffic away from whatever runs beside it.
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 rec_tc_kernel(const __grid_constant__ CUtensorMap mR,
               const __grid_constant__ CUtensorMap mShi, const __grid_constant__ CUtensorMap mSlo,
