@@ -9,25 +9,25 @@
 // recmat is streamed from HBM as it is (FP32, 4 bytes per element) and split INSIDE the pipeline; the
 // (small) slope planes are written by a split kernel per call.
 //
-// Kernel (one 128 x 128 output tile of one K split per CTA, 320 threads):
-//   warp 0 (one lane)  TMA producer: three 128 x 32 FP32 boxes per stage (recmat raw, Shi, Slo;
-//                      128-byte swizzle) into a 4-stage ring, completion on the stage's "full" mbarrier;
-//   warps 2-9          converters: two warps per TMEM lane quarter, thread = (row of the recmat tile, half of
-//                      its 32 K values); reads its 16 raw values (undoing the swizzle in the address),
-//                      hi = tf32(x), lo = tf32(x - hi), and writes both planes into TENSOR MEMORY
-//                      (tcgen05.st 32x32b.x16: lane = row, column = k), then arrives on the stage's "conv"
-//                      mbarrier;
-//   warp 1 (one lane)  MMA issuer: waits for "conv", per stage 4 K steps x 3 UMMAs (M 128, N = frames rounded
-//                      up to 16, K 8),
-//                      A (recmat hi / lo) from tensor memory, B (slope planes) from shared-memory
-//                      descriptors, into 128 TMEM columns; tcgen05.commit releases the stage ("empty")
-//                      and, after the last one, signals the epilogue;
+// Kernel (TWO neighbouring 128 x 128 output tiles of one K split per CTA, 320 threads):
+//   warp 0 (one lane)  TMA producer: four 128 x 32 FP32 boxes per stage (two raw recmat tiles, Shi, Slo; 128-byte
+//                      swizzle) into a 3-stage ring of 64 KB, completion on the stage's "full" mbarrier;
+//   warps 2-9          converters: two warps per TMEM lane quarter, thread = (row of a recmat tile, half of its 32 K
+//                      values); reads its 16 raw values of each tile (undoing the swizzle in the address),
+//                      hi = tf32(x), lo = tf32(x - hi), and writes both planes into one of two slots of TENSOR MEMORY
+//                      (tcgen05.st 32x32b.x16: lane = row, column = k) once the MMAs that read the slot last have
+//                      retired ("tfree" mbarrier), then arrives on the slot's "conv" mbarrier;
+//   warp 1 (one lane)  MMA issuer: waits for "conv", per stage 4 K steps x 2 tiles x 3 UMMAs (M 128, N = frames
+//                      rounded up to 16, K 8), A (recmat hi / lo) from tensor memory, B (slope planes) from
+//                      shared-memory descriptors, into two accumulators of 128 TMEM columns; tcgen05.commit
+//                      releases the stage ("empty") and the slot ("tfree") and, after the last one, signals the
+//                      epilogue;
 //   warps 2-9 again    epilogue: tcgen05.ld 32 lanes x 32 columns at a time, rows = modes so that a
 //                      column store is one coalesced 128-byte line of modes[b][m0..m0+32).
-// Tiles x K splits ~ number of SMs; the split-K partial sums are added in a fixed order by a second
-// kernel (deterministic, no atomics).  Per stage the CTA needs 16 KB from HBM, 768 tensor-core cycles
-// (12 UMMAs of 64 cycles) and 64 KB of shared-memory reads (16 KB by the converters, 48 KB of B operands):
-// with recmat's planes in tensor memory the shared-memory port is no longer the limiter.
+// Tile pairs x K splits ~ number of SMs; the split-K partial sums are added in a fixed order by a second
+// kernel (deterministic, no atomics).  Per stage the CTA needs 32 KB from HBM and 32 KB of slope planes out of L2
+// and issues 24 UMMAs; measured, the kernel runs at the rate those short UMMAs issue at (~97 cycles each, tensor pipe
+// 61 %; DESIGN.md 11 f2, profiles/r2_tuning.md section 11).
 #include "rec_tc.cuh"
 
 #include <cuda.h>
@@ -40,13 +40,16 @@
 
 namespace {
 
-constexpr int BM = 128, BN = 128, BK = 32, UK = 8, STAGES = 4;
+constexpr int BM = 128, BN = 128, BK = 32, UK = 8, STAGES = 3;
+constexpr int TM = 2;                                 // m tiles (of 128 modes) per CTA: they share the slope planes of a stage
+constexpr int TSLOTS = 2;                             // slots of converted recmat planes in tensor memory
 constexpr int kTileBytes = BM * BK * 4;               // 16 KB, one operand plane of one stage
-constexpr int kStageBytes = 3 * kTileBytes;           // recmat raw, Shi, Slo
+constexpr int kStageBytes = (TM + 2) * kTileBytes;    // TM raw recmat tiles, Shi, Slo
 constexpr int kThreads = 320;                         // warp 0 TMA, warp 1 MMA, warps 2..9 converters / epilogue
-constexpr uint32_t kAccCols = 128;                    // accumulator: TMEM columns [0, 128)
-constexpr uint32_t kTmemCols = 512;                   // + per stage 32 columns of recmat hi and 32 of lo: 128 + 4 * 64 = 384 -> 512
-constexpr int kLoadBytes = 3 * kTileBytes;            // what TMA brings per stage
+constexpr uint32_t kAccCols = 128 * TM;               // accumulators: TMEM columns [0, 128 TM)
+constexpr uint32_t kTmemCols = 512;                   // + per slot and m tile 32 columns of recmat hi and 32 of lo: 256 + 2 * 2 * 64
+static_assert(kAccCols + TSLOTS * TM * 64 <= kTmemCols, "tensor memory budget");
+constexpr int kLoadBytes = kStageBytes;               // what TMA brings per stage
 constexpr int kConvThreads = 256;                     // warps 2..9: two per TMEM lane quarter, 16 K values each
 constexpr size_t kSmemBytes = (size_t)STAGES * kStageBytes + 1024 /* alignment slack */ + 256 /* barriers */;
 static_assert(BK * 4 == 128, "one K block is one 128-byte swizzle row");
@@ -90,22 +93,6 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map
         "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
         ::"r"(dst), "l"((uint64_t)map), "r"(bar), "r"(c0), "r"(c1) : "memory");
 }
-// The same load delivered to the CTAs of the cluster named in cta_mask (same shared-memory offset in each, completion
-// bytes on the mbarrier at the same offset in each)
-__device__ __forceinline__ void tma_load_2d_mc(uint32_t dst, const CUtensorMap *map, uint32_t bar, int c0, int c1, uint16_t cta_mask) {
-    asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster [%0], [%1, {%3, %4}], [%2], %5;"
-        ::"r"(dst), "l"((uint64_t)map), "r"(bar), "r"(c0), "r"(c1), "h"(cta_mask) : "memory");
-}
-__device__ __forceinline__ uint32_t cluster_ctarank() {
-    uint32_t r;
-    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
-    return r;
-}
-__device__ __forceinline__ void cluster_sync_all() {
-    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
-    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
-}
 // Shared-memory matrix descriptor, K-major operand in the canonical 128-byte-swizzle layout (what TMA
 // SWIZZLE_128B writes for a box of 32 floats x rows): start >> 4 at bits 0-13, leading offset unused for
 // swizzled K-major (1), stride offset = 8 rows x 128 B = 1024 >> 4 at bits 32-45, descriptor version 1
@@ -133,11 +120,6 @@ __device__ __forceinline__ void tmem_st_32x16(uint32_t taddr, const uint32_t (&r
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
-// the same arrival on the mbarrier at this offset in every CTA of cta_mask
-__device__ __forceinline__ void umma_commit_mc(uint32_t bar, uint16_t cta_mask) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
-                 ::"r"(bar), "h"(cta_mask) : "memory");
-}
 __device__ __forceinline__ void tmem_ld_32x32(uint32_t taddr, uint32_t (&r)[32]) {
     asm volatile(
         "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
@@ -151,37 +133,40 @@ __device__ __forceinline__ void tmem_ld_32x32(uint32_t taddr, uint32_t (&r)[32])
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
 
-// grid (m_tiles rounded up to 2, ksplit, n_tiles) in clusters of two CTAs along x; block 320; dynamic smem kSmemBytes.
+// grid (ceil(m_tiles / TM), ksplit, n_tiles); block 320; dynamic smem kSmemBytes.
 // dst: modes [B][n_modes] when ksplit == 1, else partials [ksplit][B][n_modes].
 //
-// The two CTAs of a cluster work on neighbouring m tiles of the SAME K range and frame tile, so they need the same
-// slope planes: rank 0 loads Shi, rank 1 loads Slo, each as one TMA multicast to both CTAs.  Every recmat byte then
-// costs 2 instead of 3 bytes of L2 -> SM traffic (576 -> 384 MB per call on cfg 4).  A stage of either CTA may be
-// overwritten by the other's multicast, so a stage is free when BOTH MMA warps are done with it: tcgen05.commit
-// arrives on the "empty" barrier of both CTAs (count 2).  Measured: the call takes the same time with and without the
-// multicast (ncu: the converters wait for TMA, DRAM 40 %, tensor pipe 60 %) -- the traffic out of L2 is not what limits
-// the kernel (nor is the depth of the ring: three stages cost 5 %; profiles/r2_tuning.md section 11); kept because it
-// takes a third of that traffic away from whatever runs beside it.
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
+// A CTA works on TM = 2 neighbouring m tiles of one K range and frame tile, so that one copy of the slope planes in
+// shared memory serves both: per stage 2 x 16 KB of recmat + 32 KB of slope planes instead of 16 + 32.  The kernel is
+// bound by what comes out of L2 (every byte TMA delivers to an SM passes through it: 3 bytes per recmat byte with one
+// m tile per CTA = 576 MB in 63 us = 9.1 TB/s of the ~12 TB/s the L2 slices deliver; ncu: tensor pipe 60 %, DRAM 40 %,
+// the converters waiting for TMA), so the ratio is what counts: now 2 bytes per recmat byte.  (Clusters of two CTAs
+// with the slope planes multicast gave nothing: at cluster sizes up to 4 a multicast costs L2 what two loads cost.)
+// Tensor memory: two accumulators of 128 columns, and TSLOTS = 2 slots of converted recmat planes (2 m tiles x (32 hi
+// + 32 lo) columns each) that the converters fill one stage ahead of the MMA warp.
+__global__ void __launch_bounds__(kThreads, 1)
 rec_tc_kernel(const __grid_constant__ CUtensorMap mR,
               const __grid_constant__ CUtensorMap mShi, const __grid_constant__ CUtensorMap mSlo,
               float *__restrict__ dst, int n_modes, int B, int nkb, int ksplit, int m_tiles) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;          // 128-byte swizzle needs 1024-byte tiles
     const uint32_t bars = base + STAGES * kStageBytes;
-    // barriers: full[s] at +8 s, empty[s] at +8 (STAGES + s), conv[s] at +8 (2 STAGES + s), accumulator-ready at
-    // +8 (3 STAGES); then the TMEM address
-    const uint32_t bar_acc = bars + 8 * (3 * STAGES);
-    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem_raw + (bars - smem_u32(smem_raw)) + 8 * (3 * STAGES + 1));
+    // barriers: full[s] at +8 s, empty[s] at +8 (STAGES + s), conv[ts] at +8 (2 STAGES + ts), tfree[ts] at
+    // +8 (2 STAGES + TSLOTS + ts), accumulator-ready after them; then the TMEM address
+    const uint32_t bar_conv = bars + 8 * (2 * STAGES), bar_tfree = bar_conv + 8 * TSLOTS, bar_acc = bar_tfree + 8 * TSLOTS;
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem_raw + (bar_acc + 8 - smem_u32(smem_raw)));
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int m_tile = blockIdx.x, ks = blockIdx.y, n_tile = blockIdx.z;
+    const int m_pair = blockIdx.x, ks = blockIdx.y, n_tile = blockIdx.z;
     const int kb_lo = (int)(((long long)ks * nkb) / ksplit), kb_hi = (int)(((long long)(ks + 1) * nkb) / ksplit);
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < STAGES; ++s) {
             mbar_init(bars + 8 * s, 1);
-            mbar_init(bars + 8 * (STAGES + s), 2);                        // both CTAs of the cluster release a stage
-            mbar_init(bars + 8 * (2 * STAGES + s), kConvThreads);
+            mbar_init(bars + 8 * (STAGES + s), 1);
+        }
+        for (int ts = 0; ts < TSLOTS; ++ts) {
+            mbar_init(bar_conv + 8 * ts, kConvThreads);
+            mbar_init(bar_tfree + 8 * ts, 1);
         }
         mbar_init(bar_acc, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -192,11 +177,8 @@ rec_tc_kernel(const __grid_constant__ CUtensorMap mR,
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
-    cluster_sync_all();                                                   // the peer's barriers exist before anything is sent to them
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tmem = *tmem_slot;
-    const uint32_t crank = cluster_ctarank();
-    const int m_load = min(m_tile, m_tiles - 1);                          // padding CTA of an odd m_tiles: same protocol, nothing stored
 
     if (warp == 0) {
         if (lane == 0) {                                                  // ---- TMA producer
@@ -206,9 +188,13 @@ rec_tc_kernel(const __grid_constant__ CUtensorMap mR,
                 const uint32_t full = bars + 8 * s, empty = bars + 8 * (STAGES + s), st = base + s * kStageBytes;
                 mbar_wait(empty, ((it / STAGES) & 1) ^ 1);
                 mbar_expect_tx(full, kLoadBytes);
-                tma_load_2d(st + 0 * kTileBytes, &mR, full, kb * BK, m_load * BM);      // raw FP32 recmat
-                if (crank == 0) tma_load_2d_mc(st + 1 * kTileBytes, &mShi, full, kb * BK, n_tile * BN, (uint16_t)3);
-                else tma_load_2d_mc(st + 2 * kTileBytes, &mSlo, full, kb * BK, n_tile * BN, (uint16_t)3);
+#pragma unroll
+                for (int t = 0; t < TM; ++t) {                            // raw FP32 recmat; a tile beyond the matrix re-reads the last one
+                    const int mt = min(m_pair * TM + t, m_tiles - 1);
+                    tma_load_2d(st + t * kTileBytes, &mR, full, kb * BK, mt * BM);
+                }
+                tma_load_2d(st + TM * kTileBytes, &mShi, full, kb * BK, n_tile * BN);
+                tma_load_2d(st + (TM + 1) * kTileBytes, &mSlo, full, kb * BK, n_tile * BN);
             }
         }
     } else if (warp == 1) {
@@ -217,77 +203,87 @@ rec_tc_kernel(const __grid_constant__ CUtensorMap mR,
             const uint32_t idesc = idesc_for(n_here);
             int it = 0;
             for (int kb = kb_lo; kb < kb_hi; ++kb, ++it) {
-                const int s = it % STAGES;
-                const uint32_t conv = bars + 8 * (2 * STAGES + s), empty = bars + 8 * (STAGES + s), st = base + s * kStageBytes;
-                mbar_wait(conv, (it / STAGES) & 1);                       // TMA landed AND recmat has been split
+                const int s = it % STAGES, ts = it % TSLOTS;
+                const uint32_t conv = bar_conv + 8 * ts, tfree = bar_tfree + 8 * ts, empty = bars + 8 * (STAGES + s);
+                const uint32_t st = base + s * kStageBytes;
+                mbar_wait(conv, (it / TSLOTS) & 1);                       // TMA landed AND recmat has been split
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                const uint32_t a_hi = tmem + kAccCols + (uint32_t)s * 64u, a_lo = a_hi + 32u;
 #pragma unroll
                 for (int k = 0; k < BK / UK; ++k) {
                     const uint32_t ko = k * UK * 4;                      // 32 bytes along the swizzled row
-                    const uint64_t shi = smem_desc(st + 1 * kTileBytes + ko), slo = smem_desc(st + 2 * kTileBytes + ko);
-                    umma_tf32_ts(tmem, a_lo + k * UK, shi, idesc, (it > 0 || k > 0) ? 1u : 0u);   // small terms first
-                    umma_tf32_ts(tmem, a_hi + k * UK, slo, idesc, 1u);
-                    umma_tf32_ts(tmem, a_hi + k * UK, shi, idesc, 1u);
+                    const uint64_t shi = smem_desc(st + TM * kTileBytes + ko), slo = smem_desc(st + (TM + 1) * kTileBytes + ko);
+#pragma unroll
+                    for (int t = 0; t < TM; ++t) {
+                        const uint32_t acc = tmem + (uint32_t)t * 128u;
+                        const uint32_t a_hi = tmem + kAccCols + (uint32_t)(ts * TM + t) * 64u, a_lo = a_hi + 32u;
+                        umma_tf32_ts(acc, a_lo + k * UK, shi, idesc, (it > 0 || k > 0) ? 1u : 0u);   // small terms first
+                        umma_tf32_ts(acc, a_hi + k * UK, slo, idesc, 1u);
+                        umma_tf32_ts(acc, a_hi + k * UK, shi, idesc, 1u);
+                    }
                 }
-                umma_commit_mc(empty, (uint16_t)3);                       // frees the stage in BOTH CTAs when these UMMAs retire
+                umma_commit(empty);                                       // frees the stage when these UMMAs retire
+                umma_commit(tfree);                                       // ... and the slot of converted planes
             }
             umma_commit(bar_acc);
         }
     } else {                                                              // ---- warps 2..9: converters, then epilogue
         // A warp may touch the TMEM lanes 32 (warp % 4) .. + 32 only; the two warps of a lane quarter (warp, warp + 4)
-        // share its rows: `half` 0 takes the K values 0..15 of a row, `half` 1 the values 16..31.  (One warp per
-        // quarter converting all 32 values was the pipeline's bottleneck: ~300 dependent ALU instructions per stage
-        // on a scheduler that has nothing else to issue, against 768 tensor-core cycles.)
+        // share its rows: `half` 0 takes the K values 0..15 of a row, `half` 1 the values 16..31.
         const int q = warp & 3, half = (warp - 2) >> 2;
         {
             int it = 0;
             for (int kb = kb_lo; kb < kb_hi; ++kb, ++it) {
-                const int s = it % STAGES;
-                const uint32_t full = bars + 8 * s, conv = bars + 8 * (2 * STAGES + s);
-                mbar_wait(full, (it / STAGES) & 1);
+                const int s = it % STAGES, ts = it % TSLOTS;
+                mbar_wait(bars + 8 * s, (it / STAGES) & 1);               // the stage has landed
+                mbar_wait(bar_tfree + 8 * ts, ((it / TSLOTS) & 1) ^ 1);   // the MMAs that read this slot have retired
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 // thread = (row of the tile = TMEM lane 32 q + lane, half); a row's 32 K values are 8 chunks of 16 bytes
                 // that TMA's 128-byte swizzle has stored at chunk position c ^ (row % 8)
                 const int row = q * 32 + lane;
-                const uint8_t *tile = smem_raw + (base - smem_u32(smem_raw)) + s * kStageBytes + row * 128;
-                uint32_t hi[16], lo[16];
 #pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    const float4 x = *reinterpret_cast<const float4 *>(tile + (((4 * half + c) ^ (row & 7)) << 4));
-                    const float xv[4] = {x.x, x.y, x.z, x.w};
+                for (int t = 0; t < TM; ++t) {
+                    const uint8_t *tile = smem_raw + (base - smem_u32(smem_raw)) + s * kStageBytes + t * kTileBytes + row * 128;
+                    uint32_t hi[16], lo[16];
 #pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        hi[4 * c + e] = to_tf32(xv[e]);
-                        lo[4 * c + e] = to_tf32(xv[e] - __uint_as_float(hi[4 * c + e]));
+                    for (int c = 0; c < 4; ++c) {
+                        const float4 x = *reinterpret_cast<const float4 *>(tile + (((4 * half + c) ^ (row & 7)) << 4));
+                        const float xv[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) {
+                            hi[4 * c + e] = to_tf32(xv[e]);
+                            lo[4 * c + e] = to_tf32(xv[e] - __uint_as_float(hi[4 * c + e]));
+                        }
                     }
+                    const uint32_t t_hi = tmem + ((uint32_t)(q * 32) << 16) + kAccCols + (uint32_t)(ts * TM + t) * 64u + (uint32_t)half * 16u;
+                    tmem_st_32x16(t_hi, hi);
+                    tmem_st_32x16(t_hi + 32u, lo);
                 }
-                const uint32_t t_hi = tmem + ((uint32_t)(q * 32) << 16) + kAccCols + (uint32_t)s * 64u + (uint32_t)half * 16u;
-                tmem_st_32x16(t_hi, hi);
-                tmem_st_32x16(t_hi + 32u, lo);
                 asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
                 asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-                mbar_arrive(conv);
+                mbar_arrive(bar_conv + 8 * ts);
             }
         }
         mbar_wait(bar_acc, 0);
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        const int m = m_tile * BM + q * 32 + lane;
         float *out = dst + (size_t)ks * B * n_modes;
-        for (int c0 = 32 * half; c0 < BN; c0 += 64) {                    // the quarter's two warps alternate over the columns
-            const int n0 = n_tile * BN + c0;
-            if (n0 >= B) break;                                           // warp-uniform
-            uint32_t r[32];
-            tmem_ld_32x32(tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)c0, r);
-            if (m < n_modes) {
 #pragma unroll
-                for (int j = 0; j < 32; ++j)
-                    if (n0 + j < B) out[(size_t)(n0 + j) * n_modes + m] = __uint_as_float(r[j]);
+        for (int t = 0; t < TM; ++t) {
+            const int m = (m_pair * TM + t) * BM + q * 32 + lane;
+            for (int c0 = 32 * half; c0 < BN; c0 += 64) {                // the quarter's two warps alternate over the columns
+                const int n0 = n_tile * BN + c0;
+                if (n0 >= B) break;                                       // warp-uniform
+                uint32_t r[32];
+                tmem_ld_32x32(tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)t * 128u + (uint32_t)c0, r);
+                if (m < n_modes) {
+#pragma unroll
+                    for (int j = 0; j < 32; ++j)
+                        if (n0 + j < B) out[(size_t)(n0 + j) * n_modes + m] = __uint_as_float(r[j]);
+                }
             }
         }
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
-    cluster_sync_all();                                                   // no CTA leaves while the peer may still signal it
     if (warp == 2)
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(kTmemCols) : "memory");
 }
@@ -375,7 +371,7 @@ int rec_tc_create(RecTc **out, const float *d_R, int n_modes, int n_slopes, int 
 
 static int rec_tc_ksplit(const RecTc *h, int B) {
     const int m_tiles = (h->n_modes + BM - 1) / BM, n_tiles = (B + BN - 1) / BN, nkb = h->ldp / BK;
-    int ksplit = h->num_sms / ((m_tiles + 1) / 2 * 2 * n_tiles);
+    int ksplit = h->num_sms / ((m_tiles + TM - 1) / TM * n_tiles);
     if (const char *e = std::getenv("PWFS_REC_KSPLIT")) { const int v = std::atoi(e); if (v > 0) ksplit = v; }   // tuning hook
     if (ksplit > nkb / 4) ksplit = nkb / 4;                               // at least 4 K blocks per split
     return ksplit < 1 ? 1 : ksplit;
@@ -420,7 +416,7 @@ int rec_tc_run(RecTc *h, const float *d_slopes, int B, float *d_modes, cudaStrea
     if (int rc = rec_tc_reserve(h, B, st)) return rc;                     // no-op once sized (pwfs_rec_reserve)
     split_tf32_kernel<<<dim3((h->ldp + 255) / 256, B), 256, 0, st>>>(d_slopes, (size_t)h->n_slopes, h->n_slopes, h->ldp,
                                                                     h->d_Shi, h->d_Slo);
-    rec_tc_kernel<<<dim3((m_tiles + 1) / 2 * 2, ksplit, n_tiles), kThreads, kSmemBytes, st>>>(
+    rec_tc_kernel<<<dim3((m_tiles + TM - 1) / TM, ksplit, n_tiles), kThreads, kSmemBytes, st>>>(
         h->mR, h->mShi, h->mSlo, ksplit > 1 ? h->d_part : d_modes, h->n_modes, B, nkb, ksplit, m_tiles);
     if (ksplit > 1) {
         const size_t n = (size_t)B * h->n_modes;
