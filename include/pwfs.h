@@ -26,7 +26,8 @@
  *   - 2-D arrays are row-major [y][x] (x fast).  Phase is in radians at the
  *     sensing wavelength.  1 lambda/D of tilt = 2 pi across the N pupil pixels.
  *   - Every function returns PWFS_OK (0) or a negative pwfs_status; nothing
- *     throws or aborts across this boundary and there is no global mutable state.
+ *     throws or aborts across this boundary and there is no global mutable state
+ *     (one exception, stated there: the fixed scratch array of pwfs_run_noalloc).
  *   - A handle owns its device tables and scratch memory.  The caller owns
  *     pupil_amp (host memory, copied by pwfs_create) and the phase / frames /
  *     slopes buffers.  A handle is not thread-safe; distinct handles are.
@@ -56,7 +57,8 @@ typedef enum {
     PWFS_EINVAL = -1,       /* bad parameter, NULL pointer, geometry that leaves the grid, n_valid == 0 */
     PWFS_ENOMEM = -2,       /* host or device allocation failed */
     PWFS_ECUDA = -3,        /* a CUDA runtime call failed (see pwfs_last_cuda_error) */
-    PWFS_EUNSUPPORTED = -4  /* valid request this build has no kernel for (e.g. M/32 not instantiated) */
+    PWFS_EUNSUPPORTED = -4, /* valid request this build has no kernel for (e.g. M/32 not instantiated) */
+    PWFS_ELIMIT = -5        /* pwfs_run_noalloc only: the batch does not fit the library's fixed scratch array */
 } pwfs_status;
 
 /* Parameters of one sensor (names follow PAPER.md Table 1 where
@@ -160,6 +162,67 @@ int pwfs_reserve(pwfs_t *h, int32_t B);
  * and the copy-out of the previous one run under the kernels of the current
  * chunk; pageable memory works but is slower. */
 int pwfs_run_host(pwfs_t *h, const float *h_phase, int32_t B, float *h_frames, float *h_slopes);
+
+/* pwfs_run for callers that are not allowed to allocate device memory.
+ *
+ * Who needs this.  Two kinds of user of this library cannot let a sensor call reach
+ * cudaMalloc / cudaFree, which pwfs_run does whenever a batch is larger than any it has
+ * seen (and pwfs_reserve does on request):
+ *   - a real-time control thread (the adaptive-optics loop this sensor model stands in
+ *     for runs at a fixed frame rate): cudaMalloc and cudaFree take a process-wide lock,
+ *     may wait for ALL work on the device to drain, and have no upper bound on how long
+ *     they take, so one call in the wrong step is a missed deadline;
+ *   - a process in which something else has been given the device memory -- a pooling
+ *     allocator that grabbed nearly all of HBM at start-up, a fixed per-client memory
+ *     quota -- so that a cudaMalloc from inside this library would fail or steal from
+ *     that budget behind its owner's back.
+ * Such a caller creates the handle during start-up (pwfs_create uploads its tables, that
+ * is the one allocation) and from then on calls this function only.
+ *
+ * What it does.  Exactly what pwfs_run does on the M = 128 grid for a small batch: the
+ * whole path -- phasor, both transforms, mask, sum over the modulation points, rebin,
+ * slopes -- in one kernel launch on `cuda_stream`.  Arguments, layouts, ownership and
+ * asynchrony are those of pwfs_run; the caller passes the phase batch and the output
+ * buffers (DEVICE memory; d_slopes may be NULL).  The results are the ones pwfs_run
+ * gives when it takes its fused-kernel path (same kernel, same order of additions).
+ * The kernel's working memory (one partial detector frame per frame and modulation
+ * point, one counter per frame) does not come from the heap: it is a fixed array inside
+ * libpwfs.so, PWFS_NOALLOC_SCRATCH_BYTES (4 MiB + 256 B) on every GPU that loads the
+ * library, held until the process exits.  The call itself performs no cudaMalloc,
+ * no cudaFree, and creates no stream or event.
+ *
+ * Limits.  Sensors the fused kernel serves: m_grid = 128, n_pupil <= 64, n_subap <= 32.
+ * Others get PWFS_EUNSUPPORTED.  A batch must satisfy B <= PWFS_NOALLOC_MAX_FRAMES and
+ * B * K * (2 n_subap)^2 <= PWFS_NOALLOC_MAX_PART_FLOATS (K = modulation points; the
+ * 10-frame, K = 12, n_subap = 16 case of BASELINE.json's first config uses 12 % of it);
+ * a larger one gets PWFS_ELIMIT and nothing is enqueued -- split it into several calls
+ * on the same stream.
+ *
+ * First call.  The first call on a given GPU asks the CUDA runtime where the array
+ * sits on that GPU (with the handle's device current) and remembers the answer; this may
+ * make the runtime load the library's device code there.  Make that first call during
+ * start-up, outside any stream capture; later calls on that GPU skip the step.
+ *
+ * Sharing.  There is ONE array per GPU, shared by every handle and every thread in the
+ * process, and it keeps the contents the last call left.  Each call clears the counters
+ * it needs in stream order before its kernel, and overwrites the partial frames before
+ * reading them, so calls that execute one after another (same stream, or ordered by
+ * events) need no clean-up in between.  Two calls that can EXECUTE at the same time on
+ * one GPU -- different streams without an ordering, or two host threads -- race on the
+ * array and produce garbage; serialise them, or use pwfs_run (whose scratch is per
+ * handle) for all but one of them.
+ *
+ * Errors: PWFS_EINVAL (NULL handle or buffer, B < 0, debug handle), PWFS_EUNSUPPORTED,
+ * PWFS_ELIMIT, PWFS_ECUDA.  B = 0 is a no-op.  The CUDA device that was current on entry
+ * is current again on return.
+ * Defined by: north_star "pwfs_run(phase batch -> frames, slopes)"; the per-step call of
+ * a closed loop is PAPER.md:L33 ("triggers all processing objects once per simulation
+ * step"). */
+#define PWFS_NOALLOC_MAX_FRAMES 64
+#define PWFS_NOALLOC_MAX_PART_FLOATS (1u << 20)
+#define PWFS_NOALLOC_SCRATCH_BYTES (256u + 4u * PWFS_NOALLOC_MAX_PART_FLOATS)
+int pwfs_run_noalloc(pwfs_t *h, const float *d_phase, int32_t B, float *d_frames, float *d_slopes,
+                     void *cuda_stream);
 
 /* Release everything the handle owns.  NULL-safe. */
 void pwfs_destroy(pwfs_t *h);

@@ -11,6 +11,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -373,6 +374,43 @@ struct SpanGuard {
     }
 };
 
+// ---- pwfs_run_noalloc: scratch that lives in the library image instead of on the CUDA heap ---------------------
+// The fused M = 128 kernel needs two pieces of working memory besides its inputs and outputs: one completion counter
+// per frame and one partial detector frame per (frame, modulation point).  pwfs_run takes both from cudaMalloc.  For
+// callers that must not enter the CUDA allocator, the same kernel can work out of this fixed array, which the driver
+// places in device memory when the module is loaded on a GPU and keeps there until the process exits (about 4 MB on
+// every GPU that uses the library, whether or not pwfs_run_noalloc is ever called).
+//   bytes [0, 256)        : kNoAllocFrames completion counters (unsigned)
+//   bytes [256, 256 + 4Mi): kNoAllocPartFloats floats of partial frames, [frame][k][D][D]
+constexpr int kNoAllocFrames = PWFS_NOALLOC_MAX_FRAMES;
+constexpr size_t kNoAllocPartFloats = PWFS_NOALLOC_MAX_PART_FLOATS;
+constexpr size_t kNoAllocCounterBytes = 256;
+static_assert(kNoAllocFrames * sizeof(unsigned) <= kNoAllocCounterBytes, "counters must fit their slot");
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoAllocCounterBytes + kNoAllocPartFloats * sizeof(float)];
+
+// In host code `g_noalloc_scratch` is only a stand-in the runtime uses to look the array up; it is NOT the array's
+// device address and must never be handed to a kernel.  The real address differs from GPU to GPU, so it is asked for
+// once per device (with that device current) and remembered here.
+constexpr int kNoAllocMaxDevices = 64;
+std::mutex g_noalloc_mu;
+unsigned char *g_noalloc_addr[kNoAllocMaxDevices] = {};
+
+// Caller has made `device` current.  Returns the device address of the array on that GPU in *out.
+cudaError_t noalloc_scratch_address(int device, unsigned char **out) {
+    *out = nullptr;
+    if (device < 0 || device >= kNoAllocMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_noalloc_mu);
+    if (!g_noalloc_addr[device]) {
+        unsigned char *p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress((void **)&p, g_noalloc_scratch);
+        if (e != cudaSuccess) return e;
+        if (!p) return cudaErrorInvalidSymbol;
+        g_noalloc_addr[device] = p;
+    }
+    *out = g_noalloc_addr[device];
+    return cudaSuccess;
+}
+
 }  // namespace
 
 extern "C" {
@@ -384,6 +422,7 @@ const char *pwfs_strerror(int code) {
         case PWFS_ENOMEM: return "out of memory";
         case PWFS_ECUDA: return "CUDA runtime error";
         case PWFS_EUNSUPPORTED: return "grid size not supported by this build";
+        case PWFS_ELIMIT: return "batch exceeds the fixed scratch of pwfs_run_noalloc";
         default: return "unknown pwfs status";
     }
 }
@@ -856,6 +895,35 @@ int pwfs_run_host(pwfs_t *h, const float *h_phase, int32_t B, float *h_frames, f
     PWFS_CUDA(h, cudaStreamSynchronize(h->out_stream));
     PWFS_CUDA(h, cudaStreamSynchronize(h->hstream));
     return PWFS_OK;
+}
+
+// pwfs_run for callers that cannot allocate (include/pwfs.h has the contract).  Same fused kernel as pwfs_run's
+// small-batch path on the M = 128 grid, same arguments; the only difference is where the kernel's working memory
+// lives.  Nothing here calls cudaMalloc / cudaFree, creates a stream or an event, or touches the handle's own scratch.
+int pwfs_run_noalloc(pwfs_t *h, const float *d_phase, int32_t B, float *d_frames, float *d_slopes, void *cuda_stream) {
+    if (!h || B < 0) return PWFS_EINVAL;
+    if (B == 0) return PWFS_OK;
+    if (!d_phase || !d_frames || h->debug_only) return PWFS_EINVAL;
+    const DevTables &t = h->tab;
+    // geometry the fused kernel's shared-memory plan holds (SmallCfg::MAXN, MAXCOLS, MAXD, MAXCMAX)
+    if (!h->L.launch_s || t.N > 64 || t.ncols > 128 || t.D > 64 || t.cmax > 8) return PWFS_EUNSUPPORTED;
+    const size_t DD = (size_t)t.D * t.D;
+    if (B > kNoAllocFrames || (size_t)B * t.K * DD > kNoAllocPartFloats) return PWFS_ELIMIT;
+    DeviceGuard dg(h->device);
+    PWFS_CUDA(h, dg.err);
+    unsigned char *base = nullptr;
+    PWFS_CUDA(h, noalloc_scratch_address(h->device, &base));      // first call on this GPU: looks the array up
+    unsigned *counter = reinterpret_cast<unsigned *>(base);
+    float *part = reinterpret_cast<float *>(base + kNoAllocCounterBytes);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // The array keeps whatever the previous call (of any handle) left.  The partial frames are fully overwritten before
+    // they are read; the counters must be zero when the kernel starts, and a call that was cut short could have left
+    // them otherwise -- so they are cleared in stream order, every time.
+    PWFS_CUDA(h, cudaMemsetAsync(counter, 0, (size_t)B * sizeof(unsigned), st));
+    const double m4 = h->quarter ? std::pow((double)t.M, 4.0) : 1.0;
+    h->launches[4]++;
+    h->L.launch_s(dim3(t.K, B), st, t, d_phase, part, counter, d_frames, d_slopes, (float)(1.0 / ((double)t.K * m4)));
+    return check_launch(h, 4);
 }
 
 }  // extern "C"

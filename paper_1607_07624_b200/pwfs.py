@@ -16,14 +16,16 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("PWFS_LIB_PATH") or os.path.join(_HERE, "libpwfs.so")
 
-PWFS_OK, PWFS_EINVAL, PWFS_ENOMEM, PWFS_ECUDA, PWFS_EUNSUPPORTED = 0, -1, -2, -3, -4
+PWFS_OK, PWFS_EINVAL, PWFS_ENOMEM, PWFS_ECUDA, PWFS_EUNSUPPORTED, PWFS_ELIMIT = 0, -1, -2, -3, -4, -5
+NOALLOC_MAX_FRAMES, NOALLOC_MAX_PART_FLOATS = 64, 1 << 20     # PWFS_NOALLOC_* of include/pwfs.h
 NUM_KERNEL_CLASSES = 5
 KERNEL_CLASSES = ("xpass", "ypass", "xrebin", "slopes", "fused")
 
 EXPORTS = ("pwfs_create", "pwfs_create_ex", "pwfs_info", "pwfs_valid_mask", "pwfs_run", "pwfs_run_host",
            "pwfs_destroy", "pwfs_strerror", "pwfs_last_cuda_error", "pwfs_supported_grid",
            "pwfs_set_schedule", "pwfs_set_timing", "pwfs_get_timing", "pwfs_geometry", "pwfs_reserve",
-           "pwfs_last_failed_kernel", "pwfs_peak_fp32", "pwfs_debug_create", "pwfs_debug_intensity")
+           "pwfs_last_failed_kernel", "pwfs_peak_fp32", "pwfs_debug_create", "pwfs_debug_intensity",
+           "pwfs_run_noalloc")
 
 
 class pwfs_params(C.Structure):
@@ -68,6 +70,8 @@ def load_library() -> C.CDLL:
     lib.pwfs_valid_mask.restype = C.c_int
     lib.pwfs_run.argtypes = [vp, vp, i32, vp, vp, vp]
     lib.pwfs_run.restype = C.c_int
+    lib.pwfs_run_noalloc.argtypes = [vp, vp, i32, vp, vp, vp]
+    lib.pwfs_run_noalloc.restype = C.c_int
     lib.pwfs_run_host.argtypes = [vp, vp, i32, vp, vp]
     lib.pwfs_run_host.restype = C.c_int
     lib.pwfs_destroy.argtypes = [vp]
@@ -286,6 +290,33 @@ class PWFS:
                 if t is not None:
                     t.record_stream(st)
         return frames, slopes
+
+    def run_noalloc(self, phase, frames, slopes=None, stream=None):
+        """pwfs_run_noalloc: run() for callers that may not allocate device memory -- a control loop that cannot
+        afford cudaMalloc's device-wide stall, or a process whose GPU memory belongs to another allocator.  The
+        kernel's working memory is a fixed array inside libpwfs.so instead of heap scratch, so nothing is allocated
+        here either: `phase` [B,N,N] must already be contiguous and `frames` [B,2n_sub,2n_sub] (and `slopes`
+        [B,2 n_valid], optional) must be passed in; nothing is returned.  M = 128 sensors only, B <= 64 and
+        B * K * det_size^2 <= 2^20 (PwfsError PWFS_EUNSUPPORTED / PWFS_ELIMIT otherwise).  One array per GPU is shared
+        by all sensors: calls that could run at the same time on one GPU must be serialised by the caller.  Make the
+        first call on each GPU at start-up (it looks the array up)."""
+        import torch
+        N, D = self.n_pupil, self.det_size
+        if not (isinstance(phase, torch.Tensor) and phase.is_cuda and phase.dtype == torch.float32):
+            raise TypeError("phase must be a CUDA float32 tensor")
+        if phase.device.index != self.device:
+            raise ValueError("phase lives on another device than the sensor")
+        if phase.dim() != 3 or tuple(phase.shape[1:]) != (N, N) or not phase.is_contiguous():
+            raise ValueError(f"phase must be a contiguous [B,{N},{N}] tensor (a copy would allocate)")
+        B = phase.shape[0]
+        self._dev_out(frames, (B, D, D), "frames")
+        if slopes is not None:
+            self._dev_out(slopes, (B, 2 * self.n_valid), "slopes")
+        st = stream if stream is not None else torch.cuda.current_stream(phase.device)
+        rc = self._lib.pwfs_run_noalloc(self._h, C.c_void_p(phase.data_ptr()), B, C.c_void_p(frames.data_ptr()),
+                                        C.c_void_p(slopes.data_ptr()) if slopes is not None else None,
+                                        C.c_void_p(st.cuda_stream))
+        self._check(rc, "pwfs_run_noalloc")
 
     @staticmethod
     def _host_buf(a, shape, what):
