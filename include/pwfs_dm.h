@@ -51,8 +51,14 @@ int pwfs_dm_create(int32_t n_act, int32_t n_pupil, int32_t n_pix, const int32_t 
  * d_cmd: DEVICE float [B][n_act].  d_phase: DEVICE float [B][n_pupil][n_pupil]; with beta = 0 it
  * is overwritten (pixels outside the influence functions become 0), with beta = 1 the scaled layer
  * is added in place -- the residual phase the sensor sees is atmosphere + alpha * DM layer, the sign
- * and the unit conversion being the caller's alpha.  FP32 FMA, summed in the order m = 0, 1, ...
- * per pixel (deterministic).  HBM-bound: the matrix is streamed once per group of up to 8 frames.
+ * and the unit conversion being the caller's alpha.  FP32 FMA in a fixed order (deterministic):
+ * the actuators are cut into `msplit` contiguous ranges, each range is summed per pixel in the
+ * order m ascending, and the range sums are then added in range order.  msplit is fixed at create
+ * (1 when n_act < 64; otherwise chosen from n_act, n_pix and the SM count of `device` so that the
+ * kernel fills the machine), so results repeat bit for bit from call to call and do not depend on
+ * B, but they can differ in the last bits between GPUs with different SM counts and are not the
+ * plain m = 0, 1, ... sum once msplit > 1.  HBM-bound: the matrix is streamed once per group of up
+ * to 8 frames.
  * PWFS_EINVAL for beta other than 0 or 1. */
 int pwfs_dm_apply(pwfs_dm_t *h, const float *d_cmd, int32_t B, float *d_phase, float alpha, float beta,
                   void *cuda_stream);
