@@ -33,13 +33,17 @@
  *     slopes buffers.  A handle is not thread-safe; distinct handles are.
  *   - Non-finite phase values propagate to the outputs (no checking on the hot
  *     path).
- *   - Environment, read once when a handle is created (tuning and measurement
- *     hooks; none is needed for normal use): PWFS_SCRATCH_MB (scratch budget, default
- *     32768), PWFS_SMALL=0/1 (never / always take the fused M = 128 kernel),
- *     PWFS_DEBUG_T_ALIAS=1 (every frame aliases the intermediate of frame 0: timing
- *     experiment, results are wrong), PWFS_REC_KSPLIT (K split of the tensor-core
- *     reconstructor, pwfs_chain.h).  The Python binding loads the library named by
- *     PWFS_LIB_PATH, else the in-tree libpwfs.so.
+ *   - Environment, read once when a handle is created (none is needed for normal
+ *     use, none changes a result beyond FP32 summation order): PWFS_SCRATCH_MB
+ *     (scratch budget, default 32768), PWFS_SMALL=0/1 (never / always take the fused
+ *     M = 128 kernel), PWFS_REC_TC=0 (pwfs_chain.h).  The measurement hooks that DO
+ *     change results or schedules behind the caller's back -- PWFS_DEBUG_T_ALIAS=1
+ *     (every frame aliases the intermediate of frame 0: a timing experiment with
+ *     wrong output) and PWFS_REC_KSPLIT (forced K split of the tensor-core
+ *     reconstructor) -- exist only in a build made with -DPWFS_TUNING
+ *     (`python -m paper_1607_07624_b200.build --tuning` -> libpwfs_tuning.so);
+ *     libpwfs.so does not contain them.  The Python binding loads the library named
+ *     by PWFS_LIB_PATH, else the in-tree libpwfs.so.
  */
 #ifndef PWFS_H
 #define PWFS_H
@@ -152,7 +156,12 @@ int pwfs_run(pwfs_t *h, const float *d_phase, int32_t B, float *d_frames, float 
  * that those calls neither allocate nor create anything.  Required before a
  * pwfs_run of a batch size the handle has not seen is captured into a CUDA graph:
  * cudaMalloc is not allowed during stream capture, and pwfs_run then returns
- * PWFS_EINVAL instead of allocating.  Synchronous; may free and re-allocate. */
+ * PWFS_EINVAL instead of allocating.  "Up to B" is meant literally: the scratch is
+ * sized for the largest need over ALL batch sizes 1..B -- a smaller batch may take the
+ * fused M = 128 kernel where B itself does not, or split its modulation loop further
+ * and so need more column scratch per frame than B does.  Call it again after
+ * pwfs_set_schedule (the knobs change the need).  Synchronous; may free and
+ * re-allocate. */
 int pwfs_reserve(pwfs_t *h, int32_t B);
 
 /* Same computation with HOST buffers (h_slopes may be NULL): copies the phase

@@ -130,8 +130,10 @@ int pwfs_rec_create(int32_t n_modes, int32_t n_slopes, const float *h_recmat, in
  * allocate returns PWFS_EINVAL instead. */
 int pwfs_rec_run(pwfs_rec_t *h, const float *d_slopes, int32_t B, float *d_modes, void *cuda_stream);
 
-/* Size the tensor-core path's scratch for batches of up to B frames (no-op for
- * batch sizes the FP32 kernels serve).  Synchronous; allocates. */
+/* Size the tensor-core path's scratch for every batch of 1..B frames (no-op for
+ * batch sizes the FP32 kernels serve): the need is taken as the largest over the
+ * batch sizes up to B, because a smaller batch is split further along K and can
+ * write more partial sums than B itself.  Synchronous; allocates. */
 int pwfs_rec_reserve(pwfs_rec_t *h, int32_t B);
 
 void pwfs_rec_destroy(pwfs_rec_t *h); /* NULL-safe */

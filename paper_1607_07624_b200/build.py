@@ -1,9 +1,14 @@
 """Build libpwfs.so (the C-ABI CUDA library) in-tree with nvcc for sm_100a.
 
-    python -m paper_1607_07624_b200.build [--force] [--verbose]
+    python -m paper_1607_07624_b200.build [--force] [--verbose] [--tuning]
 
 nvcc cross-compiles without a GPU.  The .so is git-ignored but travels to the
-GPU box with the repo snapshot."""
+GPU box with the repo snapshot.
+
+--tuning builds a SEPARATE library, libpwfs_tuning.so (objects in build_tuning/), with
+-DPWFS_TUNING: it adds the measurement hooks PWFS_DEBUG_T_ALIAS and PWFS_REC_KSPLIT
+(include/pwfs.h), which change results or schedules from the environment and therefore
+are not compiled into libpwfs.so.  Select it with PWFS_LIB_PATH."""
 from __future__ import annotations
 
 import os
@@ -15,6 +20,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libpwfs.so")
+LIB_TUNING = os.path.join(HERE, "libpwfs_tuning.so")      # --tuning: measurement hooks compiled in (never the default)
 GRID_R1 = (4, 5, 6, 8, 9, 10, 12, 15, 16, 18, 20, 24, 25, 27, 30, 32, 36, 40, 45, 48, 50, 54, 60, 64)   # PWFS_FOR_EACH_R1 of csrc/pwfs_launch.cuh
 # (source, extra flags, object name): the FFT kernels of each grid size M = 32 R1 are their own translation unit
 UNITS = [(os.path.join(CSRC, n), [], n[:-3] + ".o")
@@ -43,34 +49,35 @@ def up_to_date() -> bool:
     return _newer(LIB, SOURCES + HEADERS)
 
 
-def _compile(unit, force: bool, verbose: bool) -> str:
+def _compile(unit, force: bool, verbose: bool, objdir: str = OBJDIR, flags=()) -> str:
     src, extra, name = unit
-    obj = os.path.join(OBJDIR, name)
+    obj = os.path.join(objdir, name)
     if not force and _newer(obj, [src] + HEADERS):
         return obj
-    cmd = [nvcc_path()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, src]
+    cmd = [nvcc_path()] + NVCC_FLAGS + list(flags) + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, src]
     if verbose:
         print(" ".join(cmd), flush=True)
     subprocess.run(cmd, check=True)
     return obj
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, tuning: bool = False) -> str:
     """One nvcc -c per source (in parallel; unchanged objects are kept), then one link."""
-    if not force and up_to_date():
-        return LIB
-    os.makedirs(OBJDIR, exist_ok=True)
+    lib, objdir, flags = (LIB_TUNING, OBJDIR + "_tuning", ["-DPWFS_TUNING"]) if tuning else (LIB, OBJDIR, [])
+    if not force and _newer(lib, SOURCES + HEADERS):
+        return lib
+    os.makedirs(objdir, exist_ok=True)
     with ThreadPoolExecutor(max_workers=min(len(UNITS), os.cpu_count() or 4)) as pool:
-        objs = list(pool.map(lambda u: _compile(u, force, verbose), UNITS))
-    tmp = os.path.join(OBJDIR, f"libpwfs.so.{os.getpid()}")     # link inside the ignored build/ directory
+        objs = list(pool.map(lambda u: _compile(u, force, verbose, objdir, flags), UNITS))
+    tmp = os.path.join(objdir, f"libpwfs.so.{os.getpid()}")     # link inside the ignored build directory
     try:
         subprocess.run([nvcc_path(), "--shared", "-o", tmp] + objs, check=True)
-        os.replace(tmp, LIB)
+        os.replace(tmp, lib)
     finally:
         if os.path.exists(tmp):
             os.remove(tmp)
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv, tuning="--tuning" in sys.argv))

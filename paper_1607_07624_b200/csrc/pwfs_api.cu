@@ -174,10 +174,14 @@ int build_tables(pwfs *h) {
     DevTables &t = h->tab;
     t.N = N; t.M = M; t.NP = (N + 31) / 32 * 32; t.K = K;
     t.D = 2 * n_sub; t.n_sub = n_sub; t.slope_norm = p.slope_norm;
-    // PWFS_DEBUG_T_ALIAS=1 (measurement only, results are wrong): every frame of a chunk uses the T slabs of frame 0,
-    // so the row<->column intermediate stays L2-resident -- what the step would cost if T never reached HBM
+    t.t_frames = 0;
+#ifdef PWFS_TUNING
+    // Tuning builds only (python -m paper_1607_07624_b200.build --tuning -> libpwfs_tuning.so; never in libpwfs.so):
+    // PWFS_DEBUG_T_ALIAS=1 makes every frame of a chunk use the T slabs of frame 0, so the row<->column intermediate
+    // stays L2-resident -- what the step would cost if T never reached HBM.  The results are WRONG by construction.
     const char *alias = std::getenv("PWFS_DEBUG_T_ALIAS");
-    t.t_frames = (alias && alias[0] == '1') ? 1 : 0;
+    if (alias && alias[0] == '1') t.t_frames = 1;
+#endif
 
     // O0: modulation points; distinct x-tilts (the row pass depends on k only through dx_k)
     // f3: an explicit list (dx, dy, w) replaces the circle; I = sum_k w_k |E_k|^2 / sum_k w_k.  The weight
@@ -281,25 +285,20 @@ int build_tables(pwfs *h) {
     return PWFS_OK;
 }
 
-// frames per chunk and k-split for a batch of B frames
-// Frames per chunk and split of the modulation loop.  Chunks are as large as the scratch budget allows: every launch
-// ends with a partly filled wave of CTAs, so fewer, larger launches waste less of the machine (cfg 4: 13.9 ms per 100
-// frames in chunks of 15, 13.4 ms in one chunk).  `min_chunks` > 1 (host-buffer path) keeps at least that many chunks so
-// that copies still overlap the kernels.
-void schedule(const pwfs *h, int B, int *fpc, int *ksplit, int min_chunks = 1) {
+// The most frames one chunk may hold: what the scratch budget (and grid.z) allows, or the caller's pinned chunk size.
+size_t max_chunk_frames(const pwfs *h) {
     const DevTables &t = h->tab;
     const size_t T_frame = (size_t)t.KX * t.M * t.NP * sizeof(float2);   // T[f][j][x][y], x over the whole grid
+    size_t maxF = std::min<size_t>(65535 /* grid.z */, std::max<size_t>(1, h->scratch_budget / std::max<size_t>(T_frame, 1)));
+    if (h->user_fpc > 0) maxF = std::min<size_t>(maxF, (size_t)h->user_fpc);
+    return maxF;
+}
+
+// Split of the modulation loop for chunks of F frames (a function of F alone).
+int ksplit_for(const pwfs *h, int F) {
+    const DevTables &t = h->tab;
     const int col_warps = (t.ncols + h->L.NB - 1) / h->L.NB;           // column-pass warps per frame
     const int slots = h->num_sms * 12;                                  // resident warps we aim to fill
-    const size_t maxF = std::min<size_t>(65535 /* grid.z */, std::max<size_t>(1, h->scratch_budget / std::max<size_t>(T_frame, 1)));
-    int F = h->user_fpc > 0 ? h->user_fpc : (int)std::min<size_t>(maxF, (size_t)std::max(B, 1));
-    if (h->user_fpc <= 0 && min_chunks > 1 && B >= 2 * min_chunks) F = std::min(F, (B + min_chunks - 1) / min_chunks);
-    F = (int)std::min<size_t>((size_t)F, maxF);
-    F = std::max(1, std::min(F, std::max(B, 1)));
-    if (h->user_fpc <= 0 && F < B) {          // equal chunks: ceil(B / n) frames for the smallest n that fits
-        const int n = (B + F - 1) / F;
-        F = (B + n - 1) / n;
-    }
     int ks = h->user_ksplit > 0 ? h->user_ksplit : 1;
     if (h->user_ksplit <= 0 && (long long)F * col_warps < 2LL * slots) {
         // too few warps for the machine (small batches, B = 1 in a closed loop): split the modulation loop, >= 4
@@ -313,18 +312,31 @@ void schedule(const pwfs *h, int B, int *fpc, int *ksplit, int min_chunks = 1) {
             if (cost < best * (1.0 - 1e-9)) { best = cost; ks = c; }
         }
     }
-    ks = std::max(1, std::min(ks, t.K));
-    *fpc = F; *ksplit = ks;
+    return std::max(1, std::min(ks, t.K));
+}
+
+// Frames per chunk and split of the modulation loop for a batch of B frames.  Chunks are as large as the scratch
+// budget allows: every launch
+// ends with a partly filled wave of CTAs, so fewer, larger launches waste less of the machine (cfg 4: 13.9 ms per 100
+// frames in chunks of 15, 13.4 ms in one chunk).  `min_chunks` > 1 (host-buffer path) keeps at least that many chunks so
+// that copies still overlap the kernels.
+void schedule(const pwfs *h, int B, int *fpc, int *ksplit, int min_chunks = 1) {
+    const size_t maxF = max_chunk_frames(h);
+    int F = (int)std::min<size_t>(maxF, (size_t)std::max(B, 1));
+    if (h->user_fpc <= 0 && min_chunks > 1 && B >= 2 * min_chunks) F = std::min(F, (B + min_chunks - 1) / min_chunks);
+    F = std::max(1, std::min(F, std::max(B, 1)));
+    if (h->user_fpc <= 0 && F < B) {          // equal chunks: ceil(B / n) frames for the smallest n that fits
+        const int n = (B + F - 1) / F;
+        F = (B + n - 1) / n;
+    }
+    *fpc = F; *ksplit = ksplit_for(h, F);
 }
 
 // `st`: the stream the caller is about to enqueue on.  cudaMalloc/cudaFree are not allowed while it is being
 // captured into a CUDA graph: a batch that needs more scratch than the handle holds is refused with PWFS_EINVAL
 // (pwfs_reserve, or one eager pwfs_run of that size, before the capture avoids it).
-int ensure_scratch(pwfs *h, int F, int ksplit, cudaStream_t st = nullptr, bool check_capture = false) {
-    const DevTables &t = h->tab;
-    const size_t needT = (size_t)F * t.KX * t.M * t.NP;
-    const size_t needC = (size_t)F * ksplit * t.ncols * t.D;
-    if (check_capture && (needT > h->T_elems || needC > h->colbin_elems || (size_t)F * t.D > h->nsum_elems)) {
+int ensure_scratch_elems(pwfs *h, size_t needT, size_t needC, size_t needN, cudaStream_t st = nullptr, bool check_capture = false) {
+    if (check_capture && (needT > h->T_elems || needC > h->colbin_elems || needN > h->nsum_elems)) {
         cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
         if (cudaStreamIsCapturing(st, &cs) == cudaSuccess && cs != cudaStreamCaptureStatusNone) return PWFS_EINVAL;
     }
@@ -335,7 +347,6 @@ int ensure_scratch(pwfs *h, int F, int ksplit, cudaStream_t st = nullptr, bool c
         if (e != cudaSuccess) { h->last_cuda = (int)e; return e == cudaErrorMemoryAllocation ? PWFS_ENOMEM : PWFS_ECUDA; }
         h->T_elems = needT;
     }
-    const size_t needN = (size_t)F * t.D;
     if (needN > h->nsum_elems) {
         if (h->nsum) cudaFree(h->nsum);
         h->nsum = nullptr; h->nsum_elems = 0;
@@ -351,6 +362,20 @@ int ensure_scratch(pwfs *h, int F, int ksplit, cudaStream_t st = nullptr, bool c
         h->colbin_elems = needC;
     }
     return PWFS_OK;
+}
+
+// scratch of one chunk of F frames whose modulation loop is split `ksplit` ways: T, colbin, nsum [elements]
+void scratch_need(const pwfs *h, int F, int ksplit, size_t *needT, size_t *needC, size_t *needN) {
+    const DevTables &t = h->tab;
+    *needT = (size_t)F * t.KX * t.M * t.NP;
+    *needC = (size_t)F * ksplit * t.ncols * t.D;
+    *needN = (size_t)F * t.D;
+}
+
+int ensure_scratch(pwfs *h, int F, int ksplit, cudaStream_t st = nullptr, bool check_capture = false) {
+    size_t needT, needC, needN;
+    scratch_need(h, F, ksplit, &needT, &needC, &needN);
+    return ensure_scratch_elems(h, needT, needC, needN, st, check_capture);
 }
 
 struct SpanGuard {
@@ -736,15 +761,33 @@ static int run_small(pwfs_t *h, const float *d_phase, int B, float *d_frames, fl
     return PWFS_OK;
 }
 
+// Sizes everything a pwfs_run of ANY batch of 1..B frames can need, not just the schedule of exactly B frames: a
+// smaller batch may take the other path (the fused kernel serves small batches only) or split its modulation loop
+// further (more colbin per frame), and must find its scratch in place when it is captured into a graph.
 int pwfs_reserve(pwfs_t *h, int32_t B) {
     if (!h || B < 1) return PWFS_EINVAL;
     DeviceGuard dg(h->device);
     PWFS_CUDA(h, dg.err);
-    if (small_applies(h, B)) return ensure_small(h, B, nullptr, false);
-    int F, ks;
-    schedule(h, B, &F, &ks);
-    int rc = ensure_scratch(h, F, ks);
+    if (small_applies(h, 1)) {                    // the fused kernel takes batches of 1..bs frames
+        const long long cap = h->small_mode == 1 ? (long long)B : 16LL * h->num_sms / std::max(1, h->tab.K);
+        const int bs = (int)std::min<long long>(B, cap);
+        if (bs >= 1)
+            if (int rc = ensure_small(h, bs, nullptr, false)) return rc;
+        if (bs == B) return PWFS_OK;              // ... which is all of them
+    }
+    // two-kernel path: a batch of b <= B frames runs in chunks of F <= min(b, max_chunk_frames) frames, every such F
+    // is some batch's chunk size, and the k-split is a function of F
+    const int Fmax = (int)std::min<size_t>((size_t)B, max_chunk_frames(h));
+    size_t needT = 0, needC = 0, needN = 0;
+    for (int F = 1; F <= Fmax; ++F) {
+        size_t nT, nC, nN;
+        scratch_need(h, F, ksplit_for(h, F), &nT, &nC, &nN);
+        needT = std::max(needT, nT); needC = std::max(needC, nC); needN = std::max(needN, nN);
+    }
+    int rc = ensure_scratch_elems(h, needT, needC, needN);
     if (rc) return rc;
+    int F, ks;
+    schedule(h, B, &F, &ks);                      // the largest batch has the most chunks
     const size_t n_chunks = ((size_t)B + F - 1) / F;
     if (n_chunks > 1) {
         if (!h->out_stream) PWFS_CUDA(h, cudaStreamCreateWithFlags(&h->out_stream, cudaStreamNonBlocking));

@@ -32,6 +32,7 @@
 
 #include <cuda.h>
 
+#include <algorithm>
 #include <cstdint>
 #include <cstdlib>
 #include <new>
@@ -345,6 +346,7 @@ struct RecTc {
     EncodeTiledFn enc = nullptr;
     float *d_Shi = nullptr, *d_Slo = nullptr, *d_part = nullptr;
     int b_cap = 0;                  // frames the slope planes / partials are sized for
+    int ksplit_env = 0;             // PWFS_REC_KSPLIT (tuning builds only), read once at create; 0 = heuristic
     size_t part_cap = 0;            // floats in d_part
     CUtensorMap mR, mShi, mSlo;
 };
@@ -357,6 +359,9 @@ int rec_tc_create(RecTc **out, const float *d_R, int n_modes, int n_slopes, int 
     h->ldp = (n_slopes + BK - 1) / BK * BK;
     h->enc = encode_tiled_fn();
     if (!h->enc) { delete h; return PWFS_EUNSUPPORTED; }
+#ifdef PWFS_TUNING   // tuning builds only (libpwfs_tuning.so): K split forced from the environment, read once here
+    if (const char *e = std::getenv("PWFS_REC_KSPLIT")) h->ksplit_env = std::max(0, std::atoi(e));
+#endif
     // recmat itself is the TMA source: [n_modes][ldk] FP32, ldk % 4 == 0 (16-byte row pitch), zero padded; K blocks
     // beyond ldk are filled with zeros by TMA
     cudaError_t e = cudaFuncSetAttribute(rec_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
@@ -369,19 +374,26 @@ int rec_tc_create(RecTc **out, const float *d_R, int n_modes, int n_slopes, int 
     return PWFS_OK;
 }
 
-static int rec_tc_ksplit(const RecTc *h, int B) {
-    const int m_tiles = (h->n_modes + BM - 1) / BM, n_tiles = (B + BN - 1) / BN, nkb = h->ldp / BK;
+// K split for a batch that fills n_tiles frame tiles (a function of the tile count, not of B itself)
+static int rec_tc_ksplit_tiles(const RecTc *h, int n_tiles) {
+    const int m_tiles = (h->n_modes + BM - 1) / BM, nkb = h->ldp / BK;
     int ksplit = h->num_sms / ((m_tiles + TM - 1) / TM * n_tiles);
-    if (const char *e = std::getenv("PWFS_REC_KSPLIT")) { const int v = std::atoi(e); if (v > 0) ksplit = v; }   // tuning hook
+    if (h->ksplit_env > 0) ksplit = h->ksplit_env;
     if (ksplit > nkb / 4) ksplit = nkb / 4;                               // at least 4 K blocks per split
     return ksplit < 1 ? 1 : ksplit;
 }
 
-// Sizes the slope planes and the split-K partials for batches of up to B frames (allocates; synchronises `st` first
-// when it has to replace buffers that may be in use).  Returns 1 if nothing had to be done.
-int rec_tc_reserve(RecTc *h, int B, cudaStream_t st) {
-    const int ksplit = rec_tc_ksplit(h, B);
-    const size_t part_need = ksplit > 1 ? (size_t)ksplit * ((size_t)(B + BN - 1) / BN * BN) * h->n_modes : 0;
+static int rec_tc_ksplit(const RecTc *h, int B) { return rec_tc_ksplit_tiles(h, (B + BN - 1) / BN); }
+
+// floats of split-K partials a batch of n_tiles frame tiles writes
+static size_t rec_tc_part_need(const RecTc *h, int n_tiles) {
+    const int ksplit = rec_tc_ksplit_tiles(h, n_tiles);
+    return ksplit > 1 ? (size_t)ksplit * ((size_t)n_tiles * BN) * h->n_modes : 0;
+}
+
+// Makes the slope planes hold B frames and the partials hold part_need floats (allocates; synchronises `st` first
+// when it has to replace buffers that may be in use).
+static int rec_tc_size(RecTc *h, int B, size_t part_need, cudaStream_t st) {
     if (B <= h->b_cap && part_need <= h->part_cap) return PWFS_OK;
     cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
     if (cudaStreamIsCapturing(st, &cs) == cudaSuccess && cs != cudaStreamCaptureStatusNone) return PWFS_EINVAL;
@@ -410,10 +422,19 @@ int rec_tc_reserve(RecTc *h, int B, cudaStream_t st) {
     return PWFS_OK;
 }
 
+// Sizes the slope planes and the split-K partials for every batch of 1..B frames: a smaller batch fills fewer frame
+// tiles, is split further along K, and can need MORE partials than B itself (148 x 128 floats per mode for one tile
+// against 49 x 384 for three), so the need is the largest over the tile counts up to B's.
+int rec_tc_reserve(RecTc *h, int B, cudaStream_t st) {
+    size_t part_need = 0;
+    for (int nt = 1; nt <= (B + BN - 1) / BN; ++nt) part_need = std::max(part_need, rec_tc_part_need(h, nt));
+    return rec_tc_size(h, B, part_need, st);
+}
+
 int rec_tc_run(RecTc *h, const float *d_slopes, int B, float *d_modes, cudaStream_t st) {
     const int m_tiles = (h->n_modes + BM - 1) / BM, n_tiles = (B + BN - 1) / BN, nkb = h->ldp / BK;
     const int ksplit = rec_tc_ksplit(h, B);
-    if (int rc = rec_tc_reserve(h, B, st)) return rc;                     // no-op once sized (pwfs_rec_reserve)
+    if (int rc = rec_tc_size(h, B, rec_tc_part_need(h, n_tiles), st)) return rc;   // no-op once sized (pwfs_rec_reserve)
     split_tf32_kernel<<<dim3((h->ldp + 255) / 256, B), 256, 0, st>>>(d_slopes, (size_t)h->n_slopes, h->n_slopes, h->ldp,
                                                                     h->d_Shi, h->d_Slo);
     rec_tc_kernel<<<dim3((m_tiles + TM - 1) / TM, ksplit, n_tiles), kThreads, kSmemBytes, st>>>(

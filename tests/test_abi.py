@@ -210,6 +210,15 @@ def test_no_cpu_fallback_without_a_device(lib):
     assert ei.value.code == PWFS_ECUDA
 
 
+def test_result_changing_hooks_are_not_in_the_production_library(lib):
+    """PWFS_DEBUG_T_ALIAS (wrong frames, PWFS_OK returned) and PWFS_REC_KSPLIT exist in -DPWFS_TUNING builds only
+    (build.py --tuning -> libpwfs_tuning.so): the strings must not occur in libpwfs.so."""
+    from paper_1607_07624_b200 import pwfs
+    blob = open(pwfs.LIB_PATH, "rb").read()
+    for name in (b"PWFS_DEBUG_T_ALIAS", b"PWFS_REC_KSPLIT"):
+        assert name not in blob, name
+
+
 def test_product_path_does_not_touch_the_oracle():
     pkg = os.path.join(ROOT, "paper_1607_07624_b200")
     for dirpath, _, files in os.walk(pkg):

@@ -282,3 +282,28 @@ def test_batched_reconstructor_is_capturable_after_reserve(torch_cuda):
         g.replay()
         torch.cuda.synchronize()
         assert torch.equal(out, want)
+
+
+def test_reconstructor_reserve_covers_smaller_batches(torch_cuda):
+    """pwfs_rec_reserve(B) must serve every batch up to B.  A smaller batch fills fewer frame tiles and is split
+    further along K: with 10 048 slopes on 148 SMs, 200 frames (2 tiles x 74 splits) write more split-K partials than
+    300 (3 tiles x 49), so a reserve sized for exactly 300 frames would refuse the capture of 200."""
+    from paper_1607_07624_b200.chain import Reconstructor
+    torch = torch_cuda
+    rng = np.random.default_rng(10)
+    R = (rng.standard_normal((128, 10048)) / 100.0).astype(np.float32)
+    S = _dev(torch, 0.1 * rng.standard_normal((300, 10048)))
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with Reconstructor(R) as ref:
+        want = {b: ref.run(S[:b]).clone() for b in (200, 100, 300)}
+    with Reconstructor(R) as rec:
+        rec.reserve(300)
+        for b in (200, 100, 300):
+            out = torch.zeros((b, 128), device="cuda")
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=side):
+                rec.run(S[:b], out=out, stream=side)
+            g.replay()
+            torch.cuda.synchronize()
+            assert torch.equal(out, want[b]), b

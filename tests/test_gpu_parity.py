@@ -364,6 +364,39 @@ def test_cuda_graph_capture_needs_reserved_scratch(torch_cuda):
         assert torch.equal(fr, f_ref) and torch.equal(sl, s_ref)
 
 
+@pytest.mark.parametrize("name,big,small", [("cfg1_tiny", 1000, 10), ("cfg2_flao", 300, 1), ("cfg2_flao", 300, 7)])
+def test_reserve_covers_every_smaller_batch_under_capture(torch_cuda, monkeypatch, name, big, small):
+    """pwfs_reserve(B) promises allocation-free pwfs_run calls of UP TO B frames.  A smaller batch can take another
+    path (M = 128: 1000 frames run the two-kernel path, 10 the fused kernel with its own scratch) or a larger k-split
+    (M = 320: one frame splits the modulation loop, 300 do not, so it needs more column scratch per frame): both
+    must capture into a graph right after the reserve, with nothing run eagerly before."""
+    from paper_1607_07624_b200.pwfs import from_config
+    torch = torch_cuda
+    monkeypatch.delenv("PWFS_SMALL", raising=False)
+    cfg = wl.CONFIGS[name]
+    ph = torch.from_numpy(wl.phase_batch(cfg, steps=small)).cuda()
+    with from_config(cfg) as ref:
+        f_ref, s_ref = ref.run(ph)
+        g_big, g_small = ref.geometry(big), ref.geometry(small)
+    if name == "cfg2_flao":
+        assert g_small["k_split"] > g_big["k_split"] == 1
+    with from_config(cfg) as sensor:
+        fr = torch.empty((small, sensor.det_size, sensor.det_size), device="cuda")
+        sl = torch.empty((small, 2 * sensor.n_valid), device="cuda")
+        sensor.reserve(big)
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            sensor.run(ph, fr, sl)                           # PWFS_EINVAL here if the reserve sized B = big only
+        fr.zero_(); sl.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(fr, f_ref) and torch.equal(sl, s_ref)
+        _, launches = sensor.get_timing()
+        assert (launches["fused"] == 1) == (name == "cfg1_tiny")
+
+
 def test_host_buffer_entry_point_matches_device_entry_point(torch_cuda):
     from paper_1607_07624_b200.pwfs import from_config
     torch = torch_cuda
