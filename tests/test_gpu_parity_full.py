@@ -74,11 +74,25 @@ def _full_batch(name):
     return cfg, phase
 
 
-def _oracle(cfg, A, phase):
+_REF = {}   # config name -> (frames, slopes) of the oracle on that config's batch, kept for the schedule tests below
+
+
+def _oracle(cfg, A, phase, keep_as=None):
     from oracle import pwfs_oracle as orc
     t0 = time.perf_counter()
     fr, sl = orc.pwfs_run(A, cfg.m_grid, cfg.mod_radius, cfg.mod_points, cfg.n_subap, phase)
+    if keep_as is not None:
+        _REF[keep_as] = (fr, sl)
     return fr, sl, time.perf_counter() - t0
+
+
+def _reference(name, cfg, A, phase, n):
+    """Oracle frames and slopes of the first n frames of `phase`: those the every-frame tests above left behind
+    (frame b of a batch is the same input whatever the batch size), else computed now."""
+    if name in _REF and _REF[name][0].shape[0] >= n:
+        return _REF[name][0][:n], _REF[name][1][:n]
+    fr, sl, _ = _oracle(cfg, A, phase[:n])
+    return fr, sl
 
 
 @pytest.mark.parametrize("name", ["cfg2_flao", "cfg3_npot", "cfg5_multi"])
@@ -92,7 +106,7 @@ def test_every_frame_of_the_bench_batch(torch_cuda, name):
         fr, sl = sensor.run(torch.from_numpy(phase).cuda())               # one call, as bench.py makes it
         torch.cuda.synchronize()
         fr, sl = fr.cpu().numpy(), sl.cpu().numpy()
-    fr_ref, sl_ref, secs = _oracle(cfg, A, phase)
+    fr_ref, sl_ref, secs = _oracle(cfg, A, phase, keep_as=name)
     ef, es = _errors(fr, sl, fr_ref, sl_ref)
     _report(name, f"pwfs_run, {phase.shape[0]} frames in chunks of {geo['frames_per_chunk']}", ef, es, secs)
     assert ef.max() <= TOL_FRAME, f"frame {ef.argmax()}: {ef.max():.3e} > {TOL_FRAME}"
@@ -117,10 +131,64 @@ def test_cfg4_every_frame_device_and_host_paths(torch_cuda):
         fh = torch.zeros((B, cfg.det_size, cfg.det_size), dtype=torch.float32).pin_memory()
         sh = torch.zeros((B, 2 * sensor.n_valid), dtype=torch.float32).pin_memory()
         sensor.run_host(h_phase, fh, sh)
-    fr_ref, sl_ref, secs = _oracle(cfg, A, phase)
+    fr_ref, sl_ref, secs = _oracle(cfg, A, phase, keep_as="cfg4_elt")
     ef, es = _errors(fr, sl, fr_ref, sl_ref)
     _report("cfg4_elt", f"pwfs_run, {B} frames in chunks of {geo['frames_per_chunk']}", ef, es, secs)
     efh, esh = _errors(fh.numpy(), sh.numpy(), fr_ref, sl_ref)
     _report("cfg4_elt", f"pwfs_run_host, {B} frames, chunked pipeline", efh, esh, 0.0)
     assert ef.max() <= TOL_FRAME and es.max() <= TOL_SLOPE, (ef.max(), es.max())
     assert efh.max() <= TOL_FRAME and esh.max() <= TOL_SLOPE, (efh.max(), esh.max())
+
+
+@pytest.mark.parametrize("name", ["cfg2_flao", "cfg3_npot", "cfg4_elt", "cfg5_multi"])
+def test_per_step_batches_against_the_oracle(torch_cuda, name):
+    """The closed loop calls the sensor with ONE step's frames ("triggers all processing objects once
+    per simulation step"): B = 1, or the 12 instances of cfg5.  Such a batch runs another schedule than the bench
+    batch -- the modulation loop split over several warps per column (k_split > 1, partial sums added in the x-rebin
+    kernel) and the x-tilt loop of the row pass split by the wave-cost model -- which the every-frame tests above
+    never take.  B = 1, 2, 3 and the instance count, on the benchmark grids, element by element against the oracle."""
+    from paper_1607_07624_b200.pwfs import from_config
+    torch = torch_cuda
+    cfg, phase = _full_batch(name)
+    A = wl.make_pupil(cfg)
+    sizes = sorted({1, 2, 3, cfg.instances})
+    fr_ref, sl_ref = _reference(name, cfg, A, phase, max(sizes))
+    d_phase = torch.from_numpy(phase[:max(sizes)]).cuda()
+    with from_config(cfg) as sensor:
+        assert sensor.geometry(1)["k_split"] > 1 and sensor.geometry(phase.shape[0])["k_split"] == 1
+        for b in sizes:
+            geo = sensor.geometry(b)
+            fr, sl = sensor.run(d_phase[:b])
+            torch.cuda.synchronize()
+            ef, es = _errors(fr.cpu().numpy(), sl.cpu().numpy(), fr_ref[:b], sl_ref[:b])
+            _report(name, f"pwfs_run, per-step batch of {b}, k_split {geo['k_split']}", ef, es, 0.0)
+            assert ef.max() <= TOL_FRAME and es.max() <= TOL_SLOPE, (b, ef.max(), es.max())
+
+
+def test_cfg5_in_several_chunks_against_the_oracle(torch_cuda, monkeypatch):
+    """pwfs_run with a scratch budget that holds a quarter of the batch: four chunks, the tail kernels of chunk c on
+    the side stream under the row pass of chunk c + 1 -- against the oracle (the device path's chunking is otherwise
+    only compared with itself)."""
+    from paper_1607_07624_b200.pwfs import from_config
+    torch = torch_cuda
+    name = "cfg5_multi"
+    cfg, phase = _full_batch(name)
+    if name not in _REF:                                                  # run on its own: 4 steps keep the oracle short
+        phase = phase[:4 * cfg.instances]
+    B = phase.shape[0]
+    A = wl.make_pupil(cfg)
+    with from_config(cfg) as probe:
+        k_unique = probe.geometry(B)["k_unique"]
+    t_frame = k_unique * cfg.m_grid * (-(-cfg.n_pupil // 32) * 32) * 8    # bytes of the row<->column intermediate per frame
+    monkeypatch.setenv("PWFS_SCRATCH_MB", str(-(-t_frame * -(-B // 4) // 2 ** 20)))
+    fr_ref, sl_ref = _reference(name, cfg, A, phase, B)
+    with from_config(cfg) as sensor:
+        geo = sensor.geometry(B)
+        assert -(-B // geo["frames_per_chunk"]) == 4
+        fr, sl = sensor.run(torch.from_numpy(phase).cuda())
+        torch.cuda.synchronize()
+        _, launches = sensor.get_timing()
+        assert launches["xpass"] == 4 and launches["ypass"] == 4 and launches["slopes"] == 4
+    ef, es = _errors(fr.cpu().numpy(), sl.cpu().numpy(), fr_ref, sl_ref)
+    _report(name, f"pwfs_run, {B} frames in 4 chunks of {geo['frames_per_chunk']}", ef, es, 0.0)
+    assert ef.max() <= TOL_FRAME and es.max() <= TOL_SLOPE, (ef.max(), es.max())
