@@ -26,17 +26,29 @@ _lib = None
 
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (double precision, OpenMP).  -O2, no
-    fast-math: the oracle is never tuned."""
+    fast-math: the oracle is never tuned.
+
+    PWFS_ORACLE_SANITIZE=1 builds and loads a second library, libpwfs_oracle_san.so,
+    with -fsanitize=address,undefined (host-side sanitizer pass
+    over the oracle pins).  Python is not an ASan binary, so the runtime must be
+    preloaded:
+        LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0 \
+        PWFS_ORACLE_SANITIZE=1 python -m pytest tests -m "not gpu" -k oracle
+    Same source, same arithmetic; only the instrumentation differs."""
+    san = os.environ.get("PWFS_ORACLE_SANITIZE") == "1"
+    lib = _LIB.replace(".so", "_san.so") if san else _LIB
     with _lock:
-        if (not force and os.path.exists(_LIB)
-                and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
-            return _LIB
-        tmp = _LIB + f".tmp{os.getpid()}"
-        cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared",
-               "-Wall", "-Wextra", "-o", tmp, _SRC, "-lm"]
+        if (not force and os.path.exists(lib)
+                and os.path.getmtime(lib) >= os.path.getmtime(_SRC)):
+            return lib
+        tmp = lib + f".tmp{os.getpid()}"
+        opt = ["-O1", "-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined",
+               "-fno-sanitize-recover=undefined"] if san else ["-O2"]
+        cmd = ["gcc"] + opt + ["-std=c11", "-fopenmp", "-fPIC", "-shared",
+                               "-Wall", "-Wextra", "-o", tmp, _SRC, "-lm"]
         subprocess.run(cmd, check=True)
-        os.replace(tmp, _LIB)
-        return _LIB
+        os.replace(tmp, lib)
+        return lib
 
 
 def _load():
