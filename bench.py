@@ -454,6 +454,38 @@ def roofline_numbers(cfg, geo, B, steps, ms_per_step, kernel_ms, launches, peak_
             "kernel_ms_per_step": {k: v / steps for k, v in kernel_ms.items()}}
 
 
+def latency_per_call(sensor, phase_b, dev, stream, reps: int = 100) -> dict:
+    """Device time of ONE pwfs_run call on a small batch (the closed loop's per-step call: 1 frame, or a config's
+    sensor instances), back to back on one stream: eager launches, and the same call replayed from a CUDA graph."""
+    import torch
+    b = phase_b.shape[0]
+    fr = torch.empty((b, sensor.det_size, sensor.det_size), dtype=torch.float32, device=dev)
+    sl = torch.empty((b, 2 * sensor.n_valid), dtype=torch.float32, device=dev)
+
+    def timed(fn):
+        for _ in range(5):
+            fn()
+        torch.cuda.synchronize(dev)
+        a, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(reps):
+            fn()
+        e.record(stream)
+        torch.cuda.synchronize(dev)
+        return a.elapsed_time(e) / reps
+
+    eager_ms = timed(lambda: sensor.run(phase_b, fr, sl))
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):                        # pwfs_run only enqueues kernels: capturable as is
+        sensor.run(phase_b, fr, sl)
+    graph_ms = timed(graph.replay)
+    del graph
+    geo = sensor.geometry(b)
+    return {"frames_per_call": b, "eager_ms": eager_ms, "cuda_graph_ms": graph_ms, "calls": reps,
+            "k_split": geo["k_split"], "us_per_frame_cuda_graph": 1e3 * graph_ms / b,
+            "note": "back-to-back calls on one stream, device time per call (CUDA events)"}
+
+
 def bench_other_configs(main_name, dev, flush, steps, warmup) -> dict:
     """Every BASELINE.json config timed like the headline one (full batch per step, warm-up, L2 flushed before each
     timed step, CUDA events, per-kernel brackets): frames/s, ms per step, fraction of the FP32 roofline for the path
@@ -484,6 +516,7 @@ def bench_other_configs(main_name, dev, flush, steps, warmup) -> dict:
             slopes = torch.empty((B, 2 * nv), dtype=torch.float32, device=dev)
             sync = lambda: torch.cuda.synchronize(dev)
             ms_total, kernel_ms, launches, _ = time_hot_path(sensor, phase, frames, slopes, steps, warmup, flush, stream, sync)
+            lat_step = latency_per_call(sensor, phase[:cfg.instances].contiguous(), dev, stream)   # one simulation step
         ms = ms_total / steps
         r = roofline_numbers(cfg, geo, B, steps, ms, kernel_ms, launches, FP32_PEAK_TFLOPS)
         out[name] = {"frames_per_step": B, "frames_per_s": B / (ms * 1e-3), "ms_per_step": ms,
@@ -491,14 +524,14 @@ def bench_other_configs(main_name, dev, flush, steps, warmup) -> dict:
                      "mod_points": cfg.mod_points, "frames_per_chunk": geo["frames_per_chunk"], "k_split": geo["k_split"],
                      "path_frac": r["path_frac"], "dominant_kernel": r["kernel"], "dominant_frac": r["frac"],
                      "executed_pair_ratio": r["executed_pair_ratio"], "kernel_ms_per_step": r["kernel_ms_per_step"],
-                     "steps": steps, "warmup": warmup, "input": src}
+                     "steps": steps, "warmup": warmup, "input": src, "latency_step": lat_step}
         del phase, frames, slopes
     return out
 
 
 def measure_fp32_peak(local: int) -> dict:
     """pwfs_peak_fp32 (FFMA and FFMA2 streams on every SM) with the SM clock sampled while it runs."""
-    from paper_1607_07624_b200.pwfs import peak_fp32
+    from paper_1607_07624_b200.peak import peak_fp32
     sampler = ClockSampler(local)
     sampler.start()
     res = {}
@@ -509,7 +542,7 @@ def measure_fp32_peak(local: int) -> dict:
     clk = sampler.stop()
     best = max(res.values())
     return {"tflops": best, "ffma_tflops": res["ffma"], "ffma2_tflops": res["ffma2"], "sm_mhz": clk["sm_mhz"],
-            "how": "pwfs_peak_fp32: independent FFMA / FFMA2 chains, 64 warps per SM, best of 3 x 5 launches, CUDA events"}
+            "how": "pwfs_peak_fp32 (libpwfs_peak.so): independent FFMA / FFMA2 chains, 64 warps per SM, best of 3 x 5 launches, CUDA events"}
 
 
 def run_ours(args, cfg):
@@ -605,31 +638,8 @@ def run_ours(args, cfg):
     # ---- closed-loop latency: one frame per call (B = 1), eager and replayed from a CUDA graph
     latency = None
     if rank == 0:
-        ph1 = phase[:1].contiguous()
-        fr1 = torch.empty((1, D, D), dtype=torch.float32, device=dev)
-        sl1 = torch.empty((1, 2 * nv), dtype=torch.float32, device=dev)
-        reps = 100
-
-        def timed(fn):
-            for _ in range(5):
-                fn()
-            torch.cuda.synchronize(dev)
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(stream)
-            for _ in range(reps):
-                fn()
-            b.record(stream)
-            torch.cuda.synchronize(dev)
-            return a.elapsed_time(b) / reps
-
-        eager_ms = timed(lambda: sensor.run(ph1, fr1, sl1))
-        graph = torch.cuda.CUDAGraph()
-        with torch.cuda.graph(graph):                    # pwfs_run only enqueues kernels: capturable as is
-            sensor.run(ph1, fr1, sl1)
-        graph_ms = timed(graph.replay)
-        latency = {"frames_per_call": 1, "eager_ms": eager_ms, "cuda_graph_ms": graph_ms, "calls": reps,
-                   "note": "back-to-back calls on one stream, device time per call (CUDA events)"}
-        del graph
+        latency = latency_per_call(sensor, phase[:1].contiguous(), dev, stream)
+        latency_step = latency if cfg.instances == 1 else latency_per_call(sensor, phase[:cfg.instances].contiguous(), dev, stream)
 
     # ---- end to end through the host-buffer entry point (e2e) ----------------
     h_phase = torch.from_numpy(phase_np).pin_memory()
@@ -650,7 +660,7 @@ def run_ours(args, cfg):
         M, K = cfg.m_grid, cfg.mod_points
         r = roofline_numbers(cfg, geo, B, args.steps, ms_per_step, kernel_ms, launches, FP32_PEAK_TFLOPS)
         dom, n_launch = r["kernel"], r["launches"]
-        traffic = None                                                   # dram bytes per launch, from the committed ncu capture
+        traffic, traffic_src = None, None                                # dram bytes per launch, from the committed ncu capture
         tpath = os.path.join(ROOT, "profiles", "traffic.csv")
         if os.path.exists(tpath):
             import csv
@@ -659,9 +669,10 @@ def run_ours(args, cfg):
                     if row["config"] == cfg.name and row["kernel"] == dom:
                         per_frame = float(row["dram_bytes_per_launch"]) / float(row["frames_per_launch"])
                         traffic = per_frame * B * args.steps / n_launch
+                        traffic_src = ("copied from profiles/traffic.csv, not measured by this run -- " + row["source"])
         peak_m = measure_fp32_peak(local)
         roof = {"bound": "alu", "kernel": dom, "achieved": r["achieved"], "peak": FP32_PEAK_TFLOPS,
-                "unit": "TFLOP/s", "frac": r["frac"], "traffic": traffic,
+                "unit": "TFLOP/s", "frac": r["frac"], "traffic": traffic, "traffic_source": traffic_src,
                 "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (guide unit counts/clocks)",
                 "peak_measured": peak_m["tflops"], "peak_measured_detail": peak_m,
                 "frac_vs_measured": r["achieved"] / peak_m["tflops"],
@@ -700,7 +711,8 @@ def run_ours(args, cfg):
                 "m_grid": M, "n_pupil": cfg.n_pupil, "mod_points": K, "frames_per_chunk": geo["frames_per_chunk"],
                 "k_split": geo["k_split"], "path_frac": r["path_frac"], "dominant_kernel": dom, "dominant_frac": r["frac"],
                 "executed_pair_ratio": r["executed_pair_ratio"], "kernel_ms_per_step": r["kernel_ms_per_step"],
-                "steps": args.steps, "warmup": args.warmup, "input": "numpy generator (the headline run above)"}
+                "steps": args.steps, "warmup": args.warmup, "input": "numpy generator (the headline run above)",
+                "latency_step": latency_step}
         if not args.no_stages:
             line["stages"] = bench_stages(cfg, dev, phase, frames, flush, loops=not args.no_loops)
         if not args.no_cpu_baseline:

@@ -295,15 +295,6 @@ int pwfs_debug_create(const pwfs_params *p, const pwfs_ext *x, int32_t mask_shif
 int pwfs_debug_intensity(pwfs_t *h, const float *d_phase, int32_t B, float *d_intensity,
                          void *cuda_stream);
 
-/* Measurement aid, not part of the hot path: the FP32 arithmetic peak of `device`
- * as a stream of independent FFMA (packed = 0) or packed FFMA2 (packed = 1)
- * instructions on every SM (64 resident warps each, 8 independent accumulator
- * pairs per thread), best of five launches of ~10^12 flop, timed with CUDA events.
- * *tflops counts an FMA as 2 flop.  This is the measured counterpart of the
- * derived "148 SMs x 128 lanes x 2 x f_SM" roofline denominator that SURVEY.md
- * 8(d) asks for.  Synchronous; uses the legacy default stream. */
-int pwfs_peak_fp32(int32_t device, int32_t packed, double *tflops, double *elapsed_ms);
-
 #ifdef __cplusplus
 }
 #endif

@@ -1,8 +1,10 @@
 // peak_fp32.cu -- the FP32 "plain ALU" roofline denominator, MEASURED: a dependent-chain-free stream of FFMA
 // (scalar) or FFMA2 (packed FP32x2, the instruction the FFT butterflies are written in) on every SM, timed with
 // CUDA events.  SURVEY.md 8(d) asks for this number next to the derived 148 x 128 x 2 x f_SM figure; bench.py
-// reports both (roofline.peak_measured, roofline.frac_vs_measured).  Not part of the hot path.
-#include "../../include/pwfs.h"
+// reports both (roofline.peak_measured, roofline.frac_vs_measured).  Not part of the hot path and not part of
+// libpwfs.so: built into its own small library, libpwfs_peak.so, which only bench.py loads.
+#include "../../include/pwfs.h"        // status codes
+#include "../../include/pwfs_peak.h"
 
 #include <cuda_runtime.h>
 

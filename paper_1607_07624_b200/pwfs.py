@@ -24,7 +24,7 @@ KERNEL_CLASSES = ("xpass", "ypass", "xrebin", "slopes", "fused")
 EXPORTS = ("pwfs_create", "pwfs_create_ex", "pwfs_info", "pwfs_valid_mask", "pwfs_run", "pwfs_run_host",
            "pwfs_destroy", "pwfs_strerror", "pwfs_last_cuda_error", "pwfs_supported_grid",
            "pwfs_set_schedule", "pwfs_set_timing", "pwfs_get_timing", "pwfs_geometry", "pwfs_reserve",
-           "pwfs_last_failed_kernel", "pwfs_peak_fp32", "pwfs_debug_create", "pwfs_debug_intensity",
+           "pwfs_last_failed_kernel", "pwfs_debug_create", "pwfs_debug_intensity",
            "pwfs_run_noalloc")
 
 
@@ -88,8 +88,6 @@ def load_library() -> C.CDLL:
     lib.pwfs_debug_create.restype = C.c_int
     lib.pwfs_debug_intensity.argtypes = [vp, vp, i32, vp, vp]
     lib.pwfs_debug_intensity.restype = C.c_int
-    lib.pwfs_peak_fp32.argtypes = [i32, i32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
-    lib.pwfs_peak_fp32.restype = C.c_int
     lib.pwfs_supported_grid.argtypes = [i32]
     lib.pwfs_supported_grid.restype = C.c_int
     lib.pwfs_set_schedule.argtypes = [vp, i32, i32]
@@ -106,15 +104,6 @@ def load_library() -> C.CDLL:
 
 def strerror(code: int) -> str:
     return load_library().pwfs_strerror(code).decode()
-
-
-def peak_fp32(device: int = 0, packed: bool = True) -> Tuple[float, float]:
-    """(TFLOP/s, ms) of the FFMA / FFMA2 stream micro-benchmark (pwfs_peak_fp32)."""
-    tf, ms = C.c_double(), C.c_double()
-    rc = load_library().pwfs_peak_fp32(device, int(packed), C.byref(tf), C.byref(ms))
-    if rc != PWFS_OK:
-        raise PwfsError(rc, "pwfs_peak_fp32", strerror(rc))
-    return tf.value, ms.value
 
 
 def supported_grid(m_grid: int) -> bool:
