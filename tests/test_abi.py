@@ -199,6 +199,9 @@ def test_null_and_invalid_arguments_do_not_crash(lib):
     lib.pwfs_destroy(None)                                                      # NULL-safe
     assert lib.pwfs_info(None, None, None) == pwfs.PWFS_EINVAL
     assert lib.pwfs_run(None, None, 1, None, None, None) == pwfs.PWFS_EINVAL
+    assert lib.pwfs_run_noalloc(None, None, 1, None, None, None) == pwfs.PWFS_EINVAL
+    assert lib.pwfs_reserve(None, 1) == pwfs.PWFS_EINVAL
+    assert "pwfs_run_noalloc" in pwfs.strerror(pwfs.PWFS_ELIMIT)
     assert lib.pwfs_last_cuda_error(None) == 0
 
 
