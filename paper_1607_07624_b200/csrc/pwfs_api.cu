@@ -664,9 +664,11 @@ static int launch_k1(pwfs_t *h, const float *d_phase, int Fc, cudaStream_t st) {
         // split the x-tilt loop only as far as needed to fill the machine (>= 8 waves of 2 CTAs/SM),
         // keeping >= 3 tilts per CTA so the one-off phasor stays amortised
         while ((long long)row_ctas * Fc * jsplit < 16LL * h->num_sms && t.KX / (jsplit + 1) >= 3) ++jsplit;
-    } else {   // small batch: (waves of resident CTAs) x (x-tilts per CTA + 1 for the phasor), >= 3 tilts per CTA
+    } else {   // small batch (less than two waves of CTAs): (waves of resident CTAs) x (x-tilts per CTA + 1 for the
+        // phasor), down to ONE tilt per CTA -- with SMs to spare the critical path counts, not the repeated phasor
+        // (cfg 2, one frame: 28 CTAs of 4 tilts on 148 SMs ran at 13 % SM-active, profiles/r3_ncu_b1.md)
         double best = 1e300;
-        for (int c = 1; c <= t.KX / 3; ++c) {
+        for (int c = 1; c <= t.KX; ++c) {
             const long long ctas = (long long)row_ctas * Fc * c;
             const double waves = (double)((ctas + h->x_resident_ctas - 1) / h->x_resident_ctas);
             const double cost = waves * ((t.KX + c - 1) / c + 1.0);
